@@ -1,0 +1,165 @@
+"""ORACLE — test infrastructure.  Thin ctypes wrappers over ``liboracle.so``.
+
+Argument marshalling only; every step of the method is in ``spin_oracle.cpp``.
+Lattices are numpy int8 arrays in the natural layout ``[batch][L][L]``.
+"""
+import ctypes
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "spin_oracle.cpp")
+_LIB = os.path.join(_HERE, "liboracle.so")
+
+__all__ = [
+    "build", "philox4x32_10", "ising_table", "potts_table", "init", "ising_half_sweep",
+    "potts_half_sweep", "ising_observables", "potts_observables", "accumulate_moments", "sweep",
+]
+
+
+def build(force=False):
+    """Compile the oracle with ``g++ -O2 -ffp-contract=off`` (no FMA contraction)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = _LIB + ".%d.tmp" % os.getpid()
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-o", tmp, _SRC])
+        os.replace(tmp, _LIB)
+    return _LIB
+
+
+_lib = None
+
+
+def _l():
+    global _lib
+    if _lib is None:
+        lib = ctypes.CDLL(build())
+        c = ctypes
+        p = c.c_void_p
+        lib.oracle_philox4x32_10.argtypes = [p, p, p]
+        lib.oracle_ising_table.argtypes = [c.c_double, c.c_double, c.c_double, p, p]
+        lib.oracle_potts_table.argtypes = [c.c_double, c.c_double, p, p]
+        lib.oracle_init.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, c.c_uint64, c.c_int64]
+        lib.oracle_ising_half_sweep.argtypes = [p, c.c_int32, c.c_int32, p, c.c_double, c.c_double,
+                                                c.c_uint64, c.c_int64, c.c_int64, c.c_int32]
+        lib.oracle_potts_half_sweep.argtypes = [p, c.c_int32, c.c_int32, p, p, c.c_double, c.c_uint64,
+                                                c.c_int64, c.c_int64, c.c_int32]
+        lib.oracle_ising_observables.argtypes = [p, c.c_int32, c.c_int32, p, p]
+        lib.oracle_potts_observables.argtypes = [p, c.c_int32, c.c_int32, p, p, p]
+        lib.oracle_accumulate_moments.argtypes = [p, c.c_int32, p, p]
+        lib.oracle_sweep.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, p, c.c_double, c.c_double,
+                                     c.c_uint64, c.c_int64, c.c_int64, c.c_int64, p, p, p]
+        _lib = lib
+    return _lib
+
+
+def _ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def _lattice(spins):
+    assert spins.dtype == np.int8 and spins.ndim == 3 and spins.shape[1] == spins.shape[2]
+    assert spins.flags["C_CONTIGUOUS"]
+    return spins.shape[0], spins.shape[1]
+
+
+def _q_array(q, batch):
+    if q is None:
+        return None
+    qa = np.ascontiguousarray(np.broadcast_to(np.asarray(q, dtype=np.int32), (batch,)))
+    return qa
+
+
+def _beta_array(beta, batch):
+    return np.ascontiguousarray(np.broadcast_to(np.asarray(beta, dtype=np.float64), (batch,)))
+
+
+def philox4x32_10(ctr, key):
+    ctr = np.asarray(ctr, dtype=np.uint32)
+    key = np.asarray(key, dtype=np.uint32)
+    out = np.zeros(4, dtype=np.uint32)
+    _l().oracle_philox4x32_10(_ptr(ctr), _ptr(key), _ptr(out))
+    return out
+
+
+def ising_table(beta, J, h):
+    """-> (T uint32[10], always bool[10]); class = 5*(s+1)/2 + (nn+4)/2."""
+    T = np.zeros(10, dtype=np.uint32)
+    a = np.zeros(10, dtype=np.uint8)
+    _l().oracle_ising_table(float(beta), float(J), float(h), _ptr(T), _ptr(a))
+    return T, a.astype(bool)
+
+
+def potts_table(beta, J):
+    """-> (T uint32[9], always bool[9]); class = dn+4."""
+    T = np.zeros(9, dtype=np.uint32)
+    a = np.zeros(9, dtype=np.uint8)
+    _l().oracle_potts_table(float(beta), float(J), _ptr(T), _ptr(a))
+    return T, a.astype(bool)
+
+
+def init(batch, L, seed, q=None, replica_offset=0):
+    """Initial lattices (O3).  q=None -> Ising; q int or int[batch] -> Potts."""
+    spins = np.zeros((batch, L, L), dtype=np.int8)
+    qa = _q_array(q, batch)
+    _l().oracle_init(_ptr(spins), batch, L, 0 if q is None else 1, _ptr(qa), int(seed), int(replica_offset))
+    return spins
+
+
+def ising_half_sweep(spins, beta, J, h, seed, t, colour, replica_offset=0):
+    B, L = _lattice(spins)
+    ba = _beta_array(beta, B)
+    _l().oracle_ising_half_sweep(_ptr(spins), B, L, _ptr(ba), float(J), float(h), int(seed),
+                                 int(replica_offset), int(t), int(colour))
+
+
+def potts_half_sweep(spins, q, beta, J, seed, t, colour, replica_offset=0):
+    B, L = _lattice(spins)
+    ba = _beta_array(beta, B)
+    qa = _q_array(q, B)
+    _l().oracle_potts_half_sweep(_ptr(spins), B, L, _ptr(qa), _ptr(ba), float(J), int(seed),
+                                 int(replica_offset), int(t), int(colour))
+
+
+def ising_observables(spins):
+    B, L = _lattice(spins)
+    E = np.zeros(B, dtype=np.int64)
+    M = np.zeros(B, dtype=np.int64)
+    _l().oracle_ising_observables(_ptr(spins), B, L, _ptr(E), _ptr(M))
+    return E, M
+
+
+def potts_observables(spins, q):
+    B, L = _lattice(spins)
+    qa = _q_array(q, B)
+    E = np.zeros(B, dtype=np.int64)
+    M = np.zeros(B, dtype=np.int64)
+    _l().oracle_potts_observables(_ptr(spins), B, L, _ptr(qa), _ptr(E), _ptr(M))
+    return E, M
+
+
+def accumulate_moments(moments, E, M):
+    B = moments.shape[0]
+    assert moments.dtype == np.int64 and moments.shape == (B, 8) and moments.flags["C_CONTIGUOUS"]
+    E = np.ascontiguousarray(E, dtype=np.int64)
+    M = np.ascontiguousarray(M, dtype=np.int64)
+    _l().oracle_accumulate_moments(_ptr(moments), B, _ptr(E), _ptr(M))
+
+
+def sweep(spins, beta, J, h, seed, n_sweeps, sweep_offset=0, q=None, replica_offset=0,
+          trace=False, moments=None):
+    """Run sweeps in place.  Returns (E_trace, M_trace) int64[n_sweeps][batch] if trace else None."""
+    B, L = _lattice(spins)
+    ba = _beta_array(beta, B)
+    qa = _q_array(q, B)
+    Et = Mt = None
+    if trace:
+        Et = np.zeros((n_sweeps, B), dtype=np.int64)
+        Mt = np.zeros((n_sweeps, B), dtype=np.int64)
+    if moments is not None:
+        assert moments.dtype == np.int64 and moments.shape == (B, 8) and moments.flags["C_CONTIGUOUS"]
+    _l().oracle_sweep(_ptr(spins), B, L, 0 if q is None else 1, _ptr(qa), _ptr(ba), float(J), float(h),
+                      int(seed), int(replica_offset), int(n_sweeps), int(sweep_offset),
+                      _ptr(Et), _ptr(Mt), _ptr(moments))
+    return (Et, Mt) if trace else None
