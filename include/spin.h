@@ -1,0 +1,161 @@
+/* spin.h — C ABI of libspin.so: batched checkerboard Metropolis sweeps for the 2D Ising and q-state
+ * Potts models on one NVIDIA B200 (sm_100a).
+ *
+ * What the library computes is the hot path of arXiv 2304.01772, "A differentiable programming
+ * framework for spin models" (citations are line numbers of /root/reference/PAPER.md):
+ *   - Algorithm 1, "Standard Metropolis-Hastings algorithm with parallelization":
+ *     propose a new state per site, evaluate the local energy change dE from the 4 nearest
+ *     neighbours, accept if dE <= 0, else with probability exp(-beta dH);
+ *   - the checkerboard method (Fig. 1): all sites of one colour are updated in
+ *     parallel, black squares first, then white squares;
+ *   - the Ising Hamiltonian Eq. 1 with the 4-neighbour stencil Eq. 2 and the
+ *     Potts Hamiltonian Eq. 5 with the four one-neighbour stencils Eq. 6 and the "one of the other
+ *     q-1 states" proposal;
+ *   - the batch dimension = independent lattices, each with its own temperature;
+ *   - energy / magnetisation bookkeeping.
+ * The readings taken where the paper is silent (sign of J, colour order, RNG, dE == 0, ...) are
+ * listed in DESIGN.md section 3.  Library sign convention: H = -J sum_<ij> s_i s_j - h sum_i s_i
+ * (Ising, s = +-1) and H = -J sum_<ij> delta(s_i, s_j) (Potts, s in 0..q-1); J > 0 is the
+ * ferromagnet (the paper's J = -1).  k_B = 1, beta = 1/T.
+ *
+ * Random numbers: Philox-4x32-10 keyed by (seed; group, replica, sweep t, colour, domain); see
+ * DESIGN.md section 3 (O2).  Results are a pure function of (seed, replica index, t): running
+ * n sweeps from offset 0 equals running them in chunks, and replica b of a batch equals replica 0
+ * of a handle created with replica_offset = b.
+ *
+ * General conventions
+ *   - Every function is extern "C"; no exception crosses the boundary; no global state other than a
+ *     thread-local last-error string.
+ *   - "host" pointers are ordinary CPU memory (pinned or pageable); "device" pointers are CUDA device
+ *     memory on the handle's device.  Unless stated otherwise pointers are host pointers.
+ *   - The caller owns every array it passes; the library keeps no caller pointer after a call returns,
+ *     except device_buffer of spin_create_ex (owned by the caller, must outlive the handle).
+ *   - int functions return SPIN_OK or a negative code; on SPIN_ERR_INVALID / SPIN_ERR_UNSUPPORTED no
+ *     caller array and no lattice has been modified.  spin_create* return NULL on failure.  The reason
+ *     is available from spin_last_error().
+ *   - One handle is used from one host thread at a time.  All work of a handle is enqueued on the
+ *     handle's CUDA stream; calls that return results in host memory synchronise that stream.
+ *   - There is no CPU fallback: without a CUDA device spin_create* fail with SPIN_ERR_CUDA text.
+ */
+#ifndef SPIN_H_
+#define SPIN_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#if defined(__GNUC__)
+#define SPIN_API __attribute__((visibility("default")))
+#else
+#define SPIN_API
+#endif
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct spin_sim spin_sim; /* opaque handle, owned by the library */
+
+enum { SPIN_OK = 0, SPIN_ERR_INVALID = -1, SPIN_ERR_NOMEM = -2, SPIN_ERR_CUDA = -3, SPIN_ERR_UNSUPPORTED = -4 };
+enum { SPIN_MODEL_ISING = 0, SPIN_MODEL_POTTS = 1 };
+enum { SPIN_LAYOUT_INT8 = 0, SPIN_LAYOUT_BITPACKED = 1 }; /* bit-packed: Ising only, L % 64 == 0 */
+
+/* ---------------------------------------------------------------------------------------------
+ * Core calls (BASELINE.json north star; problem statement PAPER.md:93-95, 127-138)
+ * ------------------------------------------------------------------------------------------- */
+
+/* Create `batch` periodic L x L lattices on the current CUDA device and initialise them uniformly at
+ * random from Philox(seed) ("a random initial state"; O3).
+ * q == 2: Ising, int8 spins -1/+1.  q >= 3: Potts, uint8 states 0..q-1, the same q in every replica.
+ * Layout int8, replica_offset 0, library-owned memory, the default (NULL) stream.
+ * Invalid: batch < 1, L < 2 or odd, q < 2 or q > 127.  Returns NULL on failure. */
+SPIN_API spin_sim* spin_create(int32_t batch, int32_t L, int32_t q, uint64_t seed);
+
+/* Run Metropolis sweeps t = sweep_offset .. sweep_offset + n_sweeps - 1; each sweep updates colour 0
+ * ((i+j) even) and then colour 1 (Alg. 1 + checkerboard).
+ * beta: host, [batch], inverse temperature of each replica (finite, >= 0); copied before return.
+ * J, h: coupling and field (finite).  h must be 0 for Potts (SPIN_ERR_UNSUPPORTED otherwise).
+ * n_sweeps >= 0, sweep_offset >= 0, sweep_offset + n_sweeps <= 2^56.
+ * Asynchronous on the handle's stream. */
+SPIN_API int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_sweeps, int64_t sweep_offset);
+
+/* Exact integer observables of the current lattices (O8).
+ * E: host, [batch]: E_int = -(sum over bonds of s_i s_j) (Ising) or -(number of equal bonds) (Potts),
+ *    every bond once, double bonds of L == 2 counted twice.  Energy = J E_int - h M (Ising), J E_int (Potts).
+ * M: host, [batch]: sum of spins (Ising) or the population of the most common state (Potts).
+ * Either pointer may be NULL.  Synchronises the stream. */
+SPIN_API int spin_observables(spin_sim* sim, int64_t* E, int64_t* M);
+
+/* Destroy a handle (frees library-owned device memory).  NULL is a no-op. */
+SPIN_API void spin_destroy(spin_sim* sim);
+
+/* Thread-local description of the last failure in this thread; valid until the next failing call. */
+SPIN_API const char* spin_last_error(void);
+
+/* ---------------------------------------------------------------------------------------------
+ * Calls needed by the five BASELINE.json configurations and the parity tests
+ * ------------------------------------------------------------------------------------------- */
+
+/* Bytes of device memory a lattice buffer of this shape needs (0 if the shape is invalid).
+ * int8 layout: batch * L * L bytes, stored [batch][colour][L][L/2] (colour = (i+j)&1, column index
+ * k = j >> 1), Ising bytes are -1/+1, Potts bytes 0..q-1.
+ * bit-packed layout: batch * L * L / 8 bytes, stored [batch][colour][L][L/64] uint32 words, bit b of
+ * word w = site k = 32 w + b, bit set = spin -1. */
+SPIN_API size_t spin_buffer_bytes(int32_t batch, int32_t L, int32_t model, int32_t layout);
+
+/* Full constructor.
+ * model: SPIN_MODEL_*.  q_per_replica: host, [batch], or NULL to use q_uniform for every replica
+ * (Ising: q is ignored and taken as 2).  layout: SPIN_LAYOUT_*.  replica_offset >= 0: replica b is
+ * keyed in the generator as b + replica_offset (must stay below 2^32).
+ * device_buffer: NULL (library allocates and owns spin_buffer_bytes(...) bytes) or a 16-byte-aligned
+ * device pointer to at least that many bytes, owned by the caller, which must outlive the handle;
+ * buffer_bytes is its size (ignored when NULL).  cuda_stream: a cudaStream_t, NULL = default stream.
+ * The lattice is initialised from Philox(seed) as in spin_create.
+ * SPIN_ERR_UNSUPPORTED (NULL return): bit-packed with Potts or with L % 64 != 0. */
+SPIN_API spin_sim* spin_create_ex(int32_t batch, int32_t L, int32_t model, const int32_t* q_per_replica, int32_t q_uniform,
+                         uint64_t seed, int32_t layout, int64_t replica_offset, void* device_buffer,
+                         size_t buffer_bytes, void* cuda_stream);
+
+/* Use another CUDA stream for subsequent work (the previous stream is synchronised first). */
+SPIN_API int spin_set_stream(spin_sim* sim, void* cuda_stream);
+
+/* Copy the lattices out / in, in the natural layout [batch][L][L] int8 (Ising -1/+1, Potts 0..q-1).
+ * Host pointers; both synchronise the stream.  spin_set_spins validates every value
+ * (SPIN_ERR_INVALID, lattice unchanged). */
+SPIN_API int spin_get_spins(spin_sim* sim, int8_t* out);
+SPIN_API int spin_set_spins(spin_sim* sim, const int8_t* in);
+
+/* spin_sweep with measurements after every full sweep (rows a5-a7 of DESIGN.md section 1).
+ * E_trace, M_trace: host, [n_sweeps][batch] or NULL: (E_int, M) after each sweep.
+ * moments: host, [batch][8], in/out, or NULL: every sweep adds one sample to
+ *   {n, sum E, sum E^2 (low 64 bits), sum E^2 (high 64 bits), sum M, sum |M|, sum M^2, sum E*M}
+ *   with E = E_int; all int64, sum E^2 is one 128-bit integer in two limbs.
+ * Synchronises the stream. */
+SPIN_API int spin_sweep_measure(spin_sim* sim, const double* beta, double J, double h, int64_t n_sweeps, int64_t sweep_offset,
+                       int64_t* E_trace, int64_t* M_trace, int64_t* moments);
+
+/* spin_observables into device memory (E_dev, M_dev: device, [batch], either may be NULL); enqueued on
+ * the stream, no synchronisation. */
+SPIN_API int spin_observables_dev(spin_sim* sim, int64_t* E_dev, int64_t* M_dev);
+
+/* Wait for all work enqueued on the handle's stream. */
+SPIN_API int spin_synchronize(spin_sim* sim);
+
+/* The acceptance table of one replica, computed on the host in IEEE double exactly as the sweeps use it
+ * (Alg. 1 lines 6-9; O4).  Needs no GPU.
+ * Ising: 10 classes, index 5*(s+1)/2 + (nn+4)/2 (s = -1 first, neighbour sum nn ascending), dE = 2 s (J nn + h).
+ * Potts: 9 classes, index dn + 4, dn = n_new - n_old, dE = -J dn (h ignored).
+ * T[c] = floor(exp(-beta dE) 2^32) clipped to 2^32-1; always[c] = 1 iff beta*dE <= 0 (accept regardless of
+ * the random word).  A move of class c is accepted iff always[c] or r < T[c] (r: 32-bit Philox word).
+ * Returns the number of classes written (10 or 9), or SPIN_ERR_INVALID. */
+SPIN_API int spin_threshold_table(int32_t model, double beta, double J, double h, uint32_t* T, uint8_t* always);
+
+/* Number of kernels this handle has launched since creation (for bench.py's gpu_launches). */
+SPIN_API int64_t spin_kernel_launches(const spin_sim* sim);
+
+/* Human-readable name of the sweep kernel variant the handle selects for its shape (diagnostics). */
+SPIN_API const char* spin_kernel_variant(const spin_sim* sim);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SPIN_H_ */

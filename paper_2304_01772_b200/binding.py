@@ -1,0 +1,204 @@
+"""ctypes binding of include/spin.h.  Same names, argument marshalling only: every step of the path runs in
+the CUDA kernels of libspin.so.  There is no fallback: if the library is missing it is built with nvcc, and if
+that fails, or no CUDA device is present at spin_create time, an exception is raised."""
+import ctypes
+import os
+
+import numpy as np
+
+from . import build as _build
+
+SPIN_OK, SPIN_ERR_INVALID, SPIN_ERR_NOMEM, SPIN_ERR_CUDA, SPIN_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
+SPIN_MODEL_ISING, SPIN_MODEL_POTTS = 0, 1
+SPIN_LAYOUT_INT8, SPIN_LAYOUT_BITPACKED = 0, 1
+
+__all__ = [
+    "SPIN_OK", "SPIN_ERR_INVALID", "SPIN_ERR_NOMEM", "SPIN_ERR_CUDA", "SPIN_ERR_UNSUPPORTED",
+    "SPIN_MODEL_ISING", "SPIN_MODEL_POTTS", "SPIN_LAYOUT_INT8", "SPIN_LAYOUT_BITPACKED",
+    "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim",
+    "spin_create", "spin_create_ex",
+]
+
+_lib = None
+
+
+class SpinError(RuntimeError):
+    def __init__(self, code, message):
+        super().__init__("libspin error %d: %s" % (code, message))
+        self.code = code
+
+
+def load_library():
+    """Load (building if needed) libspin.so and declare the prototypes of include/spin.h."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    if not os.path.exists(path):
+        raise RuntimeError("libspin.so is missing and could not be built; there is no fallback path")
+    lib = ctypes.CDLL(path)
+    c = ctypes
+    vp, i32, i64, u64, dbl, sz = c.c_void_p, c.c_int32, c.c_int64, c.c_uint64, c.c_double, c.c_size_t
+    protos = {
+        "spin_create": (vp, [i32, i32, i32, u64]),
+        "spin_sweep": (c.c_int, [vp, vp, dbl, dbl, i64, i64]),
+        "spin_observables": (c.c_int, [vp, vp, vp]),
+        "spin_destroy": (None, [vp]),
+        "spin_last_error": (c.c_char_p, []),
+        "spin_buffer_bytes": (sz, [i32, i32, i32, i32]),
+        "spin_create_ex": (vp, [i32, i32, i32, vp, i32, u64, i32, i64, vp, sz, vp]),
+        "spin_set_stream": (c.c_int, [vp, vp]),
+        "spin_get_spins": (c.c_int, [vp, vp]),
+        "spin_set_spins": (c.c_int, [vp, vp]),
+        "spin_sweep_measure": (c.c_int, [vp, vp, dbl, dbl, i64, i64, vp, vp, vp]),
+        "spin_observables_dev": (c.c_int, [vp, vp, vp]),
+        "spin_synchronize": (c.c_int, [vp]),
+        "spin_threshold_table": (c.c_int, [i32, dbl, dbl, dbl, vp, vp]),
+        "spin_kernel_launches": (i64, [vp]),
+        "spin_kernel_variant": (c.c_char_p, [vp]),
+    }
+    for name, (res, args) in protos.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+EXPORTED_SYMBOLS = (
+    "spin_create", "spin_sweep", "spin_observables", "spin_destroy", "spin_last_error", "spin_buffer_bytes",
+    "spin_create_ex", "spin_set_stream", "spin_get_spins", "spin_set_spins", "spin_sweep_measure",
+    "spin_observables_dev", "spin_synchronize", "spin_threshold_table", "spin_kernel_launches",
+    "spin_kernel_variant",
+)
+
+
+def spin_last_error():
+    return load_library().spin_last_error().decode()
+
+
+def _check(rc):
+    if rc != SPIN_OK:
+        raise SpinError(rc, spin_last_error())
+
+
+def _np_ptr(a):
+    return None if a is None else a.ctypes.data_as(ctypes.c_void_p)
+
+
+def spin_buffer_bytes(batch, L, model, layout):
+    return int(load_library().spin_buffer_bytes(batch, L, model, layout))
+
+
+def spin_threshold_table(model, beta, J, h=0.0):
+    """-> (T uint32[n], always bool[n]); n = 10 (Ising) or 9 (Potts).  Host only, needs no GPU."""
+    T = np.zeros(10, dtype=np.uint32)
+    a = np.zeros(10, dtype=np.uint8)
+    n = load_library().spin_threshold_table(model, float(beta), float(J), float(h), _np_ptr(T), _np_ptr(a))
+    if n < 0:
+        raise SpinError(n, spin_last_error())
+    return T[:n].copy(), a[:n].astype(bool)
+
+
+class SpinSim:
+    """Owner of one spin_sim* handle.  Methods are the C calls with numpy / raw-pointer marshalling."""
+
+    def __init__(self, handle, batch, L, model, layout, keepalive=None):
+        self._h = handle
+        self.batch, self.L, self.model, self.layout = batch, L, model, layout
+        self._keepalive = keepalive  # e.g. the torch tensor backing device_buffer
+
+    def _beta(self, beta):
+        b = np.ascontiguousarray(np.broadcast_to(np.asarray(beta, dtype=np.float64), (self.batch,)))
+        return b
+
+    def spin_sweep(self, beta, J, h, n_sweeps, sweep_offset=0):
+        b = self._beta(beta)
+        _check(load_library().spin_sweep(self._h, _np_ptr(b), float(J), float(h), int(n_sweeps), int(sweep_offset)))
+
+    def spin_observables(self):
+        E = np.zeros(self.batch, dtype=np.int64)
+        M = np.zeros(self.batch, dtype=np.int64)
+        _check(load_library().spin_observables(self._h, _np_ptr(E), _np_ptr(M)))
+        return E, M
+
+    def spin_observables_dev(self, E_ptr, M_ptr):
+        _check(load_library().spin_observables_dev(self._h, E_ptr, M_ptr))
+
+    def spin_get_spins(self, out=None):
+        if out is None:
+            out = np.empty((self.batch, self.L, self.L), dtype=np.int8)
+        assert out.dtype == np.int8 and out.size == self.batch * self.L * self.L and out.flags["C_CONTIGUOUS"]
+        _check(load_library().spin_get_spins(self._h, _np_ptr(out)))
+        return out
+
+    def spin_set_spins(self, spins):
+        s = np.ascontiguousarray(spins, dtype=np.int8)
+        assert s.size == self.batch * self.L * self.L
+        _check(load_library().spin_set_spins(self._h, _np_ptr(s)))
+
+    def spin_set_spins_ptr(self, host_ptr):
+        """spin_set_spins from a raw host pointer (e.g. a pinned torch tensor's data_ptr())."""
+        _check(load_library().spin_set_spins(self._h, host_ptr))
+
+    def spin_sweep_measure(self, beta, J, h, n_sweeps, sweep_offset=0, trace=True, moments=None):
+        b = self._beta(beta)
+        Et = Mt = None
+        if trace:
+            Et = np.zeros((n_sweeps, self.batch), dtype=np.int64)
+            Mt = np.zeros((n_sweeps, self.batch), dtype=np.int64)
+        if moments is not None:
+            assert moments.dtype == np.int64 and moments.shape == (self.batch, 8) and moments.flags["C_CONTIGUOUS"]
+        _check(load_library().spin_sweep_measure(self._h, _np_ptr(b), float(J), float(h), int(n_sweeps),
+                                                 int(sweep_offset), _np_ptr(Et), _np_ptr(Mt), _np_ptr(moments)))
+        return Et, Mt
+
+    def spin_set_stream(self, cuda_stream):
+        _check(load_library().spin_set_stream(self._h, cuda_stream))
+
+    def spin_synchronize(self):
+        _check(load_library().spin_synchronize(self._h))
+
+    def spin_kernel_launches(self):
+        return int(load_library().spin_kernel_launches(self._h))
+
+    def spin_kernel_variant(self):
+        return load_library().spin_kernel_variant(self._h).decode()
+
+    def spin_destroy(self):
+        if self._h:
+            load_library().spin_destroy(self._h)
+            self._h = None
+            self._keepalive = None
+
+    def __del__(self):
+        try:
+            self.spin_destroy()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.spin_destroy()
+
+
+def spin_create(batch, L, q, seed):
+    h = load_library().spin_create(batch, L, q, seed)
+    if not h:
+        raise SpinError(SPIN_ERR_INVALID, spin_last_error())
+    return SpinSim(h, batch, L, SPIN_MODEL_ISING if q == 2 else SPIN_MODEL_POTTS, SPIN_LAYOUT_INT8)
+
+
+def spin_create_ex(batch, L, model, q_per_replica=None, q_uniform=2, seed=0, layout=SPIN_LAYOUT_INT8,
+                   replica_offset=0, device_buffer=None, buffer_bytes=0, cuda_stream=None, keepalive=None):
+    qa = None
+    if q_per_replica is not None:
+        qa = np.ascontiguousarray(q_per_replica, dtype=np.int32)
+        assert qa.shape == (batch,)
+    h = load_library().spin_create_ex(batch, L, model, _np_ptr(qa), int(q_uniform), int(seed), layout,
+                                      int(replica_offset), device_buffer, int(buffer_bytes), cuda_stream)
+    if not h:
+        raise SpinError(SPIN_ERR_INVALID, spin_last_error())
+    return SpinSim(h, batch, L, model, layout, keepalive=keepalive)

@@ -1,0 +1,184 @@
+// init_layout.cu — row a0 (initial lattice from Philox, O3) and the natural <-> checkerboard-split
+// layout conversions used by spin_get_spins / spin_set_spins.  None of this is on the hot loop.
+#include "spin_internal.cuh"
+
+namespace spin {
+
+namespace {
+
+// Position of natural site (i, j) in the colour-split layouts.
+__device__ __forceinline__ size_t int8_index(int b, int L, int i, int j) {
+    const int c = (i + j) & 1;
+    const int W = L >> 1;
+    return (((size_t)b * 2 + c) * L + i) * W + (j >> 1);
+}
+
+// O3: one thread per Philox group of 4 consecutive natural sites p = 4g .. 4g+3.
+// int8 layout: scattered byte stores (init is not hot).
+__global__ void init_int8_kernel(InitArgs a, int potts) {
+    const long long N = (long long)a.L * a.L;
+    const long long groups = (N + 3) >> 2;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= groups * a.batch) return;
+    const int b = (int)(gid / groups);
+    const uint32_t g = (uint32_t)(gid % groups);
+    uint32_t out[4];
+    philox4x32_10(a.rk, g, (uint32_t)b + a.replica_offset, 0u, (uint32_t)kDomainInit << 28, out);
+    int8_t* lat = (int8_t*)a.lattice;
+    const uint32_t q = potts ? (uint32_t)a.q[b] : 2u;
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const long long p = 4ll * g + e;
+        if (p >= N) break;
+        const int i = (int)(p / a.L), j = (int)(p % a.L);
+        int8_t v;
+        if (potts) v = (int8_t)__umulhi(out[e], q);
+        else v = (out[e] & 0x80000000u) ? (int8_t)1 : (int8_t)-1;
+        lat[int8_index(b, a.L, i, j)] = v;
+    }
+}
+
+// Bit-packed layout: one thread per 64 consecutive natural sites of a row (j = 64 x .. 64 x + 63), which are
+// exactly word x of colour 0 and word x of colour 1 of that row (bit = 1 means spin -1).
+__global__ void init_bits_kernel(InitArgs a) {
+    const int wordsPerRow = a.L >> 6;
+    const long long total = (long long)a.batch * a.L * wordsPerRow;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= total) return;
+    const int x = (int)(gid % wordsPerRow);
+    const int i = (int)((gid / wordsPerRow) % a.L);
+    const int b = (int)(gid / ((long long)wordsPerRow * a.L));
+    uint32_t w[2] = {0u, 0u};
+    const long long p0 = (long long)i * a.L + 64ll * x;  // multiple of 4
+    for (int gq = 0; gq < 16; ++gq) {
+        uint32_t out[4];
+        philox4x32_10(a.rk, (uint32_t)((p0 >> 2) + gq), (uint32_t)b + a.replica_offset, 0u,
+                      (uint32_t)kDomainInit << 28, out);
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int jj = 4 * gq + e;          // j - 64 x
+            const int c = (i + jj) & 1;         // 64 x is even
+            const uint32_t down = (out[e] & 0x80000000u) ? 0u : 1u;
+            w[c] |= down << (jj >> 1);
+        }
+    }
+    uint32_t* lat = (uint32_t*)a.lattice;
+    lat[(((size_t)b * 2 + 0) * a.L + i) * wordsPerRow + x] = w[0];
+    lat[(((size_t)b * 2 + 1) * a.L + i) * wordsPerRow + x] = w[1];
+}
+
+__global__ void from_natural_int8_kernel(const int8_t* __restrict__ nat, int8_t* __restrict__ lat, int batch, int L) {
+    const long long N = (long long)L * L;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= N * batch) return;
+    const int b = (int)(gid / N);
+    const long long p = gid % N;
+    const int i = (int)(p / L), j = (int)(p % L);
+    lat[int8_index(b, L, i, j)] = nat[gid];
+}
+
+__global__ void to_natural_int8_kernel(const int8_t* __restrict__ lat, int8_t* __restrict__ nat, int batch, int L) {
+    const long long N = (long long)L * L;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= N * batch) return;
+    const int b = (int)(gid / N);
+    const long long p = gid % N;
+    const int i = (int)(p / L), j = (int)(p % L);
+    nat[gid] = lat[int8_index(b, L, i, j)];
+}
+
+// one thread per (b, i, x): 64 natural sites <-> two words
+__global__ void from_natural_bits_kernel(const int8_t* __restrict__ nat, uint32_t* __restrict__ lat, int batch, int L) {
+    const int wordsPerRow = L >> 6;
+    const long long total = (long long)batch * L * wordsPerRow;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= total) return;
+    const int x = (int)(gid % wordsPerRow);
+    const int i = (int)((gid / wordsPerRow) % L);
+    const int b = (int)(gid / ((long long)wordsPerRow * L));
+    const int8_t* row = nat + ((size_t)b * L + i) * L + 64 * x;
+    uint32_t w[2] = {0u, 0u};
+    for (int jj = 0; jj < 64; ++jj) {
+        const int c = (i + jj) & 1;
+        w[c] |= (row[jj] < 0 ? 1u : 0u) << (jj >> 1);
+    }
+    lat[(((size_t)b * 2 + 0) * L + i) * wordsPerRow + x] = w[0];
+    lat[(((size_t)b * 2 + 1) * L + i) * wordsPerRow + x] = w[1];
+}
+
+__global__ void to_natural_bits_kernel(const uint32_t* __restrict__ lat, int8_t* __restrict__ nat, int batch, int L) {
+    const int wordsPerRow = L >> 6;
+    const long long total = (long long)batch * L * wordsPerRow;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= total) return;
+    const int x = (int)(gid % wordsPerRow);
+    const int i = (int)((gid / wordsPerRow) % L);
+    const int b = (int)(gid / ((long long)wordsPerRow * L));
+    uint32_t w[2];
+    w[0] = lat[(((size_t)b * 2 + 0) * L + i) * wordsPerRow + x];
+    w[1] = lat[(((size_t)b * 2 + 1) * L + i) * wordsPerRow + x];
+    int8_t* row = nat + ((size_t)b * L + i) * L + 64 * x;
+    for (int jj = 0; jj < 64; ++jj) {
+        const int c = (i + jj) & 1;
+        row[jj] = ((w[c] >> (jj >> 1)) & 1u) ? (int8_t)-1 : (int8_t)1;
+    }
+}
+
+__global__ void validate_natural_kernel(const int8_t* __restrict__ nat, int batch, int L, int potts,
+                                        const int32_t* __restrict__ q, unsigned int* bad) {
+    const long long N = (long long)L * L;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= N * batch) return;
+    const int v = nat[gid];
+    bool ok;
+    if (potts) ok = v >= 0 && v < q[gid / N];
+    else ok = (v == 1 || v == -1);
+    if (!ok) atomicAdd(bad, 1u);
+}
+
+inline unsigned blocks_for(long long n, int tpb) { return (unsigned)((n + tpb - 1) / tpb); }
+
+}  // namespace
+
+int launch_init(const InitArgs& a, int model, int layout, cudaStream_t s) {
+    if (layout == 1) {
+        const long long total = (long long)a.batch * a.L * (a.L >> 6);
+        init_bits_kernel<<<blocks_for(total, 128), 128, 0, s>>>(a);
+    } else {
+        const long long N = (long long)a.L * a.L;
+        const long long total = ((N + 3) >> 2) * a.batch;
+        init_int8_kernel<<<blocks_for(total, 256), 256, 0, s>>>(a, model);
+    }
+    return 1;
+}
+
+int launch_from_natural(const int8_t* natural, void* lattice, int batch, int L, int layout, cudaStream_t s) {
+    if (layout == 1) {
+        const long long total = (long long)batch * L * (L >> 6);
+        from_natural_bits_kernel<<<blocks_for(total, 128), 128, 0, s>>>(natural, (uint32_t*)lattice, batch, L);
+    } else {
+        const long long total = (long long)batch * L * L;
+        from_natural_int8_kernel<<<blocks_for(total, 256), 256, 0, s>>>(natural, (int8_t*)lattice, batch, L);
+    }
+    return 1;
+}
+
+int launch_to_natural(const void* lattice, int8_t* natural, int batch, int L, int layout, cudaStream_t s) {
+    if (layout == 1) {
+        const long long total = (long long)batch * L * (L >> 6);
+        to_natural_bits_kernel<<<blocks_for(total, 128), 128, 0, s>>>((const uint32_t*)lattice, natural, batch, L);
+    } else {
+        const long long total = (long long)batch * L * L;
+        to_natural_int8_kernel<<<blocks_for(total, 256), 256, 0, s>>>((const int8_t*)lattice, natural, batch, L);
+    }
+    return 1;
+}
+
+int launch_validate_natural(const int8_t* natural, int batch, int L, int model, const int32_t* q, unsigned int* bad,
+                            cudaStream_t s) {
+    const long long total = (long long)batch * L * L;
+    validate_natural_kernel<<<blocks_for(total, 256), 256, 0, s>>>(natural, batch, L, model, q, bad);
+    return 1;
+}
+
+}  // namespace spin

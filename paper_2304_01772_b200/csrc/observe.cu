@@ -1,0 +1,192 @@
+// observe.cu — rows a5-a7: exact integer per-replica reductions.
+//   Ising: E_int = -sum_bonds s_i s_j, M = sum s.  Every bond of an even periodic lattice has exactly one
+//          colour-0 end, so E_int = -sum_{colour-0 sites} s * (up + down + left + right)  (the
+//          Hamiltonian is the neighbour-sum map times the lattice; each bond once, P2).
+//   Potts: E_int = -sum_{colour-0 sites} #(neighbours equal), M = max_k N_k (P8).
+//   Moments: n, sum E, sum E^2 (128 bit), sum M, sum |M|, sum M^2, sum E*M.
+// Warp-shuffle + shared-memory block reduction, one 64-bit atomic per block and quantity.
+#include "spin_internal.cuh"
+
+namespace spin {
+
+namespace {
+
+__device__ __forceinline__ int warp_sum(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    return v;
+}
+
+// Block-reduce two ints and add them to 64-bit accumulators.  All threads of the block must call.
+__device__ __forceinline__ void block_add2(int e, int m, long long* E_acc, long long* M_acc) {
+    __shared__ int se[32], sm[32];
+    e = warp_sum(e);
+    m = warp_sum(m);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) { se[w] = e; sm[w] = m; }
+    __syncthreads();
+    if (w == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        e = lane < nw ? se[lane] : 0;
+        m = lane < nw ? sm[lane] : 0;
+        e = warp_sum(e);
+        m = warp_sum(m);
+        if (lane == 0) {
+            if (E_acc && e) atomicAdd((unsigned long long*)E_acc, (unsigned long long)(long long)e);
+            if (M_acc && m) atomicAdd((unsigned long long*)M_acc, (unsigned long long)(long long)m);
+        }
+    }
+}
+
+// Ising int8, any even L: one thread per row-pair position; grid = (blocks per replica) * batch.
+// Thread handles column index k of row i for both colours.
+__global__ void ising_int8_observe_kernel(const int8_t* __restrict__ lat, int L, int bpr, long long* E_acc,
+                                          long long* M_acc) {
+    const int W = L >> 1;
+    const int b = blockIdx.x / bpr, blk = blockIdx.x - b * bpr;
+    const size_t half = (size_t)L * W;
+    const int8_t* c0 = lat + (size_t)b * 2 * half;
+    const int8_t* c1 = c0 + half;
+    int e = 0, m = 0;
+    for (long long n = (long long)blk * blockDim.x + threadIdx.x; n < (long long)half; n += (long long)bpr * blockDim.x) {
+        const int i = (int)(n / W), k = (int)(n % W);
+        const int p = i & 1;                                  // colour 0: column parity = row parity
+        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+        const int ks = p ? (k == W - 1 ? 0 : k + 1) : (k == 0 ? W - 1 : k - 1);
+        const int s = c0[n];
+        const int nn = c1[(size_t)iu * W + k] + c1[(size_t)id * W + k] + c1[(size_t)i * W + k] + c1[(size_t)i * W + ks];
+        e -= s * nn;
+        m += s + c1[n];
+    }
+    block_add2(e, m, E_acc ? E_acc + b : nullptr, M_acc ? M_acc + b : nullptr);
+}
+
+__global__ void ising_bits_observe_kernel(const uint32_t* __restrict__ lat, int L, int bpr, long long* E_acc,
+                                          long long* M_acc) {
+    const int WW = L >> 6;
+    const int b = blockIdx.x / bpr, blk = blockIdx.x - b * bpr;
+    const size_t half = (size_t)L * WW;
+    const uint32_t* c0 = lat + (size_t)b * 2 * half;
+    const uint32_t* c1 = c0 + half;
+    int e = 0, m = 0;
+    for (long long n = (long long)blk * blockDim.x + threadIdx.x; n < (long long)half; n += (long long)bpr * blockDim.x) {
+        const int i = (int)(n / WW), x = (int)(n % WW);
+        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+        const uint32_t own = c0[n], ct = c1[(size_t)i * WW + x];
+        uint32_t sd;
+        if (i & 1) sd = (ct >> 1) | (c1[(size_t)i * WW + (x == WW - 1 ? 0 : x + 1)] << 31);
+        else sd = (ct << 1) | (c1[(size_t)i * WW + (x == 0 ? WW - 1 : x - 1)] >> 31);
+        // s * nbr = +1 if equal, -1 if different: sum over 32 sites and 4 neighbours = 128 - 2 * (#different)
+        const int diff = __popc(own ^ c1[(size_t)iu * WW + x]) + __popc(own ^ c1[(size_t)id * WW + x]) +
+                         __popc(own ^ ct) + __popc(own ^ sd);
+        e -= 128 - 2 * diff;
+        m += 64 - 2 * (__popc(own) + __popc(c1[n]));
+    }
+    block_add2(e, m, E_acc ? E_acc + b : nullptr, M_acc ? M_acc + b : nullptr);
+}
+
+__global__ void potts_int8_observe_kernel(const uint8_t* __restrict__ lat, int L, int bpr, long long* E_acc,
+                                          unsigned int* hist) {
+    __shared__ unsigned int sh[128];
+    const int W = L >> 1;
+    const int b = blockIdx.x / bpr, blk = blockIdx.x - b * bpr;
+    const size_t half = (size_t)L * W;
+    const uint8_t* c0 = lat + (size_t)b * 2 * half;
+    const uint8_t* c1 = c0 + half;
+    for (int t = threadIdx.x; t < 128; t += blockDim.x) sh[t] = 0u;
+    __syncthreads();
+    int e = 0;
+    for (long long n = (long long)blk * blockDim.x + threadIdx.x; n < (long long)half; n += (long long)bpr * blockDim.x) {
+        const int i = (int)(n / W), k = (int)(n % W);
+        const int p = i & 1;
+        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+        const int ks = p ? (k == W - 1 ? 0 : k + 1) : (k == 0 ? W - 1 : k - 1);
+        const unsigned s = c0[n];
+        e -= (c1[(size_t)iu * W + k] == s) + (c1[(size_t)id * W + k] == s) + (c1[(size_t)i * W + k] == s) +
+             (c1[(size_t)i * W + ks] == s);
+        if (hist) {
+            atomicAdd(&sh[s & 127u], 1u);
+            atomicAdd(&sh[c1[n] & 127u], 1u);
+        }
+    }
+    __syncthreads();
+    if (hist)
+        for (int t = threadIdx.x; t < 128; t += blockDim.x)
+            if (sh[t]) atomicAdd(&hist[(size_t)b * 128 + t], sh[t]);
+    block_add2(e, 0, E_acc ? E_acc + b : nullptr, nullptr);
+}
+
+__global__ void potts_finalize_kernel(unsigned int* hist, const int32_t* __restrict__ q, int batch, long long* M_out) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    unsigned int best = 0u;
+    for (int k = 0; k < 128; ++k) {
+        const unsigned int v = hist[(size_t)b * 128 + k];
+        if (k < q[b] && v > best) best = v;
+        hist[(size_t)b * 128 + k] = 0u;
+    }
+    if (M_out) M_out[b] = (long long)best;
+}
+
+__global__ void accumulate_moments_kernel(long long* moments, const long long* __restrict__ E,
+                                          const long long* __restrict__ M, int batch) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    long long* m = moments + 8 * (size_t)b;
+    const long long e = E[b], mag = M[b];
+    const unsigned long long ae = e < 0 ? (unsigned long long)(-e) : (unsigned long long)e;
+    const unsigned long long lo = ae * ae, hi = __umul64hi(ae, ae);
+    const unsigned long long old_lo = (unsigned long long)m[2];
+    const unsigned long long new_lo = old_lo + lo;
+    m[0] += 1;
+    m[1] += e;
+    m[2] = (long long)new_lo;
+    m[3] = (long long)((unsigned long long)m[3] + hi + (new_lo < old_lo ? 1ull : 0ull));
+    m[4] += mag;
+    m[5] += mag < 0 ? -mag : mag;
+    m[6] += mag * mag;
+    m[7] += e * mag;
+}
+
+inline int blocks_per_replica(long long items, int tpb, int batch) {
+    // enough blocks to fill the GPU a few times over, but never more than the work
+    long long want = (items + tpb - 1) / tpb;
+    long long cap = (148ll * 16 + batch - 1) / batch;
+    if (cap < 1) cap = 1;
+    return (int)(want < cap ? want : cap);
+}
+
+}  // namespace
+
+int launch_ising_int8_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s) {
+    const long long half = (long long)L * (L >> 1);
+    const int tpb = 256, bpr = blocks_per_replica(half, tpb, batch);
+    ising_int8_observe_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const int8_t*)lattice, L, bpr, E_acc, M_acc);
+    return 1;
+}
+
+int launch_ising_bits_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s) {
+    const long long half = (long long)L * (L >> 6);
+    const int tpb = 256, bpr = blocks_per_replica(half, tpb, batch);
+    ising_bits_observe_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const uint32_t*)lattice, L, bpr, E_acc, M_acc);
+    return 1;
+}
+
+int launch_potts_int8_observe(const void* lattice, int batch, int L, long long* E_acc, unsigned int* hist, cudaStream_t s) {
+    const long long half = (long long)L * (L >> 1);
+    const int tpb = 256, bpr = blocks_per_replica(half, tpb, batch);
+    potts_int8_observe_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const uint8_t*)lattice, L, bpr, E_acc, hist);
+    return 1;
+}
+
+int launch_potts_finalize(unsigned int* hist, const int32_t* q, int batch, long long* M_out, cudaStream_t s) {
+    potts_finalize_kernel<<<(batch + 127) / 128, 128, 0, s>>>(hist, q, batch, M_out);
+    return 1;
+}
+
+int launch_accumulate_moments(long long* moments, const long long* E, const long long* M, int batch, cudaStream_t s) {
+    accumulate_moments_kernel<<<(batch + 127) / 128, 128, 0, s>>>(moments, E, M, batch);
+    return 1;
+}
+
+}  // namespace spin

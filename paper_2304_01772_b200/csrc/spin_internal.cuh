@@ -1,0 +1,98 @@
+// spin_internal.cuh — declarations shared by the translation units of libspin.so (CUDA side only).
+// Nothing here is shared with oracle/: the oracle has its own generator, tables and loops.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace spin {
+
+// ---- Philox-4x32-10 (O2).  Round keys are precomputed on the host. -------------
+constexpr uint32_t kPhiloxM0 = 0xD2511F53u;
+constexpr uint32_t kPhiloxM1 = 0xCD9E8D57u;
+constexpr uint32_t kPhiloxW0 = 0x9E3779B9u;
+constexpr uint32_t kPhiloxW1 = 0xBB67AE85u;
+
+enum : uint32_t { kDomainInit = 0, kDomainIsing = 1, kDomainPotts = 2 };
+
+struct RoundKeys {
+    uint32_t k0[10];
+    uint32_t k1[10];
+};
+
+// One Philox call.  c1..c3 are uniform over a launch in every kernel of this library, so the compiler
+// keeps them (and the round keys, which come from the constant bank) in uniform registers.
+__device__ __forceinline__ void philox4x32_10(const RoundKeys& rk, uint32_t c0, uint32_t c1, uint32_t c2,
+                                              uint32_t c3, uint32_t out[4]) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)kPhiloxM0 * c0;
+        const uint64_t p1 = (uint64_t)kPhiloxM1 * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ rk.k0[r];
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ rk.k1[r];
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// ---- device-side acceptance tables -------------------------------------------------------------------
+// One record of kTableStride uint32 per replica.
+//   Ising: U[d*8 + nd] at [0..15], d = 1 iff the site's spin is -1, nd = number of -1 neighbours (0..4);
+//          a flip of that class is accepted iff r <= U (U = T-1, or 0xFFFFFFFF for "always").
+//   Potts: U[dn + 4] at [0..8].
+//   [16] = bit mask of classes that can never be accepted (T == 0: r <= U cannot express it);
+//   [17] = q of the replica (Potts).
+constexpr int kTableStride = 32;
+constexpr int kTabNever = 16;
+constexpr int kTabQ = 17;
+
+struct SweepArgs {
+    void* lattice;            // int8: [B][2][L][L/2] bytes; bit-packed: [B][2][L][L/64] uint32
+    const uint32_t* tables;   // [B][kTableStride]
+    int32_t batch;
+    int32_t L;
+    uint32_t replica_offset;
+    uint32_t c2;              // low 32 bits of the sweep index t
+    uint32_t c3;              // (t >> 32) & 0xFFFFFF | colour << 24 | domain << 28
+    int32_t colour;
+    RoundKeys rk;
+};
+
+struct InitArgs {
+    void* lattice;
+    const int32_t* q;         // [B] (Potts) or nullptr
+    int32_t batch;
+    int32_t L;
+    uint32_t replica_offset;
+    RoundKeys rk;
+};
+
+// ---- launchers (each returns the number of kernels it launched; errors via cudaGetLastError) --------
+int launch_init(const InitArgs& a, int model, int layout, cudaStream_t s);
+
+int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s);      // picks generic / vectorised
+int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s);
+int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s);
+const char* ising_int8_variant(int L);
+const char* potts_int8_variant(int L);
+
+// Observables: accumulate into E_acc[b], M_acc[b] (int64, must be zero on entry; Potts uses hist).
+int launch_ising_int8_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);
+int launch_ising_bits_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);
+// Potts: E_acc as above; hist: [B][128] uint32, zero on entry; M is produced by launch_potts_finalize.
+int launch_potts_int8_observe(const void* lattice, int batch, int L, long long* E_acc, unsigned int* hist, cudaStream_t s);
+// M_out[b] = max_k hist[b][k], then hist is cleared for the next use.
+int launch_potts_finalize(unsigned int* hist, const int32_t* q, int batch, long long* M_out, cudaStream_t s);
+// moments[b][8] += sample (E[b], M[b])
+int launch_accumulate_moments(long long* moments, const long long* E, const long long* M, int batch, cudaStream_t s);
+
+// Natural <-> internal layout.  natural: [B][L][L] int8 on the device.
+int launch_from_natural(const int8_t* natural, void* lattice, int batch, int L, int layout, cudaStream_t s);
+int launch_to_natural(const void* lattice, int8_t* natural, int batch, int L, int layout, cudaStream_t s);
+// bad[0] = number of invalid values (Ising: not +-1; Potts: outside 0..q[b]-1).  bad must be zero on entry.
+int launch_validate_natural(const int8_t* natural, int batch, int L, int model, const int32_t* q, unsigned int* bad, cudaStream_t s);
+
+}  // namespace spin

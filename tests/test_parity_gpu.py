@@ -1,0 +1,246 @@
+"""GPU parity tests (-m gpu): the CUDA path through the C ABI vs the CPU oracle, bit for bit.
+
+Bar (BASELINE.json north star): lattices identical after every compared sweep, E_int and M identical as exact
+integers, threshold tables identical.  Small cases compare everything; the full-size cases compare all
+replicas for a few sweeps and single replicas (via replica_offset on the oracle side) for longer."""
+import math
+
+import numpy as np
+import pytest
+
+import paper_2304_01772_b200 as sp
+
+pytestmark = pytest.mark.gpu
+
+
+def _layout(name):
+    return sp.SPIN_LAYOUT_BITPACKED if name == "bits" else sp.SPIN_LAYOUT_INT8
+
+
+def _mk_ising(batch, L, seed, layout="int8", replica_offset=0):
+    return sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed, layout=_layout(layout),
+                             replica_offset=replica_offset)
+
+
+def _mk_potts(batch, L, q, seed, replica_offset=0):
+    q = np.broadcast_to(np.asarray(q, dtype=np.int32), (batch,))
+    return sp.spin_create_ex(batch, L, sp.SPIN_MODEL_POTTS, q_per_replica=q, seed=seed, replica_offset=replica_offset)
+
+
+# ----------------------------------------------------------------------------------------- init (row a0)
+@pytest.mark.parametrize("L,layout", [(2, "int8"), (4, "int8"), (6, "int8"), (10, "int8"), (32, "int8"),
+                                      (96, "int8"), (64, "bits"), (192, "bits")])
+def test_init_matches_oracle_ising(oracle_mod, L, layout):
+    with _mk_ising(3, L, seed=11, layout=layout, replica_offset=5) as sim:
+        got = sim.spin_get_spins()
+    assert np.array_equal(got, oracle_mod.init(3, L, seed=11, replica_offset=5))
+
+
+def test_init_matches_oracle_potts(oracle_mod):
+    q = [3, 8, 2, 127, 5]
+    for L in (2, 6, 32, 64):
+        with _mk_potts(5, L, q, seed=4) as sim:
+            got = sim.spin_get_spins()
+        assert np.array_equal(got, oracle_mod.init(5, L, seed=4, q=q))
+
+
+def test_set_get_roundtrip_and_validation():
+    for L, layout in [(2, "int8"), (6, "int8"), (32, "int8"), (64, "bits"), (128, "bits")]:
+        with _mk_ising(3, L, seed=1, layout=layout) as sim:
+            lat = sp.workloads.random_ising_lattice(3, L, seed=L)
+            sim.spin_set_spins(lat)
+            assert np.array_equal(sim.spin_get_spins(), lat)
+            bad = lat.copy()
+            bad[1, 0, 1] = 0
+            with pytest.raises(sp.SpinError):
+                sim.spin_set_spins(bad)
+            assert np.array_equal(sim.spin_get_spins(), lat)  # unchanged after a rejected set
+    with _mk_potts(2, 8, [3, 8], seed=1) as sim:
+        lat = sp.workloads.random_potts_lattice(2, 8, [3, 8], seed=2)
+        sim.spin_set_spins(lat)
+        assert np.array_equal(sim.spin_get_spins(), lat)
+        bad = lat.copy()
+        bad[0, 0, 0] = 3
+        with pytest.raises(sp.SpinError):
+            sim.spin_set_spins(bad)
+
+
+# ----------------------------------------------------------------------------------------- Ising sweeps
+ISING_CASES = [
+    # L, batch, layout, J, h, betas
+    (2, 3, "int8", 1.0, 0.0, [0.2, 0.44, 0.9]),
+    (4, 4, "int8", 1.0, 0.01, [0.1, 0.44, 0.6, 20.0]),
+    (6, 2, "int8", 1.0, 0.0, [0.3, 0.5]),
+    (10, 3, "int8", -1.0, 0.2, [0.3, 0.44, 0.0]),
+    (32, 4, "int8", 1.0, 0.0, [0.44] * 4),
+    (64, 3, "int8", 1.0, 0.01, [0.3, 0.4407, 20.0]),
+    (96, 2, "int8", 0.7, -0.3, [0.5, 1.0]),
+    (160, 2, "int8", 1.0, 0.0, [0.44, 0.6]),
+    (64, 3, "bits", 1.0, 0.01, [0.3, 0.4407, 20.0]),
+    (128, 2, "bits", 1.0, 0.0, [0.44, 0.0]),
+    (192, 2, "bits", -1.0, 0.2, [0.4, 0.8]),
+]
+
+
+@pytest.mark.parametrize("L,batch,layout,J,h,betas", ISING_CASES)
+def test_ising_sweeps_match_oracle_every_sweep(oracle_mod, L, batch, layout, J, h, betas):
+    seed, n = 100 + L, 12
+    ref = oracle_mod.init(batch, L, seed=seed)
+    with _mk_ising(batch, L, seed=seed, layout=layout) as sim:
+        for t in range(n):
+            sim.spin_sweep(betas, J, h, 1, t)
+            oracle_mod.sweep(ref, betas, J, h, seed=seed, n_sweeps=1, sweep_offset=t)
+            got = sim.spin_get_spins()
+            assert np.array_equal(got, ref), "lattice differs after sweep %d" % t
+            E, M = sim.spin_observables()
+            Eo, Mo = oracle_mod.ising_observables(ref)
+            assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+
+
+def test_ising_chunking_offsets_and_replica_offset(oracle_mod):
+    L, seed = 64, 9
+    beta = [0.3, 0.44, 0.6]
+    with _mk_ising(3, L, seed=seed) as a, _mk_ising(3, L, seed=seed) as b, \
+            _mk_ising(1, L, seed=seed, replica_offset=2) as solo:
+        a.spin_sweep(beta, 1.0, 0.0, 10, 0)
+        b.spin_sweep(beta, 1.0, 0.0, 4, 0)
+        b.spin_sweep(beta, 1.0, 0.0, 6, 4)
+        solo.spin_sweep(beta[2:], 1.0, 0.0, 10, 0)
+        la = a.spin_get_spins()
+        assert np.array_equal(la, b.spin_get_spins())
+        assert np.array_equal(la[2], solo.spin_get_spins()[0])
+    big = (1 << 32) + 3  # sweep index beyond 32 bits goes into counter word 3
+    ref = oracle_mod.init(1, 32, seed=seed)
+    oracle_mod.sweep(ref, 0.44, 1.0, 0.0, seed=seed, n_sweeps=2, sweep_offset=big)
+    with _mk_ising(1, 32, seed=seed) as sim:
+        sim.spin_sweep(0.44, 1.0, 0.0, 2, big)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+    seed64 = (0xDEADBEEF << 32) | 0x12345678  # both key words
+    ref = oracle_mod.init(2, 32, seed=seed64)
+    oracle_mod.sweep(ref, 0.44, 1.0, 0.0, seed=seed64, n_sweeps=3)
+    with _mk_ising(2, 32, seed=seed64) as sim:
+        sim.spin_sweep(0.44, 1.0, 0.0, 3, 0)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+
+
+def test_bitpacked_equals_int8(oracle_mod):
+    L, seed = 256, 3
+    with _mk_ising(2, L, seed=seed, layout="int8") as a, _mk_ising(2, L, seed=seed, layout="bits") as b:
+        assert np.array_equal(a.spin_get_spins(), b.spin_get_spins())
+        a.spin_sweep(0.4407, 1.0, 0.01, 25, 0)
+        b.spin_sweep(0.4407, 1.0, 0.01, 25, 0)
+        assert np.array_equal(a.spin_get_spins(), b.spin_get_spins())
+        Ea, Ma = a.spin_observables()
+        Eb, Mb = b.spin_observables()
+        assert np.array_equal(Ea, Eb) and np.array_equal(Ma, Mb)
+
+
+def test_set_spins_then_sweep(oracle_mod):
+    L = 32
+    lat = sp.workloads.random_ising_lattice(2, L, seed=77)
+    ref = lat.copy()
+    oracle_mod.sweep(ref, [0.4, 0.5], 1.0, 0.0, seed=5, n_sweeps=3, sweep_offset=7)
+    with _mk_ising(2, L, seed=5) as sim:
+        sim.spin_set_spins(lat)
+        sim.spin_sweep([0.4, 0.5], 1.0, 0.0, 3, 7)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+
+
+# ----------------------------------------------------------------------------------------- Potts sweeps
+POTTS_CASES = [
+    (2, [3, 8], [1.0, 1.3]),
+    (4, [3, 8, 2], [0.5, 1.34, 0.88]),
+    (6, [3, 5], [1.0, 20.0]),
+    (10, [8, 127], [1.2, 2.0]),
+    (32, [3, 8, 2, 127], [1.005, 1.342, 0.0, 3.0]),
+    (64, [3, 8], [20.0, 0.7]),
+    (96, [4, 7], [1.1, 1.3]),
+]
+
+
+@pytest.mark.parametrize("L,q,betas", POTTS_CASES)
+def test_potts_sweeps_match_oracle_every_sweep(oracle_mod, L, q, betas):
+    seed, n, batch = 200 + L, 10, len(q)
+    ref = oracle_mod.init(batch, L, seed=seed, q=q)
+    with _mk_potts(batch, L, q, seed=seed) as sim:
+        for t in range(n):
+            sim.spin_sweep(betas, 1.0, 0.0, 1, t)
+            oracle_mod.sweep(ref, betas, 1.0, 0.0, seed=seed, n_sweeps=1, sweep_offset=t, q=q)
+            assert np.array_equal(sim.spin_get_spins(), ref), "lattice differs after sweep %d" % t
+            E, M = sim.spin_observables()
+            Eo, Mo = oracle_mod.potts_observables(ref, q)
+            assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+
+
+def test_potts_negative_J_and_field_rejected(oracle_mod):
+    q, L, seed = [3, 6], 32, 8
+    ref = oracle_mod.init(2, L, seed=seed, q=q)
+    oracle_mod.sweep(ref, [0.8, 1.1], -1.0, 0.0, seed=seed, n_sweeps=4, q=q)
+    with _mk_potts(2, L, q, seed=seed) as sim:
+        with pytest.raises(sp.SpinError) as e:
+            sim.spin_sweep([0.8, 1.1], 1.0, 0.1, 1, 0)
+        assert e.value.code == sp.SPIN_ERR_UNSUPPORTED
+        sim.spin_sweep([0.8, 1.1], -1.0, 0.0, 4, 0)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+
+
+# ----------------------------------------------------------------------------------------- measurements
+def test_sweep_measure_trace_and_moments(oracle_mod):
+    L, seed, n = 32, 1, 40
+    beta = [0.3, 0.44, 0.5, 0.6]
+    ref = oracle_mod.init(4, L, seed=seed)
+    mom_o = np.zeros((4, 8), dtype=np.int64)
+    Eo, Mo = oracle_mod.sweep(ref, beta, 1.0, 0.05, seed=seed, n_sweeps=n, trace=True, moments=mom_o)
+    with _mk_ising(4, L, seed=seed) as sim:
+        mom = np.zeros((4, 8), dtype=np.int64)
+        E1, M1 = sim.spin_sweep_measure(beta, 1.0, 0.05, 15, 0, moments=mom)
+        E2, M2 = sim.spin_sweep_measure(beta, 1.0, 0.05, n - 15, 15, moments=mom)   # moments are in/out
+        assert np.array_equal(np.vstack([E1, E2]), Eo) and np.array_equal(np.vstack([M1, M2]), Mo)
+        assert np.array_equal(mom, mom_o)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+    q = [3, 8]
+    ref = oracle_mod.init(2, 16, seed=seed, q=q)
+    mom_o = np.zeros((2, 8), dtype=np.int64)
+    Eo, Mo = oracle_mod.sweep(ref, [1.0, 1.3], 1.0, 0.0, seed=seed, n_sweeps=20, q=q, trace=True, moments=mom_o)
+    with _mk_potts(2, 16, q, seed=seed) as sim:
+        mom = np.zeros((2, 8), dtype=np.int64)
+        E, M = sim.spin_sweep_measure([1.0, 1.3], 1.0, 0.0, 20, 0, moments=mom)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo) and np.array_equal(mom, mom_o)
+
+
+def test_invalid_sweep_arguments_leave_lattice_untouched():
+    with _mk_ising(2, 32, seed=1) as sim:
+        before = sim.spin_get_spins()
+        for beta, n, off in [([0.4, float("nan")], 1, 0), ([0.4, -1.0], 1, 0), ([0.4, 0.4], -1, 0),
+                             ([0.4, 0.4], 1, -1), ([0.4, 0.4], 1, 1 << 56)]:
+            with pytest.raises(sp.SpinError):
+                sim.spin_sweep(beta, 1.0, 0.0, n, off)
+        sim.spin_sweep([0.4, 0.4], 1.0, 0.0, 0, 0)  # zero sweeps is a no-op
+        assert np.array_equal(sim.spin_get_spins(), before)
+
+
+def test_caller_owned_buffer_and_stream(oracle_mod):
+    import torch
+    L, batch, seed = 64, 2, 6
+    buf = torch.empty(sp.spin_buffer_bytes(batch, L, 0, 0), dtype=torch.int8, device="cuda")
+    stream = torch.cuda.Stream()
+    sim = sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed, device_buffer=buf.data_ptr(),
+                            buffer_bytes=buf.numel(), cuda_stream=stream.cuda_stream, keepalive=buf)
+    ref = oracle_mod.init(batch, L, seed=seed)
+    oracle_mod.sweep(ref, 0.44, 1.0, 0.0, seed=seed, n_sweeps=5)
+    sim.spin_sweep(0.44, 1.0, 0.0, 5, 0)
+    sim.spin_synchronize()
+    # the caller's tensor holds the split layout [B][2][L][L/2]
+    split = buf.view(batch, 2, L, L // 2).cpu().numpy()
+    nat = np.empty((batch, L, L), dtype=np.int8)
+    for i in range(L):
+        for c in range(2):
+            nat[:, i, ((i + c) & 1)::2] = split[:, c, i, :]
+    assert np.array_equal(nat, ref) and np.array_equal(sim.spin_get_spins(), ref)
+    Ed = torch.zeros(batch, dtype=torch.int64, device="cuda")
+    Md = torch.zeros(batch, dtype=torch.int64, device="cuda")
+    sim.spin_observables_dev(Ed.data_ptr(), Md.data_ptr())
+    sim.spin_synchronize()
+    Eo, Mo = oracle_mod.ising_observables(ref)
+    assert np.array_equal(Ed.cpu().numpy(), Eo) and np.array_equal(Md.cpu().numpy(), Mo)
+    sim.spin_destroy()
