@@ -44,95 +44,191 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
     }
 }
 
-// ---- vectorised kernel: L % 32 == 0.  One thread per 16 consecutive same-colour sites of a row (one 128-bit
-// word): 4 coalesced 128-bit loads (own, up, centre, down of the other colour), one byte for the 17th
-// neighbour, 4 Philox calls, byte-SIMD neighbour counts, one LDS + compare + predicated XOR per site.
-template <bool kHasNever>
-__device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t ct, uint32_t sd,
-                                                const uint32_t r[4], const uint32_t* stab) {
-    // bit 1 of a +-1 byte is set iff the spin is -1
-    const uint32_t m = 0x02020202u;
-    const uint32_t sum2 = (up & m) + (dn & m) + (ct & m) + (sd & m);   // 2*nd per byte (0..8)
-    const uint32_t off = (sum2 << 1) + ((own & m) << 4);               // byte offset 4*(d*8 + nd)
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const uint32_t o = (off >> (8 * e)) & 0xFFu;
-        const uint32_t U = *(const uint32_t*)((const char*)stab + o);
-        bool acc = r[e] <= U;
-        if (kHasNever) acc = acc && !((stab[kTabNever] >> (o >> 2)) & 1u);
-        if (acc) own ^= 0xFEu << (8 * e);
+// ---- row-marching kernel: L % 32 == 0.
+// Measured on B200 (profiles/r1_microbench.md): every integer instruction (LOP3, IADD3, PRMT, ISETP, IMAD, ...) is
+// dispatched at 16 lanes/clk per SM sub-partition, i.e. 2 cycles per warp instruction whatever its pipe, so the
+// kernel is bound by the NUMBER of integer instructions per site; loads/stores (LSU) are dispatched beside them.
+// The design therefore minimises integer instructions and pushes byte extraction onto the LSU:
+//   * one thread owns a strip of 16 consecutive same-colour sites (one 128-bit word) and marches down kRows rows,
+//     keeping the three other-colour rows it needs in registers, already masked to "4 if spin is -1" per byte
+//     (one LOP3 per loaded word, reused as up / centre / down of three rows and for the shifted side word);
+//   * per 4-site word the class byte offset 4*nd + 32*d is two IADD3 (up+centre+down, + side + own&0x20);
+//   * the four offset bytes are written to a per-thread shared-memory slot (STS) and read back one byte at a
+//     time (LDS.U8) straight into the address of the threshold LDS: no extraction instruction;
+//   * per site: one ISETP (r <= U) and one predicated LOP3 (flip), nothing else.
+// Loads of row i+1 are issued before row i is computed; rows are fully unrolled so the register window rotates by
+// renaming.
+constexpr int kRows = 8;
+constexpr int kRowsThreads = 128;
+
+template <int kOff>
+__device__ __forceinline__ uint32_t slot_load_u8(uint32_t saddr) {
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1+%2];" : "=r"(v) : "r"(saddr), "n"(kOff));
+    return v;
+}
+
+template <int kOff>
+__device__ __forceinline__ void slot_store_u32(uint32_t saddr, uint32_t v) {
+    asm volatile("st.shared.u32 [%0+%1], %2;" :: "r"(saddr), "n"(kOff), "r"(v));
+}
+
+// One site: threshold fetch (LDS with the class byte as address), compare, flip.
+template <bool kHasNever, int kE>
+__device__ __forceinline__ void site_step(uint32_t& own, uint32_t o, uint32_t r, const uint32_t* stab) {
+    const uint32_t U = *(const uint32_t*)((const char*)stab + o);
+    if (kHasNever) {
+        const bool acc = (r <= U) && !((stab[kTabNever] >> (o >> 2)) & 1u);
+        if (acc) own ^= 0xFEu << (8 * kE);
+    } else {
+        // kept in PTX so that it stays one ISETP + one predicated LOP3
+        asm("{\n\t.reg .pred p;\n\tsetp.ls.u32 p, %1, %2;\n\t@p xor.b32 %0, %0, %3;\n\t}"
+            : "+r"(own) : "r"(r), "r"(U), "n"(0xFEu << (8 * kE)));
     }
+}
+
+// One 4-site word.  t = byte offsets 4*nd + 32*d of its four sites; kJ = index of the word in the strip.
+template <bool kHasNever, int kJ>
+__device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t t, const uint32_t r[4], const uint32_t* stab,
+                                                uint32_t slot) {
+    slot_store_u32<kJ * kRowsThreads * 4>(slot, t);
+    const uint32_t o0 = slot_load_u8<kJ * kRowsThreads * 4 + 0>(slot);
+    const uint32_t o1 = slot_load_u8<kJ * kRowsThreads * 4 + 1>(slot);
+    const uint32_t o2 = slot_load_u8<kJ * kRowsThreads * 4 + 2>(slot);
+    const uint32_t o3 = slot_load_u8<kJ * kRowsThreads * 4 + 3>(slot);
+    site_step<kHasNever, 0>(own, o0, r[0], stab);
+    site_step<kHasNever, 1>(own, o1, r[1], stab);
+    site_step<kHasNever, 2>(own, o2, r[2], stab);
+    site_step<kHasNever, 3>(own, o3, r[3], stab);
     return own;
 }
 
-template <bool kHasNever>
-__device__ __forceinline__ void update_vec(SweepArgs& a, const uint32_t* stab, int b, int i, int x) {
-    const int L = a.L, W = L >> 1, W16 = W >> 4;
-    const size_t half = (size_t)L * W;
-    uint4* ownp = (uint4*)((int8_t*)a.lattice + ((size_t)b * 2 + a.colour) * half) + (size_t)i * W16 + x;
-    const int8_t* oth = (const int8_t*)a.lattice + ((size_t)b * 2 + (1 - a.colour)) * half;
-    const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
-    const uint4 own = *ownp;
-    const uint4 up = __ldg((const uint4*)(oth + (size_t)iu * W) + x);
-    const uint4 dn = __ldg((const uint4*)(oth + (size_t)id * W) + x);
-    const uint4 ct = __ldg((const uint4*)(oth + (size_t)i * W) + x);
-    const int p = (i + a.colour) & 1;
+// One row of one strip.  um / cm / dm: masked (4 per -1 spin) other-colour words of rows i-1, i, i+1;
+// kParity = 1: the side neighbour of site k is other[i][k+1], else other[i][k-1]; `edge` is the masked 32-bit
+// word holding the 17th byte (next strip's first word, or previous strip's last word).
+template <bool kHasNever, int kParity>
+__device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const uint4& um, const uint4& cm,
+                                            const uint4& dm, uint32_t edge, uint32_t g0, uint32_t c1,
+                                            const uint32_t* stab, uint32_t slot) {
     uint32_t s0, s1, s2, s3;
-    if (p) {  // side neighbour of site k is other[i][k+1]
-        const int kn = (x == W16 - 1) ? 0 : 16 * x + 16;
-        const uint32_t nx = (uint32_t)(uint8_t)__ldg(oth + (size_t)i * W + kn);
-        s0 = __byte_perm(ct.x, ct.y, 0x4321);
-        s1 = __byte_perm(ct.y, ct.z, 0x4321);
-        s2 = __byte_perm(ct.z, ct.w, 0x4321);
-        s3 = __byte_perm(ct.w, nx, 0x4321);
-    } else {  // side neighbour of site k is other[i][k-1]
-        const int kp = (x == 0) ? W - 1 : 16 * x - 1;
-        const uint32_t pv = (uint32_t)(uint8_t)__ldg(oth + (size_t)i * W + kp);
-        s0 = __byte_perm(pv, ct.x, 0x6540);
-        s1 = __byte_perm(ct.x, ct.y, 0x6543);
-        s2 = __byte_perm(ct.y, ct.z, 0x6543);
-        s3 = __byte_perm(ct.z, ct.w, 0x6543);
+    if (kParity) {
+        s0 = __byte_perm(cm.x, cm.y, 0x4321);
+        s1 = __byte_perm(cm.y, cm.z, 0x4321);
+        s2 = __byte_perm(cm.z, cm.w, 0x4321);
+        s3 = __byte_perm(cm.w, edge, 0x4321);
+    } else {
+        s0 = __byte_perm(edge, cm.x, 0x6543);
+        s1 = __byte_perm(cm.x, cm.y, 0x6543);
+        s2 = __byte_perm(cm.y, cm.z, 0x6543);
+        s3 = __byte_perm(cm.z, cm.w, 0x6543);
     }
-    const uint32_t g0 = (uint32_t)i * (uint32_t)(W >> 2) + 4u * (uint32_t)x;
-    const uint32_t c1 = (uint32_t)b + a.replica_offset;
+    const uint32_t kOwn = 0x20202020u;   // bit 5 of a +-1 byte is set iff the spin is -1: contributes 32*d
+    const uint32_t t0 = (um.x + cm.x + dm.x) + s0 + (own.x & kOwn);
+    const uint32_t t1 = (um.y + cm.y + dm.y) + s1 + (own.y & kOwn);
+    const uint32_t t2 = (um.z + cm.z + dm.z) + s2 + (own.z & kOwn);
+    const uint32_t t3 = (um.w + cm.w + dm.w) + s3 + (own.w & kOwn);
+    uint32_t r0[4], r1[4], r2[4], r3[4];
+    philox4x32_10(a.rk, g0 + 0, c1, a.c2, a.c3, r0);
+    philox4x32_10(a.rk, g0 + 1, c1, a.c2, a.c3, r1);
+    philox4x32_10(a.rk, g0 + 2, c1, a.c2, a.c3, r2);
+    philox4x32_10(a.rk, g0 + 3, c1, a.c2, a.c3, r3);
     uint4 res;
-    uint32_t r[4];
-    philox4x32_10(a.rk, g0 + 0, c1, a.c2, a.c3, r);
-    res.x = update_word<kHasNever>(own.x, up.x, dn.x, ct.x, s0, r, stab);
-    philox4x32_10(a.rk, g0 + 1, c1, a.c2, a.c3, r);
-    res.y = update_word<kHasNever>(own.y, up.y, dn.y, ct.y, s1, r, stab);
-    philox4x32_10(a.rk, g0 + 2, c1, a.c2, a.c3, r);
-    res.z = update_word<kHasNever>(own.z, up.z, dn.z, ct.z, s2, r, stab);
-    philox4x32_10(a.rk, g0 + 3, c1, a.c2, a.c3, r);
-    res.w = update_word<kHasNever>(own.w, up.w, dn.w, ct.w, s3, r, stab);
-    *ownp = res;
+    res.x = update_word<kHasNever, 0>(own.x, t0, r0, stab, slot);
+    res.y = update_word<kHasNever, 1>(own.y, t1, r1, stab, slot);
+    res.z = update_word<kHasNever, 2>(own.z, t2, r2, stab, slot);
+    res.w = update_word<kHasNever, 3>(own.w, t3, r3, stab, slot);
+    return res;
 }
 
-// One block covers blockDim.x consecutive 128-bit words of one replica; bpr = blocks per replica.
-__global__ void __launch_bounds__(256) ising_int8_vec_kernel(SweepArgs a, int bpr) {
+__device__ __forceinline__ uint4 mask4(const uint4& v) {
+    const uint32_t m = 0x04040404u;      // 4 per -1 spin
+    return make_uint4(v.x & m, v.y & m, v.z & m, v.w & m);
+}
+
+template <int kColour, bool kHasNever>
+__device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, uint32_t slot, int b, int rb,
+                                           int x) {
+    const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
+    const size_t half = (size_t)L * W;
+    const int i0 = rb * kRows;
+    uint4* own4 = (uint4*)((int8_t*)a.lattice + ((size_t)b * 2 + kColour) * half);
+    const int8_t* oth = (const int8_t*)a.lattice + ((size_t)b * 2 + (1 - kColour)) * half;
+    const uint4* oth4 = (const uint4*)oth;
+    const uint32_t* oth1 = (const uint32_t*)oth;
+    // 32-bit element offsets inside the replica (L <= 65536 keeps them below 2^32)
+    const uint32_t eNext = (x == W16 - 1) ? 0u : 4u * x + 4u;    // word index of the edge word inside a row
+    const uint32_t ePrev = (x == 0) ? (uint32_t)W4 - 1u : 4u * x - 1u;
+    const int iu = i0 == 0 ? L - 1 : i0 - 1;
+    uint4 win[3];
+    win[0] = mask4(__ldg(oth4 + (uint32_t)iu * W16 + x));
+    win[1] = mask4(__ldg(oth4 + (uint32_t)i0 * W16 + x));
+    win[2] = mask4(__ldg(oth4 + (uint32_t)(i0 + 1) * W16 + x));
+    uint32_t ownIdx = (uint32_t)i0 * W16 + x;
+    uint4 own = own4[ownIdx];
+    // even rows have parity kColour, odd rows 1 - kColour (i0 is even)
+    uint32_t edge = __ldg(oth1 + (uint32_t)i0 * W4 + (kColour ? eNext : ePrev)) & 0x04040404u;
+    uint32_t g0 = (uint32_t)i0 * (uint32_t)W4 + 4u * (uint32_t)x;
+    const uint32_t c1 = (uint32_t)b + a.replica_offset;
+#pragma unroll
+    for (int r = 0; r < kRows; ++r) {
+        const int i = i0 + r;
+        uint4 nwin = win[0], nown = own;
+        uint32_t nedge = edge;
+        if (r + 1 < kRows) {   // prefetch the inputs of row i+1
+            int i2 = i + 2;
+            if (i2 >= L) i2 -= L;
+            nwin = __ldg(oth4 + (uint32_t)i2 * W16 + x);
+            nown = own4[ownIdx + W16];
+            const bool nextParity = ((r + 1) & 1) ? (1 - kColour) : kColour;
+            nedge = __ldg(oth1 + (uint32_t)(i + 1) * W4 + (nextParity ? eNext : ePrev));
+        }
+        const uint4& um = win[r % 3];
+        const uint4& cm = win[(r + 1) % 3];
+        const uint4& dm = win[(r + 2) % 3];
+        uint4 res;
+        if (r & 1) res = update_row<kHasNever, 1 - kColour>(a, own, um, cm, dm, edge, g0, c1, stab, slot);
+        else res = update_row<kHasNever, kColour>(a, own, um, cm, dm, edge, g0, c1, stab, slot);
+        own4[ownIdx] = res;
+        if (r + 1 < kRows) {
+            win[r % 3] = mask4(nwin);       // row i+2 replaces row i-1
+            own = nown;
+            edge = nedge & 0x04040404u;
+            ownIdx += W16;
+            g0 += (uint32_t)W4;
+        }
+    }
+}
+
+// One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
+template <int kColour>
+__global__ void __launch_bounds__(kRowsThreads) ising_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[kTableStride];
+    __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
-    if (threadIdx.x < kTableStride) stab[threadIdx.x] = a.tables[(size_t)b * kTableStride + threadIdx.x];
+    for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
     __syncthreads();
     const int W16 = a.L >> 5;
-    const int u = blk * blockDim.x + threadIdx.x;          // < L * W16 by construction
-    const int i = u / W16, x = u - i * W16;
-    if (stab[kTabNever]) update_vec<true>(a, stab, b, i, x);
-    else update_vec<false>(a, stab, b, i, x);
+    const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
+    const int rb = u / W16, x = u - rb * W16;
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
+    if (stab[kTabNever]) march_rows<kColour, true>(a, stab, slot, b, rb, x);
+    else march_rows<kColour, false>(a, stab, slot, b, rb, x);
 }
 
 }  // namespace
 
-const char* ising_int8_variant(int L) { return (L % 32 == 0) ? "ising_int8_vec128" : "ising_int8_generic"; }
+const char* ising_int8_variant(int L) { return (L % 32 == 0) ? "ising_int8_rows128" : "ising_int8_generic"; }
 
 int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
-        const int perReplica = a.L * (a.L >> 5);            // 128-bit words of one colour
-        int tpb = 256;
-        while (perReplica % tpb) tpb >>= 1;                  // L = 32 -> 32 threads
+        const int perReplica = (a.L / kRows) * (a.L >> 5);   // strips x row blocks of one colour
+        int tpb = kRowsThreads;
+        while (perReplica % tpb) tpb >>= 1;                  // L = 32 -> 4 threads
         const int bpr = perReplica / tpb;
-        ising_int8_vec_kernel<<<(unsigned)((long long)bpr * a.batch), tpb, 0, s>>>(a, bpr);
+        const unsigned grid = (unsigned)((long long)bpr * a.batch);
+        if (a.colour == 0) ising_int8_rows_kernel<0><<<grid, tpb, 0, s>>>(a, bpr);
+        else ising_int8_rows_kernel<1><<<grid, tpb, 0, s>>>(a, bpr);
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 3) >> 2) * a.batch;
