@@ -45,10 +45,11 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 }
 
 // ---- row-marching kernel: L % 32 == 0.
-// Measured on B200 (profiles/r1_microbench.md): every integer instruction (LOP3, IADD3, PRMT, ISETP, IMAD, ...) is
-// dispatched at 16 lanes/clk per SM sub-partition, i.e. 2 cycles per warp instruction whatever its pipe, so the
-// kernel is bound by the NUMBER of integer instructions per site; loads/stores (LSU) are dispatched beside them.
-// The design therefore minimises integer instructions and pushes byte extraction onto the LSU:
+// Measured on B200 (profiles/r1_microbench.md): LOP3 / PRMT / SHF / IMAD issue at 64 lanes/SM/clk, IMAD.WIDE at 32,
+// two-operand IADD3 / ISETP at 128, LDS at 32.  An IMAD.WIDE + LOP3 pair (one Philox half-round) completes in 4.1
+// cycles per SM sub-partition, but every further instruction adds its own issue time, and the kernel runs at the
+// same speed with 20 or 32 resident warps per SM: it is bound by the number of integer instructions per site, not by
+// latency or memory.  The design therefore minimises integer instructions and pushes byte extraction onto the LSU:
 //   * one thread owns a strip of 16 consecutive same-colour sites (one 128-bit word) and marches down kRows rows,
 //     keeping the three other-colour rows it needs in registers, already masked to "4 if spin is -1" per byte
 //     (one LOP3 per loaded word, reused as up / centre / down of three rows and for the shifted side word);
@@ -56,8 +57,10 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 //   * the four offset bytes are written to a per-thread shared-memory slot (STS) and read back one byte at a
 //     time (LDS.U8) straight into the address of the threshold LDS: no extraction instruction;
 //   * per site: one ISETP (r <= U) and one predicated LOP3 (flip), nothing else.
-// Loads of row i+1 are issued before row i is computed; rows are fully unrolled so the register window rotates by
-// renaming.
+// Loads of the next rows are issued before the current row is computed, through running pointers (no per-load index
+// arithmetic); the loop is rolled two rows per iteration (the side-neighbour parity alternates) so that the body
+// (about 540 instructions) stays resident in the instruction caches.  Launched with programmatic dependent launch:
+// the next half-sweep's blocks are scheduled while this one drains.
 constexpr int kRows = 8;
 constexpr int kRowsThreads = 128;
 
@@ -151,61 +154,76 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
     const size_t half = (size_t)L * W;
     const int i0 = rb * kRows;
-    uint4* own4 = (uint4*)((int8_t*)a.lattice + ((size_t)b * 2 + kColour) * half);
+    int8_t* ownBase = (int8_t*)a.lattice + ((size_t)b * 2 + kColour) * half;
     const int8_t* oth = (const int8_t*)a.lattice + ((size_t)b * 2 + (1 - kColour)) * half;
     const uint4* oth4 = (const uint4*)oth;
     const uint32_t* oth1 = (const uint32_t*)oth;
-    // 32-bit element offsets inside the replica (L <= 65536 keeps them below 2^32)
-    const uint32_t eNext = (x == W16 - 1) ? 0u : 4u * x + 4u;    // word index of the edge word inside a row
+    // word index of the edge word inside a row: next strip's first word / previous strip's last word (periodic)
+    const uint32_t eNext = (x == W16 - 1) ? 0u : 4u * x + 4u;
     const uint32_t ePrev = (x == 0) ? (uint32_t)W4 - 1u : 4u * x - 1u;
     const int iu = i0 == 0 ? L - 1 : i0 - 1;
-    uint4 win[3];
-    win[0] = mask4(__ldg(oth4 + (uint32_t)iu * W16 + x));
-    win[1] = mask4(__ldg(oth4 + (uint32_t)i0 * W16 + x));
-    win[2] = mask4(__ldg(oth4 + (uint32_t)(i0 + 1) * W16 + x));
-    uint32_t ownIdx = (uint32_t)i0 * W16 + x;
-    uint4 own = own4[ownIdx];
-    // even rows have parity kColour, odd rows 1 - kColour (i0 is even)
-    uint32_t edge = __ldg(oth1 + (uint32_t)i0 * W4 + (kColour ? eNext : ePrev)) & 0x04040404u;
+    const int iLast = (i0 + kRows == L) ? 0 : i0 + kRows;       // the only prefetched row that can wrap
+    // Running pointers, advanced by one row stride per row: no per-load index arithmetic inside the unrolled rows.
+    const size_t rowStride = (size_t)W16;                        // in uint4
+    const size_t edgeStride2 = 2 * (size_t)W4;                   // two rows, in uint32
+    const uint4* pOth = oth4 + (size_t)(i0 + 2) * W16 + x;       // next other-colour row to prefetch
+    const uint4* pOthLast = oth4 + (size_t)iLast * W16 + x;
+    uint4* pOwn = (uint4*)ownBase + (size_t)i0 * W16 + x;
+    // even rows of the block have parity kColour, odd rows 1 - kColour (i0 is even)
+    const uint32_t* pEdgeEven = oth1 + (size_t)i0 * W4 + (kColour ? eNext : ePrev);
+    const uint32_t* pEdgeOdd = oth1 + (size_t)(i0 + 1) * W4 + (kColour ? ePrev : eNext);
+    uint4 wU = mask4(__ldg(oth4 + (size_t)iu * W16 + x));     // masked other-colour rows i-1, i, i+1
+    uint4 wC = mask4(__ldg(pOth - 2 * rowStride));
+    uint4 wD = mask4(__ldg(pOth - rowStride));
+    uint4 own = *pOwn;
+    uint32_t edge = __ldg(pEdgeEven) & 0x04040404u;
     uint32_t g0 = (uint32_t)i0 * (uint32_t)W4 + 4u * (uint32_t)x;
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
-#pragma unroll
-    for (int r = 0; r < kRows; ++r) {
-        const int i = i0 + r;
-        uint4 nwin = win[0], nown = own;
-        uint32_t nedge = edge;
-        if (r + 1 < kRows) {   // prefetch the inputs of row i+1
-            int i2 = i + 2;
-            if (i2 >= L) i2 -= L;
-            nwin = __ldg(oth4 + (uint32_t)i2 * W16 + x);
-            nown = own4[ownIdx + W16];
-            const bool nextParity = ((r + 1) & 1) ? (1 - kColour) : kColour;
-            nedge = __ldg(oth1 + (uint32_t)(i + 1) * W4 + (nextParity ? eNext : ePrev));
+    // Two rows per iteration (the side-neighbour parity alternates), rolled: the body stays small enough for the
+    // instruction caches, and all warps of the SM share it.
+#pragma unroll 1
+    for (int rr = 0; rr < kRows; rr += 2) {
+        const bool more = rr + 2 < kRows;
+        // inputs of the odd row i+1: other-colour row i+2 (the only one that can wrap), own row i+1, its edge word
+        const uint4 n1 = __ldg(more ? pOth : pOthLast);
+        const uint4 own1 = *(pOwn + rowStride);
+        const uint32_t edge1 = __ldg(pEdgeOdd);
+        uint4 res = update_row<kHasNever, kColour>(a, own, wU, wC, wD, edge, g0, c1, stab, slot);
+        *pOwn = res;
+        // inputs of the next even row i+2: other-colour row i+3, own row i+2, its edge word
+        uint4 n2 = n1, own2 = own1;
+        uint32_t edge2 = edge1;
+        if (more) {
+            n2 = __ldg(pOth + rowStride);
+            own2 = *(pOwn + 2 * rowStride);
+            edge2 = __ldg(pEdgeEven + edgeStride2);
         }
-        const uint4& um = win[r % 3];
-        const uint4& cm = win[(r + 1) % 3];
-        const uint4& dm = win[(r + 2) % 3];
-        uint4 res;
-        if (r & 1) res = update_row<kHasNever, 1 - kColour>(a, own, um, cm, dm, edge, g0, c1, stab, slot);
-        else res = update_row<kHasNever, kColour>(a, own, um, cm, dm, edge, g0, c1, stab, slot);
-        own4[ownIdx] = res;
-        if (r + 1 < kRows) {
-            win[r % 3] = mask4(nwin);       // row i+2 replaces row i-1
-            own = nown;
-            edge = nedge & 0x04040404u;
-            ownIdx += W16;
-            g0 += (uint32_t)W4;
-        }
+        const uint4 n1m = mask4(n1);
+        res = update_row<kHasNever, 1 - kColour>(a, own1, wC, wD, n1m, edge1 & 0x04040404u, g0 + (uint32_t)W4, c1, stab,
+                                                 slot);
+        *(pOwn + rowStride) = res;
+        wU = wD;
+        wC = n1m;
+        wD = mask4(n2);
+        own = own2;
+        edge = edge2 & 0x04040404u;
+        pOth += 2 * rowStride;
+        pOwn += 2 * rowStride;
+        pEdgeEven += edgeStride2;
+        pEdgeOdd += edgeStride2;
+        g0 += 2u * (uint32_t)W4;
     }
 }
 
 // One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
 template <int kColour>
-__global__ void __launch_bounds__(kRowsThreads) ising_int8_rows_kernel(SweepArgs a, int bpr) {
+__global__ void __launch_bounds__(kRowsThreads, 1) ising_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[kTableStride];
     __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
+    pdl_launch_dependents();
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
+    pdl_wait();
     for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
     __syncthreads();
     const int W16 = a.L >> 5;
@@ -227,8 +245,8 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
         while (perReplica % tpb) tpb >>= 1;                  // L = 32 -> 4 threads
         const int bpr = perReplica / tpb;
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
-        if (a.colour == 0) ising_int8_rows_kernel<0><<<grid, tpb, 0, s>>>(a, bpr);
-        else ising_int8_rows_kernel<1><<<grid, tpb, 0, s>>>(a, bpr);
+        if (a.colour == 0) launch_pdl(ising_int8_rows_kernel<0>, grid, (unsigned)tpb, s, a, bpr);
+        else launch_pdl(ising_int8_rows_kernel<1>, grid, (unsigned)tpb, s, a, bpr);
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 3) >> 2) * a.batch;

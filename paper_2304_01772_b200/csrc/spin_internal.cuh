@@ -70,6 +70,30 @@ struct InitArgs {
     RoundKeys rk;
 };
 
+// ---- programmatic dependent launch -------------------------------------------------------------------
+// The sweep is a chain of short dependent kernels (two per sweep).  Launching them with the programmatic
+// stream-serialisation attribute lets the blocks of launch n+1 be scheduled, and run their index arithmetic, while
+// the last blocks of launch n drain; pdl_wait() then blocks until launch n has completed and its writes are
+// visible.  Every kernel launched this way calls pdl_launch_dependents() first and pdl_wait() before its first
+// global-memory access.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, cudaStream_t s, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid, 1, 1);
+    cfg.blockDim = dim3(block, 1, 1);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
+}
+
 // ---- launchers (each returns the number of kernels it launched; errors via cudaGetLastError) --------
 int launch_init(const InitArgs& a, int model, int layout, cudaStream_t s);
 

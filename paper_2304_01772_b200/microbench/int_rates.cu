@@ -12,7 +12,7 @@
 constexpr int kChains = 8;     // independent dependency chains per thread
 constexpr int kInner = 64;     // unrolled ops per chain per outer iteration
 
-enum Op { OP_LOP3, OP_IADD3, OP_IMAD, OP_WIDE, OP_HI, OP_HI_LO, OP_PRMT, OP_SETP_XOR, OP_WIDE_LOP3, OP_SHF, OP_WIDE_2LOP3, OP_WIDE_LOP3_ADD, OP_WIDE_LOP3_SETP, OP_L2I, OP_L2R, OP_L3R, OP_L3I, OP_ADD3R, OP_SETP_DEP, OP_VOTE, OP_LDS, OP_LDS_U8, OP_SEL, OP_DP4A, OP_PLOP_IMM, OP_COUNT };
+enum Op { OP_LOP3, OP_IADD3, OP_IMAD, OP_WIDE, OP_HI, OP_HI_LO, OP_PRMT, OP_SETP_XOR, OP_WIDE_LOP3, OP_SHF, OP_WIDE_2LOP3, OP_WIDE_LOP3_ADD, OP_WIDE_LOP3_SETP, OP_L2I, OP_L2R, OP_L3R, OP_L3I, OP_ADD3R, OP_SETP_DEP, OP_VOTE, OP_LDS, OP_LDS_U8, OP_SEL, OP_DP4A, OP_PLOP_IMM, OP_CARRY, OP_COUNT };
 static const char* kOpName[OP_COUNT] = {
     "LOP3 (3-input xor)", "IADD3", "IMAD (mad.lo.u32)", "IMAD.WIDE.U32 (mul.wide.u32)", "IMAD.HI.U32 (mul.hi.u32)",
     "mul.hi.u32 + mul.lo.u32 pair", "PRMT", "ISETP + predicated LOP3", "IMAD.WIDE.U32 + LOP3 (one Philox half-round)",
@@ -20,8 +20,9 @@ static const char* kOpName[OP_COUNT] = {
     "LOP3 reg ^ imm", "LOP3 reg ^ reg", "LOP3 reg ^ reg ^ reg", "LOP3 reg ^ reg ^ imm", "IADD3 reg + reg + reg",
     "ISETP (data dependent) + predicated LOP3 imm", "VOTE.ballot + LOP3", "LDS (32-bit, data-dependent address)",
     "LDS.U8 (data-dependent address)", "ISETP + SEL", "IDP4A (dp4a.s32.u32 with accumulate)",
-    "ISETP (uniform threshold) + predicated LOP3 reg | imm (2 ops; the per-site pair of the bit-sliced kernels)"};
-static const int kOpsPerStep[OP_COUNT] = {1, 1, 1, 1, 1, 2, 1, 2, 2, 1, 3, 3, 4, 1, 1, 1, 1, 1, 2, 2, 1, 1, 2, 1, 2};
+    "ISETP (uniform threshold) + predicated LOP3 reg | imm (2 ops; the per-site pair of the bit-sliced kernels)",
+    "IADD3 carry-out + IADD3.X shift-in (add.cc / addc: compare bit shifted into a mask, 2 ops)"};
+static const int kOpsPerStep[OP_COUNT] = {1, 1, 1, 1, 1, 2, 1, 2, 2, 1, 3, 3, 4, 1, 1, 1, 1, 1, 2, 2, 1, 1, 2, 1, 2, 2};
 
 template <int kOp>
 __device__ __forceinline__ void step(uint32_t& a, uint32_t& b, uint32_t k) {
@@ -74,6 +75,10 @@ __device__ __forceinline__ void step(uint32_t& a, uint32_t& b, uint32_t k) {
     else if (kOp == OP_PLOP_IMM) {
         // a plays the random word (changes every step), b collects the predicate bits
         asm volatile("{\n\t.reg .pred p;\n\tsetp.ls.u32 p, %1, %2;\n\t@p or.b32 %0, %0, 0x10;\n\t}" : "+r"(b) : "r"(a), "r"(k));
+        asm volatile("add.u32 %0, %0, %1;" : "+r"(a) : "r"(b));
+    }
+    else if (kOp == OP_CARRY) {
+        asm volatile("{\n\t.reg .u32 t;\n\tadd.cc.u32 t, %1, %2;\n\taddc.u32 %0, %0, %0;\n\t}" : "+r"(b) : "r"(a), "r"(k));
         asm volatile("add.u32 %0, %0, %1;" : "+r"(a) : "r"(b));
     }
     else if (kOp == OP_SHF) { asm volatile("shf.l.wrap.b32 %0, %0, %1, 7;" : "+r"(a) : "r"(b)); }
@@ -207,7 +212,7 @@ int main(int argc, char** argv) {
         if (only_philox) { if (run_op<OP_WIDE_LOP3>(d, w) || run_op<OP_WIDE_2LOP3>(d, w) || run_op<OP_WIDE_LOP3_ADD>(d, w) || run_op<OP_WIDE_LOP3_SETP>(d, w)) return 1; continue; }
         if (run_op<OP_LOP3>(d, w) || run_op<OP_IADD3>(d, w) || run_op<OP_IMAD>(d, w) || run_op<OP_WIDE>(d, w) ||
             run_op<OP_HI>(d, w) || run_op<OP_HI_LO>(d, w) || run_op<OP_PRMT>(d, w) || run_op<OP_SHF>(d, w) ||
-            run_op<OP_SETP_XOR>(d, w) || run_op<OP_WIDE_LOP3>(d, w) || run_op<OP_WIDE_2LOP3>(d, w) || run_op<OP_WIDE_LOP3_ADD>(d, w) || run_op<OP_WIDE_LOP3_SETP>(d, w) || run_op<OP_L2I>(d, w) || run_op<OP_L2R>(d, w) || run_op<OP_L3R>(d, w) || run_op<OP_L3I>(d, w) || run_op<OP_ADD3R>(d, w) || run_op<OP_SETP_DEP>(d, w) || run_op<OP_VOTE>(d, w) || run_op<OP_SEL>(d, w) || run_op<OP_LDS>(d, w) || run_op<OP_LDS_U8>(d, w) || run_op<OP_DP4A>(d, w) || run_op<OP_PLOP_IMM>(d, w)) return 1;
+            run_op<OP_SETP_XOR>(d, w) || run_op<OP_WIDE_LOP3>(d, w) || run_op<OP_WIDE_2LOP3>(d, w) || run_op<OP_WIDE_LOP3_ADD>(d, w) || run_op<OP_WIDE_LOP3_SETP>(d, w) || run_op<OP_L2I>(d, w) || run_op<OP_L2R>(d, w) || run_op<OP_L3R>(d, w) || run_op<OP_L3I>(d, w) || run_op<OP_ADD3R>(d, w) || run_op<OP_SETP_DEP>(d, w) || run_op<OP_VOTE>(d, w) || run_op<OP_SEL>(d, w) || run_op<OP_LDS>(d, w) || run_op<OP_LDS_U8>(d, w) || run_op<OP_DP4A>(d, w) || run_op<OP_PLOP_IMM>(d, w) || run_op<OP_CARRY>(d, w)) return 1;
     }
     printf("\n| kernel | warps/SMSP | rate | | |\n|---|---|---|---|---|\n");
     for (int w : {4, 8}) {
