@@ -46,10 +46,31 @@ __global__ void potts_int8_generic_kernel(SweepArgs a) {
     }
 }
 
-// ---- vectorised kernel: L % 32 == 0, one thread per 16 consecutive same-colour sites (8 Philox calls).
+// ---- row-marching kernel: L % 32 == 0.  Same skeleton as the Ising int8 kernel (ising_int8.cu): one thread owns a
+// strip of 16 consecutive same-colour sites (8 Philox calls per row) and marches down kRows rows with the three
+// other-colour rows it needs in registers, running pointers, a rolled two-row loop and programmatic dependent launch.
 // Byte-SIMD throughout: states are < 128, so for x = a ^ b (per byte < 128) bit 7 of x + 0x7F is "a != b".
 // The 4 "differs from old" bits and the 4 "differs from new" bits of a site are gathered into one byte that
-// indexes a 256-entry shared table holding U[dn + 4] (dn = n_new - n_old = #(!= old) - #(!= new)).
+// indexes a 256-entry shared table holding U[dn + 4] (dn = n_new - n_old = #(!= old) - #(!= new)); the four index
+// bytes of a word go through a per-thread shared-memory slot (STS, then LDS.U8 straight into the table address).
+constexpr int kRows = 8;
+constexpr int kRowsThreads = 128;
+#ifndef POTTS_MINB
+#define POTTS_MINB 5
+#endif
+
+template <int kOff>
+__device__ __forceinline__ uint32_t slot_load_u8(uint32_t saddr) {
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1+%2];" : "=r"(v) : "r"(saddr), "n"(kOff));
+    return v;
+}
+
+template <int kOff>
+__device__ __forceinline__ void slot_store_u32(uint32_t saddr, uint32_t v) {
+    asm volatile("st.shared.u32 [%0+%1], %2;" :: "r"(saddr), "n"(kOff), "r"(v));
+}
+
 __device__ __forceinline__ uint32_t neq_bits(uint32_t v, uint32_t u, uint32_t d, uint32_t c, uint32_t s) {
     const uint32_t k = 0x7F7F7F7Fu;
     const uint32_t a0 = (v ^ u) + k, a1 = ((v ^ d) + k) >> 1, a2 = ((v ^ c) + k) >> 2, a3 = ((v ^ s) + k) >> 3;
@@ -60,115 +81,182 @@ __device__ __forceinline__ uint32_t neq_bits(uint32_t v, uint32_t u, uint32_t d,
     return t;
 }
 
-template <bool kHasNever>
+// One site: threshold fetch (the index byte scales into the table address), compare, replace the byte by the proposal.
+template <bool kHasNever, int kE>
+__device__ __forceinline__ void site_step(uint32_t& own, uint32_t nw, uint32_t o, uint32_t r, const uint32_t* stab,
+                                          const uint32_t* snever) {
+    // two byte-addressed loads (no address arithmetic): pattern byte -> 4 * class -> U[class]
+    const uint32_t c4 = ((const uint8_t*)(stab + 16))[o];
+    bool acc = r <= *(const uint32_t*)((const char*)stab + c4);
+    if (kHasNever) acc = acc && !((snever[0] >> (c4 >> 2)) & 1u);
+    if (acc) own = __byte_perm(own, nw, 0x3210 ^ ((0x4 + kE) << (4 * kE)) ^ (kE << (4 * kE)));
+}
+
+// One 4-site word: r0 feeds sites 0, 1 (proposal words r0[0], r0[2]; acceptance words r0[1], r0[3]), r1 sites 2, 3.
+template <bool kHasNever, int kJ>
 __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t ct, uint32_t sd,
-                                                const uint32_t r0[4], const uint32_t r1[4], uint32_t q,
-                                                const uint32_t* stab, const uint32_t* snever) {
+                                                const uint32_t r0[4], const uint32_t r1[4], uint32_t q, uint32_t geAdd,
+                                                const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
     // proposal (O6): new = old + 1 + floor(r_prop (q-1) / 2^32), minus q if >= q
     const uint32_t qm1 = q - 1u;
     const uint32_t d = __umulhi(r0[0], qm1) | (__umulhi(r0[2], qm1) << 8) | (__umulhi(r1[0], qm1) << 16) |
                        (__umulhi(r1[2], qm1) << 24);
     uint32_t nw = own + 0x01010101u + d;                              // <= 2q-2 per byte
-    const uint32_t ge = ((nw + (0x80u - q) * 0x01010101u) >> 7) & 0x01010101u;   // 1 where nw >= q
+    const uint32_t ge = ((nw + geAdd) >> 7) & 0x01010101u;            // 1 where nw >= q (geAdd = (0x80 - q) per byte)
     nw -= ge * q;
     const uint32_t mo = neq_bits(own, up, dn, ct, sd);
     const uint32_t mn = neq_bits(nw, up, dn, ct, sd);
     const uint32_t idx = (mo & 0xF0F0F0F0u) | ((mn >> 4) & 0x0F0F0F0Fu);
-    const uint32_t racc[4] = {r0[1], r0[3], r1[1], r1[3]};
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const uint32_t o = (idx >> (8 * e)) & 0xFFu;
-        bool acc = racc[e] <= stab[o];
-        if (kHasNever) acc = acc && !((snever[o >> 5] >> (o & 31u)) & 1u);
-        if (acc) own = __byte_perm(own, nw, 0x3210 ^ ((0x4 + e) << (4 * e)) ^ (e << (4 * e)));
-    }
+    slot_store_u32<kJ * kRowsThreads * 4>(slot, idx);
+    const uint32_t o0 = slot_load_u8<kJ * kRowsThreads * 4 + 0>(slot);
+    const uint32_t o1 = slot_load_u8<kJ * kRowsThreads * 4 + 1>(slot);
+    const uint32_t o2 = slot_load_u8<kJ * kRowsThreads * 4 + 2>(slot);
+    const uint32_t o3 = slot_load_u8<kJ * kRowsThreads * 4 + 3>(slot);
+    site_step<kHasNever, 0>(own, nw, o0, r0[1], stab, snever);
+    site_step<kHasNever, 1>(own, nw, o1, r0[3], stab, snever);
+    site_step<kHasNever, 2>(own, nw, o2, r1[1], stab, snever);
+    site_step<kHasNever, 3>(own, nw, o3, r1[3], stab, snever);
     return own;
 }
 
-template <bool kHasNever>
-__device__ __forceinline__ void update_vec(SweepArgs& a, const uint32_t* stab, const uint32_t* snever, uint32_t q,
-                                           int b, int i, int x) {
-    const int L = a.L, W = L >> 1, W16 = W >> 4;
-    const size_t half = (size_t)L * W;
-    uint4* ownp = (uint4*)((uint8_t*)a.lattice + ((size_t)b * 2 + a.colour) * half) + (size_t)i * W16 + x;
-    const uint8_t* oth = (const uint8_t*)a.lattice + ((size_t)b * 2 + (1 - a.colour)) * half;
-    const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
-    const uint4 own = *ownp;
-    const uint4 up = __ldg((const uint4*)(oth + (size_t)iu * W) + x);
-    const uint4 dn = __ldg((const uint4*)(oth + (size_t)id * W) + x);
-    const uint4 ct = __ldg((const uint4*)(oth + (size_t)i * W) + x);
-    const int p = (i + a.colour) & 1;
+// One row of one strip.  up / ct / dn: other-colour words of rows i-1, i, i+1; kParity = 1: the side neighbour of
+// site k is other[i][k+1], else other[i][k-1]; `edge` is the 32-bit word holding the 17th byte.
+template <bool kHasNever, int kParity>
+__device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const uint4& up, const uint4& ct,
+                                            const uint4& dn, uint32_t edge, uint32_t g0, uint32_t c1, uint32_t q,
+                                            uint32_t geAdd, const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
     uint32_t s0, s1, s2, s3;
-    if (p) {
-        const int kn = (x == W16 - 1) ? 0 : 16 * x + 16;
-        const uint32_t nx = (uint32_t)__ldg(oth + (size_t)i * W + kn);
+    if (kParity) {
         s0 = __byte_perm(ct.x, ct.y, 0x4321);
         s1 = __byte_perm(ct.y, ct.z, 0x4321);
         s2 = __byte_perm(ct.z, ct.w, 0x4321);
-        s3 = __byte_perm(ct.w, nx, 0x4321);
+        s3 = __byte_perm(ct.w, edge, 0x4321);
     } else {
-        const int kp = (x == 0) ? W - 1 : 16 * x - 1;
-        const uint32_t pv = (uint32_t)__ldg(oth + (size_t)i * W + kp);
-        s0 = __byte_perm(pv, ct.x, 0x6540);
+        s0 = __byte_perm(edge, ct.x, 0x6543);
         s1 = __byte_perm(ct.x, ct.y, 0x6543);
         s2 = __byte_perm(ct.y, ct.z, 0x6543);
         s3 = __byte_perm(ct.z, ct.w, 0x6543);
     }
-    // same-colour index n = i*W + 16x + ...; Philox group = n >> 1
-    const uint32_t g0 = (uint32_t)i * (uint32_t)(W >> 1) + 8u * (uint32_t)x;
-    const uint32_t c1 = (uint32_t)b + a.replica_offset;
     uint4 res;
     uint32_t r0[4], r1[4];
     philox4x32_10(a.rk, g0 + 0, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 1, c1, a.c2, a.c3, r1);
-    res.x = update_word<kHasNever>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, stab, snever);
+    res.x = update_word<kHasNever, 0>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 2, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 3, c1, a.c2, a.c3, r1);
-    res.y = update_word<kHasNever>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, stab, snever);
+    res.y = update_word<kHasNever, 1>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 4, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 5, c1, a.c2, a.c3, r1);
-    res.z = update_word<kHasNever>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, stab, snever);
+    res.z = update_word<kHasNever, 2>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 6, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 7, c1, a.c2, a.c3, r1);
-    res.w = update_word<kHasNever>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, stab, snever);
-    *ownp = res;
+    res.w = update_word<kHasNever, 3>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, geAdd, stab, snever, slot);
+    return res;
 }
 
-__global__ void __launch_bounds__(256) potts_int8_vec_kernel(SweepArgs a, int bpr) {
-    __shared__ uint32_t stab[256];
-    __shared__ uint32_t snever[8];
+template <int kColour, bool kHasNever>
+__device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint32_t* snever, uint32_t q,
+                                           uint32_t slot, int b, int rb, int x) {
+    const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
+    const size_t half = (size_t)L * W;
+    const int i0 = rb * kRows;
+    uint8_t* ownBase = (uint8_t*)a.lattice + ((size_t)b * 2 + kColour) * half;
+    const uint8_t* oth = (const uint8_t*)a.lattice + ((size_t)b * 2 + (1 - kColour)) * half;
+    const uint4* oth4 = (const uint4*)oth;
+    const uint32_t* oth1 = (const uint32_t*)oth;
+    const uint32_t eNext = (x == W16 - 1) ? 0u : 4u * x + 4u;    // word index of the edge word inside a row
+    const uint32_t ePrev = (x == 0) ? (uint32_t)W4 - 1u : 4u * x - 1u;
+    const int iu = i0 == 0 ? L - 1 : i0 - 1;
+    const int iLast = (i0 + kRows == L) ? 0 : i0 + kRows;        // the only prefetched row that can wrap
+    const size_t rowStride = (size_t)W16;                         // in uint4
+    const size_t edgeStride2 = 2 * (size_t)W4;                    // two rows, in uint32
+    const uint4* pOth = oth4 + (size_t)(i0 + 2) * W16 + x;
+    const uint4* pOthLast = oth4 + (size_t)iLast * W16 + x;
+    uint4* pOwn = (uint4*)ownBase + (size_t)i0 * W16 + x;
+    // even rows of the block have parity kColour, odd rows 1 - kColour (i0 is even)
+    const uint32_t* pEdgeEven = oth1 + (size_t)i0 * W4 + (kColour ? eNext : ePrev);
+    const uint32_t* pEdgeOdd = oth1 + (size_t)(i0 + 1) * W4 + (kColour ? ePrev : eNext);
+    uint4 wU = __ldg(oth4 + (size_t)iu * W16 + x);               // other-colour rows i-1, i, i+1
+    uint4 wC = __ldg(pOth - 2 * rowStride);
+    uint4 wD = __ldg(pOth - rowStride);
+    uint4 own = *pOwn;
+    uint32_t edge = __ldg(pEdgeEven);
+    uint32_t g0 = (uint32_t)i0 * (uint32_t)(W >> 1) + 8u * (uint32_t)x;   // Philox group = n >> 1
+    const uint32_t c1 = (uint32_t)b + a.replica_offset;
+    const uint32_t geAdd = (0x80u - q) * 0x01010101u;
+#pragma unroll 1
+    for (int rr = 0; rr < kRows; rr += 2) {
+        const bool more = rr + 2 < kRows;
+        const uint4 n1 = __ldg(more ? pOth : pOthLast);
+        const uint4 own1 = *(pOwn + rowStride);
+        const uint32_t edge1 = __ldg(pEdgeOdd);
+        uint4 res = update_row<kHasNever, kColour>(a, own, wU, wC, wD, edge, g0, c1, q, geAdd, stab, snever, slot);
+        *pOwn = res;
+        uint4 n2 = n1, own2 = own1;
+        uint32_t edge2 = edge1;
+        if (more) {
+            n2 = __ldg(pOth + rowStride);
+            own2 = *(pOwn + 2 * rowStride);
+            edge2 = __ldg(pEdgeEven + edgeStride2);
+        }
+        res = update_row<kHasNever, 1 - kColour>(a, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd, stab,
+                                                 snever, slot);
+        *(pOwn + rowStride) = res;
+        wU = wD;
+        wC = n1;
+        wD = n2;
+        own = own2;
+        edge = edge2;
+        pOth += 2 * rowStride;
+        pOwn += 2 * rowStride;
+        pEdgeEven += edgeStride2;
+        pEdgeOdd += edgeStride2;
+        g0 += (uint32_t)W;
+    }
+}
+
+// One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
+template <int kColour>
+__global__ void __launch_bounds__(kRowsThreads, POTTS_MINB) potts_int8_rows_kernel(SweepArgs a, int bpr) {
+    __shared__ uint32_t stab[16 + 64];            // U[dn + 4] in [0..8]; from word 16: 256-byte pattern -> 4 * class table
+    __shared__ uint32_t snever[1];
+    __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
+    pdl_launch_dependents();
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
+    pdl_wait();
     const uint32_t* tab = a.tables + (size_t)b * kTableStride;
     const uint32_t never = tab[kTabNever];
-    if (threadIdx.x < 8) snever[threadIdx.x] = 0u;
-    __syncthreads();
+    for (int m = threadIdx.x; m < 16; m += blockDim.x) stab[m] = tab[m];
+    if (threadIdx.x == 0) snever[0] = never;
     for (int m = threadIdx.x; m < 256; m += blockDim.x) {
         // high nibble: "neighbour != old" bits, low nibble: "neighbour != new" bits
         const int cls = __popc(m >> 4) - __popc(m & 15) + 4;
-        stab[m] = tab[cls];
-        if ((never >> cls) & 1u) atomicOr(&snever[m >> 5], 1u << (m & 31));
+        ((uint8_t*)(stab + 16))[m] = (uint8_t)(4 * cls);
     }
     __syncthreads();
     const uint32_t q = tab[kTabQ];
     const int W16 = a.L >> 5;
-    const int u = blk * blockDim.x + threadIdx.x;
-    const int i = u / W16, x = u - i * W16;
-    if (never) update_vec<true>(a, stab, snever, q, b, i, x);
-    else update_vec<false>(a, stab, snever, q, b, i, x);
+    const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
+    const int rb = u / W16, x = u - rb * W16;
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
+    if (never) march_rows<kColour, true>(a, stab, snever, q, slot, b, rb, x);
+    else march_rows<kColour, false>(a, stab, snever, q, slot, b, rb, x);
 }
 
 }  // namespace
 
-const char* potts_int8_variant(int L) { return (L % 32 == 0) ? "potts_int8_vec128" : "potts_int8_generic"; }
+const char* potts_int8_variant(int L) { return (L % 32 == 0) ? "potts_int8_rows128" : "potts_int8_generic"; }
 
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
-        const int perReplica = a.L * (a.L >> 5);
-        int tpb = 256;
-        while (perReplica % tpb) tpb >>= 1;
+        const int perReplica = (a.L / kRows) * (a.L >> 5);   // strips x row blocks of one colour
+        int tpb = kRowsThreads;
+        while (perReplica % tpb) tpb >>= 1;                  // L = 32 -> 4 threads
         const int bpr = perReplica / tpb;
-        potts_int8_vec_kernel<<<(unsigned)((long long)bpr * a.batch), tpb, 0, s>>>(a, bpr);
+        const unsigned grid = (unsigned)((long long)bpr * a.batch);
+        if (a.colour == 0) launch_pdl(potts_int8_rows_kernel<0>, grid, (unsigned)tpb, s, a, bpr);
+        else launch_pdl(potts_int8_rows_kernel<1>, grid, (unsigned)tpb, s, a, bpr);
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 1) >> 1) * a.batch;
