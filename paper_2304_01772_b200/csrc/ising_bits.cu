@@ -26,6 +26,13 @@ __device__ __forceinline__ int decode_class(int e, int nib) {
     return D * 8 + P2 * 4 + P1 * 2 + P0;
 }
 
+constexpr int kRows = 8;
+constexpr int kThreads = 128;
+
+// One word = 32 sites = 8 Philox calls.  up / dn / ct: other-colour words of rows i-1, i+1, i; sd: the side
+// neighbours (ct shifted by one site, with the bit of the adjacent word).  stab[e][nibble] holds U for the class
+// whose bits sit in that nibble order; the nibble of site 4c+e is read pre-scaled (x4) so that it is the byte offset
+// of the threshold: per site SHF + LOP3 (extract), LDS, ISETP, predicated OR.
 template <bool kHasNever>
 __device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own, uint32_t up, uint32_t dn, uint32_t ct,
                                                 uint32_t sd, uint32_t g0, uint32_t c1, const uint32_t (*stab)[16],
@@ -50,24 +57,84 @@ __device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own
         philox4x32_10(a.rk, g0 + c, c1, a.c2, a.c3, r);
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const uint32_t o = (t[e] >> (4 * c)) & 0xFu;
-            bool acc = r[e] <= stab[e][o];
-            if (kHasNever) acc = acc && !((snever[e] >> o) & 1u);
+            // byte offset 4 * nibble of site 4c+e
+            const uint32_t o4 = (c == 0 ? (t[e] << 2) : (t[e] >> (4 * c - 2))) & 0x3Cu;
+            bool acc = r[e] <= *(const uint32_t*)((const char*)stab[e] + o4);
+            if (kHasNever) acc = acc && !((snever[e] >> (o4 >> 2)) & 1u);
             if (acc) flip |= 1u << (4 * c + e);
         }
     }
     return own ^ flip;
 }
 
-__global__ void __launch_bounds__(128) ising_bits_kernel(SweepArgs a, int bpr) {
+// Row-marching: one thread owns word x of kRows consecutive rows (same skeleton as ising_int8.cu: the three
+// other-colour words it needs stay in registers, running pointers, two rows per rolled iteration because the side
+// of the horizontal neighbour alternates, programmatic dependent launch).
+template <int kColour, bool kHasNever>
+__device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t (*stab)[16], const uint32_t* snever, int b,
+                                           int rb, int x) {
+    const int L = a.L, WW = L >> 6;                       // words per colour-row
+    const size_t half = (size_t)L * WW;
+    const int i0 = rb * kRows;
+    uint32_t* pOwn = (uint32_t*)a.lattice + ((size_t)b * 2 + kColour) * half + (size_t)i0 * WW + x;
+    const uint32_t* oth = (const uint32_t*)a.lattice + ((size_t)b * 2 + (1 - kColour)) * half;
+    const int xNext = (x == WW - 1) ? 0 : x + 1, xPrev = (x == 0) ? WW - 1 : x - 1;
+    const int iu = i0 == 0 ? L - 1 : i0 - 1;
+    const int iLast = (i0 + kRows == L) ? 0 : i0 + kRows;
+    const uint32_t* pOth = oth + (size_t)(i0 + 2) * WW + x;
+    const uint32_t* pOthLast = oth + (size_t)iLast * WW + x;
+    // even rows of the block have parity kColour (side neighbour k+1 iff parity 1), odd rows 1 - kColour
+    const uint32_t* pEdgeEven = oth + (size_t)i0 * WW + (kColour ? xNext : xPrev);
+    const uint32_t* pEdgeOdd = oth + (size_t)(i0 + 1) * WW + (kColour ? xPrev : xNext);
+    const size_t rowStride = (size_t)WW;
+    uint32_t wU = __ldg(oth + (size_t)iu * WW + x);
+    uint32_t wC = __ldg(pOth - 2 * rowStride);
+    uint32_t wD = __ldg(pOth - rowStride);
+    uint32_t own = *pOwn;
+    uint32_t edge = __ldg(pEdgeEven);
+    uint32_t g0 = (uint32_t)i0 * (uint32_t)(L >> 3) + 8u * (uint32_t)x;   // (i*(L/2) + 32x) >> 2
+    const uint32_t c1 = (uint32_t)b + a.replica_offset;
+#pragma unroll 1
+    for (int rr = 0; rr < kRows; rr += 2) {
+        const bool more = rr + 2 < kRows;
+        const uint32_t n1 = __ldg(more ? pOth : pOthLast);
+        const uint32_t own1 = *(pOwn + rowStride);
+        const uint32_t edge1 = __ldg(pEdgeOdd);
+        uint32_t sd = kColour ? ((wC >> 1) | (edge << 31)) : ((wC << 1) | (edge >> 31));
+        *pOwn = update_word<kHasNever>(a, own, wU, wD, wC, sd, g0, c1, stab, snever);
+        uint32_t n2 = n1, own2 = own1, edge2 = edge1;
+        if (more) {
+            n2 = __ldg(pOth + rowStride);
+            own2 = *(pOwn + 2 * rowStride);
+            edge2 = __ldg(pEdgeEven + 2 * rowStride);
+        }
+        sd = kColour ? ((wD << 1) | (edge1 >> 31)) : ((wD >> 1) | (edge1 << 31));
+        *(pOwn + rowStride) = update_word<kHasNever>(a, own1, wC, n1, wD, sd, g0 + (uint32_t)(L >> 3), c1, stab, snever);
+        wU = wD;
+        wC = n1;
+        wD = n2;
+        own = own2;
+        edge = edge2;
+        pOth += 2 * rowStride;
+        pOwn += 2 * rowStride;
+        pEdgeEven += 2 * rowStride;
+        pEdgeOdd += 2 * rowStride;
+        g0 += (uint32_t)(L >> 2);
+    }
+}
+
+template <int kColour>
+__global__ void __launch_bounds__(kThreads) ising_bits_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[4][16];
     __shared__ uint32_t snever[4];
+    pdl_launch_dependents();
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
+    pdl_wait();
     const uint32_t* tab = a.tables + (size_t)b * kTableStride;
     const uint32_t never = tab[kTabNever];
-    if (threadIdx.x < 64) {
-        const int e = threadIdx.x >> 4, nib = threadIdx.x & 15;
+    for (int m = threadIdx.x; m < 64; m += blockDim.x) {
+        const int e = m >> 4, nib = m & 15;
         stab[e][nib] = tab[decode_class(e, nib)];
     }
     if (threadIdx.x < 4) {
@@ -76,41 +143,23 @@ __global__ void __launch_bounds__(128) ising_bits_kernel(SweepArgs a, int bpr) {
         snever[threadIdx.x] = m;
     }
     __syncthreads();
-    const int L = a.L, WW = L >> 6;                       // words per colour-row
-    const int u = blk * blockDim.x + threadIdx.x;         // < L * WW by construction
-    const int i = u / WW, x = u - i * WW;
-    const size_t half = (size_t)L * WW;
-    uint32_t* ownp = (uint32_t*)a.lattice + ((size_t)b * 2 + a.colour) * half + (size_t)i * WW + x;
-    const uint32_t* oth = (const uint32_t*)a.lattice + ((size_t)b * 2 + (1 - a.colour)) * half;
-    const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
-    const uint32_t own = *ownp;
-    const uint32_t up = __ldg(oth + (size_t)iu * WW + x);
-    const uint32_t dn = __ldg(oth + (size_t)id * WW + x);
-    const uint32_t ct = __ldg(oth + (size_t)i * WW + x);
-    uint32_t sd;
-    if ((i + a.colour) & 1) {   // side neighbour of site k is other[i][k+1]
-        const uint32_t nx = __ldg(oth + (size_t)i * WW + (x == WW - 1 ? 0 : x + 1));
-        sd = (ct >> 1) | (nx << 31);
-    } else {                    // other[i][k-1]
-        const uint32_t pv = __ldg(oth + (size_t)i * WW + (x == 0 ? WW - 1 : x - 1));
-        sd = (ct << 1) | (pv >> 31);
-    }
-    const uint32_t g0 = (uint32_t)i * (uint32_t)(L >> 3) + 8u * (uint32_t)x;   // (i*(L/2) + 32x) >> 2
-    const uint32_t c1 = (uint32_t)b + a.replica_offset;
-    uint32_t res;
-    if (never) res = update_word<true>(a, own, up, dn, ct, sd, g0, c1, stab, snever);
-    else res = update_word<false>(a, own, up, dn, ct, sd, g0, c1, stab, snever);
-    *ownp = res;
+    const int WW = a.L >> 6;
+    const int u = blk * blockDim.x + threadIdx.x;         // < (L / kRows) * WW by construction
+    const int rb = u / WW, x = u - rb * WW;
+    if (never) march_rows<kColour, true>(a, stab, snever, b, rb, x);
+    else march_rows<kColour, false>(a, stab, snever, b, rb, x);
 }
 
 }  // namespace
 
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
-    const int perReplica = a.L * (a.L >> 6);
-    int tpb = 128;
+    const int perReplica = (a.L / kRows) * (a.L >> 6);
+    int tpb = kThreads;
     while (perReplica % tpb) tpb >>= 1;
     const int bpr = perReplica / tpb;
-    ising_bits_kernel<<<(unsigned)((long long)bpr * a.batch), tpb, 0, s>>>(a, bpr);
+    const unsigned grid = (unsigned)((long long)bpr * a.batch);
+    if (a.colour == 0) launch_pdl(ising_bits_kernel<0>, grid, (unsigned)tpb, s, a, bpr);
+    else launch_pdl(ising_bits_kernel<1>, grid, (unsigned)tpb, s, a, bpr);
     return 1;
 }
 
