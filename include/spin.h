@@ -155,6 +155,15 @@ SPIN_API int64_t spin_kernel_launches(const spin_sim* sim);
 /* Human-readable name of the sweep kernel variant the handle selects for its shape (diagnostics). */
 SPIN_API const char* spin_kernel_variant(const spin_sim* sim);
 
+/* Kernel selection policy (diagnostics / tests; the results never depend on it: every path computes the same
+ * lattice).  SPIN_POLICY_AUTO picks per shape; SPIN_POLICY_STREAMING forces the two-launches-
+ * per-sweep HBM kernels; SPIN_POLICY_RESIDENT uses the shared-memory-resident multi-sweep kernel (one CTA per
+ * replica, all sweeps of a call in one launch, E / M reductions fused) whenever the shape allows it (Ising, int8
+ * layout, L a multiple of 32, L*L <= 192 KiB) and falls back to streaming otherwise.
+ * Returns SPIN_OK or SPIN_ERR_INVALID (NULL handle, unknown policy). */
+enum { SPIN_POLICY_AUTO = 0, SPIN_POLICY_STREAMING = 1, SPIN_POLICY_RESIDENT = 2 };
+SPIN_API int spin_set_policy(spin_sim* sim, int32_t policy);
+
 #ifdef __cplusplus
 }
 #endif

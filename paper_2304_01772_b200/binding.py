@@ -11,10 +11,12 @@ from . import build as _build
 SPIN_OK, SPIN_ERR_INVALID, SPIN_ERR_NOMEM, SPIN_ERR_CUDA, SPIN_ERR_UNSUPPORTED = 0, -1, -2, -3, -4
 SPIN_MODEL_ISING, SPIN_MODEL_POTTS = 0, 1
 SPIN_LAYOUT_INT8, SPIN_LAYOUT_BITPACKED = 0, 1
+SPIN_POLICY_AUTO, SPIN_POLICY_STREAMING, SPIN_POLICY_RESIDENT = 0, 1, 2
 
 __all__ = [
     "SPIN_OK", "SPIN_ERR_INVALID", "SPIN_ERR_NOMEM", "SPIN_ERR_CUDA", "SPIN_ERR_UNSUPPORTED",
     "SPIN_MODEL_ISING", "SPIN_MODEL_POTTS", "SPIN_LAYOUT_INT8", "SPIN_LAYOUT_BITPACKED",
+    "SPIN_POLICY_AUTO", "SPIN_POLICY_STREAMING", "SPIN_POLICY_RESIDENT",
     "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim",
     "spin_create", "spin_create_ex",
 ]
@@ -56,6 +58,7 @@ def load_library():
         "spin_threshold_table": (c.c_int, [i32, dbl, dbl, dbl, vp, vp]),
         "spin_kernel_launches": (i64, [vp]),
         "spin_kernel_variant": (c.c_char_p, [vp]),
+        "spin_set_policy": (c.c_int, [vp, i32]),
     }
     for name, (res, args) in protos.items():
         fn = getattr(lib, name)
@@ -69,7 +72,7 @@ EXPORTED_SYMBOLS = (
     "spin_create", "spin_sweep", "spin_observables", "spin_destroy", "spin_last_error", "spin_buffer_bytes",
     "spin_create_ex", "spin_set_stream", "spin_get_spins", "spin_set_spins", "spin_sweep_measure",
     "spin_observables_dev", "spin_synchronize", "spin_threshold_table", "spin_kernel_launches",
-    "spin_kernel_variant",
+    "spin_kernel_variant", "spin_set_policy",
 )
 
 
@@ -161,6 +164,9 @@ class SpinSim:
 
     def spin_kernel_launches(self):
         return int(load_library().spin_kernel_launches(self._h))
+
+    def spin_set_policy(self, policy):
+        _check(load_library().spin_set_policy(self._h, int(policy)))
 
     def spin_kernel_variant(self):
         return load_library().spin_kernel_variant(self._h).decode()

@@ -110,8 +110,8 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t t, const 
 // kParity = 1: the side neighbour of site k is other[i][k+1], else other[i][k-1]; `edge` is the masked 32-bit
 // word holding the 17th byte (next strip's first word, or previous strip's last word).
 template <bool kHasNever, int kParity>
-__device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const uint4& um, const uint4& cm,
-                                            const uint4& dm, uint32_t edge, uint32_t g0, uint32_t c1,
+__device__ __forceinline__ uint4 update_row(const RoundKeys& rk, uint32_t c2, uint32_t c3, uint4 own, const uint4& um,
+                                            const uint4& cm, const uint4& dm, uint32_t edge, uint32_t g0, uint32_t c1,
                                             const uint32_t* stab, uint32_t slot) {
     uint32_t s0, s1, s2, s3;
     if (kParity) {
@@ -131,10 +131,10 @@ __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const
     const uint32_t t2 = (um.z + cm.z + dm.z) + s2 + (own.z & kOwn);
     const uint32_t t3 = (um.w + cm.w + dm.w) + s3 + (own.w & kOwn);
     uint32_t r0[4], r1[4], r2[4], r3[4];
-    philox4x32_10(a.rk, g0 + 0, c1, a.c2, a.c3, r0);
-    philox4x32_10(a.rk, g0 + 1, c1, a.c2, a.c3, r1);
-    philox4x32_10(a.rk, g0 + 2, c1, a.c2, a.c3, r2);
-    philox4x32_10(a.rk, g0 + 3, c1, a.c2, a.c3, r3);
+    philox4x32_10(rk, g0 + 0, c1, c2, c3, r0);
+    philox4x32_10(rk, g0 + 1, c1, c2, c3, r1);
+    philox4x32_10(rk, g0 + 2, c1, c2, c3, r2);
+    philox4x32_10(rk, g0 + 3, c1, c2, c3, r3);
     uint4 res;
     res.x = update_word<kHasNever, 0>(own.x, t0, r0, stab, slot);
     res.y = update_word<kHasNever, 1>(own.y, t1, r1, stab, slot);
@@ -188,7 +188,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
         const uint4 n1 = __ldg(more ? pOth : pOthLast);
         const uint4 own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
-        uint4 res = update_row<kHasNever, kColour>(a, own, wU, wC, wD, edge, g0, c1, stab, slot);
+        uint4 res = update_row<kHasNever, kColour>(a.rk, a.c2, a.c3, own, wU, wC, wD, edge, g0, c1, stab, slot);
         *pOwn = res;
         // inputs of the next even row i+2: other-colour row i+3, own row i+2, its edge word
         uint4 n2 = n1, own2 = own1;
@@ -199,8 +199,8 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             edge2 = __ldg(pEdgeEven + edgeStride2);
         }
         const uint4 n1m = mask4(n1);
-        res = update_row<kHasNever, 1 - kColour>(a, own1, wC, wD, n1m, edge1 & 0x04040404u, g0 + (uint32_t)W4, c1, stab,
-                                                 slot);
+        res = update_row<kHasNever, 1 - kColour>(a.rk, a.c2, a.c3, own1, wC, wD, n1m, edge1 & 0x04040404u,
+                                                 g0 + (uint32_t)W4, c1, stab, slot);
         *(pOwn + rowStride) = res;
         wU = wD;
         wC = n1m;
@@ -234,6 +234,145 @@ __global__ void __launch_bounds__(kRowsThreads, 1) ising_int8_rows_kernel(SweepA
     else march_rows<kColour, false>(a, stab, slot, b, rb, x);
 }
 
+// ---- shared-memory-resident kernel: L % 32 == 0 and the replica (L^2 bytes) fits one CTA's shared memory.
+// One CTA per replica runs every sweep of the call: both colours stay in shared memory, the half-sweeps are
+// separated by __syncthreads() (a colour only reads the other colour), the Philox counter words of sweep t are
+// formed in the kernel, and after each sweep the exact E_int and M of the replica are reduced from shared memory
+// (same byte-SIMD bond count as observe.cu), written to the traces and accumulated into the moments by thread 0.
+// Per row strip the work is the same update_row as the HBM kernel.
+constexpr int kResThreads = 256;
+constexpr size_t kResMaxLatticeBytes = 196608;   // 3 CTAs of L = 256 per SM; one CTA up to L = 416
+
+__device__ __forceinline__ int block_sum(int v, int* scratch) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __syncthreads();                       // scratch may still be read from the previous call
+    if (lane == 0) scratch[w] = v;
+    __syncthreads();
+    int t = 0;
+    const int nw = (blockDim.x + 31) >> 5;
+    for (int k = 0; k < nw; ++k) t += scratch[k];
+    return t;
+}
+
+// Rows of one parity at a time: the side of the horizontal neighbour depends on (row + colour) & 1, and a warp spans
+// several rows when L/32 < 32, so mixing parities in one pass would make every warp execute both variants.
+template <bool kHasNever, int kParity>
+__device__ __forceinline__ void resident_rows(const ResidentArgs& a, int colour, uint32_t c2, uint32_t c3, uint8_t* lat,
+                                              const uint32_t* stab, uint32_t slot, uint32_t c1) {
+    const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
+    uint4* own4 = (uint4*)(lat + (size_t)colour * L * W);
+    const uint4* oth4 = (const uint4*)(lat + (size_t)(1 - colour) * L * W);
+    const uint32_t* oth1 = (const uint32_t*)oth4;
+    const int rowPar = (kParity + colour) & 1;                  // rows i with (i + colour) & 1 == kParity
+    const int units = (L >> 1) * W16;
+    for (int v = threadIdx.x; v < units; v += blockDim.x) {
+        const int ih = v / W16, x = v - ih * W16;
+        const int i = 2 * ih + rowPar, u = i * W16 + x;
+        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+        const uint4 um = mask4(oth4[iu * W16 + x]), cm = mask4(oth4[u]), dm = mask4(oth4[id * W16 + x]);
+        const uint4 own = own4[u];
+        const uint32_t g0 = (uint32_t)u * 4u;                   // (i * W + 16 x) >> 2
+        const int ew = kParity ? ((x == W16 - 1) ? 0 : 4 * x + 4) : ((x == 0) ? W4 - 1 : 4 * x - 1);
+        const uint32_t edge = oth1[i * W4 + ew] & 0x04040404u;
+        own4[u] = update_row<kHasNever, kParity>(a.rk, c2, c3, own, um, cm, dm, edge, g0, c1, stab, slot);
+    }
+}
+
+template <bool kHasNever>
+__device__ __forceinline__ void resident_half_sweep(const ResidentArgs& a, int colour, uint32_t c2, uint32_t c3,
+                                                    uint8_t* lat, const uint32_t* stab, uint32_t slot, uint32_t c1) {
+    resident_rows<kHasNever, 0>(a, colour, c2, c3, lat, stab, slot, c1);
+    resident_rows<kHasNever, 1>(a, colour, c2, c3, lat, stab, slot, c1);
+}
+
+__global__ void __launch_bounds__(kResThreads) ising_int8_resident_kernel(ResidentArgs a) {
+    extern __shared__ __align__(16) uint8_t smem[];
+    const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
+    const size_t latBytes = (size_t)L * L;
+    uint8_t* lat = smem;
+    uint32_t* stab = (uint32_t*)(smem + latBytes);
+    uint32_t* sidx = stab + kTableStride;                       // per-thread slots, word j of thread t at [j * 256 + t]
+    int* scratch = (int*)(sidx + 4 * kResThreads);
+    const int b = blockIdx.x;
+    uint4* g4 = (uint4*)((uint8_t*)a.lattice + (size_t)b * latBytes);
+    for (int k = threadIdx.x; k < (int)(latBytes >> 4); k += blockDim.x) ((uint4*)lat)[k] = g4[k];
+    for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
+    __syncthreads();
+    // update_word addresses word j of a thread at slot + j * 128 words: one 512-word region per 128 threads
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[(threadIdx.x >> 7) * 512 + (threadIdx.x & 127)]);
+    const uint32_t c1 = (uint32_t)b + a.replica_offset;
+    const bool never = stab[kTabNever] != 0u;
+    long long mom[8];
+    if (a.moments && threadIdx.x == 0)
+        for (int k = 0; k < 8; ++k) mom[k] = a.moments[(size_t)b * 8 + k];
+    for (long long s = 0; s < a.n_sweeps; ++s) {
+        const unsigned long long t = a.t0 + (unsigned long long)s;
+        const uint32_t c2 = (uint32_t)(t & 0xFFFFFFFFull);
+        const uint32_t c3lo = (uint32_t)((t >> 32) & 0xFFFFFFull) | (kDomainIsing << 28);
+        for (int colour = 0; colour < 2; ++colour) {
+            const uint32_t c3 = c3lo | ((uint32_t)colour << 24);
+            if (never) resident_half_sweep<true>(a, colour, c2, c3, lat, stab, slot, c1);
+            else resident_half_sweep<false>(a, colour, c2, c3, lat, stab, slot, c1);
+            __syncthreads();
+        }
+        if (a.measure) {
+            // exact E_int = -(bonds equal - bonds different) from the colour-0 sites, M = sites - 2 * (#spins -1)
+            const uint4* c0 = (const uint4*)lat;
+            const uint4* c1p = (const uint4*)(lat + (size_t)L * W);
+            const uint32_t* c1w = (const uint32_t*)c1p;
+            int diff = 0, neg = 0;
+            const uint32_t m2 = 0x02020202u, m8 = 0x80808080u;
+            for (int u = threadIdx.x; u < L * W16; u += blockDim.x) {
+                const int i = u / W16, x = u - i * W16;
+                const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+                const uint4 own = c0[u], ct = c1p[u], up = c1p[iu * W16 + x], dn = c1p[id * W16 + x];
+                uint32_t s0, s1, s2, s3;
+                if (i & 1) {
+                    const uint32_t e = c1w[i * W4 + (x == W16 - 1 ? 0 : 4 * x + 4)];
+                    s0 = __byte_perm(ct.x, ct.y, 0x4321); s1 = __byte_perm(ct.y, ct.z, 0x4321);
+                    s2 = __byte_perm(ct.z, ct.w, 0x4321); s3 = __byte_perm(ct.w, e, 0x4321);
+                } else {
+                    const uint32_t e = c1w[i * W4 + (x == 0 ? W4 - 1 : 4 * x - 1)];
+                    s0 = __byte_perm(e, ct.x, 0x6543); s1 = __byte_perm(ct.x, ct.y, 0x6543);
+                    s2 = __byte_perm(ct.y, ct.z, 0x6543); s3 = __byte_perm(ct.z, ct.w, 0x6543);
+                }
+                diff += __popc((own.x ^ up.x) & m2) + __popc((own.x ^ dn.x) & m2) + __popc((own.x ^ ct.x) & m2) + __popc((own.x ^ s0) & m2);
+                diff += __popc((own.y ^ up.y) & m2) + __popc((own.y ^ dn.y) & m2) + __popc((own.y ^ ct.y) & m2) + __popc((own.y ^ s1) & m2);
+                diff += __popc((own.z ^ up.z) & m2) + __popc((own.z ^ dn.z) & m2) + __popc((own.z ^ ct.z) & m2) + __popc((own.z ^ s2) & m2);
+                diff += __popc((own.w ^ up.w) & m2) + __popc((own.w ^ dn.w) & m2) + __popc((own.w ^ ct.w) & m2) + __popc((own.w ^ s3) & m2);
+                neg += __popc(own.x & m8) + __popc(own.y & m8) + __popc(own.z & m8) + __popc(own.w & m8);
+                neg += __popc(ct.x & m8) + __popc(ct.y & m8) + __popc(ct.z & m8) + __popc(ct.w & m8);
+            }
+            diff = block_sum(diff, scratch);
+            neg = block_sum(neg, scratch);
+            if (threadIdx.x == 0) {
+                const long long N = (long long)L * L;
+                const long long e = -(2 * N - 2 * (long long)diff), mag = N - 2 * (long long)neg;
+                if (a.E_trace) a.E_trace[(size_t)s * a.batch + b] = e;
+                if (a.M_trace) a.M_trace[(size_t)s * a.batch + b] = mag;
+                if (a.moments) {
+                    const unsigned long long ae = e < 0 ? (unsigned long long)(-e) : (unsigned long long)e;
+                    const unsigned long long lo = ae * ae, hi = __umul64hi(ae, ae);
+                    const unsigned long long old_lo = (unsigned long long)mom[2], new_lo = old_lo + lo;
+                    mom[0] += 1;
+                    mom[1] += e;
+                    mom[2] = (long long)new_lo;
+                    mom[3] = (long long)((unsigned long long)mom[3] + hi + (new_lo < old_lo ? 1ull : 0ull));
+                    mom[4] += mag;
+                    mom[5] += mag < 0 ? -mag : mag;
+                    mom[6] += mag * mag;
+                    mom[7] += e * mag;
+                }
+            }
+        }
+    }
+    if (a.moments && threadIdx.x == 0)
+        for (int k = 0; k < 8; ++k) a.moments[(size_t)b * 8 + k] = mom[k];
+    for (int k = threadIdx.x; k < (int)(latBytes >> 4); k += blockDim.x) g4[k] = ((uint4*)lat)[k];
+}
+
 }  // namespace
 
 const char* ising_int8_variant(int L) { return (L % 32 == 0) ? "ising_int8_rows128" : "ising_int8_generic"; }
@@ -252,6 +391,31 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
         const long long total = ((half + 3) >> 2) * a.batch;
         ising_int8_generic_kernel<<<(unsigned)((total + 127) / 128), 128, 0, s>>>(a);
     }
+    return 1;
+}
+
+}  // namespace spin
+
+namespace spin {
+
+static size_t resident_smem_bytes(int L) {
+    return (size_t)L * L + sizeof(uint32_t) * (kTableStride + 4 * kResThreads) + sizeof(int) * 32;
+}
+
+bool ising_int8_resident_fits(int L) { return L % 32 == 0 && (size_t)L * L <= kResMaxLatticeBytes; }
+
+int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s) {
+    const size_t smem = resident_smem_bytes(a.L);
+    static bool configured = false;
+    if (!configured) {
+        cudaFuncSetAttribute(ising_int8_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(kResMaxLatticeBytes + sizeof(uint32_t) * (kTableStride + 4 * kResThreads) + 128));
+        configured = true;
+    }
+    const int units = a.L * (a.L >> 5);
+    int tpb = kResThreads;
+    while (tpb > 32 && tpb / 2 >= units) tpb >>= 1;           // L = 32: 32 strips -> one warp
+    ising_int8_resident_kernel<<<(unsigned)a.batch, tpb, smem, s>>>(a);
     return 1;
 }
 

@@ -61,6 +61,47 @@ __global__ void ising_int8_observe_kernel(const int8_t* __restrict__ lat, int L,
     block_add2(e, m, E_acc ? E_acc + b : nullptr, M_acc ? M_acc + b : nullptr);
 }
 
+// Ising int8, L % 32 == 0: one thread per 16-site strip of a colour-0 row, 128-bit loads, byte-SIMD.
+// For +-1 bytes own ^ nbr is 0x00 (equal) or 0xFE (different): s * nbr summed over a strip and its 4 neighbours is
+// 64 - 2 * #different; the number of -1 spins of a word is popc(word & 0x80808080).
+__global__ void __launch_bounds__(256) ising_int8_observe_vec_kernel(const int8_t* __restrict__ lat, int L, int bpr,
+                                                                     long long* E_acc, long long* M_acc) {
+    const int W = L >> 1, W16 = W >> 4, W4 = W >> 2;
+    const int b = blockIdx.x / bpr, blk = blockIdx.x - b * bpr;
+    const size_t half = (size_t)L * W;
+    const uint4* c0 = (const uint4*)(lat + (size_t)b * 2 * half);
+    const uint4* c1 = (const uint4*)(lat + (size_t)b * 2 * half + half);
+    const uint32_t* c1w = (const uint32_t*)c1;
+    const int strips = L * W16;
+    int diff = 0, neg = 0, cnt = 0;
+    for (int n = blk * blockDim.x + threadIdx.x; n < strips; n += bpr * blockDim.x) {
+        const int i = n / W16, x = n - i * W16;
+        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+        const uint4 own = __ldg(c0 + n), ct = __ldg(c1 + n);
+        const uint4 up = __ldg(c1 + (size_t)iu * W16 + x), dn = __ldg(c1 + (size_t)id * W16 + x);
+        uint32_t s0, s1, s2, s3;
+        if (i & 1) {                                           // colour 0: side neighbour is other[i][k+1] on odd rows
+            const uint32_t e = __ldg(c1w + (size_t)i * W4 + (x == W16 - 1 ? 0 : 4 * x + 4));
+            s0 = __byte_perm(ct.x, ct.y, 0x4321); s1 = __byte_perm(ct.y, ct.z, 0x4321);
+            s2 = __byte_perm(ct.z, ct.w, 0x4321); s3 = __byte_perm(ct.w, e, 0x4321);
+        } else {
+            const uint32_t e = __ldg(c1w + (size_t)i * W4 + (x == 0 ? W4 - 1 : 4 * x - 1));
+            s0 = __byte_perm(e, ct.x, 0x6543); s1 = __byte_perm(ct.x, ct.y, 0x6543);
+            s2 = __byte_perm(ct.y, ct.z, 0x6543); s3 = __byte_perm(ct.z, ct.w, 0x6543);
+        }
+        const uint32_t m2 = 0x02020202u, m8 = 0x80808080u;
+        diff += __popc((own.x ^ up.x) & m2) + __popc((own.x ^ dn.x) & m2) + __popc((own.x ^ ct.x) & m2) + __popc((own.x ^ s0) & m2);
+        diff += __popc((own.y ^ up.y) & m2) + __popc((own.y ^ dn.y) & m2) + __popc((own.y ^ ct.y) & m2) + __popc((own.y ^ s1) & m2);
+        diff += __popc((own.z ^ up.z) & m2) + __popc((own.z ^ dn.z) & m2) + __popc((own.z ^ ct.z) & m2) + __popc((own.z ^ s2) & m2);
+        diff += __popc((own.w ^ up.w) & m2) + __popc((own.w ^ dn.w) & m2) + __popc((own.w ^ ct.w) & m2) + __popc((own.w ^ s3) & m2);
+        neg += __popc(own.x & m8) + __popc(own.y & m8) + __popc(own.z & m8) + __popc(own.w & m8);
+        neg += __popc(ct.x & m8) + __popc(ct.y & m8) + __popc(ct.z & m8) + __popc(ct.w & m8);
+        ++cnt;
+    }
+    // per strip: 16 sites x 4 bonds, and 32 spins (both colours)
+    block_add2(-(64 * cnt - 2 * diff), 32 * cnt - 2 * neg, E_acc ? E_acc + b : nullptr, M_acc ? M_acc + b : nullptr);
+}
+
 __global__ void ising_bits_observe_kernel(const uint32_t* __restrict__ lat, int L, int bpr, long long* E_acc,
                                           long long* M_acc) {
     const int WW = L >> 6;
@@ -159,6 +200,12 @@ inline int blocks_per_replica(long long items, int tpb, int batch) {
 }  // namespace
 
 int launch_ising_int8_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s) {
+    if (L % 32 == 0) {
+        const long long strips = (long long)L * (L >> 5);
+        const int tpb = 256, bpr = blocks_per_replica(strips, tpb, batch);
+        ising_int8_observe_vec_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const int8_t*)lattice, L, bpr, E_acc, M_acc);
+        return 1;
+    }
     const long long half = (long long)L * (L >> 1);
     const int tpb = 256, bpr = blocks_per_replica(half, tpb, batch);
     ising_int8_observe_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const int8_t*)lattice, L, bpr, E_acc, M_acc);

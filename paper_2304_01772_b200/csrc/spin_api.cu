@@ -101,6 +101,7 @@ struct spin_sim {
     uint32_t* h_tables = nullptr;
     RoundKeys rk;
     int64_t launches = 0;
+    int32_t policy = SPIN_POLICY_AUTO;
 };
 
 namespace {
@@ -170,6 +171,35 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     a.colour = colour;
     a.rk = sim->rk;
     return a;
+}
+
+// Shared-memory-resident path (ising_int8.cu): Ising, int8 layout, replica fits one CTA.  AUTO uses it when the
+// batch gives every SM work (or when the lattice is so small that the streaming kernels are launch-bound anyway).
+bool use_resident(const spin_sim* sim, bool measure) {
+    if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || !ising_int8_resident_fits(sim->L)) return false;
+    if (sim->policy == SPIN_POLICY_STREAMING) return false;
+    if (sim->policy == SPIN_POLICY_RESIDENT) return true;
+    const long long sites = (long long)sim->batch * sim->L * sim->L;
+    if (sites <= (1ll << 20)) return true;                         // launch-latency-bound shapes
+    return measure && sim->batch >= 296;                           // fused per-sweep reductions, >= 2 CTAs per SM
+}
+
+void enqueue_resident(spin_sim* sim, int64_t t0, int64_t n_sweeps, bool measure, long long* E_trace, long long* M_trace,
+                      long long* moments) {
+    ResidentArgs a;
+    a.lattice = sim->lattice;
+    a.tables = sim->d_tables;
+    a.batch = sim->batch;
+    a.L = sim->L;
+    a.replica_offset = sim->replica_offset;
+    a.measure = measure ? 1u : 0u;
+    a.t0 = (unsigned long long)t0;
+    a.n_sweeps = n_sweeps;
+    a.E_trace = E_trace;
+    a.M_trace = M_trace;
+    a.moments = moments;
+    a.rk = sim->rk;
+    sim->launches += launch_ising_int8_resident(a, sim->stream);
 }
 
 void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour) {
@@ -362,8 +392,17 @@ int64_t spin_kernel_launches(const spin_sim* sim) { return sim ? sim->launches :
 const char* spin_kernel_variant(const spin_sim* sim) {
     if (!sim) return "";
     if (sim->model == SPIN_MODEL_POTTS) return potts_int8_variant(sim->L);
-    if (sim->layout == SPIN_LAYOUT_BITPACKED) return "ising_bits_word32";
+    if (sim->layout == SPIN_LAYOUT_BITPACKED) return "ising_bits_rows32";
+    if (use_resident(sim, false)) return "ising_int8_resident";
     return ising_int8_variant(sim->L);
+}
+
+int spin_set_policy(spin_sim* sim, int32_t policy) {
+    if (!sim) return fail(SPIN_ERR_INVALID, "spin_set_policy: NULL handle");
+    if (policy != SPIN_POLICY_AUTO && policy != SPIN_POLICY_STREAMING && policy != SPIN_POLICY_RESIDENT)
+        return fail(SPIN_ERR_INVALID, "spin_set_policy: unknown policy %d", (int)policy);
+    sim->policy = policy;
+    return SPIN_OK;
 }
 
 int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_sweeps, int64_t sweep_offset) {
@@ -373,9 +412,13 @@ int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_
     CUDA_TRY(cudaSetDevice(sim->device));
     const int rt = upload_tables(sim, beta, J, h);
     if (rt != SPIN_OK) return rt;
-    for (int64_t t = sweep_offset; t < sweep_offset + n_sweeps; ++t) {
-        enqueue_half_sweep(sim, t, 0);
-        enqueue_half_sweep(sim, t, 1);
+    if (use_resident(sim, false)) {
+        enqueue_resident(sim, sweep_offset, n_sweeps, false, nullptr, nullptr, nullptr);
+    } else {
+        for (int64_t t = sweep_offset; t < sweep_offset + n_sweeps; ++t) {
+            enqueue_half_sweep(sim, t, 0);
+            enqueue_half_sweep(sim, t, 1);
+        }
     }
     CUDA_TRY(cudaGetLastError());
     return SPIN_OK;
@@ -466,7 +509,9 @@ int spin_sweep_measure(spin_sim* sim, const double* beta, double J, double h, in
             e = cudaMemcpyAsync(d_mom, moments, sizeof(long long) * 8 * B, cudaMemcpyHostToDevice, sim->stream);
             if (e != cudaSuccess) { result = cuda_fail(e, "copy moments"); break; }
         }
-        for (int64_t local = 0; local < n_sweeps && result == SPIN_OK; ++local) {
+        if (use_resident(sim, true))
+            enqueue_resident(sim, sweep_offset, n_sweeps, true, d_trace, d_trace + trace_elems, d_mom);
+        else for (int64_t local = 0; local < n_sweeps && result == SPIN_OK; ++local) {
             const int64_t t = sweep_offset + local;
             enqueue_half_sweep(sim, t, 0);
             enqueue_half_sweep(sim, t, 1);

@@ -61,6 +61,23 @@ struct SweepArgs {
     RoundKeys rk;
 };
 
+// Shared-memory-resident multi-sweep kernel (small lattices: one CTA holds a whole replica and runs all sweeps of a
+// call in one launch, with the per-sweep E / M reductions and the moment accumulation fused in).
+struct ResidentArgs {
+    void* lattice;            // int8: [B][2][L][L/2]
+    const uint32_t* tables;   // [B][kTableStride]
+    int32_t batch;
+    int32_t L;
+    uint32_t replica_offset;
+    uint32_t measure;         // 1: reduce E, M after every sweep
+    unsigned long long t0;    // first sweep index
+    long long n_sweeps;
+    long long* E_trace;       // device [n_sweeps][B] or nullptr
+    long long* M_trace;       // device [n_sweeps][B] or nullptr
+    long long* moments;       // device [B][8] in/out or nullptr
+    RoundKeys rk;
+};
+
 struct InitArgs {
     void* lattice;
     const int32_t* q;         // [B] (Potts) or nullptr
@@ -101,6 +118,8 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s);      // pi
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s);
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s);
 const char* ising_int8_variant(int L);
+bool ising_int8_resident_fits(int L);                                       // a replica fits one CTA's shared memory
+int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s);      // all n_sweeps in one launch
 const char* potts_int8_variant(int L);
 
 // Observables: accumulate into E_acc[b], M_acc[b] (int64, must be zero on entry; Potts uses hist).

@@ -17,9 +17,17 @@ def _layout(name):
     return sp.SPIN_LAYOUT_BITPACKED if name == "bits" else sp.SPIN_LAYOUT_INT8
 
 
-def _mk_ising(batch, L, seed, layout="int8", replica_offset=0):
-    return sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed, layout=_layout(layout),
-                             replica_offset=replica_offset)
+def _mk_ising(batch, L, seed, layout="int8", replica_offset=0, policy=None):
+    sim = sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed, layout=_layout(layout),
+                            replica_offset=replica_offset)
+    if policy is not None:
+        sim.spin_set_policy(policy)
+    return sim
+
+
+# every int8 Ising case runs through both kernel families: the two-launches-per-sweep HBM kernels and the
+# shared-memory-resident multi-sweep kernel (used when the shape allows it, else it falls back to streaming)
+POLICIES = [sp.SPIN_POLICY_STREAMING, sp.SPIN_POLICY_RESIDENT]
 
 
 def _mk_potts(batch, L, q, seed, replica_offset=0):
@@ -82,11 +90,16 @@ ISING_CASES = [
 ]
 
 
+@pytest.mark.parametrize("policy", POLICIES)
 @pytest.mark.parametrize("L,batch,layout,J,h,betas", ISING_CASES)
-def test_ising_sweeps_match_oracle_every_sweep(oracle_mod, L, batch, layout, J, h, betas):
+def test_ising_sweeps_match_oracle_every_sweep(oracle_mod, L, batch, layout, J, h, betas, policy):
+    if layout == "bits" and policy == sp.SPIN_POLICY_RESIDENT:
+        pytest.skip("the resident kernel is int8 only; bits always stream")
     seed, n = 100 + L, 12
     ref = oracle_mod.init(batch, L, seed=seed)
-    with _mk_ising(batch, L, seed=seed, layout=layout) as sim:
+    with _mk_ising(batch, L, seed=seed, layout=layout, policy=policy) as sim:
+        if policy == sp.SPIN_POLICY_RESIDENT and L % 32 == 0:
+            assert sim.spin_kernel_variant() == "ising_int8_resident"
         for t in range(n):
             sim.spin_sweep(betas, J, h, 1, t)
             oracle_mod.sweep(ref, betas, J, h, seed=seed, n_sweeps=1, sweep_offset=t)
@@ -185,19 +198,39 @@ def test_potts_negative_J_and_field_rejected(oracle_mod):
 
 
 # ----------------------------------------------------------------------------------------- measurements
-def test_sweep_measure_trace_and_moments(oracle_mod):
-    L, seed, n = 32, 1, 40
+@pytest.mark.parametrize("policy", POLICIES)
+@pytest.mark.parametrize("L", [32, 96, 256])
+def test_sweep_measure_trace_and_moments(oracle_mod, policy, L):
+    seed, n = 1, 40
     beta = [0.3, 0.44, 0.5, 0.6]
     ref = oracle_mod.init(4, L, seed=seed)
     mom_o = np.zeros((4, 8), dtype=np.int64)
     Eo, Mo = oracle_mod.sweep(ref, beta, 1.0, 0.05, seed=seed, n_sweeps=n, trace=True, moments=mom_o)
-    with _mk_ising(4, L, seed=seed) as sim:
+    with _mk_ising(4, L, seed=seed, policy=policy) as sim:
         mom = np.zeros((4, 8), dtype=np.int64)
         E1, M1 = sim.spin_sweep_measure(beta, 1.0, 0.05, 15, 0, moments=mom)
         E2, M2 = sim.spin_sweep_measure(beta, 1.0, 0.05, n - 15, 15, moments=mom)   # moments are in/out
         assert np.array_equal(np.vstack([E1, E2]), Eo) and np.array_equal(np.vstack([M1, M2]), Mo)
         assert np.array_equal(mom, mom_o)
         assert np.array_equal(sim.spin_get_spins(), ref)
+
+
+def test_resident_multi_sweep_call_equals_streaming(oracle_mod):
+    """One resident launch for 25 sweeps (t crossing 2^32, beta = 20 never-classes, odd batch) == streaming == oracle."""
+    L, seed, off = 64, 77, (1 << 32) - 10
+    beta = [0.2, 0.4407, 20.0, 0.6, 0.0]
+    ref = oracle_mod.init(5, L, seed=seed, replica_offset=3)
+    oracle_mod.sweep(ref, beta, 1.0, 0.01, seed=seed, n_sweeps=25, sweep_offset=off, replica_offset=3)
+    for policy in POLICIES:
+        with _mk_ising(5, L, seed=seed, replica_offset=3, policy=policy) as sim:
+            sim.spin_sweep(beta, 1.0, 0.01, 25, off)
+            assert np.array_equal(sim.spin_get_spins(), ref)
+            with pytest.raises(sp.SpinError):
+                sim.spin_set_policy(7)
+
+
+def test_sweep_measure_potts(oracle_mod):
+    seed = 1
     q = [3, 8]
     ref = oracle_mod.init(2, 16, seed=seed, q=q)
     mom_o = np.zeros((2, 8), dtype=np.int64)
