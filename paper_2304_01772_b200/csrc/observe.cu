@@ -157,6 +157,88 @@ __global__ void potts_int8_observe_kernel(const uint8_t* __restrict__ lat, int L
     block_add2(e, 0, E_acc ? E_acc + b : nullptr, nullptr);
 }
 
+// Potts uint8, L % 32 == 0: one thread per 16-site strip of a colour-0 row (128-bit loads, byte-SIMD).  States are
+// < 128, so bit 7 of (a ^ b) + 0x7F is "a != b" per byte.  The histogram is counted in registers by comparing whole
+// words with each state when q <= 8 (no shared-memory atomics on a handful of hot bins), else with shared atomics.
+__device__ __forceinline__ int neq_count(uint32_t a, uint32_t b) {
+    return __popc(((a ^ b) + 0x7F7F7F7Fu) & 0x80808080u);
+}
+
+__global__ void __launch_bounds__(256) potts_int8_observe_vec_kernel(const uint8_t* __restrict__ lat, int L, int bpr,
+                                                                     const int32_t* __restrict__ qv, long long* E_acc,
+                                                                     unsigned int* hist) {
+    __shared__ unsigned int sh[128];
+    const int W = L >> 1, W16 = W >> 4, W4 = W >> 2;
+    const int b = blockIdx.x / bpr, blk = blockIdx.x - b * bpr;
+    const size_t half = (size_t)L * W;
+    const uint4* c0 = (const uint4*)(lat + (size_t)b * 2 * half);
+    const uint4* c1 = (const uint4*)(lat + (size_t)b * 2 * half + half);
+    const uint32_t* c1w = (const uint32_t*)c1;
+    const int q = qv[b];
+    const bool small = q <= 8;
+    for (int t = threadIdx.x; t < 128; t += blockDim.x) sh[t] = 0u;
+    __syncthreads();
+    const int strips = L * W16;
+    int diff = 0, cnt = 0;
+    int hk[8] = {0, 0, 0, 0, 0, 0, 0, 0};                    // sites NOT in state k (q <= 8)
+    for (int n = blk * blockDim.x + threadIdx.x; n < strips; n += bpr * blockDim.x) {
+        const int i = n / W16, x = n - i * W16;
+        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+        const uint4 own = __ldg(c0 + n), ct = __ldg(c1 + n);
+        const uint4 up = __ldg(c1 + (size_t)iu * W16 + x), dn = __ldg(c1 + (size_t)id * W16 + x);
+        uint32_t s0, s1, s2, s3;
+        if (i & 1) {
+            const uint32_t e = __ldg(c1w + (size_t)i * W4 + (x == W16 - 1 ? 0 : 4 * x + 4));
+            s0 = __byte_perm(ct.x, ct.y, 0x4321); s1 = __byte_perm(ct.y, ct.z, 0x4321);
+            s2 = __byte_perm(ct.z, ct.w, 0x4321); s3 = __byte_perm(ct.w, e, 0x4321);
+        } else {
+            const uint32_t e = __ldg(c1w + (size_t)i * W4 + (x == 0 ? W4 - 1 : 4 * x - 1));
+            s0 = __byte_perm(e, ct.x, 0x6543); s1 = __byte_perm(ct.x, ct.y, 0x6543);
+            s2 = __byte_perm(ct.y, ct.z, 0x6543); s3 = __byte_perm(ct.z, ct.w, 0x6543);
+        }
+        diff += neq_count(own.x, up.x) + neq_count(own.x, dn.x) + neq_count(own.x, ct.x) + neq_count(own.x, s0);
+        diff += neq_count(own.y, up.y) + neq_count(own.y, dn.y) + neq_count(own.y, ct.y) + neq_count(own.y, s1);
+        diff += neq_count(own.z, up.z) + neq_count(own.z, dn.z) + neq_count(own.z, ct.z) + neq_count(own.z, s2);
+        diff += neq_count(own.w, up.w) + neq_count(own.w, dn.w) + neq_count(own.w, ct.w) + neq_count(own.w, s3);
+        ++cnt;
+        if (hist) {
+            const uint32_t w[8] = {own.x, own.y, own.z, own.w, ct.x, ct.y, ct.z, ct.w};
+            if (small) {
+#pragma unroll
+                for (int k = 0; k < 8; ++k) {
+                    if (k >= q) break;                        // block-uniform
+                    const uint32_t kk = 0x01010101u * (uint32_t)k;
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) hk[k] += neq_count(w[j], kk);
+                }
+            } else {
+#pragma unroll
+                for (int j = 0; j < 8; ++j) {
+                    atomicAdd(&sh[w[j] & 127u], 1u);
+                    atomicAdd(&sh[(w[j] >> 8) & 127u], 1u);
+                    atomicAdd(&sh[(w[j] >> 16) & 127u], 1u);
+                    atomicAdd(&sh[(w[j] >> 24) & 127u], 1u);
+                }
+            }
+        }
+    }
+    if (hist && small) {
+#pragma unroll
+        for (int k = 0; k < 8; ++k) {
+            int v = k < q ? 32 * cnt - hk[k] : 0;             // sites in state k
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
+            if ((threadIdx.x & 31) == 0 && v) atomicAdd(&sh[k], (unsigned int)v);
+        }
+    }
+    __syncthreads();
+    if (hist)
+        for (int t = threadIdx.x; t < 128; t += blockDim.x)
+            if (sh[t]) atomicAdd(&hist[(size_t)b * 128 + t], sh[t]);
+    // per strip: 16 sites x 4 bonds; E_int = -(#equal bonds)
+    block_add2(-(64 * cnt - diff), 0, E_acc ? E_acc + b : nullptr, nullptr);
+}
+
 __global__ void potts_finalize_kernel(unsigned int* hist, const int32_t* __restrict__ q, int batch, long long* M_out) {
     const int b = blockIdx.x * blockDim.x + threadIdx.x;
     if (b >= batch) return;
@@ -219,7 +301,14 @@ int launch_ising_bits_observe(const void* lattice, int batch, int L, long long* 
     return 1;
 }
 
-int launch_potts_int8_observe(const void* lattice, int batch, int L, long long* E_acc, unsigned int* hist, cudaStream_t s) {
+int launch_potts_int8_observe(const void* lattice, int batch, int L, const int32_t* q, long long* E_acc,
+                              unsigned int* hist, cudaStream_t s) {
+    if (L % 32 == 0) {
+        const long long strips = (long long)L * (L >> 5);
+        const int tpb = 256, bpr = blocks_per_replica(strips, tpb, batch);
+        potts_int8_observe_vec_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const uint8_t*)lattice, L, bpr, q, E_acc, hist);
+        return 1;
+    }
     const long long half = (long long)L * (L >> 1);
     const int tpb = 256, bpr = blocks_per_replica(half, tpb, batch);
     potts_int8_observe_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const uint8_t*)lattice, L, bpr, E_acc, hist);

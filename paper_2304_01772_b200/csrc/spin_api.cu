@@ -215,7 +215,7 @@ int enqueue_observe(spin_sim* sim, long long* E_out, long long* M_out) {
     const size_t nb = sizeof(long long) * (size_t)sim->batch;
     if (E_out) CUDA_TRY(cudaMemsetAsync(E_out, 0, nb, sim->stream));
     if (sim->model == SPIN_MODEL_POTTS) {
-        sim->launches += launch_potts_int8_observe(sim->lattice, sim->batch, sim->L, E_out, M_out ? sim->d_hist : nullptr, sim->stream);
+        sim->launches += launch_potts_int8_observe(sim->lattice, sim->batch, sim->L, sim->d_q, E_out, M_out ? sim->d_hist : nullptr, sim->stream);
         if (M_out) sim->launches += launch_potts_finalize(sim->d_hist, sim->d_q, sim->batch, M_out, sim->stream);
     } else {
         if (M_out) CUDA_TRY(cudaMemsetAsync(M_out, 0, nb, sim->stream));

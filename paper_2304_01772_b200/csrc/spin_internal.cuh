@@ -126,7 +126,7 @@ const char* potts_int8_variant(int L);
 int launch_ising_int8_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);
 int launch_ising_bits_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);
 // Potts: E_acc as above; hist: [B][128] uint32, zero on entry; M is produced by launch_potts_finalize.
-int launch_potts_int8_observe(const void* lattice, int batch, int L, long long* E_acc, unsigned int* hist, cudaStream_t s);
+int launch_potts_int8_observe(const void* lattice, int batch, int L, const int32_t* q, long long* E_acc, unsigned int* hist, cudaStream_t s);
 // M_out[b] = max_k hist[b][k], then hist is cleared for the next use.
 int launch_potts_finalize(unsigned int* hist, const int32_t* q, int batch, long long* M_out, cudaStream_t s);
 // moments[b][8] += sample (E[b], M[b])
