@@ -28,6 +28,9 @@ __device__ __forceinline__ int decode_class(int e, int nib) {
 
 constexpr int kRows = 8;
 constexpr int kThreads = 128;
+#ifndef BITS_MINB
+#define BITS_MINB 8
+#endif
 
 // One word = 32 sites = 8 Philox calls.  up / dn / ct: other-colour words of rows i-1, i+1, i; sd: the side
 // neighbours (ct shifted by one site, with the bit of the adjacent word).  stab[e][nibble] holds U for the class
@@ -124,7 +127,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t (*
 }
 
 template <int kColour>
-__global__ void __launch_bounds__(kThreads) ising_bits_kernel(SweepArgs a, int bpr) {
+__global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[4][16];
     __shared__ uint32_t snever[4];
     pdl_launch_dependents();

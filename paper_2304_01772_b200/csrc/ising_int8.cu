@@ -62,6 +62,9 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 // (about 540 instructions) stays resident in the instruction caches.  Launched with programmatic dependent launch:
 // the next half-sweep's blocks are scheduled while this one drains.
 constexpr int kRows = 8;
+#ifndef ISING_MINB
+#define ISING_MINB 7
+#endif
 constexpr int kRowsThreads = 128;
 
 template <int kOff>
@@ -217,7 +220,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 
 // One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
 template <int kColour>
-__global__ void __launch_bounds__(kRowsThreads, 1) ising_int8_rows_kernel(SweepArgs a, int bpr) {
+__global__ void __launch_bounds__(kRowsThreads, ISING_MINB) ising_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[kTableStride];
     __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
     pdl_launch_dependents();

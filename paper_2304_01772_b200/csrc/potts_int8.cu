@@ -56,7 +56,7 @@ __global__ void potts_int8_generic_kernel(SweepArgs a) {
 constexpr int kRows = 8;
 constexpr int kRowsThreads = 128;
 #ifndef POTTS_MINB
-#define POTTS_MINB 5
+#define POTTS_MINB 4
 #endif
 
 template <int kOff>
@@ -83,24 +83,37 @@ __device__ __forceinline__ uint32_t neq_bits(uint32_t v, uint32_t u, uint32_t d,
 
 // One site: threshold fetch (the index byte scales into the table address), compare, replace the byte by the proposal.
 template <bool kHasNever, int kE>
-__device__ __forceinline__ void site_step(uint32_t& own, uint32_t nw, uint32_t o, uint32_t r, const uint32_t* stab,
+__device__ __forceinline__ void site_step(uint32_t& acc_mask, uint32_t o, uint32_t r, const uint32_t* stab,
                                           const uint32_t* snever) {
     // two byte-addressed loads (no address arithmetic): pattern byte -> 4 * class -> U[class]
     const uint32_t c4 = ((const uint8_t*)(stab + 16))[o];
     bool acc = r <= *(const uint32_t*)((const char*)stab + c4);
     if (kHasNever) acc = acc && !((snever[0] >> (c4 >> 2)) & 1u);
-    if (acc) own = __byte_perm(own, nw, 0x3210 ^ ((0x4 + kE) << (4 * kE)) ^ (kE << (4 * kE)));
+    if (kHasNever) {
+        if (acc) acc_mask |= 0xFFu << (8 * kE);
+    } else {
+        // kept in PTX so that it stays one ISETP + one predicated two-input OR (issues at twice the PRMT rate)
+        asm("{\n\t.reg .pred p;\n\tsetp.ls.u32 p, %1, %2;\n\t@p or.b32 %0, %0, %3;\n\t}"
+            : "+r"(acc_mask) : "r"(r), "r"(*(const uint32_t*)((const char*)stab + c4)), "n"(0xFFu << (8 * kE)));
+    }
 }
 
 // One 4-site word: r0 feeds sites 0, 1 (proposal words r0[0], r0[2]; acceptance words r0[1], r0[3]), r1 sites 2, 3.
-template <bool kHasNever, int kJ>
+// floor(r (q-1) / 2^32): a shift when q-1 is a power of two (psh = 32 - log2(q-1)), else a multiply-high
+template <bool kPow2>
+__device__ __forceinline__ uint32_t propose(uint32_t r, uint32_t qm1, uint32_t psh) {
+    return kPow2 ? (r >> psh) : __umulhi(r, qm1);
+}
+
+template <bool kHasNever, bool kPow2, int kJ>
 __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t ct, uint32_t sd,
-                                                const uint32_t r0[4], const uint32_t r1[4], uint32_t q, uint32_t geAdd,
-                                                const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
+                                                const uint32_t r0[4], const uint32_t r1[4], uint32_t q, uint32_t psh,
+                                                uint32_t geAdd, const uint32_t* stab, const uint32_t* snever,
+                                                uint32_t slot) {
     // proposal (O6): new = old + 1 + floor(r_prop (q-1) / 2^32), minus q if >= q
     const uint32_t qm1 = q - 1u;
-    const uint32_t d = __umulhi(r0[0], qm1) | (__umulhi(r0[2], qm1) << 8) | (__umulhi(r1[0], qm1) << 16) |
-                       (__umulhi(r1[2], qm1) << 24);
+    const uint32_t d = propose<kPow2>(r0[0], qm1, psh) | (propose<kPow2>(r0[2], qm1, psh) << 8) |
+                       (propose<kPow2>(r1[0], qm1, psh) << 16) | (propose<kPow2>(r1[2], qm1, psh) << 24);
     uint32_t nw = own + 0x01010101u + d;                              // <= 2q-2 per byte
     const uint32_t ge = ((nw + geAdd) >> 7) & 0x01010101u;            // 1 where nw >= q (geAdd = (0x80 - q) per byte)
     nw -= ge * q;
@@ -112,19 +125,21 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
     const uint32_t o1 = slot_load_u8<kJ * kRowsThreads * 4 + 1>(slot);
     const uint32_t o2 = slot_load_u8<kJ * kRowsThreads * 4 + 2>(slot);
     const uint32_t o3 = slot_load_u8<kJ * kRowsThreads * 4 + 3>(slot);
-    site_step<kHasNever, 0>(own, nw, o0, r0[1], stab, snever);
-    site_step<kHasNever, 1>(own, nw, o1, r0[3], stab, snever);
-    site_step<kHasNever, 2>(own, nw, o2, r1[1], stab, snever);
-    site_step<kHasNever, 3>(own, nw, o3, r1[3], stab, snever);
-    return own;
+    uint32_t am = 0u;                                                 // 0xFF in the bytes whose proposal is accepted
+    site_step<kHasNever, 0>(am, o0, r0[1], stab, snever);
+    site_step<kHasNever, 1>(am, o1, r0[3], stab, snever);
+    site_step<kHasNever, 2>(am, o2, r1[1], stab, snever);
+    site_step<kHasNever, 3>(am, o3, r1[3], stab, snever);
+    return (own & ~am) | (nw & am);
 }
 
 // One row of one strip.  up / ct / dn: other-colour words of rows i-1, i, i+1; kParity = 1: the side neighbour of
 // site k is other[i][k+1], else other[i][k-1]; `edge` is the 32-bit word holding the 17th byte.
-template <bool kHasNever, int kParity>
+template <bool kHasNever, bool kPow2, int kParity>
 __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const uint4& up, const uint4& ct,
                                             const uint4& dn, uint32_t edge, uint32_t g0, uint32_t c1, uint32_t q,
-                                            uint32_t geAdd, const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
+                                            uint32_t psh, uint32_t geAdd, const uint32_t* stab, const uint32_t* snever,
+                                            uint32_t slot) {
     uint32_t s0, s1, s2, s3;
     if (kParity) {
         s0 = __byte_perm(ct.x, ct.y, 0x4321);
@@ -141,22 +156,22 @@ __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const
     uint32_t r0[4], r1[4];
     philox4x32_10(a.rk, g0 + 0, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 1, c1, a.c2, a.c3, r1);
-    res.x = update_word<kHasNever, 0>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, geAdd, stab, snever, slot);
+    res.x = update_word<kHasNever, kPow2, 0>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, psh, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 2, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 3, c1, a.c2, a.c3, r1);
-    res.y = update_word<kHasNever, 1>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, geAdd, stab, snever, slot);
+    res.y = update_word<kHasNever, kPow2, 1>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, psh, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 4, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 5, c1, a.c2, a.c3, r1);
-    res.z = update_word<kHasNever, 2>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, geAdd, stab, snever, slot);
+    res.z = update_word<kHasNever, kPow2, 2>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, psh, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 6, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 7, c1, a.c2, a.c3, r1);
-    res.w = update_word<kHasNever, 3>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, geAdd, stab, snever, slot);
+    res.w = update_word<kHasNever, kPow2, 3>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, psh, geAdd, stab, snever, slot);
     return res;
 }
 
-template <int kColour, bool kHasNever>
+template <int kColour, bool kHasNever, bool kPow2>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint32_t* snever, uint32_t q,
-                                           uint32_t slot, int b, int rb, int x) {
+                                           uint32_t psh, uint32_t slot, int b, int rb, int x) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
     const size_t half = (size_t)L * W;
     const int i0 = rb * kRows;
@@ -190,7 +205,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
         const uint4 n1 = __ldg(more ? pOth : pOthLast);
         const uint4 own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
-        uint4 res = update_row<kHasNever, kColour>(a, own, wU, wC, wD, edge, g0, c1, q, geAdd, stab, snever, slot);
+        uint4 res = update_row<kHasNever, kPow2, kColour>(a, own, wU, wC, wD, edge, g0, c1, q, psh, geAdd, stab, snever, slot);
         *pOwn = res;
         uint4 n2 = n1, own2 = own1;
         uint32_t edge2 = edge1;
@@ -199,8 +214,8 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             own2 = *(pOwn + 2 * rowStride);
             edge2 = __ldg(pEdgeEven + edgeStride2);
         }
-        res = update_row<kHasNever, 1 - kColour>(a, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd, stab,
-                                                 snever, slot);
+        res = update_row<kHasNever, kPow2, 1 - kColour>(a, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, psh,
+                                                        geAdd, stab, snever, slot);
         *(pOwn + rowStride) = res;
         wU = wD;
         wC = n1;
@@ -240,8 +255,12 @@ __global__ void __launch_bounds__(kRowsThreads, POTTS_MINB) potts_int8_rows_kern
     const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
-    if (never) march_rows<kColour, true>(a, stab, snever, q, slot, b, rb, x);
-    else march_rows<kColour, false>(a, stab, snever, q, slot, b, rb, x);
+    const uint32_t qm1 = q - 1u;
+    const bool pow2 = qm1 >= 2u && (qm1 & (qm1 - 1u)) == 0u;    // q = 3, 5, 9, ...: the proposal is a shift
+    const uint32_t psh = pow2 ? (uint32_t)__clz(qm1) + 1u : 0u;    // 32 - log2(q-1)
+    if (never) march_rows<kColour, true, false>(a, stab, snever, q, psh, slot, b, rb, x);
+    else if (pow2) march_rows<kColour, false, true>(a, stab, snever, q, psh, slot, b, rb, x);
+    else march_rows<kColour, false, false>(a, stab, snever, q, psh, slot, b, rb, x);
 }
 
 }  // namespace
