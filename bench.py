@@ -93,6 +93,22 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def _ncu_traffic(kernel_variant, w):
+    """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture summary
+    (profiles/r1_traffic.csv: kernel variant, workload, dram read + write bytes per launch), or None."""
+    p = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    if not os.path.exists(p):
+        return None
+    for line in open(p):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) >= 4 and f[0] == kernel_variant and f[1] == w.name:
+            try:
+                return float(f[2]) + float(f[3])
+            except ValueError:
+                return None
+    return None
+
+
 def _cores():
     try:
         return len(os.sched_getaffinity(0))
@@ -219,14 +235,14 @@ def main():
     E_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
     M_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
 
-    def step(offset):
-        # whole hot path, inputs resident in HBM: table build + upload, all sweeps, E/M reductions (device)
-        sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, offset)
-        sim.spin_observables_dev(E_dev.data_ptr(), M_dev.data_ptr())
-
+    # a step = the whole hot path with inputs resident in HBM: table build + upload, all sweeps, E/M reductions
     offset = 0
+    launches_per_sweep_call = None
     for _ in range(args.warmup):
-        step(offset)
+        l0 = sim.spin_kernel_launches()
+        sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, offset)
+        launches_per_sweep_call = sim.spin_kernel_launches() - l0      # 2 per sweep (streaming) or 1 (resident)
+        sim.spin_observables_dev(E_dev.data_ptr(), M_dev.data_ptr())
         offset += w.n_sweeps
     sim.spin_synchronize()
     torch.cuda.synchronize()
@@ -285,14 +301,16 @@ def main():
 
     if rank == 0:
         peaks = _peaks()
-        n_half = 2 * w.n_sweeps
-        kern_ms = float(np.mean(sweep_ms)) / n_half  # average launch duration incl. launch gaps
-        upd_per_launch = float(w.sites) / 2.0
+        n_launch = launches_per_sweep_call or 2 * w.n_sweeps
+        kern_ms = float(np.mean(sweep_ms)) / n_launch  # average launch duration incl. launch gaps
+        upd_per_launch = float(w.updates) / n_launch
         ops = OPS_PER_UPDATE[w.model]
         achieved = ops * upd_per_launch / (kern_ms * 1e-3) / 1e12
         peak = INT32_LANES_PER_SM * N_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
         bytes_per_site = 0.375 if w.layout == "bits" else 3.0  # per sweep, two launches
-        hbm_achieved = bytes_per_site / 2.0 * upd_per_launch * 2.0 / (kern_ms * 1e-3) / 1e9
+        if n_launch == 1:
+            bytes_per_site = (0.25 if w.layout == "bits" else 2.0) / w.n_sweeps  # resident: one read + one write per call
+        hbm_achieved = bytes_per_site * upd_per_launch / (kern_ms * 1e-3) / 1e9
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -306,7 +324,9 @@ def main():
             "sweep_only_flips_per_ns": float(w.updates) / (float(np.mean(sweep_ms)) * 1e6),
             "roofline": {
                 "bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tint32op/s", "frac": achieved / peak,
-                "traffic": None,
+                "traffic": _ncu_traffic(sim.spin_kernel_variant(), w),
+                "algorithmic_bytes_per_launch": bytes_per_site * upd_per_launch,
+                "launches_per_step": int(n_launch),
                 "kernel_avg_launch_us": kern_ms * 1e3, "ops_per_update": ops,
                 "peak_source": "derived: 64 INT32 lanes/SM/clk x 148 SMs x %.0f MHz (%s sm_max_mhz); DESIGN.md section 6"
                                % (peaks["sm_max_mhz"], peaks["source"]),
