@@ -71,9 +71,17 @@ __device__ __forceinline__ void slot_store_u32(uint32_t saddr, uint32_t v) {
     asm volatile("st.shared.u32 [%0+%1], %2;" :: "r"(saddr), "n"(kOff), "r"(v));
 }
 
+// kSmallQ (q <= 16, states < 16): x = a ^ b < 16, so x + 0x3F / 0x1F / 0x0F raise bit 6 / 5 / 4 iff x != 0 and leave the
+// higher bits clear: the four indicator bits land in place without shifts.
+template <bool kSmallQ>
 __device__ __forceinline__ uint32_t neq_bits(uint32_t v, uint32_t u, uint32_t d, uint32_t c, uint32_t s) {
     const uint32_t k = 0x7F7F7F7Fu;
-    const uint32_t a0 = (v ^ u) + k, a1 = ((v ^ d) + k) >> 1, a2 = ((v ^ c) + k) >> 2, a3 = ((v ^ s) + k) >> 3;
+    uint32_t a0, a1, a2, a3;
+    if (kSmallQ) {
+        a0 = (v ^ u) + k; a1 = (v ^ d) + 0x3F3F3F3Fu; a2 = (v ^ c) + 0x1F1F1F1Fu; a3 = (v ^ s) + 0x0F0F0F0Fu;
+    } else {
+        a0 = (v ^ u) + k; a1 = ((v ^ d) + k) >> 1; a2 = ((v ^ c) + k) >> 2; a3 = ((v ^ s) + k) >> 3;
+    }
     // bit 7 from a0, bit 6 from a1, bit 5 from a2, bit 4 from a3 (low nibble is garbage, masked by the caller)
     uint32_t t = (a2 & 0x20202020u) | (a3 & ~0x20202020u);
     t = (a1 & 0x40404040u) | (t & ~0x40404040u);
@@ -99,26 +107,19 @@ __device__ __forceinline__ void site_step(uint32_t& acc_mask, uint32_t o, uint32
 }
 
 // One 4-site word: r0 feeds sites 0, 1 (proposal words r0[0], r0[2]; acceptance words r0[1], r0[3]), r1 sites 2, 3.
-// floor(r (q-1) / 2^32): a shift when q-1 is a power of two (psh = 32 - log2(q-1)), else a multiply-high
-template <bool kPow2>
-__device__ __forceinline__ uint32_t propose(uint32_t r, uint32_t qm1, uint32_t psh) {
-    return kPow2 ? (r >> psh) : __umulhi(r, qm1);
-}
-
-template <bool kHasNever, bool kPow2, int kJ>
+template <bool kHasNever, bool kSmallQ, int kJ>
 __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t ct, uint32_t sd,
-                                                const uint32_t r0[4], const uint32_t r1[4], uint32_t q, uint32_t psh,
-                                                uint32_t geAdd, const uint32_t* stab, const uint32_t* snever,
-                                                uint32_t slot) {
+                                                const uint32_t r0[4], const uint32_t r1[4], uint32_t q, uint32_t geAdd,
+                                                const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
     // proposal (O6): new = old + 1 + floor(r_prop (q-1) / 2^32), minus q if >= q
     const uint32_t qm1 = q - 1u;
-    const uint32_t d = propose<kPow2>(r0[0], qm1, psh) | (propose<kPow2>(r0[2], qm1, psh) << 8) |
-                       (propose<kPow2>(r1[0], qm1, psh) << 16) | (propose<kPow2>(r1[2], qm1, psh) << 24);
+    const uint32_t d = __umulhi(r0[0], qm1) | (__umulhi(r0[2], qm1) << 8) | (__umulhi(r1[0], qm1) << 16) |
+                       (__umulhi(r1[2], qm1) << 24);
     uint32_t nw = own + 0x01010101u + d;                              // <= 2q-2 per byte
     const uint32_t ge = ((nw + geAdd) >> 7) & 0x01010101u;            // 1 where nw >= q (geAdd = (0x80 - q) per byte)
     nw -= ge * q;
-    const uint32_t mo = neq_bits(own, up, dn, ct, sd);
-    const uint32_t mn = neq_bits(nw, up, dn, ct, sd);
+    const uint32_t mo = neq_bits<kSmallQ>(own, up, dn, ct, sd);
+    const uint32_t mn = neq_bits<kSmallQ>(nw, up, dn, ct, sd);
     const uint32_t idx = (mo & 0xF0F0F0F0u) | ((mn >> 4) & 0x0F0F0F0Fu);
     slot_store_u32<kJ * kRowsThreads * 4>(slot, idx);
     const uint32_t o0 = slot_load_u8<kJ * kRowsThreads * 4 + 0>(slot);
@@ -135,11 +136,10 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
 
 // One row of one strip.  up / ct / dn: other-colour words of rows i-1, i, i+1; kParity = 1: the side neighbour of
 // site k is other[i][k+1], else other[i][k-1]; `edge` is the 32-bit word holding the 17th byte.
-template <bool kHasNever, bool kPow2, int kParity>
+template <bool kHasNever, bool kSmallQ, int kParity>
 __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const uint4& up, const uint4& ct,
                                             const uint4& dn, uint32_t edge, uint32_t g0, uint32_t c1, uint32_t q,
-                                            uint32_t psh, uint32_t geAdd, const uint32_t* stab, const uint32_t* snever,
-                                            uint32_t slot) {
+                                            uint32_t geAdd, const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
     uint32_t s0, s1, s2, s3;
     if (kParity) {
         s0 = __byte_perm(ct.x, ct.y, 0x4321);
@@ -156,22 +156,22 @@ __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const
     uint32_t r0[4], r1[4];
     philox4x32_10(a.rk, g0 + 0, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 1, c1, a.c2, a.c3, r1);
-    res.x = update_word<kHasNever, kPow2, 0>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, psh, geAdd, stab, snever, slot);
+    res.x = update_word<kHasNever, kSmallQ, 0>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 2, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 3, c1, a.c2, a.c3, r1);
-    res.y = update_word<kHasNever, kPow2, 1>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, psh, geAdd, stab, snever, slot);
+    res.y = update_word<kHasNever, kSmallQ, 1>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 4, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 5, c1, a.c2, a.c3, r1);
-    res.z = update_word<kHasNever, kPow2, 2>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, psh, geAdd, stab, snever, slot);
+    res.z = update_word<kHasNever, kSmallQ, 2>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, geAdd, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 6, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 7, c1, a.c2, a.c3, r1);
-    res.w = update_word<kHasNever, kPow2, 3>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, psh, geAdd, stab, snever, slot);
+    res.w = update_word<kHasNever, kSmallQ, 3>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, geAdd, stab, snever, slot);
     return res;
 }
 
-template <int kColour, bool kHasNever, bool kPow2>
+template <int kColour, bool kHasNever, bool kSmallQ>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint32_t* snever, uint32_t q,
-                                           uint32_t psh, uint32_t slot, int b, int rb, int x) {
+                                           uint32_t slot, int b, int rb, int x) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
     const size_t half = (size_t)L * W;
     const int i0 = rb * kRows;
@@ -205,7 +205,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
         const uint4 n1 = __ldg(more ? pOth : pOthLast);
         const uint4 own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
-        uint4 res = update_row<kHasNever, kPow2, kColour>(a, own, wU, wC, wD, edge, g0, c1, q, psh, geAdd, stab, snever, slot);
+        uint4 res = update_row<kHasNever, kSmallQ, kColour>(a, own, wU, wC, wD, edge, g0, c1, q, geAdd, stab, snever, slot);
         *pOwn = res;
         uint4 n2 = n1, own2 = own1;
         uint32_t edge2 = edge1;
@@ -214,8 +214,8 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             own2 = *(pOwn + 2 * rowStride);
             edge2 = __ldg(pEdgeEven + edgeStride2);
         }
-        res = update_row<kHasNever, kPow2, 1 - kColour>(a, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, psh,
-                                                        geAdd, stab, snever, slot);
+        res = update_row<kHasNever, kSmallQ, 1 - kColour>(a, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd,
+                                                          stab, snever, slot);
         *(pOwn + rowStride) = res;
         wU = wD;
         wC = n1;
@@ -255,12 +255,9 @@ __global__ void __launch_bounds__(kRowsThreads, POTTS_MINB) potts_int8_rows_kern
     const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
-    const uint32_t qm1 = q - 1u;
-    const bool pow2 = qm1 >= 2u && (qm1 & (qm1 - 1u)) == 0u;    // q = 3, 5, 9, ...: the proposal is a shift
-    const uint32_t psh = pow2 ? (uint32_t)__clz(qm1) + 1u : 0u;    // 32 - log2(q-1)
-    if (never) march_rows<kColour, true, false>(a, stab, snever, q, psh, slot, b, rb, x);
-    else if (pow2) march_rows<kColour, false, true>(a, stab, snever, q, psh, slot, b, rb, x);
-    else march_rows<kColour, false, false>(a, stab, snever, q, psh, slot, b, rb, x);
+    if (never) march_rows<kColour, true, false>(a, stab, snever, q, slot, b, rb, x);
+    else if (q <= 16u) march_rows<kColour, false, true>(a, stab, snever, q, slot, b, rb, x);   // shift-free indicators
+    else march_rows<kColour, false, false>(a, stab, snever, q, slot, b, rb, x);
 }
 
 }  // namespace

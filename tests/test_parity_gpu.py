@@ -168,6 +168,7 @@ POTTS_CASES = [
     (32, [3, 8, 2, 127], [1.005, 1.342, 0.0, 3.0]),
     (64, [3, 8], [20.0, 0.7]),
     (96, [4, 7], [1.1, 1.3]),
+    (64, [16, 17, 15, 33], [1.6, 1.6, 20.0, 1.9]),   # both sides of the q <= 16 (shift-free indicators) boundary
 ]
 
 
