@@ -199,7 +199,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     uint32_t g0 = (uint32_t)i0 * (uint32_t)(W >> 1) + 8u * (uint32_t)x;   // Philox group = n >> 1
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
     const uint32_t geAdd = (0x80u - q) * 0x01010101u;
-#pragma unroll 1
+#pragma unroll 2
     for (int rr = 0; rr < kRows; rr += 2) {
         const bool more = rr + 2 < kRows;
         const uint4 n1 = __ldg(more ? pOth : pOthLast);
