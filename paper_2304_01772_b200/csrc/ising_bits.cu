@@ -26,7 +26,8 @@ __device__ __forceinline__ int decode_class(int e, int nib) {
     return D * 8 + P2 * 4 + P1 * 2 + P0;
 }
 
-constexpr int kRows = 8;
+constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
+constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
 constexpr int kThreads = 128;
 #ifndef BITS_MINB
 #define BITS_MINB 8
@@ -73,7 +74,7 @@ __device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own
 // Row-marching: one thread owns word x of kRows consecutive rows (same skeleton as ising_int8.cu: the three
 // other-colour words it needs stay in registers, running pointers, two rows per rolled iteration because the side
 // of the horizontal neighbour alternates, programmatic dependent launch).
-template <int kColour, bool kHasNever>
+template <int kColour, bool kHasNever, int kRows>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t (*stab)[16], const uint32_t* snever, int b,
                                            int rb, int x) {
     const int L = a.L, WW = L >> 6;                       // words per colour-row
@@ -126,7 +127,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t (*
     }
 }
 
-template <int kColour>
+template <int kColour, int kRows>
 __global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[4][16];
     __shared__ uint32_t snever[4];
@@ -149,20 +150,28 @@ __global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepAr
     const int WW = a.L >> 6;
     const int u = blk * blockDim.x + threadIdx.x;         // < (L / kRows) * WW by construction
     const int rb = u / WW, x = u - rb * WW;
-    if (never) march_rows<kColour, true>(a, stab, snever, b, rb, x);
-    else march_rows<kColour, false>(a, stab, snever, b, rb, x);
+    if (never) march_rows<kColour, true, kRows>(a, stab, snever, b, rb, x);
+    else march_rows<kColour, false, kRows>(a, stab, snever, b, rb, x);
 }
 
 }  // namespace
 
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
-    const int perReplica = (a.L / kRows) * (a.L >> 6);
+    const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 6) * a.batch;
+    const bool shortRows = longThreads < 148ll * 64;      // the per-block table set-up makes short threads pay off only for tiny launches
+    const int rows = shortRows ? kRowsShort : kRowsLong;
+    const int perReplica = (a.L / rows) * (a.L >> 6);
     int tpb = kThreads;
     while (perReplica % tpb) tpb >>= 1;
     const int bpr = perReplica / tpb;
     const unsigned grid = (unsigned)((long long)bpr * a.batch);
-    if (a.colour == 0) launch_pdl(ising_bits_kernel<0>, grid, (unsigned)tpb, s, a, bpr);
-    else launch_pdl(ising_bits_kernel<1>, grid, (unsigned)tpb, s, a, bpr);
+    if (shortRows) {
+        if (a.colour == 0) launch_pdl(ising_bits_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
+        else launch_pdl(ising_bits_kernel<1, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
+    } else {
+        if (a.colour == 0) launch_pdl(ising_bits_kernel<0, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
+        else launch_pdl(ising_bits_kernel<1, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
+    }
     return 1;
 }
 

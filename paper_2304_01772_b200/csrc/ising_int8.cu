@@ -61,7 +61,8 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 // arithmetic); the loop is rolled two rows per iteration (the side-neighbour parity alternates) so that the body
 // (about 540 instructions) stays resident in the instruction caches.  Launched with programmatic dependent launch:
 // the next half-sweep's blocks are scheduled while this one drains.
-constexpr int kRows = 8;
+constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
+constexpr int kRowsShort = 2;   // ... and when it does not (latency-bound shapes): four times as many threads
 #ifndef ISING_MINB
 #define ISING_MINB 7
 #endif
@@ -151,7 +152,7 @@ __device__ __forceinline__ uint4 mask4(const uint4& v) {
     return make_uint4(v.x & m, v.y & m, v.z & m, v.w & m);
 }
 
-template <int kColour, bool kHasNever>
+template <int kColour, bool kHasNever, int kRows>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, uint32_t slot, int b, int rb,
                                            int x) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
@@ -219,7 +220,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 }
 
 // One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
-template <int kColour>
+template <int kColour, int kRows>
 __global__ void __launch_bounds__(kRowsThreads, ISING_MINB) ising_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[kTableStride];
     __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
@@ -233,8 +234,8 @@ __global__ void __launch_bounds__(kRowsThreads, ISING_MINB) ising_int8_rows_kern
     const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
-    if (stab[kTabNever]) march_rows<kColour, true>(a, stab, slot, b, rb, x);
-    else march_rows<kColour, false>(a, stab, slot, b, rb, x);
+    if (stab[kTabNever]) march_rows<kColour, true, kRows>(a, stab, slot, b, rb, x);
+    else march_rows<kColour, false, kRows>(a, stab, slot, b, rb, x);
 }
 
 // ---- shared-memory-resident kernel: L % 32 == 0 and the replica (L^2 bytes) fits one CTA's shared memory.
@@ -382,13 +383,22 @@ const char* ising_int8_variant(int L) { return (L % 32 == 0) ? "ising_int8_rows1
 
 int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
-        const int perReplica = (a.L / kRows) * (a.L >> 5);   // strips x row blocks of one colour
+        // 8 rows per thread when that still gives every SM several blocks, else 2 rows (short threads, 4x as many)
+        const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 5) * a.batch;
+        const bool shortRows = longThreads < 148ll * 4 * kRowsThreads;
+        const int rows = shortRows ? kRowsShort : kRowsLong;
+        const int perReplica = (a.L / rows) * (a.L >> 5);    // strips x row blocks of one colour
         int tpb = kRowsThreads;
         while (perReplica % tpb) tpb >>= 1;                  // L = 32 -> 4 threads
         const int bpr = perReplica / tpb;
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
-        if (a.colour == 0) launch_pdl(ising_int8_rows_kernel<0>, grid, (unsigned)tpb, s, a, bpr);
-        else launch_pdl(ising_int8_rows_kernel<1>, grid, (unsigned)tpb, s, a, bpr);
+        if (shortRows) {
+            if (a.colour == 0) launch_pdl(ising_int8_rows_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
+            else launch_pdl(ising_int8_rows_kernel<1, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
+        } else {
+            if (a.colour == 0) launch_pdl(ising_int8_rows_kernel<0, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
+            else launch_pdl(ising_int8_rows_kernel<1, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
+        }
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 3) >> 2) * a.batch;

@@ -53,7 +53,8 @@ __global__ void potts_int8_generic_kernel(SweepArgs a) {
 // The 4 "differs from old" bits and the 4 "differs from new" bits of a site are gathered into one byte that
 // indexes a 256-entry shared table holding U[dn + 4] (dn = n_new - n_old = #(!= old) - #(!= new)); the four index
 // bytes of a word go through a per-thread shared-memory slot (STS, then LDS.U8 straight into the table address).
-constexpr int kRows = 8;
+constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
+constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
 constexpr int kRowsThreads = 128;
 #ifndef POTTS_MINB
 #define POTTS_MINB 4
@@ -169,7 +170,7 @@ __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const
     return res;
 }
 
-template <int kColour, bool kHasNever, bool kSmallQ>
+template <int kColour, bool kHasNever, bool kSmallQ, int kRows>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint32_t* snever, uint32_t q,
                                            uint32_t slot, int b, int rb, int x) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
@@ -231,7 +232,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 }
 
 // One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
-template <int kColour>
+template <int kColour, int kRows>
 __global__ void __launch_bounds__(kRowsThreads, POTTS_MINB) potts_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[16 + 64];            // U[dn + 4] in [0..8]; from word 16: 256-byte pattern -> 4 * class table
     __shared__ uint32_t snever[1];
@@ -255,9 +256,9 @@ __global__ void __launch_bounds__(kRowsThreads, POTTS_MINB) potts_int8_rows_kern
     const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
-    if (never) march_rows<kColour, true, false>(a, stab, snever, q, slot, b, rb, x);
-    else if (q <= 16u) march_rows<kColour, false, true>(a, stab, snever, q, slot, b, rb, x);   // shift-free indicators
-    else march_rows<kColour, false, false>(a, stab, snever, q, slot, b, rb, x);
+    if (never) march_rows<kColour, true, false, kRows>(a, stab, snever, q, slot, b, rb, x);
+    else if (q <= 16u) march_rows<kColour, false, true, kRows>(a, stab, snever, q, slot, b, rb, x);   // shift-free indicators
+    else march_rows<kColour, false, false, kRows>(a, stab, snever, q, slot, b, rb, x);
 }
 
 }  // namespace
@@ -266,13 +267,21 @@ const char* potts_int8_variant(int L) { return (L % 32 == 0) ? "potts_int8_rows1
 
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
-        const int perReplica = (a.L / kRows) * (a.L >> 5);   // strips x row blocks of one colour
+        const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 5) * a.batch;
+        const bool shortRows = longThreads < 148ll * 4 * kRowsThreads;
+        const int rows = shortRows ? kRowsShort : kRowsLong;
+        const int perReplica = (a.L / rows) * (a.L >> 5);    // strips x row blocks of one colour
         int tpb = kRowsThreads;
         while (perReplica % tpb) tpb >>= 1;                  // L = 32 -> 4 threads
         const int bpr = perReplica / tpb;
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
-        if (a.colour == 0) launch_pdl(potts_int8_rows_kernel<0>, grid, (unsigned)tpb, s, a, bpr);
-        else launch_pdl(potts_int8_rows_kernel<1>, grid, (unsigned)tpb, s, a, bpr);
+        if (shortRows) {
+            if (a.colour == 0) launch_pdl(potts_int8_rows_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
+            else launch_pdl(potts_int8_rows_kernel<1, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
+        } else {
+            if (a.colour == 0) launch_pdl(potts_int8_rows_kernel<0, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
+            else launch_pdl(potts_int8_rows_kernel<1, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
+        }
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 1) >> 1) * a.batch;
