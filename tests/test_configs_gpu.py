@@ -20,14 +20,37 @@ def _create(w, layout=None):
     return sp.spin_create_ex(w.batch, w.L, sp.SPIN_MODEL_ISING, seed=w.seed, layout=lay)
 
 
-def test_config1_complete(oracle_mod):
+@pytest.mark.parametrize("policy", [sp.SPIN_POLICY_AUTO, sp.SPIN_POLICY_STREAMING])
+def test_config1_complete(oracle_mod, policy):
+    """All 1000 sweeps, every (E, M), final lattice: once as bench.py runs it (AUTO: one resident launch) and once
+    through the two-launches-per-sweep kernels."""
     w = sp.workloads.config(1)
     ref = oracle_mod.init(w.batch, w.L, seed=w.seed)
     Eo, Mo = oracle_mod.sweep(ref, w.beta, w.J, w.h, seed=w.seed, n_sweeps=w.n_sweeps, trace=True)
     with _create(w) as sim:
+        sim.spin_set_policy(policy)
+        assert (sim.spin_kernel_variant() == "ising_int8_resident") == (policy == sp.SPIN_POLICY_AUTO)
         E, M = sim.spin_sweep_measure(w.beta, w.J, w.h, w.n_sweeps, 0)
         assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
         assert np.array_equal(sim.spin_get_spins(), ref)
+
+
+def _compare_after_one_call(oracle_mod, w, replicas, n_sweeps, policy=sp.SPIN_POLICY_AUTO):
+    """The whole batch runs n_sweeps in ONE spin_sweep call (the way bench.py drives it); sampled replicas are then
+    compared with the oracle run alone: lattice, E_int, M."""
+    q = None if w.q is None else w.q
+    with _create(w) as sim:
+        sim.spin_set_policy(policy)
+        sim.spin_sweep(w.beta, w.J, w.h, n_sweeps, 0)
+        got = sim.spin_get_spins()
+        E, M = sim.spin_observables()
+    for b in replicas:
+        qb = None if q is None else int(q[b])
+        ref = oracle_mod.init(1, w.L, seed=w.seed, q=qb, replica_offset=b)
+        oracle_mod.sweep(ref, w.beta[b:b + 1], w.J, w.h, seed=w.seed, n_sweeps=n_sweeps, q=qb, replica_offset=b)
+        assert np.array_equal(got[b], ref[0]), "replica %d differs after %d sweeps" % (b, n_sweeps)
+        Eo, Mo = oracle_mod.ising_observables(ref) if qb is None else oracle_mod.potts_observables(ref, qb)
+        assert int(E[b]) == int(Eo[0]) and int(M[b]) == int(Mo[0])
 
 
 def _compare_sampled_replicas(oracle_mod, w, replicas, n_sweeps, layout=None):
@@ -57,6 +80,7 @@ def _compare_sampled_replicas(oracle_mod, w, replicas, n_sweeps, layout=None):
 
 def test_config2_sampled_replicas(oracle_mod):
     _compare_sampled_replicas(oracle_mod, sp.workloads.config(2), [0, 31, 63], n_sweeps=3)
+    _compare_after_one_call(oracle_mod, sp.workloads.config(2), [0, 63], n_sweeps=100)
 
 
 @pytest.mark.parametrize("layout", ["int8", "bits"])
@@ -67,20 +91,32 @@ def test_config3_sampled_replica(oracle_mod, layout):
 
 def test_config4_sampled_replicas(oracle_mod):
     _compare_sampled_replicas(oracle_mod, sp.workloads.config(4), [0, 63, 64, 127], n_sweeps=5)
+    _compare_after_one_call(oracle_mod, sp.workloads.config(4), [5, 100], n_sweeps=200)
 
 
 def test_config5_sampled_replicas_and_moments(oracle_mod):
     w = sp.workloads.config(5)
     _compare_sampled_replicas(oracle_mod, w, [0, 512, 1023], n_sweeps=5)
-    # moments over a short window, all 1024 replicas on the GPU, three checked against the oracle
-    with _create(w) as sim:
-        sim.spin_sweep(w.beta, w.J, w.h, 4, 0)
-        mom = np.zeros((w.batch, 8), dtype=np.int64)
-        sim.spin_sweep_measure(w.beta, w.J, w.h, 6, 4, trace=False, moments=mom)
+    _compare_after_one_call(oracle_mod, w, [1, 511, 1022], n_sweeps=1000)
+    _compare_after_one_call(oracle_mod, w, [2, 1000], n_sweeps=50, policy=sp.SPIN_POLICY_RESIDENT)
+    # thermalise, then moments over a window: all 1024 replicas on the GPU (AUTO: the resident kernel with fused
+    # reductions; STREAMING: half-sweep kernels + reduction kernels), three replicas checked against the oracle
+    n_therm, n_meas = 20, 60
+    expect = {}
     for b in (0, 700, 1023):
         ref = oracle_mod.init(1, w.L, seed=w.seed, replica_offset=b)
-        oracle_mod.sweep(ref, w.beta[b:b + 1], w.J, w.h, seed=w.seed, n_sweeps=4, replica_offset=b)
+        oracle_mod.sweep(ref, w.beta[b:b + 1], w.J, w.h, seed=w.seed, n_sweeps=n_therm, replica_offset=b)
         mo = np.zeros((1, 8), dtype=np.int64)
-        oracle_mod.sweep(ref, w.beta[b:b + 1], w.J, w.h, seed=w.seed, n_sweeps=6, sweep_offset=4, replica_offset=b,
-                         moments=mo)
-        assert np.array_equal(mom[b], mo[0])
+        oracle_mod.sweep(ref, w.beta[b:b + 1], w.J, w.h, seed=w.seed, n_sweeps=n_meas, sweep_offset=n_therm,
+                         replica_offset=b, moments=mo)
+        expect[b] = (mo[0], ref[0])
+    for policy in (sp.SPIN_POLICY_AUTO, sp.SPIN_POLICY_STREAMING):
+        with _create(w) as sim:
+            sim.spin_set_policy(policy)
+            sim.spin_sweep(w.beta, w.J, w.h, n_therm, 0)
+            mom = np.zeros((w.batch, 8), dtype=np.int64)
+            sim.spin_sweep_measure(w.beta, w.J, w.h, n_meas, n_therm, trace=False, moments=mom)
+            got = sim.spin_get_spins()
+        for b, (mo, lat) in expect.items():
+            assert np.array_equal(mom[b], mo), "moments differ, replica %d, policy %d" % (b, policy)
+            assert np.array_equal(got[b], lat)
