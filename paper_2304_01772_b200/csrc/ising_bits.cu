@@ -2,8 +2,8 @@
 // [B][2][L][L/64] uint32, bit b of word w = same-colour site k = 32 w + b of that row, bit set = spin -1.
 // Same rule, same Philox words as the int8 kernels (Alg. 1 + checkerboard).
 // One thread per word = 32 sites = 8 Philox calls.  The neighbour count is a bit-sliced full adder; the
-// 4-bit class index of every site is assembled nibble-parallel (8 sites per LOP3), so the per-site work is
-// extract + LDS + compare + predicated OR.
+// 4-bit class index of every site is assembled nibble-parallel (8 sites per LOP3) and looked up through shared
+// memory, so the per-site work is two byte-addressed loads + compare + select.
 #include "spin_internal.cuh"
 
 namespace spin {
@@ -11,20 +11,6 @@ namespace spin {
 namespace {
 
 __device__ __forceinline__ uint32_t sel(uint32_t m, uint32_t a, uint32_t b) { return (a & m) | (b & ~m); }
-
-// Per-e nibble tables: the 4 sites of a nibble (e = 0..3) see the class bits (D, P2, P1, P0) at different
-// nibble positions; decode_class turns a nibble value back into the standard class index d*8 + nd.
-__device__ __forceinline__ int decode_class(int e, int nib) {
-    const int b0 = nib & 1, b1 = (nib >> 1) & 1, b2 = (nib >> 2) & 1, b3 = (nib >> 3) & 1;
-    int D, P0, P1, P2;
-    switch (e) {
-        case 0: P0 = b0; P1 = b1; P2 = b2; D = b3; break;
-        case 1: D = b0; P0 = b1; P1 = b2; P2 = b3; break;
-        case 2: P2 = b0; D = b1; P0 = b2; P1 = b3; break;
-        default: P1 = b0; P2 = b1; D = b2; P0 = b3; break;
-    }
-    return D * 8 + P2 * 4 + P1 * 2 + P0;
-}
 
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
 constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
@@ -34,13 +20,64 @@ constexpr int kThreads = 128;
 #endif
 
 // One word = 32 sites = 8 Philox calls.  up / dn / ct: other-colour words of rows i-1, i+1, i; sd: the side
-// neighbours (ct shifted by one site, with the bit of the adjacent word).  stab[e][nibble] holds U for the class
-// whose bits sit in that nibble order; the nibble of site 4c+e is read pre-scaled (x4) so that it is the byte offset
-// of the threshold: per site SHF + LOP3 (extract), LDS, ISETP, predicated OR.
+// neighbours (ct shifted by one site, with the bit of the adjacent word).  The class nibbles of the 32 sites are
+// assembled nibble-parallel into t[0..3] (site 4c+e in nibble c of t[e], bit order rotated by e), stored to a
+// per-thread shared-memory slot, and read back a byte (two sites) at a time; a constant byte table turns that byte
+// into 4 * class of its low / high nibble, which is the address of the threshold: per site LDS.U8, LDS, ISETP and a
+// select, no extraction arithmetic (the LSU has the headroom, the integer issue slots do not).
+template <int kOff>
+__device__ __forceinline__ uint32_t slot_load_u8(uint32_t saddr) {
+    uint32_t v;
+    asm volatile("ld.shared.u8 %0, [%1+%2];" : "=r"(v) : "r"(saddr), "n"(kOff));
+    return v;
+}
+
+template <int kOff>
+__device__ __forceinline__ void slot_store_u32(uint32_t saddr, uint32_t v) {
+    asm volatile("st.shared.u32 [%0+%1], %2;" :: "r"(saddr), "n"(kOff), "r"(v));
+}
+
+constexpr int kAuxBytes = 2048;            // [e][half][byte] -> 4 * class
+
+template <bool kHasNever, int kC, int kE>
+__device__ __forceinline__ void site_step(uint32_t& flip, uint32_t v, uint32_t r, const uint32_t* stab,
+                                          const uint8_t* sT, uint32_t never) {
+    const uint32_t c4 = sT[(kE * 2 + (kC & 1)) * 256 + v];
+    const uint32_t U = *(const uint32_t*)((const char*)stab + c4);
+    bool acc = r <= U;
+    if (kHasNever) acc = acc && !((never >> (c4 >> 2)) & 1u);
+    if (acc) flip |= 1u << (4 * kC + kE);
+}
+
+template <bool kHasNever, int kC>
+__device__ __forceinline__ void group_step(uint32_t& flip, const uint32_t r[4], const uint32_t v[4], const uint32_t* stab,
+                                           const uint8_t* sT, uint32_t never) {
+    site_step<kHasNever, kC, 0>(flip, v[0], r[0], stab, sT, never);
+    site_step<kHasNever, kC, 1>(flip, v[1], r[1], stab, sT, never);
+    site_step<kHasNever, kC, 2>(flip, v[2], r[2], stab, sT, never);
+    site_step<kHasNever, kC, 3>(flip, v[3], r[3], stab, sT, never);
+}
+
+// Two Philox groups (sites 8p .. 8p+7) share one byte of each t[e].
+template <bool kHasNever, int kP>
+__device__ __forceinline__ void pair_step(const SweepArgs& a, uint32_t& flip, uint32_t g0, uint32_t c1,
+                                          const uint32_t* stab, const uint8_t* sT, uint32_t never, uint32_t slot) {
+    uint32_t v[4];
+    v[0] = slot_load_u8<0 * kThreads * 4 + kP>(slot);
+    v[1] = slot_load_u8<1 * kThreads * 4 + kP>(slot);
+    v[2] = slot_load_u8<2 * kThreads * 4 + kP>(slot);
+    v[3] = slot_load_u8<3 * kThreads * 4 + kP>(slot);
+    uint32_t r[4];
+    philox4x32_10(a.rk, g0 + 2 * kP, c1, a.c2, a.c3, r);
+    group_step<kHasNever, 2 * kP>(flip, r, v, stab, sT, never);
+    philox4x32_10(a.rk, g0 + 2 * kP + 1, c1, a.c2, a.c3, r);
+    group_step<kHasNever, 2 * kP + 1>(flip, r, v, stab, sT, never);
+}
+
 template <bool kHasNever>
 __device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own, uint32_t up, uint32_t dn, uint32_t ct,
-                                                uint32_t sd, uint32_t g0, uint32_t c1, const uint32_t (*stab)[16],
-                                                const uint32_t* snever) {
+                                                uint32_t sd, uint32_t g0, uint32_t c1, const uint32_t* stab,
+                                                const uint8_t* sT, uint32_t never, uint32_t slot) {
     // bit-sliced count of -1 neighbours: nd = P0 + 2 P1 + 4 P2
     const uint32_t s1 = up ^ dn ^ ct;
     const uint32_t k1 = (up & dn) | (ct & (up | dn));
@@ -49,25 +86,15 @@ __device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own
     const uint32_t P1 = k1 ^ k2;
     const uint32_t P2 = k1 & k2;
     const uint32_t P1a = P1 << 1, P1b = P1 >> 3, P2a = P2 << 2, P2b = P2 >> 2, Da = own << 3, Db = own >> 1;
-    uint32_t t[4];
-    t[0] = sel(0x11111111u, P0, sel(0x22222222u, P1a, sel(0x44444444u, P2a, Da)));
-    t[1] = sel(0x11111111u, Db, sel(0x22222222u, P0, sel(0x44444444u, P1a, P2a)));
-    t[2] = sel(0x11111111u, P2b, sel(0x22222222u, Db, sel(0x44444444u, P0, P1a)));
-    t[3] = sel(0x11111111u, P1b, sel(0x22222222u, P2b, sel(0x44444444u, Db, P0)));
+    slot_store_u32<0 * kThreads * 4>(slot, sel(0x11111111u, P0, sel(0x22222222u, P1a, sel(0x44444444u, P2a, Da))));
+    slot_store_u32<1 * kThreads * 4>(slot, sel(0x11111111u, Db, sel(0x22222222u, P0, sel(0x44444444u, P1a, P2a))));
+    slot_store_u32<2 * kThreads * 4>(slot, sel(0x11111111u, P2b, sel(0x22222222u, Db, sel(0x44444444u, P0, P1a))));
+    slot_store_u32<3 * kThreads * 4>(slot, sel(0x11111111u, P1b, sel(0x22222222u, P2b, sel(0x44444444u, Db, P0))));
     uint32_t flip = 0u;
-#pragma unroll
-    for (int c = 0; c < 8; ++c) {
-        uint32_t r[4];
-        philox4x32_10(a.rk, g0 + c, c1, a.c2, a.c3, r);
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-            // byte offset 4 * nibble of site 4c+e
-            const uint32_t o4 = (c == 0 ? (t[e] << 2) : (t[e] >> (4 * c - 2))) & 0x3Cu;
-            bool acc = r[e] <= *(const uint32_t*)((const char*)stab[e] + o4);
-            if (kHasNever) acc = acc && !((snever[e] >> (o4 >> 2)) & 1u);
-            if (acc) flip |= 1u << (4 * c + e);
-        }
-    }
+    pair_step<kHasNever, 0>(a, flip, g0, c1, stab, sT, never, slot);
+    pair_step<kHasNever, 1>(a, flip, g0, c1, stab, sT, never, slot);
+    pair_step<kHasNever, 2>(a, flip, g0, c1, stab, sT, never, slot);
+    pair_step<kHasNever, 3>(a, flip, g0, c1, stab, sT, never, slot);
     return own ^ flip;
 }
 
@@ -75,8 +102,8 @@ __device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own
 // other-colour words it needs stay in registers, running pointers, two rows per rolled iteration because the side
 // of the horizontal neighbour alternates, programmatic dependent launch).
 template <int kColour, bool kHasNever, int kRows>
-__device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t (*stab)[16], const uint32_t* snever, int b,
-                                           int rb, int x) {
+__device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint8_t* sT, uint32_t never,
+                                           uint32_t slot, int b, int rb, int x) {
     const int L = a.L, WW = L >> 6;                       // words per colour-row
     const size_t half = (size_t)L * WW;
     const int i0 = rb * kRows;
@@ -105,7 +132,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t (*
         const uint32_t own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
         uint32_t sd = kColour ? ((wC >> 1) | (edge << 31)) : ((wC << 1) | (edge >> 31));
-        *pOwn = update_word<kHasNever>(a, own, wU, wD, wC, sd, g0, c1, stab, snever);
+        *pOwn = update_word<kHasNever>(a, own, wU, wD, wC, sd, g0, c1, stab, sT, never, slot);
         uint32_t n2 = n1, own2 = own1, edge2 = edge1;
         if (more) {
             n2 = __ldg(pOth + rowStride);
@@ -113,7 +140,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t (*
             edge2 = __ldg(pEdgeEven + 2 * rowStride);
         }
         sd = kColour ? ((wD << 1) | (edge1 >> 31)) : ((wD >> 1) | (edge1 << 31));
-        *(pOwn + rowStride) = update_word<kHasNever>(a, own1, wC, n1, wD, sd, g0 + (uint32_t)(L >> 3), c1, stab, snever);
+        *(pOwn + rowStride) = update_word<kHasNever>(a, own1, wC, n1, wD, sd, g0 + (uint32_t)(L >> 3), c1, stab, sT, never, slot);
         wU = wD;
         wC = n1;
         wD = n2;
@@ -129,32 +156,55 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t (*
 
 template <int kColour, int kRows>
 __global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepArgs a, int bpr) {
-    __shared__ uint32_t stab[4][16];
-    __shared__ uint32_t snever[4];
+    __shared__ uint32_t stab[16];                          // U[class], class = d * 8 + nd
+    __shared__ __align__(16) uint8_t sT[kAuxBytes];        // [e][half][byte] -> 4 * class
+    __shared__ uint32_t sidx[4 * kThreads];                // per-thread slot: word e of thread t at sidx[e * 128 + t]
     pdl_launch_dependents();
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
+    for (int k = threadIdx.x; k < kAuxBytes / 16; k += blockDim.x) ((uint4*)sT)[k] = ((const uint4*)a.aux)[k];   // constant
     pdl_wait();
     const uint32_t* tab = a.tables + (size_t)b * kTableStride;
     const uint32_t never = tab[kTabNever];
-    for (int m = threadIdx.x; m < 64; m += blockDim.x) {
-        const int e = m >> 4, nib = m & 15;
-        stab[e][nib] = tab[decode_class(e, nib)];
-    }
-    if (threadIdx.x < 4) {
-        uint32_t m = 0u;
-        for (int nib = 0; nib < 16; ++nib) m |= ((never >> decode_class(threadIdx.x, nib)) & 1u) << nib;
-        snever[threadIdx.x] = m;
-    }
+    for (int m = threadIdx.x; m < 16; m += blockDim.x) stab[m] = tab[m];
     __syncthreads();
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
     const int WW = a.L >> 6;
     const int u = blk * blockDim.x + threadIdx.x;         // < (L / kRows) * WW by construction
     const int rb = u / WW, x = u - rb * WW;
-    if (never) march_rows<kColour, true, kRows>(a, stab, snever, b, rb, x);
-    else march_rows<kColour, false, kRows>(a, stab, snever, b, rb, x);
+    if (never) march_rows<kColour, true, kRows>(a, stab, sT, never, slot, b, rb, x);
+    else march_rows<kColour, false, kRows>(a, stab, sT, never, slot, b, rb, x);
 }
 
 }  // namespace
+
+// Host side of the constant lookup table: entry [e][half][v] = 4 * class of the low (half 0) / high (half 1) nibble
+// of v, where the nibble of a site 4c+e holds (D, P2, P1, P0) rotated by e bits (see update_word).
+const uint8_t* ising_bits_aux_table() {
+    static uint8_t* d_table = nullptr;
+    if (!d_table) {
+        uint8_t h[kAuxBytes];
+        for (int e = 0; e < 4; ++e)
+            for (int half = 0; half < 2; ++half)
+                for (int v = 0; v < 256; ++v) {
+                    const int nib = half ? (v >> 4) : (v & 15);
+                    const int b0 = nib & 1, b1 = (nib >> 1) & 1, b2 = (nib >> 2) & 1, b3 = (nib >> 3) & 1;
+                    int D, P0, P1, P2;
+                    switch (e) {
+                        case 0: P0 = b0; P1 = b1; P2 = b2; D = b3; break;
+                        case 1: D = b0; P0 = b1; P1 = b2; P2 = b3; break;
+                        case 2: P2 = b0; D = b1; P0 = b2; P1 = b3; break;
+                        default: P1 = b0; P2 = b1; D = b2; P0 = b3; break;
+                    }
+                    h[(e * 2 + half) * 256 + v] = (uint8_t)(4 * (D * 8 + P2 * 4 + P1 * 2 + P0));
+                }
+        uint8_t* p = nullptr;
+        if (cudaMalloc(&p, kAuxBytes) != cudaSuccess) return nullptr;
+        if (cudaMemcpy(p, h, kAuxBytes, cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(p); return nullptr; }
+        d_table = p;
+    }
+    return d_table;
+}
 
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
     const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 6) * a.batch;

@@ -169,6 +169,7 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     const uint32_t domain = sim->model == SPIN_MODEL_ISING ? kDomainIsing : kDomainPotts;
     a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)colour << 24) | (domain << 28);
     a.colour = colour;
+    a.aux = sim->layout == SPIN_LAYOUT_BITPACKED ? ising_bits_aux_table() : nullptr;
     a.rk = sim->rk;
     return a;
 }

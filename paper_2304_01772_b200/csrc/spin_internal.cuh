@@ -58,6 +58,7 @@ struct SweepArgs {
     uint32_t c2;              // low 32 bits of the sweep index t
     uint32_t c3;              // (t >> 32) & 0xFFFFFF | colour << 24 | domain << 28
     int32_t colour;
+    const uint8_t* aux;       // bit-packed kernel: nibble-pair -> 4 * class byte table (ising_bits_aux_table), else nullptr
     RoundKeys rk;
 };
 
@@ -117,6 +118,7 @@ int launch_init(const InitArgs& a, int model, int layout, cudaStream_t s);
 int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s);      // picks generic / vectorised
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s);
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s);
+const uint8_t* ising_bits_aux_table();     // device pointer to the constant 2 KiB lookup table (uploaded on first use)
 const char* ising_int8_variant(int L);
 bool ising_int8_resident_fits(int L);                                       // a replica fits one CTA's shared memory
 int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s);      // all n_sweeps in one launch
