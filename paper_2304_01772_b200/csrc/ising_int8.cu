@@ -64,7 +64,7 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
 constexpr int kRowsShort = 2;   // ... and when it does not (latency-bound shapes): four times as many threads
 #ifndef ISING_MINB
-#define ISING_MINB 7
+#define ISING_MINB 6
 #endif
 constexpr int kRowsThreads = 128;
 
@@ -185,6 +185,8 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     uint32_t edge = __ldg(pEdgeEven) & 0x04040404u;
     uint32_t g0 = (uint32_t)i0 * (uint32_t)W4 + 4u * (uint32_t)x;
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
+    __syncthreads();    // the block's threshold table (filled by the caller) is first read below: the loads above
+                        // are already in flight while the block waits for it
     // Two rows per iteration (the side-neighbour parity alternates), rolled: the body stays small enough for the
     // instruction caches, and all warps of the SM share it.
 #pragma unroll 1
@@ -194,8 +196,6 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
         const uint4 n1 = __ldg(more ? pOth : pOthLast);
         const uint4 own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
-        uint4 res = update_row<kHasNever, kColour>(a.rk, a.c2, a.c3, own, wU, wC, wD, edge, g0, c1, stab, slot);
-        *pOwn = res;
         // inputs of the next even row i+2: other-colour row i+3, own row i+2, its edge word
         uint4 n2 = n1, own2 = own1;
         uint32_t edge2 = edge1;
@@ -204,6 +204,8 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             own2 = *(pOwn + 2 * rowStride);
             edge2 = __ldg(pEdgeEven + edgeStride2);
         }
+        uint4 res = update_row<kHasNever, kColour>(a.rk, a.c2, a.c3, own, wU, wC, wD, edge, g0, c1, stab, slot);
+        *pOwn = res;
         const uint4 n1m = mask4(n1);
         res = update_row<kHasNever, 1 - kColour>(a.rk, a.c2, a.c3, own1, wC, wD, n1m, edge1 & 0x04040404u,
                                                  g0 + (uint32_t)W4, c1, stab, slot);
@@ -230,13 +232,13 @@ __global__ void __launch_bounds__(kRowsThreads, ISING_MINB) ising_int8_rows_kern
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
     pdl_wait();
+    const uint32_t never = a.tables[(size_t)b * kTableStride + kTabNever];   // block-uniform
     for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
-    __syncthreads();
     const int W16 = a.L >> 5;
     const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
-    if (stab[kTabNever]) march_rows<kColour, true, kRows>(a, stab, slot, b, rb, x);
+    if (never) march_rows<kColour, true, kRows>(a, stab, slot, b, rb, x);
     else march_rows<kColour, false, kRows>(a, stab, slot, b, rb, x);
 }
 
