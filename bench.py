@@ -202,6 +202,7 @@ def main():
     world = int(os.environ.get("WORLD_SIZE", "1"))
 
     import paper_2304_01772_b200 as sp
+    from paper_2304_01772_b200 import sharding
     w = sp.workloads.config(args.config, layout=args.layout)
     if args.sweeps:
         w.n_sweeps = args.sweeps
@@ -229,7 +230,7 @@ def main():
     nbytes = sp.spin_buffer_bytes(w.batch, w.L, model, lay)
     buf = torch.empty(nbytes, dtype=torch.int8, device="cuda")
     sim = sp.spin_create_ex(w.batch, w.L, model, q_per_replica=w.q, seed=w.seed, layout=lay,
-                            replica_offset=rank * w.batch, device_buffer=buf.data_ptr(), buffer_bytes=nbytes,
+                            replica_offset=sharding.replica_offset(rank, w.batch), device_buffer=buf.data_ptr(), buffer_bytes=nbytes,
                             cuda_stream=stream.cuda_stream, keepalive=buf)
     flush = torch.empty(256 << 20, dtype=torch.int8, device="cuda")
     E_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
@@ -278,10 +279,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     step_ms = [e[0].elapsed_time(e[2]) for e in ev]
     sweep_ms = [e[0].elapsed_time(e[1]) for e in ev]
-    total_ms = torch.tensor([sum(step_ms)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(total_ms, op=dist.ReduceOp.MAX)
-    total_ms = float(total_ms.item())
+    total_ms = sharding.max_over_ranks(sum(step_ms), device="cuda")      # the job is as slow as its slowest rank
     updates_per_step = float(w.updates) * world
     value = updates_per_step * args.steps / (total_ms * 1e6)  # flips per ns, whole job
 
@@ -299,10 +297,8 @@ def main():
         sim.spin_set_spins_ptr(host_lat.data_ptr())
         sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, offset)
         Eh, Mh = sim.spin_observables()
-    dt = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(dt, op=dist.ReduceOp.MAX)
-    e2e_value = updates_per_step * e2e_steps / (float(dt.item()) * 1e9)
+    dt = sharding.max_over_ranks(time.perf_counter() - t0, device="cuda")
+    e2e_value = updates_per_step * e2e_steps / (dt * 1e9)
     h2d = int(host_lat.numel() + w.batch * 8 + w.batch * 32 * 4)
     d2h = int(2 * w.batch * 8 + 4)
 

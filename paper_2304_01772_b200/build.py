@@ -62,5 +62,18 @@ def build(force=False, verbose=False):
     return LIB
 
 
+def build_microbench():
+    """Compile the stand-alone integer issue-rate microbenchmark (microbench/int_rates.cu -> microbench/int_rates)."""
+    nvcc = os.environ.get("NVCC", "nvcc")
+    src = os.path.join(_HERE, "microbench", "int_rates.cu")
+    out = os.path.join(_HERE, "microbench", "int_rates")
+    cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-o", out, src]
+    r = subprocess.run(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)
+    if r.returncode != 0:
+        raise RuntimeError("nvcc failed for %s:\n%s" % (src, r.stdout))
+    return out
+
+
 if __name__ == "__main__":
     print(build(force=True, verbose=True))
+    print(build_microbench())
