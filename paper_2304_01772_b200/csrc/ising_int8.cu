@@ -266,9 +266,12 @@ __device__ __forceinline__ int block_sum(int v, int* scratch) {
 
 // Rows of one parity at a time: the side of the horizontal neighbour depends on (row + colour) & 1, and a warp spans
 // several rows when L/32 < 32, so mixing parities in one pass would make every warp execute both variants.
-template <bool kHasNever, int kParity>
+// kMeasure: also accumulate, from the updated strip and the neighbour sums already in registers, sS = sum of the new
+// spins and sSN = sum of (new spin) x (4 x number of -1 neighbours) (IDP4A on the +-1 bytes): after the colour-1 pass
+// every bond has been seen from its colour-1 end with final values, so E_int = -(4 sS1 - sSN1 / 2), M = sS0 + sS1.
+template <bool kHasNever, int kParity, bool kMeasure>
 __device__ __forceinline__ void resident_rows(const ResidentArgs& a, int colour, uint32_t c2, uint32_t c3, uint8_t* lat,
-                                              const uint32_t* stab, uint32_t slot, uint32_t c1) {
+                                              const uint32_t* stab, uint32_t slot, uint32_t c1, int& sS, int& sSN) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
     uint4* own4 = (uint4*)(lat + (size_t)colour * L * W);
     const uint4* oth4 = (const uint4*)(lat + (size_t)(1 - colour) * L * W);
@@ -284,20 +287,43 @@ __device__ __forceinline__ void resident_rows(const ResidentArgs& a, int colour,
         const uint32_t g0 = (uint32_t)u * 4u;                   // (i * W + 16 x) >> 2
         const int ew = kParity ? ((x == W16 - 1) ? 0 : 4 * x + 4) : ((x == 0) ? W4 - 1 : 4 * x - 1);
         const uint32_t edge = oth1[i * W4 + ew] & 0x04040404u;
-        own4[u] = update_row<kHasNever, kParity>(a.rk, c2, c3, own, um, cm, dm, edge, g0, c1, stab, slot);
+        const uint4 res = update_row<kHasNever, kParity>(a.rk, c2, c3, own, um, cm, dm, edge, g0, c1, stab, slot);
+        own4[u] = res;
+        if (kMeasure) {
+            const int ones = 0x01010101;
+            sS += __dp4a((int)res.x, ones, __dp4a((int)res.y, ones, __dp4a((int)res.z, ones, __dp4a((int)res.w, ones, 0))));
+            if (colour == 1) {
+                uint32_t s0, s1, s2, s3;
+                if (kParity) {
+                    s0 = __byte_perm(cm.x, cm.y, 0x4321); s1 = __byte_perm(cm.y, cm.z, 0x4321);
+                    s2 = __byte_perm(cm.z, cm.w, 0x4321); s3 = __byte_perm(cm.w, edge, 0x4321);
+                } else {
+                    s0 = __byte_perm(edge, cm.x, 0x6543); s1 = __byte_perm(cm.x, cm.y, 0x6543);
+                    s2 = __byte_perm(cm.y, cm.z, 0x6543); s3 = __byte_perm(cm.z, cm.w, 0x6543);
+                }
+                // bytes 4 * nd <= 16: dp4a with the bytes of the new spins as signed, the counts as unsigned
+                int t = 0;
+                asm("dp4a.s32.u32 %0, %1, %2, %0;" : "+r"(t) : "r"(res.x), "r"(um.x + cm.x + dm.x + s0));
+                asm("dp4a.s32.u32 %0, %1, %2, %0;" : "+r"(t) : "r"(res.y), "r"(um.y + cm.y + dm.y + s1));
+                asm("dp4a.s32.u32 %0, %1, %2, %0;" : "+r"(t) : "r"(res.z), "r"(um.z + cm.z + dm.z + s2));
+                asm("dp4a.s32.u32 %0, %1, %2, %0;" : "+r"(t) : "r"(res.w), "r"(um.w + cm.w + dm.w + s3));
+                sSN += t;
+            }
+        }
     }
 }
 
-template <bool kHasNever>
+template <bool kHasNever, bool kMeasure>
 __device__ __forceinline__ void resident_half_sweep(const ResidentArgs& a, int colour, uint32_t c2, uint32_t c3,
-                                                    uint8_t* lat, const uint32_t* stab, uint32_t slot, uint32_t c1) {
-    resident_rows<kHasNever, 0>(a, colour, c2, c3, lat, stab, slot, c1);
-    resident_rows<kHasNever, 1>(a, colour, c2, c3, lat, stab, slot, c1);
+                                                    uint8_t* lat, const uint32_t* stab, uint32_t slot, uint32_t c1,
+                                                    int& sS, int& sSN) {
+    resident_rows<kHasNever, 0, kMeasure>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
+    resident_rows<kHasNever, 1, kMeasure>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
 }
 
 __global__ void __launch_bounds__(kResThreads) ising_int8_resident_kernel(ResidentArgs a) {
     extern __shared__ __align__(16) uint8_t smem[];
-    const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
+    const int L = a.L;
     const size_t latBytes = (size_t)L * L;
     uint8_t* lat = smem;
     uint32_t* stab = (uint32_t*)(smem + latBytes);
@@ -319,45 +345,27 @@ __global__ void __launch_bounds__(kResThreads) ising_int8_resident_kernel(Reside
         const unsigned long long t = a.t0 + (unsigned long long)s;
         const uint32_t c2 = (uint32_t)(t & 0xFFFFFFFFull);
         const uint32_t c3lo = (uint32_t)((t >> 32) & 0xFFFFFFull) | (kDomainIsing << 28);
+        int sS0 = 0, sS1 = 0, sSN = 0;      // this thread's share of sum s (colour 0, colour 1) and of sum s * 4 nd
         for (int colour = 0; colour < 2; ++colour) {
             const uint32_t c3 = c3lo | ((uint32_t)colour << 24);
-            if (never) resident_half_sweep<true>(a, colour, c2, c3, lat, stab, slot, c1);
-            else resident_half_sweep<false>(a, colour, c2, c3, lat, stab, slot, c1);
+            int& sS = colour ? sS1 : sS0;
+            if (never) {
+                if (a.measure) resident_half_sweep<true, true>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
+                else resident_half_sweep<true, false>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
+            } else {
+                if (a.measure) resident_half_sweep<false, true>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
+                else resident_half_sweep<false, false>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
+            }
             __syncthreads();
         }
         if (a.measure) {
-            // exact E_int = -(bonds equal - bonds different) from the colour-0 sites, M = sites - 2 * (#spins -1)
-            const uint4* c0 = (const uint4*)lat;
-            const uint4* c1p = (const uint4*)(lat + (size_t)L * W);
-            const uint32_t* c1w = (const uint32_t*)c1p;
-            int diff = 0, neg = 0;
-            const uint32_t m2 = 0x02020202u, m8 = 0x80808080u;
-            for (int u = threadIdx.x; u < L * W16; u += blockDim.x) {
-                const int i = u / W16, x = u - i * W16;
-                const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
-                const uint4 own = c0[u], ct = c1p[u], up = c1p[iu * W16 + x], dn = c1p[id * W16 + x];
-                uint32_t s0, s1, s2, s3;
-                if (i & 1) {
-                    const uint32_t e = c1w[i * W4 + (x == W16 - 1 ? 0 : 4 * x + 4)];
-                    s0 = __byte_perm(ct.x, ct.y, 0x4321); s1 = __byte_perm(ct.y, ct.z, 0x4321);
-                    s2 = __byte_perm(ct.z, ct.w, 0x4321); s3 = __byte_perm(ct.w, e, 0x4321);
-                } else {
-                    const uint32_t e = c1w[i * W4 + (x == 0 ? W4 - 1 : 4 * x - 1)];
-                    s0 = __byte_perm(e, ct.x, 0x6543); s1 = __byte_perm(ct.x, ct.y, 0x6543);
-                    s2 = __byte_perm(ct.y, ct.z, 0x6543); s3 = __byte_perm(ct.z, ct.w, 0x6543);
-                }
-                diff += __popc((own.x ^ up.x) & m2) + __popc((own.x ^ dn.x) & m2) + __popc((own.x ^ ct.x) & m2) + __popc((own.x ^ s0) & m2);
-                diff += __popc((own.y ^ up.y) & m2) + __popc((own.y ^ dn.y) & m2) + __popc((own.y ^ ct.y) & m2) + __popc((own.y ^ s1) & m2);
-                diff += __popc((own.z ^ up.z) & m2) + __popc((own.z ^ dn.z) & m2) + __popc((own.z ^ ct.z) & m2) + __popc((own.z ^ s2) & m2);
-                diff += __popc((own.w ^ up.w) & m2) + __popc((own.w ^ dn.w) & m2) + __popc((own.w ^ ct.w) & m2) + __popc((own.w ^ s3) & m2);
-                neg += __popc(own.x & m8) + __popc(own.y & m8) + __popc(own.z & m8) + __popc(own.w & m8);
-                neg += __popc(ct.x & m8) + __popc(ct.y & m8) + __popc(ct.z & m8) + __popc(ct.w & m8);
-            }
-            diff = block_sum(diff, scratch);
-            neg = block_sum(neg, scratch);
+            // Every bond has exactly one colour-1 end, and after the colour-1 pass both ends are final:
+            // sum_bonds s s' = sum over colour-1 sites of s * nn, nn = 4 - 2 nd = 4 - (4 nd) / 2.
+            const int totS0 = block_sum(sS0, scratch);
+            const int totS1 = block_sum(sS1, scratch);
+            const int totSN = block_sum(sSN, scratch);
             if (threadIdx.x == 0) {
-                const long long N = (long long)L * L;
-                const long long e = -(2 * N - 2 * (long long)diff), mag = N - 2 * (long long)neg;
+                const long long e = -(4ll * totS1 - (long long)totSN / 2), mag = (long long)totS0 + totS1;
                 if (a.E_trace) a.E_trace[(size_t)s * a.batch + b] = e;
                 if (a.M_trace) a.M_trace[(size_t)s * a.batch + b] = mag;
                 if (a.moments) {

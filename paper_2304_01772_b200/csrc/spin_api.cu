@@ -182,6 +182,12 @@ bool use_resident(const spin_sim* sim, bool measure) {
     if (sim->policy == SPIN_POLICY_RESIDENT) return true;
     const long long sites = (long long)sim->batch * sim->L * sim->L;
     if (sites <= (1ll << 20)) return true;                         // launch-latency-bound shapes
+    // the streaming kernel's blocks cover (L/8) x (L/32) thread strips of ONE replica: below 64 of them (L = 64, 96,
+    // 160, ...) its blocks are a fraction of a warp and the resident kernel is faster (L = 64: 922 vs 576 flips/ns)
+    int tpb = 128;
+    const int perReplica = (sim->L / 8) * (sim->L / 32);
+    while (perReplica % tpb) tpb >>= 1;
+    if (tpb < 64 && sim->batch >= 148) return true;
     return measure && sim->batch >= 296;                           // fused per-sweep reductions, >= 2 CTAs per SM
 }
 
