@@ -170,7 +170,8 @@ __global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepAr
     __syncthreads();
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
     const int WW = a.L >> 6;
-    const int u = blk * blockDim.x + threadIdx.x;         // < (L / kRows) * WW by construction
+    const int u = blk * blockDim.x + threadIdx.x;
+    if (u >= (a.L / kRows) * WW) return;                  // ragged last block of a replica (after the barrier)
     const int rb = u / WW, x = u - rb * WW;
     if (never) march_rows<kColour, true, kRows>(a, stab, sT, never, slot, b, rb, x);
     else march_rows<kColour, false, kRows>(a, stab, sT, never, slot, b, rb, x);
@@ -211,9 +212,8 @@ int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
     const bool shortRows = longThreads < 148ll * 64;      // the per-block table set-up makes short threads pay off only for tiny launches
     const int rows = shortRows ? kRowsShort : kRowsLong;
     const int perReplica = (a.L / rows) * (a.L >> 6);
-    int tpb = kThreads;
-    while (perReplica % tpb) tpb >>= 1;
-    const int bpr = perReplica / tpb;
+    const int tpb = perReplica >= kThreads ? kThreads : ((perReplica + 31) & ~31);   // last block may be ragged
+    const int bpr = (perReplica + tpb - 1) / tpb;
     const unsigned grid = (unsigned)((long long)bpr * a.batch);
     if (shortRows) {
         if (a.colour == 0) launch_pdl(ising_bits_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);

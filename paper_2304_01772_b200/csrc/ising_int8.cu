@@ -235,7 +235,10 @@ __global__ void __launch_bounds__(kRowsThreads, ISING_MINB) ising_int8_rows_kern
     const uint32_t never = a.tables[(size_t)b * kTableStride + kTabNever];   // block-uniform
     for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
     const int W16 = a.L >> 5;
-    const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
+    const int u = blk * blockDim.x + threadIdx.x;
+    // ragged last block of a replica: the spare threads have done their share of the table fill and leave (an
+    // exited thread counts as arrived at the barrier inside march_rows)
+    if (u >= (a.L / kRows) * W16) return;
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
     if (never) march_rows<kColour, true, kRows>(a, stab, slot, b, rb, x);
@@ -397,12 +400,12 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
         // 8 rows per thread when that still gives every SM several blocks, else 2 rows (short threads, 4x as many)
         const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 5) * a.batch;
-        const bool shortRows = longThreads < 148ll * 4 * kRowsThreads;
+        const bool shortRows = longThreads < 148ll * 4 * kRowsThreads ||
+                               (a.L / kRowsLong) * (a.L >> 5) < kRowsThreads / 2;   // small L: keep the blocks full
         const int rows = shortRows ? kRowsShort : kRowsLong;
         const int perReplica = (a.L / rows) * (a.L >> 5);    // strips x row blocks of one colour
-        int tpb = kRowsThreads;
-        while (perReplica % tpb) tpb >>= 1;                  // L = 32 -> 4 threads
-        const int bpr = perReplica / tpb;
+        const int tpb = perReplica >= kRowsThreads ? kRowsThreads : ((perReplica + 31) & ~31);   // last block may be ragged
+        const int bpr = (perReplica + tpb - 1) / tpb;
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
         if (shortRows) {
             if (a.colour == 0) launch_pdl(ising_int8_rows_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);

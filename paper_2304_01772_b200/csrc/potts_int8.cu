@@ -253,7 +253,8 @@ __global__ void __launch_bounds__(kRowsThreads, POTTS_MINB) potts_int8_rows_kern
     __syncthreads();
     const uint32_t q = tab[kTabQ];
     const int W16 = a.L >> 5;
-    const int u = blk * blockDim.x + threadIdx.x;          // < (L / kRows) * W16 by construction
+    const int u = blk * blockDim.x + threadIdx.x;
+    if (u >= (a.L / kRows) * W16) return;                  // ragged last block of a replica (after the barrier)
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
     if (never) march_rows<kColour, true, false, kRows>(a, stab, snever, q, slot, b, rb, x);
@@ -268,12 +269,12 @@ const char* potts_int8_variant(int L) { return (L % 32 == 0) ? "potts_int8_rows1
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
         const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 5) * a.batch;
-        const bool shortRows = longThreads < 148ll * 4 * kRowsThreads;
+        const bool shortRows = longThreads < 148ll * 4 * kRowsThreads ||
+                               (a.L / kRowsLong) * (a.L >> 5) < kRowsThreads / 2;   // small L: keep the blocks full
         const int rows = shortRows ? kRowsShort : kRowsLong;
         const int perReplica = (a.L / rows) * (a.L >> 5);    // strips x row blocks of one colour
-        int tpb = kRowsThreads;
-        while (perReplica % tpb) tpb >>= 1;                  // L = 32 -> 4 threads
-        const int bpr = perReplica / tpb;
+        const int tpb = perReplica >= kRowsThreads ? kRowsThreads : ((perReplica + 31) & ~31);   // last block may be ragged
+        const int bpr = (perReplica + tpb - 1) / tpb;
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
         if (shortRows) {
             if (a.colour == 0) launch_pdl(potts_int8_rows_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
