@@ -16,6 +16,7 @@ _LIB = os.path.join(_HERE, "liboracle.so")
 __all__ = [
     "build", "philox4x32_10", "ising_table", "potts_table", "init", "ising_half_sweep",
     "potts_half_sweep", "ising_observables", "potts_observables", "accumulate_moments", "sweep",
+    "sweep_bonds", "ising_bonds_observables", "ising_bonds_half_sweep",
 ]
 
 
@@ -50,6 +51,11 @@ def _l():
         lib.oracle_accumulate_moments.argtypes = [p, c.c_int32, p, p]
         lib.oracle_sweep.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, p, c.c_double, c.c_double,
                                      c.c_uint64, c.c_int64, c.c_int64, c.c_int64, p, p, p]
+        lib.oracle_ising_bonds_observables.argtypes = [p, p, p, c.c_int32, c.c_int32, p, p]
+        lib.oracle_ising_bonds_half_sweep.argtypes = [p, p, p, c.c_int32, c.c_int32, p, c.c_double, c.c_double,
+                                                      c.c_uint64, c.c_int64, c.c_int64, c.c_int32]
+        lib.oracle_sweep_bonds.argtypes = [p, p, p, c.c_int32, c.c_int32, p, c.c_double, c.c_double, c.c_uint64,
+                                           c.c_int64, c.c_int64, c.c_int64, p, p]
         _lib = lib
     return _lib
 
@@ -163,3 +169,41 @@ def sweep(spins, beta, J, h, seed, n_sweeps, sweep_offset=0, q=None, replica_off
                       int(seed), int(replica_offset), int(n_sweeps), int(sweep_offset),
                       _ptr(Et), _ptr(Mt), _ptr(moments))
     return (Et, Mt) if trace else None
+
+
+def _bonds(J, B, L):
+    a = np.ascontiguousarray(np.broadcast_to(np.asarray(J, dtype=np.int8), (B, L, L)))
+    assert np.all(np.abs(a) == 1), "bond signs must be +-1"
+    return a
+
+
+def ising_bonds_observables(spins, Jh, Jv):
+    """E_int = -sum_bonds J_ij s_i s_j, M = sum s for +-1 bond signs Jh (right bonds), Jv (down bonds)."""
+    B, L = _lattice(spins)
+    jh, jv = _bonds(Jh, B, L), _bonds(Jv, B, L)
+    E = np.zeros(B, dtype=np.int64)
+    M = np.zeros(B, dtype=np.int64)
+    _l().oracle_ising_bonds_observables(_ptr(spins), _ptr(jh), _ptr(jv), B, L, _ptr(E), _ptr(M))
+    return E, M
+
+
+def sweep_bonds(spins, Jh, Jv, beta, J, h, seed, n_sweeps, sweep_offset=0, replica_offset=0, trace=False):
+    """Ising sweeps with +-1 bond signs (Jh[b][i][j]: bond (i,j)-(i,j+1); Jv[b][i][j]: bond (i,j)-(i+1,j)), in place."""
+    B, L = _lattice(spins)
+    ba = _beta_array(beta, B)
+    jh, jv = _bonds(Jh, B, L), _bonds(Jv, B, L)
+    Et = Mt = None
+    if trace:
+        Et = np.zeros((n_sweeps, B), dtype=np.int64)
+        Mt = np.zeros((n_sweeps, B), dtype=np.int64)
+    _l().oracle_sweep_bonds(_ptr(spins), _ptr(jh), _ptr(jv), B, L, _ptr(ba), float(J), float(h), int(seed),
+                            int(replica_offset), int(n_sweeps), int(sweep_offset), _ptr(Et), _ptr(Mt))
+    return (Et, Mt) if trace else None
+
+
+def ising_bonds_half_sweep(spins, Jh, Jv, beta, J, h, seed, t, colour, replica_offset=0):
+    B, L = _lattice(spins)
+    ba = _beta_array(beta, B)
+    jh, jv = _bonds(Jh, B, L), _bonds(Jv, B, L)
+    _l().oracle_ising_bonds_half_sweep(_ptr(spins), _ptr(jh), _ptr(jv), B, L, _ptr(ba), float(J), float(h),
+                                       int(seed), int(replica_offset), int(t), int(colour))

@@ -325,4 +325,83 @@ void oracle_sweep(int8_t* spins, int32_t batch, int32_t L, int32_t model_potts, 
     std::free(M);
 }
 
+// ---- +-J couplings (Eq. 1 is written with per-bond J_ij, and the
+// paper's Fig. 9 minimises a +-J spin glass).  Reading: every bond carries a sign
+// Jh[b][i][j] (between (i,j) and (i,j+1 mod L)) or Jv[b][i][j] (between (i,j) and (i+1 mod L,j)), values +-1, and
+// H = -J sum_bonds J_ij s_i s_j - h sum_i s_i.  The local field of a site is the bond-weighted neighbour sum
+// nn = Jv[i-1][j] s(i-1,j) + Jv[i][j] s(i+1,j) + Jh[i][j-1] s(i,j-1) + Jh[i][j] s(i,j+1), still in {-4..4}, so
+// the class table, the random words and the accept rule are those of the uniform model (O2, O4, O5).
+void oracle_ising_bonds_half_sweep(int8_t* spins, const int8_t* Jh, const int8_t* Jv, int32_t batch, int32_t L,
+                                   const double* beta, double J, double h, uint64_t seed,
+                                   int64_t replica_offset, int64_t t, int32_t colour) {
+    const int64_t N = (int64_t)L * L;
+    const int half = L / 2;
+    for (int32_t b = 0; b < batch; ++b) {
+        uint32_t T[10];
+        uint8_t always[10];
+        oracle_ising_table(beta[b], J, h, T, always);
+        int8_t* lat = spins + (int64_t)b * N;
+        const int8_t* jh = Jh + (int64_t)b * N;
+        const int8_t* jv = Jv + (int64_t)b * N;
+        uint32_t replica = (uint32_t)(b + replica_offset);
+        for (int i = 0; i < L; ++i) {
+            for (int j = 0; j < L; ++j) {
+                if (((i + j) & 1) != colour) continue;
+                int s = lat[(int64_t)i * L + j];
+                int nn = jv[(int64_t)wrap(i - 1, L) * L + j] * lat[(int64_t)wrap(i - 1, L) * L + j] +
+                         jv[(int64_t)i * L + j] * lat[(int64_t)wrap(i + 1, L) * L + j] +
+                         jh[(int64_t)i * L + wrap(j - 1, L)] * lat[(int64_t)i * L + wrap(j - 1, L)] +
+                         jh[(int64_t)i * L + j] * lat[(int64_t)i * L + wrap(j + 1, L)];
+                int64_t n = (int64_t)i * half + (j >> 1);
+                uint32_t out[4];
+                draw(seed, (uint32_t)(n >> 2), replica, (uint64_t)t, (uint32_t)colour, DOMAIN_ISING, out);
+                uint32_t r = out[n & 3];
+                int cls = 5 * ((s + 1) / 2) + (nn + 4) / 2;
+                if (accept(r, T[cls], always[cls])) lat[(int64_t)i * L + j] = (int8_t)(-s);
+            }
+        }
+    }
+}
+
+// E_int = -sum_bonds J_ij s_i s_j (each bond once: the right and the down bond of every site), M = sum s.
+void oracle_ising_bonds_observables(const int8_t* spins, const int8_t* Jh, const int8_t* Jv, int32_t batch,
+                                    int32_t L, int64_t* E, int64_t* M) {
+    const int64_t N = (int64_t)L * L;
+    for (int32_t b = 0; b < batch; ++b) {
+        const int8_t* lat = spins + (int64_t)b * N;
+        const int8_t* jh = Jh + (int64_t)b * N;
+        const int8_t* jv = Jv + (int64_t)b * N;
+        int64_t S = 0, m = 0;
+        for (int i = 0; i < L; ++i) {
+            for (int j = 0; j < L; ++j) {
+                int s = lat[(int64_t)i * L + j];
+                S += s * (jh[(int64_t)i * L + j] * lat[(int64_t)i * L + wrap(j + 1, L)] +
+                          jv[(int64_t)i * L + j] * lat[(int64_t)wrap(i + 1, L) * L + j]);
+                m += s;
+            }
+        }
+        E[b] = -S;
+        M[b] = m;
+    }
+}
+
+void oracle_sweep_bonds(int8_t* spins, const int8_t* Jh, const int8_t* Jv, int32_t batch, int32_t L,
+                        const double* beta, double J, double h, uint64_t seed, int64_t replica_offset,
+                        int64_t n_sweeps, int64_t sweep_offset, int64_t* E_trace, int64_t* M_trace) {
+    int64_t* E = (int64_t*)std::malloc(sizeof(int64_t) * (size_t)batch);
+    int64_t* M = (int64_t*)std::malloc(sizeof(int64_t) * (size_t)batch);
+    for (int64_t local = 0; local < n_sweeps; ++local) {
+        int64_t t = sweep_offset + local;
+        for (int colour = 0; colour < 2; ++colour)
+            oracle_ising_bonds_half_sweep(spins, Jh, Jv, batch, L, beta, J, h, seed, replica_offset, t, colour);
+        if (E_trace || M_trace) {
+            oracle_ising_bonds_observables(spins, Jh, Jv, batch, L, E, M);
+            if (E_trace) std::memcpy(E_trace + local * batch, E, sizeof(int64_t) * (size_t)batch);
+            if (M_trace) std::memcpy(M_trace + local * batch, M, sizeof(int64_t) * (size_t)batch);
+        }
+    }
+    std::free(E);
+    std::free(M);
+}
+
 }  // extern "C"
