@@ -155,6 +155,16 @@ SPIN_API int64_t spin_kernel_launches(const spin_sim* sim);
 /* Human-readable name of the sweep kernel variant the handle selects for its shape (diagnostics). */
 SPIN_API const char* spin_kernel_variant(const spin_sim* sim);
 
+/* +-J couplings (the paper writes Eq. 1 with a coupling J_ij per bond, and minimises a +-J spin glass
+ * in Fig. 9).  Jh, Jv: HOST arrays, natural layout [batch][L][L], values +1 / -1:
+ * Jh[b][i][j] is the sign of the bond between (i, j) and (i, (j+1) mod L), Jv[b][i][j] of the bond between (i, j) and
+ * ((i+1) mod L, j).  From then on spin_sweep* use H = -J sum_bonds J_ij s_i s_j - h sum_i s_i (the local field is the
+ * bond-weighted neighbour sum; thresholds, random words and acceptance are unchanged) and spin_observables* return
+ * E_int = -sum_bonds J_ij s_i s_j.  Both NULL: back to uniform couplings.  The arrays are copied before return.
+ * Implemented for the Ising model in the bit-packed layout (SPIN_ERR_UNSUPPORTED otherwise); SPIN_ERR_INVALID for a
+ * NULL handle, exactly one NULL array, or a value that is not +-1 (the handle is left unchanged). */
+SPIN_API int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv);
+
 /* Kernel selection policy (diagnostics / tests; the results never depend on it: every path computes the same
  * lattice).  SPIN_POLICY_AUTO picks per shape; SPIN_POLICY_STREAMING forces the two-launches-
  * per-sweep HBM kernels; SPIN_POLICY_RESIDENT uses the shared-memory-resident multi-sweep kernel (one CTA per

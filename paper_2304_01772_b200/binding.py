@@ -59,6 +59,7 @@ def load_library():
         "spin_kernel_launches": (i64, [vp]),
         "spin_kernel_variant": (c.c_char_p, [vp]),
         "spin_set_policy": (c.c_int, [vp, i32]),
+        "spin_set_bonds": (c.c_int, [vp, vp, vp]),
     }
     for name, (res, args) in protos.items():
         fn = getattr(lib, name)
@@ -72,7 +73,7 @@ EXPORTED_SYMBOLS = (
     "spin_create", "spin_sweep", "spin_observables", "spin_destroy", "spin_last_error", "spin_buffer_bytes",
     "spin_create_ex", "spin_set_stream", "spin_get_spins", "spin_set_spins", "spin_sweep_measure",
     "spin_observables_dev", "spin_synchronize", "spin_threshold_table", "spin_kernel_launches",
-    "spin_kernel_variant", "spin_set_policy",
+    "spin_kernel_variant", "spin_set_policy", "spin_set_bonds",
 )
 
 
@@ -164,6 +165,16 @@ class SpinSim:
 
     def spin_kernel_launches(self):
         return int(load_library().spin_kernel_launches(self._h))
+
+    def spin_set_bonds(self, Jh, Jv):
+        """+-1 bond signs, natural layout [batch][L][L] (broadcast from [L][L]); (None, None) removes them."""
+        if Jh is None and Jv is None:
+            _check(load_library().spin_set_bonds(self._h, None, None))
+            return
+        shape = (self.batch, self.L, self.L)
+        jh = np.ascontiguousarray(np.broadcast_to(np.asarray(Jh, dtype=np.int8), shape))
+        jv = np.ascontiguousarray(np.broadcast_to(np.asarray(Jv, dtype=np.int8), shape))
+        _check(load_library().spin_set_bonds(self._h, _np_ptr(jh), _np_ptr(jv)))
 
     def spin_set_policy(self, policy):
         _check(load_library().spin_set_policy(self._h, int(policy)))

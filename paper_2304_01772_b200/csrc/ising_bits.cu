@@ -101,7 +101,9 @@ __device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own
 // Row-marching: one thread owns word x of kRows consecutive rows (same skeleton as ising_int8.cu: the three
 // other-colour words it needs stay in registers, running pointers, two rows per rolled iteration because the side
 // of the horizontal neighbour alternates, programmatic dependent launch).
-template <int kColour, bool kHasNever, int kRows>
+// kBonds: +-J couplings (SweepArgs::bonds): the neighbour words are XORed with the sign planes of the bonds that
+// join them to the row's sites, so the adder counts neighbours whose bond-weighted spin is -1; nothing else changes.
+template <int kColour, bool kHasNever, int kRows, bool kBonds>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint8_t* sT, uint32_t never,
                                            uint32_t slot, int b, int rb, int x) {
     const int L = a.L, WW = L >> 6;                       // words per colour-row
@@ -125,14 +127,23 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     uint32_t edge = __ldg(pEdgeEven);
     uint32_t g0 = (uint32_t)i0 * (uint32_t)(L >> 3) + 8u * (uint32_t)x;   // (i*(L/2) + 32x) >> 2
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
+    // bond sign planes of this colour: plane p of row i, word x at pB[p * half + i * WW + x]
+    const uint32_t* pB = kBonds ? a.bonds + ((size_t)b * 2 + kColour) * 4 * half + (size_t)i0 * WW + x : nullptr;
 #pragma unroll 1
     for (int rr = 0; rr < kRows; rr += 2) {
         const bool more = rr + 2 < kRows;
         const uint32_t n1 = __ldg(more ? pOth : pOthLast);
         const uint32_t own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
+        uint32_t bu = 0u, bd = 0u, bc = 0u, bs = 0u, bu1 = 0u, bd1 = 0u, bc1 = 0u, bs1 = 0u;
+        if (kBonds) {
+            bu = __ldg(pB); bd = __ldg(pB + half); bc = __ldg(pB + 2 * half); bs = __ldg(pB + 3 * half);
+            bu1 = __ldg(pB + rowStride); bd1 = __ldg(pB + half + rowStride);
+            bc1 = __ldg(pB + 2 * half + rowStride); bs1 = __ldg(pB + 3 * half + rowStride);
+            pB += 2 * rowStride;
+        }
         uint32_t sd = kColour ? ((wC >> 1) | (edge << 31)) : ((wC << 1) | (edge >> 31));
-        *pOwn = update_word<kHasNever>(a, own, wU, wD, wC, sd, g0, c1, stab, sT, never, slot);
+        *pOwn = update_word<kHasNever>(a, own, wU ^ bu, wD ^ bd, wC ^ bc, sd ^ bs, g0, c1, stab, sT, never, slot);
         uint32_t n2 = n1, own2 = own1, edge2 = edge1;
         if (more) {
             n2 = __ldg(pOth + rowStride);
@@ -140,7 +151,8 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             edge2 = __ldg(pEdgeEven + 2 * rowStride);
         }
         sd = kColour ? ((wD << 1) | (edge1 >> 31)) : ((wD >> 1) | (edge1 << 31));
-        *(pOwn + rowStride) = update_word<kHasNever>(a, own1, wC, n1, wD, sd, g0 + (uint32_t)(L >> 3), c1, stab, sT, never, slot);
+        *(pOwn + rowStride) = update_word<kHasNever>(a, own1, wC ^ bu1, n1 ^ bd1, wD ^ bc1, sd ^ bs1, g0 + (uint32_t)(L >> 3),
+                                                     c1, stab, sT, never, slot);
         wU = wD;
         wC = n1;
         wD = n2;
@@ -154,7 +166,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     }
 }
 
-template <int kColour, int kRows>
+template <int kColour, int kRows, bool kBonds>
 __global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[16];                          // U[class], class = d * 8 + nd
     __shared__ __align__(16) uint8_t sT[kAuxBytes];        // [e][half][byte] -> 4 * class
@@ -173,8 +185,8 @@ __global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepAr
     const int u = blk * blockDim.x + threadIdx.x;
     if (u >= (a.L / kRows) * WW) return;                  // ragged last block of a replica (after the barrier)
     const int rb = u / WW, x = u - rb * WW;
-    if (never) march_rows<kColour, true, kRows>(a, stab, sT, never, slot, b, rb, x);
-    else march_rows<kColour, false, kRows>(a, stab, sT, never, slot, b, rb, x);
+    if (never) march_rows<kColour, true, kRows, kBonds>(a, stab, sT, never, slot, b, rb, x);
+    else march_rows<kColour, false, kRows, kBonds>(a, stab, sT, never, slot, b, rb, x);
 }
 
 }  // namespace
@@ -215,13 +227,16 @@ int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
     const int tpb = perReplica >= kThreads ? kThreads : ((perReplica + 31) & ~31);   // last block may be ragged
     const int bpr = (perReplica + tpb - 1) / tpb;
     const unsigned grid = (unsigned)((long long)bpr * a.batch);
+    const bool bonds = a.bonds != nullptr;
+    void (*k)(SweepArgs, int);
     if (shortRows) {
-        if (a.colour == 0) launch_pdl(ising_bits_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
-        else launch_pdl(ising_bits_kernel<1, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
+        if (bonds) k = a.colour == 0 ? ising_bits_kernel<0, kRowsShort, true> : ising_bits_kernel<1, kRowsShort, true>;
+        else k = a.colour == 0 ? ising_bits_kernel<0, kRowsShort, false> : ising_bits_kernel<1, kRowsShort, false>;
     } else {
-        if (a.colour == 0) launch_pdl(ising_bits_kernel<0, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
-        else launch_pdl(ising_bits_kernel<1, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
+        if (bonds) k = a.colour == 0 ? ising_bits_kernel<0, kRowsLong, true> : ising_bits_kernel<1, kRowsLong, true>;
+        else k = a.colour == 0 ? ising_bits_kernel<0, kRowsLong, false> : ising_bits_kernel<1, kRowsLong, false>;
     }
+    launch_pdl(k, grid, (unsigned)tpb, s, a, bpr);
     return 1;
 }
 

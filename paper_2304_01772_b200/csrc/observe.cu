@@ -102,8 +102,9 @@ __global__ void __launch_bounds__(256) ising_int8_observe_vec_kernel(const int8_
     block_add2(-(64 * cnt - 2 * diff), 32 * cnt - 2 * neg, E_acc ? E_acc + b : nullptr, M_acc ? M_acc + b : nullptr);
 }
 
-__global__ void ising_bits_observe_kernel(const uint32_t* __restrict__ lat, int L, int bpr, long long* E_acc,
-                                          long long* M_acc) {
+// bonds (or nullptr): sign planes of the +-J couplings, [B][2][4][L][L/64]; only the colour-0 planes are read.
+__global__ void ising_bits_observe_kernel(const uint32_t* __restrict__ lat, const uint32_t* __restrict__ bonds, int L,
+                                          int bpr, long long* E_acc, long long* M_acc) {
     const int WW = L >> 6;
     const int b = blockIdx.x / bpr, blk = blockIdx.x - b * bpr;
     const size_t half = (size_t)L * WW;
@@ -117,9 +118,15 @@ __global__ void ising_bits_observe_kernel(const uint32_t* __restrict__ lat, int 
         uint32_t sd;
         if (i & 1) sd = (ct >> 1) | (c1[(size_t)i * WW + (x == WW - 1 ? 0 : x + 1)] << 31);
         else sd = (ct << 1) | (c1[(size_t)i * WW + (x == 0 ? WW - 1 : x - 1)] >> 31);
-        // s * nbr = +1 if equal, -1 if different: sum over 32 sites and 4 neighbours = 128 - 2 * (#different)
-        const int diff = __popc(own ^ c1[(size_t)iu * WW + x]) + __popc(own ^ c1[(size_t)id * WW + x]) +
-                         __popc(own ^ ct) + __popc(own ^ sd);
+        // s * nbr = +1 if equal, -1 if different: sum over 32 sites and 4 neighbours = 128 - 2 * (#different);
+        // with bond signs J s s' = -1 iff (s differs from s') xor (bond is -1)
+        uint32_t bu = 0u, bd = 0u, bc = 0u, bs = 0u;
+        if (bonds) {
+            const uint32_t* pb = bonds + (size_t)b * 2 * 4 * half + n;
+            bu = pb[0]; bd = pb[half]; bc = pb[2 * half]; bs = pb[3 * half];
+        }
+        const int diff = __popc(own ^ c1[(size_t)iu * WW + x] ^ bu) + __popc(own ^ c1[(size_t)id * WW + x] ^ bd) +
+                         __popc(own ^ ct ^ bc) + __popc(own ^ sd ^ bs);
         e -= 128 - 2 * diff;
         m += 64 - 2 * (__popc(own) + __popc(c1[n]));
     }
@@ -294,10 +301,11 @@ int launch_ising_int8_observe(const void* lattice, int batch, int L, long long* 
     return 1;
 }
 
-int launch_ising_bits_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s) {
+int launch_ising_bits_observe(const void* lattice, const uint32_t* bonds, int batch, int L, long long* E_acc,
+                              long long* M_acc, cudaStream_t s) {
     const long long half = (long long)L * (L >> 6);
     const int tpb = 256, bpr = blocks_per_replica(half, tpb, batch);
-    ising_bits_observe_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const uint32_t*)lattice, L, bpr, E_acc, M_acc);
+    ising_bits_observe_kernel<<<(unsigned)((long long)bpr * batch), tpb, 0, s>>>((const uint32_t*)lattice, bonds, L, bpr, E_acc, M_acc);
     return 1;
 }
 

@@ -97,6 +97,7 @@ struct spin_sim {
     long long* d_EM = nullptr;       // [2][B] accumulators
     unsigned int* d_hist = nullptr;  // [B][128] (Potts)
     unsigned int* d_bad = nullptr;   // validation counter
+    uint32_t* d_bonds = nullptr;     // +-J sign planes [B][2][4][L][L/64] (bit-packed layout) or nullptr
     // scratch (host, pinned)
     uint32_t* h_tables = nullptr;
     RoundKeys rk;
@@ -170,6 +171,7 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)colour << 24) | (domain << 28);
     a.colour = colour;
     a.aux = sim->layout == SPIN_LAYOUT_BITPACKED ? ising_bits_aux_table() : nullptr;
+    a.bonds = sim->d_bonds;
     a.rk = sim->rk;
     return a;
 }
@@ -227,7 +229,7 @@ int enqueue_observe(spin_sim* sim, long long* E_out, long long* M_out) {
     } else {
         if (M_out) CUDA_TRY(cudaMemsetAsync(M_out, 0, nb, sim->stream));
         if (sim->layout == SPIN_LAYOUT_BITPACKED)
-            sim->launches += launch_ising_bits_observe(sim->lattice, sim->batch, sim->L, E_out, M_out, sim->stream);
+            sim->launches += launch_ising_bits_observe(sim->lattice, sim->d_bonds, sim->batch, sim->L, E_out, M_out, sim->stream);
         else
             sim->launches += launch_ising_int8_observe(sim->lattice, sim->batch, sim->L, E_out, M_out, sim->stream);
     }
@@ -282,6 +284,7 @@ void spin_destroy(spin_sim* sim) {
     if (sim->stream || sim->lattice) cudaStreamSynchronize(sim->stream);
     if (sim->owns_lattice && sim->lattice) cudaFree(sim->lattice);
     if (sim->d_tables) cudaFree(sim->d_tables);
+    if (sim->d_bonds) cudaFree(sim->d_bonds);
     if (sim->d_q) cudaFree(sim->d_q);
     if (sim->d_EM) cudaFree(sim->d_EM);
     if (sim->d_hist) cudaFree(sim->d_hist);
@@ -402,6 +405,61 @@ const char* spin_kernel_variant(const spin_sim* sim) {
     if (sim->layout == SPIN_LAYOUT_BITPACKED) return "ising_bits_rows32";
     if (use_resident(sim, false)) return "ising_int8_resident";
     return ising_int8_variant(sim->L);
+}
+
+// +-J couplings (Eq. 1 with per-bond J_ij).  The natural-layout signs are
+// turned into per-colour bit planes on the host: for the colour-c site (i, k), j = 2k + p, p = (i + c) & 1,
+//   plane 0 (up)     Jv[i-1][j]          plane 1 (down)  Jv[i][j]
+//   plane 2 (centre, the other-colour site with the same k)   p ? Jh[i][j-1] : Jh[i][j]
+//   plane 3 (side,   the other-colour site k+1 if p else k-1) p ? Jh[i][j]   : Jh[i][j-1]
+// bit = 1 iff the bond is -1.
+int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv) {
+    if (!sim) return fail(SPIN_ERR_INVALID, "spin_set_bonds: NULL handle");
+    if ((Jh == nullptr) != (Jv == nullptr)) return fail(SPIN_ERR_INVALID, "spin_set_bonds: Jh and Jv must both be given or both be NULL");
+    CUDA_TRY(cudaSetDevice(sim->device));
+    if (!Jh) {   // back to uniform couplings
+        CUDA_TRY(cudaStreamSynchronize(sim->stream));
+        if (sim->d_bonds) cudaFree(sim->d_bonds);
+        sim->d_bonds = nullptr;
+        return SPIN_OK;
+    }
+    if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_BITPACKED)
+        return fail(SPIN_ERR_UNSUPPORTED, "spin_set_bonds: +-J couplings are implemented for the bit-packed Ising layout only");
+    const int L = sim->L, WW = L >> 6;
+    const size_t N = (size_t)L * L, half = (size_t)L * WW;
+    for (size_t p = 0; p < N * (size_t)sim->batch; ++p)
+        if ((Jh[p] != 1 && Jh[p] != -1) || (Jv[p] != 1 && Jv[p] != -1))
+            return fail(SPIN_ERR_INVALID, "spin_set_bonds: bond signs must be +1 or -1 (entry %zu)", p);
+    std::vector<uint32_t> planes((size_t)sim->batch * 2 * 4 * half, 0u);
+    for (int b = 0; b < sim->batch; ++b) {
+        const int8_t* jh = Jh + (size_t)b * N;
+        const int8_t* jv = Jv + (size_t)b * N;
+        for (int c = 0; c < 2; ++c) {
+            uint32_t* base = planes.data() + ((size_t)b * 2 + c) * 4 * half;
+            for (int i = 0; i < L; ++i) {
+                const int iu = i == 0 ? L - 1 : i - 1, par = (i + c) & 1;
+                for (int k = 0; k < L / 2; ++k) {
+                    const int j = 2 * k + par, jl = j == 0 ? L - 1 : j - 1;
+                    const int8_t up = jv[(size_t)iu * L + j], dn = jv[(size_t)i * L + j];
+                    const int8_t left = jh[(size_t)i * L + jl], right = jh[(size_t)i * L + j];
+                    const int8_t ct = par ? left : right, sd = par ? right : left;
+                    const size_t w = (size_t)i * WW + (k >> 5);
+                    const uint32_t bit = 1u << (k & 31);
+                    if (up < 0) base[w] |= bit;
+                    if (dn < 0) base[half + w] |= bit;
+                    if (ct < 0) base[2 * half + w] |= bit;
+                    if (sd < 0) base[3 * half + w] |= bit;
+                }
+            }
+        }
+    }
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    if (!sim->d_bonds) {
+        cudaError_t e = cudaMalloc(&sim->d_bonds, planes.size() * sizeof(uint32_t));
+        if (e != cudaSuccess) { sim->d_bonds = nullptr; return fail(SPIN_ERR_NOMEM, "spin_set_bonds: cudaMalloc: %s", cudaGetErrorString(e)); }
+    }
+    CUDA_TRY(cudaMemcpy(sim->d_bonds, planes.data(), planes.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    return SPIN_OK;
 }
 
 int spin_set_policy(spin_sim* sim, int32_t policy) {

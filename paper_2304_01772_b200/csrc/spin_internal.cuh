@@ -59,6 +59,8 @@ struct SweepArgs {
     uint32_t c3;              // (t >> 32) & 0xFFFFFF | colour << 24 | domain << 28
     int32_t colour;
     const uint8_t* aux;       // bit-packed kernel: nibble-pair -> 4 * class byte table (ising_bits_aux_table), else nullptr
+    const uint32_t* bonds;    // bit-packed +-J couplings: [B][2][4][L][L/64] words (bit = bond is -1; planes up, down,
+                              // centre, side of the colour's sites), or nullptr for uniform couplings
     RoundKeys rk;
 };
 
@@ -126,7 +128,7 @@ const char* potts_int8_variant(int L);
 
 // Observables: accumulate into E_acc[b], M_acc[b] (int64, must be zero on entry; Potts uses hist).
 int launch_ising_int8_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);
-int launch_ising_bits_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);
+int launch_ising_bits_observe(const void* lattice, const uint32_t* bonds, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);
 // Potts: E_acc as above; hist: [B][128] uint32, zero on entry; M is produced by launch_potts_finalize.
 int launch_potts_int8_observe(const void* lattice, int batch, int L, const int32_t* q, long long* E_acc, unsigned int* hist, cudaStream_t s);
 // M_out[b] = max_k hist[b][k], then hist is cleared for the next use.
