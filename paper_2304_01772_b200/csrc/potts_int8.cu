@@ -101,8 +101,9 @@ __device__ __forceinline__ void site_step(uint32_t& acc_mask, uint32_t o, uint32
     if (kHasNever) {
         if (acc) acc_mask |= 0xFFu << (8 * kE);
     } else {
-        // kept in PTX so that it stays one ISETP + one predicated two-input OR (issues at twice the PRMT rate)
-        asm("{\n\t.reg .pred p;\n\tsetp.ls.u32 p, %1, %2;\n\t@p or.b32 %0, %0, %3;\n\t}"
+        // kept in PTX so that it stays one ISETP + one predicated add (the bytes are disjoint; a two-operand add
+        // issues at twice the rate of a logic op or a PRMT)
+        asm("{\n\t.reg .pred p;\n\tsetp.ls.u32 p, %1, %2;\n\t@p add.u32 %0, %0, %3;\n\t}"
             : "+r"(acc_mask) : "r"(r), "r"(*(const uint32_t*)((const char*)stab + c4)), "n"(0xFFu << (8 * kE)));
     }
 }
