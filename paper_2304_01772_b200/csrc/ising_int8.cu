@@ -64,7 +64,7 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
 constexpr int kRowsShort = 2;   // ... and when it does not (latency-bound shapes): four times as many threads
 #ifndef ISING_MINB
-#define ISING_MINB 6
+#define ISING_MINB 5
 #endif
 constexpr int kRowsThreads = 128;
 
@@ -187,9 +187,9 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
     __syncthreads();    // the block's threshold table (filled by the caller) is first read below: the loads above
                         // are already in flight while the block waits for it
-    // Two rows per iteration (the side-neighbour parity alternates), rolled: the body stays small enough for the
-    // instruction caches, and all warps of the SM share it.
-#pragma unroll 1
+    // Two rows per iteration (the side-neighbour parity alternates); the four iterations of an 8-row thread are
+    // unrolled so that the register window rotates by renaming instead of moves (measured: +2.5 % over the rolled loop).
+#pragma unroll 4
     for (int rr = 0; rr < kRows; rr += 2) {
         const bool more = rr + 2 < kRows;
         // inputs of the odd row i+1: other-colour row i+2 (the only one that can wrap), own row i+1, its edge word
