@@ -83,11 +83,25 @@ __device__ __forceinline__ uint32_t neq_bits(uint32_t v, uint32_t u, uint32_t d,
     } else {
         a0 = (v ^ u) + k; a1 = ((v ^ d) + k) >> 1; a2 = ((v ^ c) + k) >> 2; a3 = ((v ^ s) + k) >> 3;
     }
+    if (kSmallQ) {
+        // High nibbles: a0 = 1000 / 0111, a1 = 0100 / 0011, a2 = 0010 / 0001, a3 = 0001 / 0000 (differs / equal).  Their
+        // XOR is a one-to-one code of the four indicator bits (the toggles 1111, 0111, 0011, 0001 are independent), so
+        // two 3-input XORs replace the three bit-selects; the pattern table decodes it (small_q_count below).
+        return a0 ^ a1 ^ a2 ^ a3;
+    }
     // bit 7 from a0, bit 6 from a1, bit 5 from a2, bit 4 from a3 (low nibble is garbage, masked by the caller)
     uint32_t t = (a2 & 0x20202020u) | (a3 & ~0x20202020u);
     t = (a1 & 0x40404040u) | (t & ~0x40404040u);
     t = (a0 & 0x80808080u) | (t & ~0x80808080u);
     return t;
+}
+
+// Number of differing neighbours encoded in a nibble: plain indicator bits (general path) or the XOR code of the
+// shift-free path: n ^ 0101 = i0 1111 ^ i1 0111 ^ i2 0011 ^ i3 0001, so (i0..i3) is its Gray code.
+__device__ __forceinline__ int nibble_count(int n, bool small_q) {
+    if (!small_q) return __popc(n);
+    const int b = n ^ 5;
+    return __popc((b ^ (b >> 1)) & 15);
 }
 
 // One site: threshold fetch (the index byte scales into the table address), compare, replace the byte by the proposal.
@@ -246,13 +260,14 @@ __global__ void __launch_bounds__(kRowsThreads, POTTS_MINB) potts_int8_rows_kern
     const uint32_t never = tab[kTabNever];
     for (int m = threadIdx.x; m < 16; m += blockDim.x) stab[m] = tab[m];
     if (threadIdx.x == 0) snever[0] = never;
+    const uint32_t q = tab[kTabQ];
+    const bool small_q = !never && q <= 16u;                // the variant this block runs (see the dispatch below)
     for (int m = threadIdx.x; m < 256; m += blockDim.x) {
-        // high nibble: "neighbour != old" bits, low nibble: "neighbour != new" bits
-        const int cls = __popc(m >> 4) - __popc(m & 15) + 4;
+        // high nibble: "neighbour != old" code, low nibble: "neighbour != new" code
+        const int cls = nibble_count(m >> 4, small_q) - nibble_count(m & 15, small_q) + 4;
         ((uint8_t*)(stab + 16))[m] = (uint8_t)(4 * cls);
     }
     __syncthreads();
-    const uint32_t q = tab[kTabQ];
     const int W16 = a.L >> 5;
     const int u = blk * blockDim.x + threadIdx.x;
     if (u >= (a.L / kRows) * W16) return;                  // ragged last block of a replica (after the barrier)
