@@ -224,7 +224,7 @@ int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
     const bool shortRows = longThreads < 148ll * 64;      // the per-block table set-up makes short threads pay off only for tiny launches
     const int rows = shortRows ? kRowsShort : kRowsLong;
     const int perReplica = (a.L / rows) * (a.L >> 6);
-    const int tpb = perReplica >= kThreads ? kThreads : ((perReplica + 31) & ~31);   // last block may be ragged
+    const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
     const int bpr = (perReplica + tpb - 1) / tpb;
     const unsigned grid = (unsigned)((long long)bpr * a.batch);
     const bool bonds = a.bonds != nullptr;

@@ -289,7 +289,7 @@ int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
                                (a.L / kRowsLong) * (a.L >> 5) < kRowsThreads / 2;   // small L: keep the blocks full
         const int rows = shortRows ? kRowsShort : kRowsLong;
         const int perReplica = (a.L / rows) * (a.L >> 5);    // strips x row blocks of one colour
-        const int tpb = perReplica >= kRowsThreads ? kRowsThreads : ((perReplica + 31) & ~31);   // last block may be ragged
+        const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
         const int bpr = (perReplica + tpb - 1) / tpb;
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
         if (shortRows) {

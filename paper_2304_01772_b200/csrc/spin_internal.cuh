@@ -114,6 +114,18 @@ inline cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned 
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
+// Threads per block for `units` thread-units of one replica: the multiple of 32 (at most 128) that wastes the fewest
+// lanes in the ragged last block; ties go to the larger block.
+inline int pick_block(int units) {
+    int best = 128;
+    long long bestPad = -1;
+    for (int t = 128; t >= 32; t -= 32) {
+        const long long pad = (long long)((units + t - 1) / t) * t;
+        if (bestPad < 0 || pad < bestPad) { best = t; bestPad = pad; }
+    }
+    return best;
+}
+
 // ---- launchers (each returns the number of kernels it launched; errors via cudaGetLastError) --------
 int launch_init(const InitArgs& a, int model, int layout, cudaStream_t s);
 
