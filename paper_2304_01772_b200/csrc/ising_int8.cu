@@ -88,6 +88,10 @@ __device__ __forceinline__ void site_step(uint32_t& fm, uint32_t o, uint32_t r, 
     if (kHasNever) {
         const bool acc = (r <= U) && !((stab[kTabNever] >> (o >> 2)) & 1u);
         if (acc) fm += 0xFEu << (8 * kE);
+    } else if (kE == 0) {
+        // the first site of a word defines the mask (one select, no zero-initialisation)
+        asm("{\n\t.reg .pred p;\n\tsetp.ls.u32 p, %1, %2;\n\tselp.b32 %0, %3, 0, p;\n\t}"
+            : "=r"(fm) : "r"(r), "r"(U), "n"(0xFEu));
     } else {
         // kept in PTX so that it stays one ISETP + one predicated IADD
         asm("{\n\t.reg .pred p;\n\tsetp.ls.u32 p, %1, %2;\n\t@p add.u32 %0, %0, %3;\n\t}"
