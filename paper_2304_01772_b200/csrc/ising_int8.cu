@@ -258,24 +258,31 @@ __global__ void __launch_bounds__(kRowsThreads, ISING_MINB) ising_int8_rows_kern
 constexpr int kResThreads = 256;
 constexpr size_t kResMaxLatticeBytes = 196608;   // 3 CTAs of L = 256 per SM; one CTA up to L = 416
 
-__device__ __forceinline__ int block_sum(int v, int* scratch) {
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xFFFFFFFFu, v, o);
-    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    __syncthreads();                       // scratch may still be read from the previous call
-    if (lane == 0) scratch[w] = v;
-    __syncthreads();
-    int t = 0;
-    const int nw = (blockDim.x + 31) >> 5;
-    for (int k = 0; k < nw; ++k) t += scratch[k];
-    return t;
-}
 
 // Rows of one parity at a time: the side of the horizontal neighbour depends on (row + colour) & 1, and a warp spans
 // several rows when L/32 < 32, so mixing parities in one pass would make every warp execute both variants.
 // kMeasure: also accumulate, from the updated strip and the neighbour sums already in registers, sS = sum of the new
 // spins and sSN = sum of (new spin) x (4 x number of -1 neighbours) (IDP4A on the +-1 bytes): after the colour-1 pass
 // every bond has been seen from its colour-1 end with final values, so E_int = -(4 sS1 - sSN1 / 2), M = sS0 + sS1.
+// Three block sums with one pair of barriers (valid in thread 0 only).
+__device__ __forceinline__ void block_sum3(int& a, int& b, int& c, int* scratch) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        a += __shfl_xor_sync(0xFFFFFFFFu, a, o);
+        b += __shfl_xor_sync(0xFFFFFFFFu, b, o);
+        c += __shfl_xor_sync(0xFFFFFFFFu, c, o);
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    __syncthreads();                       // scratch may still be read from the previous sweep
+    if (lane == 0) { scratch[3 * w] = a; scratch[3 * w + 1] = b; scratch[3 * w + 2] = c; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        const int nw = (blockDim.x + 31) >> 5;
+        a = b = c = 0;
+        for (int k = 0; k < nw; ++k) { a += scratch[3 * k]; b += scratch[3 * k + 1]; c += scratch[3 * k + 2]; }
+    }
+}
+
 template <bool kHasNever, int kParity, bool kMeasure>
 __device__ __forceinline__ void resident_rows(const ResidentArgs& a, int colour, uint32_t c2, uint32_t c3, uint8_t* lat,
                                               const uint32_t* stab, uint32_t slot, uint32_t c1, int& sS, int& sSN) {
@@ -320,10 +327,46 @@ __device__ __forceinline__ void resident_rows(const ResidentArgs& a, int colour,
     }
 }
 
+// Tiny lattices (L <= 64): one thread per 4-site word (= one Philox group) instead of per 16-site strip, so that a
+// half-sweep of a 32 x 32 replica is one short pass of 128 threads rather than two passes of 16 busy lanes.  The row
+// parity (which side the horizontal neighbour is on) is handled with selects on the PRMT operands: no divergence.
+template <bool kHasNever, bool kMeasure>
+__device__ __forceinline__ void resident_words(const ResidentArgs& a, int colour, uint32_t c2, uint32_t c3, uint8_t* lat,
+                                               const uint32_t* stab, uint32_t slot, uint32_t c1, int& sS, int& sSN) {
+    const int L = a.L, W = L >> 1, W4 = W >> 2;
+    uint32_t* own1 = (uint32_t*)(lat + (size_t)colour * L * W);
+    const uint32_t* oth1 = (const uint32_t*)(lat + (size_t)(1 - colour) * L * W);
+    const int words = L * W4;
+    const uint32_t m = 0x04040404u;
+    for (int w = threadIdx.x; w < words; w += blockDim.x) {
+        const int i = w / W4, x = w - i * W4;
+        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+        const bool par = ((i + colour) & 1) != 0;              // side neighbour of site k: k+1 if par else k-1
+        const uint32_t um = oth1[iu * W4 + x] & m, cm = oth1[w] & m, dm = oth1[id * W4 + x] & m;
+        const int xs = par ? (x == W4 - 1 ? 0 : x + 1) : (x == 0 ? W4 - 1 : x - 1);
+        const uint32_t nb = oth1[i * W4 + xs] & m;
+        const uint32_t sd = __byte_perm(par ? cm : nb, par ? nb : cm, par ? 0x4321u : 0x6543u);
+        const uint32_t own = own1[w];
+        const uint32_t n4 = um + cm + dm + sd;                  // 4 x number of -1 neighbours per byte
+        uint32_t r[4];
+        philox4x32_10(a.rk, (uint32_t)w, c1, c2, c3, r);       // word index = Philox group (n >> 2)
+        const uint32_t res = update_word<kHasNever, 0>(own, n4 + (own & 0x20202020u), r, stab, slot);
+        own1[w] = res;
+        if (kMeasure) {
+            sS = __dp4a((int)res, 0x01010101, sS);
+            if (colour == 1) asm("dp4a.s32.u32 %0, %1, %2, %0;" : "+r"(sSN) : "r"(res), "r"(n4));
+        }
+    }
+}
+
 template <bool kHasNever, bool kMeasure>
 __device__ __forceinline__ void resident_half_sweep(const ResidentArgs& a, int colour, uint32_t c2, uint32_t c3,
                                                     uint8_t* lat, const uint32_t* stab, uint32_t slot, uint32_t c1,
                                                     int& sS, int& sSN) {
+    if (a.L <= 64) {      // block-uniform
+        resident_words<kHasNever, kMeasure>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
+        return;
+    }
     resident_rows<kHasNever, 0, kMeasure>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
     resident_rows<kHasNever, 1, kMeasure>(a, colour, c2, c3, lat, stab, slot, c1, sS, sSN);
 }
@@ -368,9 +411,8 @@ __global__ void __launch_bounds__(kResThreads) ising_int8_resident_kernel(Reside
         if (a.measure) {
             // Every bond has exactly one colour-1 end, and after the colour-1 pass both ends are final:
             // sum_bonds s s' = sum over colour-1 sites of s * nn, nn = 4 - 2 nd = 4 - (4 nd) / 2.
-            const int totS0 = block_sum(sS0, scratch);
-            const int totS1 = block_sum(sS1, scratch);
-            const int totSN = block_sum(sSN, scratch);
+            int totS0 = sS0, totS1 = sS1, totSN = sSN;
+            block_sum3(totS0, totS1, totSN, scratch);
             if (threadIdx.x == 0) {
                 const long long e = -(4ll * totS1 - (long long)totSN / 2), mag = (long long)totS0 + totS1;
                 if (a.E_trace) a.E_trace[(size_t)s * a.batch + b] = e;
@@ -444,9 +486,9 @@ int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s) {
                              (int)(kResMaxLatticeBytes + sizeof(uint32_t) * (kTableStride + 4 * kResThreads) + 128));
         configured = true;
     }
-    const int units = a.L * (a.L >> 5);
+    const int units = a.L <= 64 ? a.L * (a.L >> 3) : a.L * (a.L >> 5);   // words (tiny lattices) or strips per colour
     int tpb = kResThreads;
-    while (tpb > 32 && tpb / 2 >= units) tpb >>= 1;           // L = 32: 32 strips -> one warp
+    while (tpb > 32 && tpb / 2 >= units) tpb >>= 1;           // L = 32: 128 words -> 128 threads
     ising_int8_resident_kernel<<<(unsigned)a.batch, tpb, smem, s>>>(a);
     return 1;
 }
