@@ -214,6 +214,12 @@ def test_sweep_measure_trace_and_moments(oracle_mod, policy, L):
         assert np.array_equal(np.vstack([E1, E2]), Eo) and np.array_equal(np.vstack([M1, M2]), Mo)
         assert np.array_equal(mom, mom_o)
         assert np.array_equal(sim.spin_get_spins(), ref)
+        # float-derived quantities (north star: relative 1e-12 in double): from exact integers, hence bit-equal
+        from paper_2304_01772_b200 import derived
+        dg = derived.thermodynamics(mom, beta, 1.0, 0.05, L)
+        do = derived.thermodynamics(mom_o, beta, 1.0, 0.05, L)
+        for k in ("u", "abs_m", "c", "chi"):
+            assert np.all(np.abs(dg[k] - do[k]) <= 1e-12 * np.abs(do[k]))
 
 
 def test_resident_multi_sweep_call_equals_streaming(oracle_mod):
