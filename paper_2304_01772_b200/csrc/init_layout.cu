@@ -181,4 +181,55 @@ int launch_validate_natural(const int8_t* natural, int batch, int L, int model, 
     return 1;
 }
 
+// ---- +-J couplings: natural-layout bond signs -> per-colour bit planes (spin_set_bonds, spin.h).
+// For the colour-c site (i, k), j = 2k + p, p = (i + c) & 1:
+//   plane 0 (up) Jv[i-1][j], plane 1 (down) Jv[i][j], plane 2 (centre) p ? Jh[i][j-1] : Jh[i][j],
+//   plane 3 (side) p ? Jh[i][j] : Jh[i][j-1];  bit = 1 iff the bond is -1.  One thread per output word quadruple.
+// bad[0] counts entries that are not +-1 (each entry is read by exactly one of colour 0 / colour 1 per role, so the
+// count is of reads, not of entries; only zero / non-zero matters).
+namespace {
+__global__ void bonds_from_natural_kernel(const int8_t* __restrict__ Jh, const int8_t* __restrict__ Jv,
+                                          uint32_t* __restrict__ planes, int batch, int L, unsigned int* bad) {
+    const int WW = L >> 6;
+    const long long half = (long long)L * WW;
+    const long long total = (long long)batch * 2 * half;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= total) return;
+    const int b = (int)(gid / (2 * half));
+    const long long rem = gid - (long long)b * 2 * half;
+    const int c = (int)(rem / half);
+    const long long w = rem - (long long)c * half;
+    const int i = (int)(w / WW), x = (int)(w - (long long)i * WW);
+    const int iu = i == 0 ? L - 1 : i - 1, par = (i + c) & 1;
+    const int8_t* jh = Jh + (size_t)b * L * L;
+    const int8_t* jv = Jv + (size_t)b * L * L;
+    uint32_t pu = 0u, pd = 0u, pc = 0u, ps = 0u;
+    unsigned int nbad = 0;
+    for (int t = 0; t < 32; ++t) {
+        const int k = 32 * x + t, j = 2 * k + par, jl = j == 0 ? L - 1 : j - 1;
+        const int up = jv[(size_t)iu * L + j], dn = jv[(size_t)i * L + j];
+        const int left = jh[(size_t)i * L + jl], right = jh[(size_t)i * L + j];
+        nbad += (up != 1 && up != -1) + (dn != 1 && dn != -1) + (left != 1 && left != -1) + (right != 1 && right != -1);
+        const int ct = par ? left : right, sd = par ? right : left;
+        pu |= (uint32_t)(up < 0) << t;
+        pd |= (uint32_t)(dn < 0) << t;
+        pc |= (uint32_t)(ct < 0) << t;
+        ps |= (uint32_t)(sd < 0) << t;
+    }
+    uint32_t* base = planes + ((size_t)b * 2 + c) * 4 * half + w;
+    base[0] = pu;
+    base[half] = pd;
+    base[2 * half] = pc;
+    base[3 * half] = ps;
+    if (nbad) atomicAdd(bad, nbad);
+}
+}  // namespace
+
+int launch_bonds_from_natural(const int8_t* Jh, const int8_t* Jv, uint32_t* planes, int batch, int L, unsigned int* bad,
+                              cudaStream_t s) {
+    const long long total = (long long)batch * 2 * L * (L >> 6);
+    bonds_from_natural_kernel<<<blocks_for(total, 128), 128, 0, s>>>(Jh, Jv, planes, batch, L, bad);
+    return 1;
+}
+
 }  // namespace spin

@@ -408,7 +408,7 @@ const char* spin_kernel_variant(const spin_sim* sim) {
 }
 
 // +-J couplings (Eq. 1 with per-bond J_ij).  The natural-layout signs are
-// turned into per-colour bit planes on the host: for the colour-c site (i, k), j = 2k + p, p = (i + c) & 1,
+// turned into per-colour bit planes (init_layout.cu): for the colour-c site (i, k), j = 2k + p, p = (i + c) & 1,
 //   plane 0 (up)     Jv[i-1][j]          plane 1 (down)  Jv[i][j]
 //   plane 2 (centre, the other-colour site with the same k)   p ? Jh[i][j-1] : Jh[i][j]
 //   plane 3 (side,   the other-colour site k+1 if p else k-1) p ? Jh[i][j]   : Jh[i][j-1]
@@ -425,40 +425,33 @@ int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv) {
     }
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_BITPACKED)
         return fail(SPIN_ERR_UNSUPPORTED, "spin_set_bonds: +-J couplings are implemented for the bit-packed Ising layout only");
-    const int L = sim->L, WW = L >> 6;
-    const size_t N = (size_t)L * L, half = (size_t)L * WW;
-    for (size_t p = 0; p < N * (size_t)sim->batch; ++p)
-        if ((Jh[p] != 1 && Jh[p] != -1) || (Jv[p] != 1 && Jv[p] != -1))
-            return fail(SPIN_ERR_INVALID, "spin_set_bonds: bond signs must be +1 or -1 (entry %zu)", p);
-    std::vector<uint32_t> planes((size_t)sim->batch * 2 * 4 * half, 0u);
-    for (int b = 0; b < sim->batch; ++b) {
-        const int8_t* jh = Jh + (size_t)b * N;
-        const int8_t* jv = Jv + (size_t)b * N;
-        for (int c = 0; c < 2; ++c) {
-            uint32_t* base = planes.data() + ((size_t)b * 2 + c) * 4 * half;
-            for (int i = 0; i < L; ++i) {
-                const int iu = i == 0 ? L - 1 : i - 1, par = (i + c) & 1;
-                for (int k = 0; k < L / 2; ++k) {
-                    const int j = 2 * k + par, jl = j == 0 ? L - 1 : j - 1;
-                    const int8_t up = jv[(size_t)iu * L + j], dn = jv[(size_t)i * L + j];
-                    const int8_t left = jh[(size_t)i * L + jl], right = jh[(size_t)i * L + j];
-                    const int8_t ct = par ? left : right, sd = par ? right : left;
-                    const size_t w = (size_t)i * WW + (k >> 5);
-                    const uint32_t bit = 1u << (k & 31);
-                    if (up < 0) base[w] |= bit;
-                    if (dn < 0) base[half + w] |= bit;
-                    if (ct < 0) base[2 * half + w] |= bit;
-                    if (sd < 0) base[3 * half + w] |= bit;
-                }
-            }
-        }
+    // natural-layout signs -> device -> per-colour bit planes (validated on the device; a rejected call leaves the
+    // handle's couplings as they were)
+    const int L = sim->L;
+    const size_t nat = (size_t)sim->batch * L * L;
+    const size_t words = (size_t)sim->batch * 2 * 4 * L * (size_t)(L >> 6);
+    int8_t* d_nat = nullptr;
+    uint32_t* d_new = nullptr;
+    cudaError_t e = cudaMalloc(&d_nat, 2 * nat);
+    if (e == cudaSuccess) e = cudaMalloc(&d_new, words * sizeof(uint32_t));
+    if (e != cudaSuccess) {
+        if (d_nat) cudaFree(d_nat);
+        return fail(SPIN_ERR_NOMEM, "spin_set_bonds: cudaMalloc: %s", cudaGetErrorString(e));
     }
-    CUDA_TRY(cudaStreamSynchronize(sim->stream));
-    if (!sim->d_bonds) {
-        cudaError_t e = cudaMalloc(&sim->d_bonds, planes.size() * sizeof(uint32_t));
-        if (e != cudaSuccess) { sim->d_bonds = nullptr; return fail(SPIN_ERR_NOMEM, "spin_set_bonds: cudaMalloc: %s", cudaGetErrorString(e)); }
+    unsigned int bad = 0;
+    e = cudaMemcpyAsync(d_nat, Jh, nat, cudaMemcpyHostToDevice, sim->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_nat + nat, Jv, nat, cudaMemcpyHostToDevice, sim->stream);
+    if (e == cudaSuccess) e = cudaMemsetAsync(sim->d_bad, 0, sizeof(unsigned int), sim->stream);
+    if (e == cudaSuccess) {
+        sim->launches += launch_bonds_from_natural(d_nat, d_nat + nat, d_new, sim->batch, L, sim->d_bad, sim->stream);
+        e = cudaMemcpyAsync(&bad, sim->d_bad, sizeof bad, cudaMemcpyDeviceToHost, sim->stream);
     }
-    CUDA_TRY(cudaMemcpy(sim->d_bonds, planes.data(), planes.size() * sizeof(uint32_t), cudaMemcpyHostToDevice));
+    if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
+    cudaFree(d_nat);
+    if (e != cudaSuccess) { cudaFree(d_new); return cuda_fail(e, "spin_set_bonds"); }
+    if (bad) { cudaFree(d_new); return fail(SPIN_ERR_INVALID, "spin_set_bonds: bond signs must be +1 or -1"); }
+    if (sim->d_bonds) cudaFree(sim->d_bonds);
+    sim->d_bonds = d_new;
     return SPIN_OK;
 }
 

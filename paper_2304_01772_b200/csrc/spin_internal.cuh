@@ -152,6 +152,10 @@ int launch_accumulate_moments(long long* moments, const long long* E, const long
 int launch_from_natural(const int8_t* natural, void* lattice, int batch, int L, int layout, cudaStream_t s);
 int launch_to_natural(const void* lattice, int8_t* natural, int batch, int L, int layout, cudaStream_t s);
 // bad[0] = number of invalid values (Ising: not +-1; Potts: outside 0..q[b]-1).  bad must be zero on entry.
+// +-J bond signs, natural [B][L][L] int8 on the device -> sign planes [B][2][4][L][L/64]; bad[0] (zero on entry) gets the
+// number of reads that were not +-1.
+int launch_bonds_from_natural(const int8_t* Jh, const int8_t* Jv, uint32_t* planes, int batch, int L, unsigned int* bad,
+                              cudaStream_t s);
 int launch_validate_natural(const int8_t* natural, int batch, int L, int model, const int32_t* q, unsigned int* bad, cudaStream_t s);
 
 }  // namespace spin
