@@ -5,9 +5,11 @@
 
 A "step" is one pass of the whole hot path over one batch: the acceptance-table build for the batch's betas,
 all sweeps of the configuration (colour 0 + colour 1 each) and the per-replica E / M reductions.  At N = 1 the
-workload is BASELINE.json configs[1] (C2: Ising 64 x 1024^2, 2000 sweeps).  With N > 1 (torchrun) every rank
-runs the same number of replicas with replica_offset = rank * batch: replicas are independent, there is no
-data-path collective ("weak" scaling).  Rank 0 prints ONE JSON line.
+headline workload is BASELINE.json configs[1] (C2: Ising 64 x 1024^2, 2000 sweeps), and the same JSON line carries a
+`per_config` block with every BASELINE.json configuration (C1, C2, C3 in both layouts, C4, C5 sweeps only and C5 with
+moments), the paper's Table III shapes, and the differentiable-MC path, each timed the same way.  With N > 1
+(torchrun) every rank runs the same number of replicas with replica_offset = rank * batch: replicas are
+independent, there is no data-path collective ("weak" scaling).  Rank 0 prints ONE JSON line.
 """
 import argparse
 import json
@@ -185,6 +187,173 @@ def _config_dict(w, world, extra=None):
     return d
 
 
+class Runner:
+    """Times one workload through the binding: device-resident steps with CUDA events on the handle's stream, then
+    end-to-end steps (host lattice in, host observables out) with the host clock around synchronising calls."""
+
+    def __init__(self, sp, torch, sharding, rank, world, local_rank):
+        self.sp, self.torch, self.sharding = sp, torch, sharding
+        self.rank, self.world, self.local_rank = rank, world, local_rank
+        self.stream = torch.cuda.Stream()
+        self.flush = torch.empty(256 << 20, dtype=torch.int8, device="cuda")
+
+    def create(self, w, policy=None):
+        sp, torch = self.sp, self.torch
+        lay = sp.SPIN_LAYOUT_BITPACKED if w.layout == "bits" else sp.SPIN_LAYOUT_INT8
+        model = sp.SPIN_MODEL_POTTS if w.model == "potts" else sp.SPIN_MODEL_ISING
+        nbytes = sp.spin_buffer_bytes(w.batch, w.L, model, lay)
+        buf = torch.empty(nbytes, dtype=torch.int8, device="cuda")
+        sim = sp.spin_create_ex(w.batch, w.L, model, q_per_replica=w.q, seed=w.seed, layout=lay,
+                                replica_offset=self.sharding.replica_offset(self.rank, w.batch),
+                                device_buffer=buf.data_ptr(), buffer_bytes=nbytes,
+                                cuda_stream=self.stream.cuda_stream, keepalive=buf)
+        if policy is not None:
+            sim.spin_set_policy(policy)
+        return sim
+
+    def run(self, w, mode, steps, warmup, policy=None, e2e_steps=None, barrier=lambda: None):
+        """mode: 'sweep' (spin_sweep + spin_observables_dev), 'trace' (spin_sweep_measure with per-sweep E, M traces),
+        'moments' (w.therm plain sweeps, then spin_sweep_measure with moments and no trace)."""
+        torch, stream = self.torch, self.stream
+        sim = self.create(w, policy)
+        E_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
+        M_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
+        state = {"offset": 0, "per_call": None}
+
+        def step(events=None):
+            off = state["offset"]
+            if events:
+                events[0].record(stream)
+            if mode == "sweep":
+                l0 = sim.spin_kernel_launches()
+                sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, off)
+                state["per_call"] = sim.spin_kernel_launches() - l0
+                if events:
+                    events[1].record(stream)
+                sim.spin_observables_dev(E_dev.data_ptr(), M_dev.data_ptr())
+            elif mode == "trace":
+                sim.spin_sweep_measure(w.beta, w.J, w.h, w.n_sweeps, off, trace=True)
+                if events:
+                    events[1].record(stream)
+            else:
+                mom = np.zeros((w.batch, 8), dtype=np.int64)
+                if w.therm:
+                    sim.spin_sweep(w.beta, w.J, w.h, w.therm, off)
+                sim.spin_sweep_measure(w.beta, w.J, w.h, w.n_sweeps - w.therm, off + w.therm, trace=False, moments=mom)
+                if events:
+                    events[1].record(stream)
+            if events:
+                events[2].record(stream)
+            state["offset"] = off + w.n_sweeps
+
+        for _ in range(warmup):
+            step()
+        sim.spin_synchronize()
+        torch.cuda.synchronize()
+        ev = [tuple(torch.cuda.Event(enable_timing=True) for _ in range(3)) for _ in range(steps)]
+        launches0 = sim.spin_kernel_launches()
+        barrier()
+        torch.cuda.synchronize()
+        for k in range(steps):
+            with torch.cuda.stream(stream):
+                self.flush.fill_(k)  # L2 flush, outside the timed interval of the step
+            step(ev[k])
+        sim.spin_synchronize()
+        torch.cuda.synchronize()
+        barrier()
+        launches = sim.spin_kernel_launches() - launches0
+        step_ms = [e[0].elapsed_time(e[2]) for e in ev]
+        sweep_ms = [e[0].elapsed_time(e[1]) for e in ev]
+        res = {"sim": sim, "step_ms": step_ms, "sweep_ms": sweep_ms, "launches": int(launches),
+               "launches_per_sweep_call": state["per_call"], "kernel": sim.spin_kernel_variant(), "state": state,
+               "step_fn": step}
+        if e2e_steps:
+            host_lat = torch.empty((w.batch, w.L, w.L), dtype=torch.int8).pin_memory()
+            sim.spin_get_spins(host_lat.numpy())
+
+            def e2e_step():
+                sim.spin_set_spins_ptr(host_lat.data_ptr())
+                if mode == "sweep":
+                    sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, state["offset"])
+                    sim.spin_observables()
+                else:
+                    step()
+            e2e_step()  # one untimed end-to-end step
+            barrier()
+            t0 = time.perf_counter()
+            for _ in range(e2e_steps):
+                e2e_step()
+            dt = self.sharding.max_over_ranks(time.perf_counter() - t0, device="cuda")
+            out_bytes = 2 * w.batch * 8 + 4
+            if mode == "trace":
+                out_bytes += 2 * w.n_sweeps * w.batch * 8
+            if mode == "moments":
+                out_bytes += 8 * w.batch * 8
+            res["e2e"] = {"value": float(w.updates) * self.world * e2e_steps / (dt * 1e9), "unit": UNIT,
+                          "h2d_bytes_per_step": int(host_lat.numel() + w.batch * 8 + w.batch * 32 * 4
+                                                    + (8 * w.batch * 8 if mode == "moments" else 0)),
+                          "d2h_bytes_per_step": int(out_bytes), "steps": e2e_steps}
+        return res
+
+
+def alu_peak(peaks):
+    return INT32_LANES_PER_SM * N_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
+
+
+def summarise(w, res, peaks, measured_words_per_ns):
+    """Per-config entry: throughput (mean, best, median over the timed steps) and the two ALU roofline fractions."""
+    step_ms = np.array(res["step_ms"])
+    sweep_ms = np.array(res["sweep_ms"])
+    ops = OPS_PER_UPDATE[w.model]
+    per_step = float(w.updates)
+    vals = per_step / (step_ms * 1e6)
+    sweep_rate = per_step / (float(np.mean(sweep_ms)) * 1e6)             # updates/ns over the sweep portion of the step
+    frac = ops * sweep_rate * 1e9 / 1e12 / alu_peak(peaks)
+    words = 1.0 if w.model == "ising" else 2.0
+    d = {"workload": "%s: %s %dx%d^2, %d sweeps, layout %s" % (w.name, w.model, w.batch, w.L, w.n_sweeps, w.layout),
+         "value": float(per_step * len(step_ms) / (step_ms.sum() * 1e6)), "unit": UNIT, "best": float(vals.max()),
+         "median": float(np.median(vals)), "ms_per_step": float(step_ms.mean()), "kernel": res["kernel"],
+         "gpu_launches_per_step": res["launches"] // len(step_ms),
+         "roofline": {"bound": "alu", "frac": float(frac), "sweep_only_flips_per_ns": float(sweep_rate),
+                      "frac_of_measured": (float(sweep_rate * words / measured_words_per_ns)
+                                           if measured_words_per_ns else None)}}
+    if "e2e" in res:
+        d["e2e"] = res["e2e"]
+    return d
+
+
+def per_config_block(runner, sp, args, peaks, measured):
+    """Every BASELINE.json configuration and the paper's Table III shapes, timed like the headline (N = 1 only)."""
+    out = {}
+    plan = [("C1", sp.workloads.config(1), "trace"), ("C2", sp.workloads.config(2), "sweep"),
+            ("C3-bits", sp.workloads.config(3, layout="bits"), "sweep"),
+            ("C3-int8", sp.workloads.config(3, layout="int8"), "sweep"),
+            ("C4", sp.workloads.config(4), "sweep"), ("C5-sweep", sp.workloads.config(5), "sweep"),
+            ("C5-measure", sp.workloads.config(5), "moments")]
+    for key, w, mode in plan:
+        if args.sweeps:
+            w.n_sweeps = args.sweeps
+            w.therm = min(w.therm, args.sweeps // 5)
+        res = runner.run(w, mode, args.steps, args.warmup, e2e_steps=max(1, min(args.steps, 2)))
+        out[key] = summarise(w, res, peaks, measured)
+        out[key]["mode"] = {"sweep": "spin_sweep + spin_observables_dev", "trace": "spin_sweep_measure, E and M after every sweep",
+                            "moments": "spin_sweep (thermalisation) + spin_sweep_measure with moments"}[mode]
+        res["sim"].spin_destroy()
+    # the paper's Table III corners (PAPER.md:252-276): context shapes, launch/latency-bound on a B200
+    paper = {"P_1x640": 0.89, "P_16x640": 1.70, "P_1x2560": 1.53, "P_16x2560": 1.71}
+    for w in sp.workloads.paper_table3_shapes():
+        if args.sweeps:
+            w.n_sweeps = args.sweeps
+        for layout in ("int8", "bits"):
+            w.layout = layout
+            res = runner.run(w, "sweep", args.steps, args.warmup)
+            d = summarise(w, res, peaks, measured)
+            d["paper_rtx3060_flips_per_ns"] = paper[w.name]
+            out["%s-%s" % (w.name, layout)] = d
+            res["sim"].spin_destroy()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -195,6 +364,7 @@ def main():
     ap.add_argument("--layout", default=None, choices=[None, "int8", "bits"])
     ap.add_argument("--sweeps", type=int, default=None, help="override sweeps per step (diagnostics only)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="headline workload only")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -224,110 +394,58 @@ def main():
         if world > 1:
             dist.barrier()
 
-    stream = torch.cuda.Stream()
-    lay = sp.SPIN_LAYOUT_BITPACKED if w.layout == "bits" else sp.SPIN_LAYOUT_INT8
-    model = sp.SPIN_MODEL_POTTS if w.model == "potts" else sp.SPIN_MODEL_ISING
-    nbytes = sp.spin_buffer_bytes(w.batch, w.L, model, lay)
-    buf = torch.empty(nbytes, dtype=torch.int8, device="cuda")
-    sim = sp.spin_create_ex(w.batch, w.L, model, q_per_replica=w.q, seed=w.seed, layout=lay,
-                            replica_offset=sharding.replica_offset(rank, w.batch), device_buffer=buf.data_ptr(), buffer_bytes=nbytes,
-                            cuda_stream=stream.cuda_stream, keepalive=buf)
-    flush = torch.empty(256 << 20, dtype=torch.int8, device="cuda")
-    E_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
-    M_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
-
-    # a step = the whole hot path with inputs resident in HBM: table build + upload, all sweeps, E/M reductions
-    offset = 0
-    launches_per_sweep_call = None
-    for _ in range(args.warmup):
-        l0 = sim.spin_kernel_launches()
-        sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, offset)
-        launches_per_sweep_call = sim.spin_kernel_launches() - l0      # 2 per sweep (streaming) or 1 (resident)
-        sim.spin_observables_dev(E_dev.data_ptr(), M_dev.data_ptr())
-        offset += w.n_sweeps
-    sim.spin_synchronize()
-    torch.cuda.synchronize()
-
+    runner = Runner(sp, torch, sharding, rank, world, local_rank)
+    measured = sp.spin_measure_philox_compare_rate()        # stand-alone Philox + compare rate, random words per ns
     sampler = ClockSampler(local_rank)
     if rank == 0:
         sampler.start()
-    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-          for _ in range(args.steps)]
-    launches0 = sim.spin_kernel_launches()
-    barrier()
-    torch.cuda.synchronize()
-    for k in range(args.steps):
-        with torch.cuda.stream(stream):
-            flush.fill_(k)  # L2 flush, outside the timed interval of the step
-        ev[k][0].record(stream)
-        sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, offset)
-        ev[k][1].record(stream)
-        sim.spin_observables_dev(E_dev.data_ptr(), M_dev.data_ptr())
-        ev[k][2].record(stream)
-        offset += w.n_sweeps
-    sim.spin_synchronize()
-    torch.cuda.synchronize()
-    barrier()
-    launches = sim.spin_kernel_launches() - launches0
+    res = runner.run(w, "sweep", args.steps, args.warmup, e2e_steps=max(1, min(args.steps, 3)), barrier=barrier)
+    sim = res["sim"]
     if rank == 0 and len(sampler.lines) < 2:
         # the timed region was shorter than the sampling period (tiny workloads): keep the same load running,
         # untimed, until the sampler has seen it
         t_end = time.perf_counter() + 0.6
         while time.perf_counter() < t_end:
-            sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, offset)
+            sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, res["state"]["offset"])
             sim.spin_synchronize()
     clocks = sampler.stop() if rank == 0 else None
-    step_ms = [e[0].elapsed_time(e[2]) for e in ev]
-    sweep_ms = [e[0].elapsed_time(e[1]) for e in ev]
+    step_ms, sweep_ms = res["step_ms"], res["sweep_ms"]
     total_ms = sharding.max_over_ranks(sum(step_ms), device="cuda")      # the job is as slow as its slowest rank
     updates_per_step = float(w.updates) * world
     value = updates_per_step * args.steps / (total_ms * 1e6)  # flips per ns, whole job
 
-    # ---- end to end through the C ABI with HOST buffers: set_spins (H2D of the natural lattice) + sweeps +
-    # observables to host.  Timed with the host clock around synchronising calls.
-    host_lat = torch.empty((w.batch, w.L, w.L), dtype=torch.int8).pin_memory()
-    sim.spin_get_spins(host_lat.numpy())
-    e2e_steps = max(1, min(args.steps, 3))
-    sim.spin_set_spins_ptr(host_lat.data_ptr())          # one untimed end-to-end step (same shape as the timed ones)
-    sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, offset)
-    sim.spin_observables()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        sim.spin_set_spins_ptr(host_lat.data_ptr())
-        sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, offset)
-        Eh, Mh = sim.spin_observables()
-    dt = sharding.max_over_ranks(time.perf_counter() - t0, device="cuda")
-    e2e_value = updates_per_step * e2e_steps / (dt * 1e9)
-    h2d = int(host_lat.numel() + w.batch * 8 + w.batch * 32 * 4)
-    d2h = int(2 * w.batch * 8 + 4)
-
     if rank == 0:
         peaks = _peaks()
-        n_launch = launches_per_sweep_call or 2 * w.n_sweeps
+        n_launch = res["launches_per_sweep_call"] or 2 * w.n_sweeps
         kern_ms = float(np.mean(sweep_ms)) / n_launch  # average launch duration incl. launch gaps
         upd_per_launch = float(w.updates) / n_launch
         ops = OPS_PER_UPDATE[w.model]
         achieved = ops * upd_per_launch / (kern_ms * 1e-3) / 1e12
-        peak = INT32_LANES_PER_SM * N_SM * peaks["sm_max_mhz"] * 1e6 / 1e12
+        peak = alu_peak(peaks)
         bytes_per_site = 0.375 if w.layout == "bits" else 3.0  # per sweep, two launches
         if n_launch == 1:
             bytes_per_site = (0.25 if w.layout == "bits" else 2.0) / w.n_sweeps  # resident: one read + one write per call
         hbm_achieved = bytes_per_site * upd_per_launch / (kern_ms * 1e-3) / 1e9
+        words = 1.0 if w.model == "ising" else 2.0
+        measured_peak = measured * (ops / words) * 1e9 / 1e12           # Tint32op/s the stand-alone kernel sustains
+        vals = float(w.updates) / (np.array(step_ms) * 1e6)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "int8" if w.layout != "bits" else "u32 bit-packed", "data": "synthetic",
             "config": _config_dict(w, world),
             "clocks": clocks,
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps},
-            "gpu_launches": int(launches),
-            "kernel": sim.spin_kernel_variant(),
+            "e2e": res["e2e"],
+            "gpu_launches": res["launches"],
+            "kernel": res["kernel"],
+            "best": float(vals.max()), "median": float(np.median(vals)),
             "sweep_only_flips_per_ns": float(w.updates) / (float(np.mean(sweep_ms)) * 1e6),
             "roofline": {
                 "bound": "alu", "achieved": achieved, "peak": peak, "unit": "Tint32op/s", "frac": achieved / peak,
-                "traffic": _ncu_traffic(sim.spin_kernel_variant(), w),
+                "measured_peak": measured_peak, "frac_of_measured": achieved / measured_peak,
+                "measured_peak_source": "spin_measure_philox_compare_rate(): register-only Philox-4x32-10 + 4 compares, "
+                                        "%.1f random words/ns on this device in this run" % measured,
+                "traffic": _ncu_traffic(res["kernel"], w),
                 "algorithmic_bytes_per_launch": bytes_per_site * upd_per_launch,
                 "launches_per_step": int(n_launch),
                 "kernel_avg_launch_us": kern_ms * 1e3, "ops_per_update": ops,
@@ -337,11 +455,19 @@ def main():
                         "bytes_per_site_per_sweep": bytes_per_site, "peak_source": peaks["source"]},
             },
         }
+        sim.spin_destroy()
+        if world == 1 and not args.no_per_config:
+            line["per_config"] = per_config_block(runner, sp, args, peaks, measured)
         if not args.no_cpu_baseline and world == 1:
-            v, threads, sample, _ = oracle_throughput(w, 15.0)
-            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample}
+            v, threads, sample, _ = oracle_throughput(w, 12.0)
+            line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
+                                    "note": "correctness oracle as it stands (one Philox call per site visit, natural "
+                                            "layout, -O2): a checker, not a tuned CPU implementation"}
+            v1, _, sample1, _ = oracle_throughput(w, 6.0, max_threads=1)
+            line["cpu_baseline"]["single_thread"] = {"value": v1, "cores": 1, "sample": sample1}
         print(json.dumps(line), flush=True)
-    sim.spin_destroy()
+    else:
+        sim.spin_destroy()
     if world > 1:
         dist.destroy_process_group()
 

@@ -75,7 +75,9 @@ SPIN_API spin_sim* spin_create(int32_t batch, int32_t L, int32_t q, uint64_t see
  * beta: host, [batch], inverse temperature of each replica (finite, >= 0); copied before return.
  * J, h: coupling and field (finite).  h must be 0 for Potts (SPIN_ERR_UNSUPPORTED otherwise).
  * n_sweeps >= 0, sweep_offset >= 0, sweep_offset + n_sweeps <= 2^56.
- * Asynchronous on the handle's stream. */
+ * Asynchronous on the handle's stream: the call builds the acceptance tables (O(batch) host work), enqueues their
+ * upload and the sweep kernels, and returns without waiting for earlier work of the stream (the two pinned table
+ * buffers alternate; only the upload issued two calls earlier is waited for). */
 SPIN_API int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_sweeps, int64_t sweep_offset);
 
 /* Exact integer observables of the current lattices (O8).
@@ -128,7 +130,11 @@ SPIN_API int spin_set_spins(spin_sim* sim, const int8_t* in);
  * E_trace, M_trace: host, [n_sweeps][batch] or NULL: (E_int, M) after each sweep.
  * moments: host, [batch][8], in/out, or NULL: every sweep adds one sample to
  *   {n, sum E, sum E^2 (low 64 bits), sum E^2 (high 64 bits), sum M, sum |M|, sum M^2, sum E*M}
- *   with E = E_int; all int64, sum E^2 is one 128-bit integer in two limbs.
+ *   with E = E_int; all int64, sum E^2 is one 128-bit integer in two limbs.  sum M^2 and sum E*M are plain int64
+ *   (|M| <= L^2, |E_int| <= 2 L^2): a call is rejected with SPIN_ERR_INVALID, nothing run, when
+ *   (max_b moments[b][0] + n_sweeps) * 2 L^4 >= 2^63, i.e. when they could wrap (L = 8192: 1024 samples; L <= 1024:
+ *   more than 4e6 samples); accumulate longer runs in several moment arrays.
+ * With both traces NULL no per-sweep trace is stored (a moments-only run of any length needs O(batch) memory).
  * Synchronises the stream. */
 SPIN_API int spin_sweep_measure(spin_sim* sim, const double* beta, double J, double h, int64_t n_sweeps, int64_t sweep_offset,
                        int64_t* E_trace, int64_t* M_trace, int64_t* moments);
@@ -173,6 +179,13 @@ SPIN_API int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv);
  * Returns SPIN_OK or SPIN_ERR_INVALID (NULL handle, unknown policy). */
 enum { SPIN_POLICY_AUTO = 0, SPIN_POLICY_STREAMING = 1, SPIN_POLICY_RESIDENT = 2 };
 SPIN_API int spin_set_policy(spin_sim* sim, int32_t policy);
+
+/* Measurement aid ("second, tighter denominator"): runs a register-only kernel on the current
+ * device that does nothing but the algorithmic work of the sweep - Philox-4x32-10 calls (precomputed round keys) whose
+ * four output words are each compared with a threshold - and returns the best-of-5 rate in random words per
+ * nanosecond (= Ising updates/ns at one word per update; Potts uses two words per update).  Synchronous, default stream,
+ * ~20 ms.  words_per_ns: host.  SPIN_ERR_INVALID for NULL, SPIN_ERR_CUDA without a device. */
+SPIN_API int spin_measure_philox_compare_rate(double* words_per_ns);
 
 #ifdef __cplusplus
 }

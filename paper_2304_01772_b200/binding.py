@@ -17,7 +17,7 @@ __all__ = [
     "SPIN_OK", "SPIN_ERR_INVALID", "SPIN_ERR_NOMEM", "SPIN_ERR_CUDA", "SPIN_ERR_UNSUPPORTED",
     "SPIN_MODEL_ISING", "SPIN_MODEL_POTTS", "SPIN_LAYOUT_INT8", "SPIN_LAYOUT_BITPACKED",
     "SPIN_POLICY_AUTO", "SPIN_POLICY_STREAMING", "SPIN_POLICY_RESIDENT",
-    "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim",
+    "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim", "spin_measure_philox_compare_rate",
     "spin_create", "spin_create_ex",
 ]
 
@@ -60,6 +60,7 @@ def load_library():
         "spin_kernel_variant": (c.c_char_p, [vp]),
         "spin_set_policy": (c.c_int, [vp, i32]),
         "spin_set_bonds": (c.c_int, [vp, vp, vp]),
+        "spin_measure_philox_compare_rate": (c.c_int, [vp]),
     }
     for name, (res, args) in protos.items():
         fn = getattr(lib, name)
@@ -73,7 +74,7 @@ EXPORTED_SYMBOLS = (
     "spin_create", "spin_sweep", "spin_observables", "spin_destroy", "spin_last_error", "spin_buffer_bytes",
     "spin_create_ex", "spin_set_stream", "spin_get_spins", "spin_set_spins", "spin_sweep_measure",
     "spin_observables_dev", "spin_synchronize", "spin_threshold_table", "spin_kernel_launches",
-    "spin_kernel_variant", "spin_set_policy", "spin_set_bonds",
+    "spin_kernel_variant", "spin_set_policy", "spin_set_bonds", "spin_measure_philox_compare_rate",
 )
 
 
@@ -102,6 +103,13 @@ def spin_threshold_table(model, beta, J, h=0.0):
     if n < 0:
         raise SpinError(n, spin_last_error())
     return T[:n].copy(), a[:n].astype(bool)
+
+
+def spin_measure_philox_compare_rate():
+    """Stand-alone Philox-4x32-10 + compare rate of the current device, random words per ns (measurement aid)."""
+    v = ctypes.c_double(0.0)
+    _check(load_library().spin_measure_philox_compare_rate(ctypes.byref(v)))
+    return float(v.value)
 
 
 class SpinSim:

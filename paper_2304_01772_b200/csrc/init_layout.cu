@@ -87,6 +87,52 @@ __global__ void to_natural_int8_kernel(const int8_t* __restrict__ lat, int8_t* _
     nat[gid] = lat[int8_index(b, L, i, j)];
 }
 
+// L % 32 == 0: one thread per 32 consecutive natural bytes of a row (two 128-bit loads) <-> one 128-bit word of each
+// colour.  In row i the even columns belong to colour i & 1 and the odd columns to the other one; PRMT separates /
+// interleaves them, and every global access is a coalesced 128-bit one.
+__global__ void __launch_bounds__(256) from_natural_int8_vec_kernel(const uint4* __restrict__ nat, int8_t* __restrict__ lat,
+                                                                    int batch, int L) {
+    const int C = L >> 5;                                       // 32-byte chunks per row
+    const long long total = (long long)batch * L * C;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= total) return;
+    const int x = (int)(gid % C);
+    const long long bi = gid / C;                               // b * L + i
+    const int i = (int)(bi % L);
+    const long long b = bi / L;
+    const uint4 a = __ldg(nat + 2 * gid), c = __ldg(nat + 2 * gid + 1);
+    const uint4 ev = make_uint4(__byte_perm(a.x, a.y, 0x6420), __byte_perm(a.z, a.w, 0x6420),
+                                __byte_perm(c.x, c.y, 0x6420), __byte_perm(c.z, c.w, 0x6420));
+    const uint4 od = make_uint4(__byte_perm(a.x, a.y, 0x7531), __byte_perm(a.z, a.w, 0x7531),
+                                __byte_perm(c.x, c.y, 0x7531), __byte_perm(c.z, c.w, 0x7531));
+    const size_t W16 = (size_t)(L >> 5);                        // uint4 per colour-row
+    uint4* l4 = (uint4*)lat;
+    const int ce = i & 1;
+    l4[(((size_t)b * 2 + ce) * L + i) * W16 + x] = ev;
+    l4[(((size_t)b * 2 + (1 - ce)) * L + i) * W16 + x] = od;
+}
+
+__global__ void __launch_bounds__(256) to_natural_int8_vec_kernel(const int8_t* __restrict__ lat, uint4* __restrict__ nat,
+                                                                  int batch, int L) {
+    const int C = L >> 5;
+    const long long total = (long long)batch * L * C;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= total) return;
+    const int x = (int)(gid % C);
+    const long long bi = gid / C;
+    const int i = (int)(bi % L);
+    const long long b = bi / L;
+    const size_t W16 = (size_t)(L >> 5);
+    const uint4* l4 = (const uint4*)lat;
+    const int ce = i & 1;
+    const uint4 ev = l4[(((size_t)b * 2 + ce) * L + i) * W16 + x];
+    const uint4 od = l4[(((size_t)b * 2 + (1 - ce)) * L + i) * W16 + x];
+    nat[2 * gid] = make_uint4(__byte_perm(ev.x, od.x, 0x5140), __byte_perm(ev.x, od.x, 0x7362),
+                              __byte_perm(ev.y, od.y, 0x5140), __byte_perm(ev.y, od.y, 0x7362));
+    nat[2 * gid + 1] = make_uint4(__byte_perm(ev.z, od.z, 0x5140), __byte_perm(ev.z, od.z, 0x7362),
+                                  __byte_perm(ev.w, od.w, 0x5140), __byte_perm(ev.w, od.w, 0x7362));
+}
+
 // one thread per (b, i, x): 64 natural sites <-> two words
 __global__ void from_natural_bits_kernel(const int8_t* __restrict__ nat, uint32_t* __restrict__ lat, int batch, int L) {
     const int wordsPerRow = L >> 6;
@@ -136,6 +182,32 @@ __global__ void validate_natural_kernel(const int8_t* __restrict__ nat, int batc
     if (!ok) atomicAdd(bad, 1u);
 }
 
+// 16 bytes per thread (N % 16 == 0): Ising bytes must be 0x01 or 0xFF, Potts bytes < q of their replica.
+__global__ void __launch_bounds__(256) validate_natural_vec_kernel(const uint4* __restrict__ nat, long long n16, long long N16,
+                                                                   int potts, const int32_t* __restrict__ q, unsigned int* bad) {
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= n16) return;
+    const uint4 v = __ldg(nat + gid);
+    const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+    unsigned int nbad = 0;
+    if (potts) {
+        const uint32_t qq = (uint32_t)q[gid / N16];            // bytes >= q (or negative): bit 7 of (byte | (byte + 0x80 - q))
+        const uint32_t add = (0x80u - qq) * 0x01010101u;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) nbad += __popc((w[k] | ((w[k] & 0x7F7F7F7Fu) + add)) & 0x80808080u);
+    } else {
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            // exact zero-byte test on w ^ 0x01.. (+1 bytes) and on ~w (-1 = 0xFF bytes)
+            const uint32_t a = w[k] ^ 0x01010101u, c = ~w[k];
+            const uint32_t za = ~(((a & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | a | 0x7F7F7F7Fu);
+            const uint32_t zc = ~(((c & 0x7F7F7F7Fu) + 0x7F7F7F7Fu) | c | 0x7F7F7F7Fu);
+            nbad += 4 - __popc(za | zc);
+        }
+    }
+    if (nbad) atomicAdd(bad, nbad);
+}
+
 inline unsigned blocks_for(long long n, int tpb) { return (unsigned)((n + tpb - 1) / tpb); }
 
 }  // namespace
@@ -156,6 +228,9 @@ int launch_from_natural(const int8_t* natural, void* lattice, int batch, int L, 
     if (layout == 1) {
         const long long total = (long long)batch * L * (L >> 6);
         from_natural_bits_kernel<<<blocks_for(total, 128), 128, 0, s>>>(natural, (uint32_t*)lattice, batch, L);
+    } else if (L % 32 == 0) {
+        const long long total = (long long)batch * L * (L >> 5);
+        from_natural_int8_vec_kernel<<<blocks_for(total, 256), 256, 0, s>>>((const uint4*)natural, (int8_t*)lattice, batch, L);
     } else {
         const long long total = (long long)batch * L * L;
         from_natural_int8_kernel<<<blocks_for(total, 256), 256, 0, s>>>(natural, (int8_t*)lattice, batch, L);
@@ -167,6 +242,9 @@ int launch_to_natural(const void* lattice, int8_t* natural, int batch, int L, in
     if (layout == 1) {
         const long long total = (long long)batch * L * (L >> 6);
         to_natural_bits_kernel<<<blocks_for(total, 128), 128, 0, s>>>((const uint32_t*)lattice, natural, batch, L);
+    } else if (L % 32 == 0) {
+        const long long total = (long long)batch * L * (L >> 5);
+        to_natural_int8_vec_kernel<<<blocks_for(total, 256), 256, 0, s>>>((const int8_t*)lattice, (uint4*)natural, batch, L);
     } else {
         const long long total = (long long)batch * L * L;
         to_natural_int8_kernel<<<blocks_for(total, 256), 256, 0, s>>>((const int8_t*)lattice, natural, batch, L);
@@ -177,6 +255,11 @@ int launch_to_natural(const void* lattice, int8_t* natural, int batch, int L, in
 int launch_validate_natural(const int8_t* natural, int batch, int L, int model, const int32_t* q, unsigned int* bad,
                             cudaStream_t s) {
     const long long total = (long long)batch * L * L;
+    if (((long long)L * L) % 16 == 0) {
+        validate_natural_vec_kernel<<<blocks_for(total >> 4, 256), 256, 0, s>>>((const uint4*)natural, total >> 4,
+                                                                                ((long long)L * L) >> 4, model, q, bad);
+        return 1;
+    }
     validate_natural_kernel<<<blocks_for(total, 256), 256, 0, s>>>(natural, batch, L, model, q, bad);
     return 1;
 }

@@ -15,9 +15,7 @@ __device__ __forceinline__ uint32_t sel(uint32_t m, uint32_t a, uint32_t b) { re
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
 constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
 constexpr int kThreads = 128;
-#ifndef BITS_MINB
-#define BITS_MINB 8
-#endif
+constexpr int kMinBlocks = 8;   // resident blocks per SM (64 registers)
 
 // One word = 32 sites = 8 Philox calls.  up / dn / ct: other-colour words of rows i-1, i+1, i; sd: the side
 // neighbours (ct shifted by one site, with the bit of the adjacent word).  The class nibbles of the 32 sites are
@@ -167,7 +165,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 }
 
 template <int kColour, int kRows, bool kBonds>
-__global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepArgs a, int bpr) {
+__global__ void __launch_bounds__(kThreads, kMinBlocks) ising_bits_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[16];                          // U[class], class = d * 8 + nd
     __shared__ __align__(16) uint8_t sT[kAuxBytes];        // [e][half][byte] -> 4 * class
     __shared__ uint32_t sidx[4 * kThreads];                // per-thread slot: word e of thread t at sidx[e * 128 + t]
@@ -193,9 +191,8 @@ __global__ void __launch_bounds__(kThreads, BITS_MINB) ising_bits_kernel(SweepAr
 
 // Host side of the constant lookup table: entry [e][half][v] = 4 * class of the low (half 0) / high (half 1) nibble
 // of v, where the nibble of a site 4c+e holds (D, P2, P1, P0) rotated by e bits (see update_word).
-const uint8_t* ising_bits_aux_table() {
-    static uint8_t* d_table = nullptr;
-    if (!d_table) {
+uint8_t* ising_bits_make_aux_table() {
+    {
         uint8_t h[kAuxBytes];
         for (int e = 0; e < 4; ++e)
             for (int half = 0; half < 2; ++half)
@@ -214,9 +211,8 @@ const uint8_t* ising_bits_aux_table() {
         uint8_t* p = nullptr;
         if (cudaMalloc(&p, kAuxBytes) != cudaSuccess) return nullptr;
         if (cudaMemcpy(p, h, kAuxBytes, cudaMemcpyHostToDevice) != cudaSuccess) { cudaFree(p); return nullptr; }
-        d_table = p;
+        return p;
     }
-    return d_table;
 }
 
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {

@@ -63,9 +63,7 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 // the next half-sweep's blocks are scheduled while this one drains.
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
 constexpr int kRowsShort = 2;   // ... and when it does not (latency-bound shapes): four times as many threads
-#ifndef ISING_MINB
-#define ISING_MINB 5
-#endif
+constexpr int kMinBlocks = 5;   // resident blocks per SM (96 registers)
 constexpr int kRowsThreads = 128;
 
 template <int kOff>
@@ -229,7 +227,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 
 // One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
 template <int kColour, int kRows>
-__global__ void __launch_bounds__(kRowsThreads, ISING_MINB) ising_int8_rows_kernel(SweepArgs a, int bpr) {
+__global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[kTableStride];
     __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
     pdl_launch_dependents();
@@ -478,14 +476,15 @@ static size_t resident_smem_bytes(int L) {
 
 bool ising_int8_resident_fits(int L) { return L % 32 == 0 && (size_t)L * L <= kResMaxLatticeBytes; }
 
+// Opt the resident kernel in to more than 48 KiB of dynamic shared memory on the CURRENT device (called once per
+// handle at creation: the attribute is per device, and cheap to set again).
+cudaError_t ising_int8_resident_configure() {
+    return cudaFuncSetAttribute(ising_int8_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)(kResMaxLatticeBytes + sizeof(uint32_t) * (kTableStride + 4 * kResThreads) + 128));
+}
+
 int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s) {
     const size_t smem = resident_smem_bytes(a.L);
-    static bool configured = false;
-    if (!configured) {
-        cudaFuncSetAttribute(ising_int8_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)(kResMaxLatticeBytes + sizeof(uint32_t) * (kTableStride + 4 * kResThreads) + 128));
-        configured = true;
-    }
     const int units = a.L <= 64 ? a.L * (a.L >> 3) : a.L * (a.L >> 5);   // words (tiny lattices) or strips per colour
     int tpb = kResThreads;
     while (tpb > 32 && tpb / 2 >= units) tpb >>= 1;           // L = 32: 128 words -> 128 threads

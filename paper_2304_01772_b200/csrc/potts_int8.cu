@@ -56,9 +56,7 @@ __global__ void potts_int8_generic_kernel(SweepArgs a) {
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
 constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
 constexpr int kRowsThreads = 128;
-#ifndef POTTS_MINB
-#define POTTS_MINB 4
-#endif
+constexpr int kMinBlocks = 4;   // resident blocks per SM (128 registers)
 
 template <int kOff>
 __device__ __forceinline__ uint32_t slot_load_u8(uint32_t saddr) {
@@ -248,7 +246,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 
 // One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
 template <int kColour, int kRows>
-__global__ void __launch_bounds__(kRowsThreads, POTTS_MINB) potts_int8_rows_kernel(SweepArgs a, int bpr) {
+__global__ void __launch_bounds__(kRowsThreads, kMinBlocks) potts_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[16 + 64];            // U[dn + 4] in [0..8]; from word 16: 256-byte pattern -> 4 * class table
     __shared__ uint32_t snever[1];
     __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]

@@ -26,7 +26,7 @@ int fail(int code, const char* fmt, ...) {
     va_start(ap, fmt);
     vsnprintf(buf, sizeof buf, fmt, ap);
     va_end(ap);
-    g_last_error = buf;
+    try { g_last_error = buf; } catch (...) {}   // no exception may cross the C boundary
     return code;
 }
 
@@ -98,8 +98,18 @@ struct spin_sim {
     unsigned int* d_hist = nullptr;  // [B][128] (Potts)
     unsigned int* d_bad = nullptr;   // validation counter
     uint32_t* d_bonds = nullptr;     // +-J sign planes [B][2][4][L][L/64] (bit-packed layout) or nullptr
-    // scratch (host, pinned)
-    uint32_t* h_tables = nullptr;
+    uint8_t* d_aux = nullptr;        // bit-packed kernel's constant 2 KiB lookup table, on this handle's device
+    int8_t* d_stage = nullptr;       // natural-layout staging for spin_get_spins / spin_set_spins / spin_set_bonds (grow-only)
+    size_t stage_bytes = 0;
+    long long* d_mom = nullptr;      // [B][8] moments of spin_sweep_measure
+    long long* d_trace = nullptr;    // trace buffer of spin_sweep_measure (grow-only)
+    size_t trace_bytes = 0;
+    // scratch (host, pinned): two table buffers used alternately, each guarded by the event recorded after its upload,
+    // so that spin_sweep never waits for earlier sweeps, only (rarely) for the copy issued two calls ago
+    uint32_t* h_tables[2] = {nullptr, nullptr};
+    cudaEvent_t table_ev[2] = {nullptr, nullptr};
+    int table_slot = 0;
+    long long* h_EM = nullptr;       // [2][B] pinned, spin_observables
     RoundKeys rk;
     int64_t launches = 0;
     int32_t policy = SPIN_POLICY_AUTO;
@@ -138,11 +148,14 @@ int check_sweep_args(const spin_sim* sim, const double* beta, double J, double h
 
 // Build the per-replica records on the host and enqueue their copy.
 int upload_tables(spin_sim* sim, const double* beta, double J, double h) {
-    // the previous upload may still be in flight from the pinned buffer
-    CUDA_TRY(cudaStreamSynchronize(sim->stream));
-    std::memset(sim->h_tables, 0, sizeof(uint32_t) * kTableStride * (size_t)sim->batch);
+    // the upload issued two calls ago may still be reading this pinned buffer; nothing else is waited for
+    const int slot = sim->table_slot;
+    sim->table_slot ^= 1;
+    uint32_t* h_tab = sim->h_tables[slot];
+    CUDA_TRY(cudaEventSynchronize(sim->table_ev[slot]));
+    std::memset(h_tab, 0, sizeof(uint32_t) * kTableStride * (size_t)sim->batch);
     for (int b = 0; b < sim->batch; ++b) {
-        uint32_t* rec = sim->h_tables + (size_t)b * kTableStride;
+        uint32_t* rec = h_tab + (size_t)b * kTableStride;
         if (sim->model == SPIN_MODEL_ISING) {
             for (int d = 0; d < 2; ++d)
                 for (int nd = 0; nd <= 4; ++nd) {
@@ -154,8 +167,9 @@ int upload_tables(spin_sim* sim, const double* beta, double J, double h) {
         }
         rec[kTabQ] = (uint32_t)sim->q[b];
     }
-    CUDA_TRY(cudaMemcpyAsync(sim->d_tables, sim->h_tables, sizeof(uint32_t) * kTableStride * (size_t)sim->batch,
+    CUDA_TRY(cudaMemcpyAsync(sim->d_tables, h_tab, sizeof(uint32_t) * kTableStride * (size_t)sim->batch,
                              cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaEventRecord(sim->table_ev[slot], sim->stream));
     return SPIN_OK;
 }
 
@@ -170,7 +184,7 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     const uint32_t domain = sim->model == SPIN_MODEL_ISING ? kDomainIsing : kDomainPotts;
     a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)colour << 24) | (domain << 28);
     a.colour = colour;
-    a.aux = sim->layout == SPIN_LAYOUT_BITPACKED ? ising_bits_aux_table() : nullptr;
+    a.aux = sim->d_aux;
     a.bonds = sim->d_bonds;
     a.rk = sim->rk;
     return a;
@@ -237,6 +251,31 @@ int enqueue_observe(spin_sim* sim, long long* E_out, long long* M_out) {
     return SPIN_OK;
 }
 
+// Grow-only device staging buffers kept in the handle (no cudaMalloc / cudaFree on the per-call paths).
+int ensure_stage(spin_sim* sim, size_t bytes) {
+    if (sim->stage_bytes >= bytes) return SPIN_OK;
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    if (sim->d_stage) cudaFree(sim->d_stage);
+    sim->d_stage = nullptr;
+    sim->stage_bytes = 0;
+    cudaError_t e = cudaMalloc(&sim->d_stage, bytes);
+    if (e != cudaSuccess) { sim->d_stage = nullptr; return fail(SPIN_ERR_NOMEM, "cudaMalloc(%zu) for staging: %s", bytes, cudaGetErrorString(e)); }
+    sim->stage_bytes = bytes;
+    return SPIN_OK;
+}
+
+int ensure_trace(spin_sim* sim, size_t bytes) {
+    if (sim->trace_bytes >= bytes) return SPIN_OK;
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    if (sim->d_trace) cudaFree(sim->d_trace);
+    sim->d_trace = nullptr;
+    sim->trace_bytes = 0;
+    cudaError_t e = cudaMalloc(&sim->d_trace, bytes);
+    if (e != cudaSuccess) { sim->d_trace = nullptr; return fail(SPIN_ERR_NOMEM, "cudaMalloc(%zu) for the trace: %s", bytes, cudaGetErrorString(e)); }
+    sim->trace_bytes = bytes;
+    return SPIN_OK;
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -289,7 +328,15 @@ void spin_destroy(spin_sim* sim) {
     if (sim->d_EM) cudaFree(sim->d_EM);
     if (sim->d_hist) cudaFree(sim->d_hist);
     if (sim->d_bad) cudaFree(sim->d_bad);
-    if (sim->h_tables) cudaFreeHost(sim->h_tables);
+    if (sim->d_aux) cudaFree(sim->d_aux);
+    if (sim->d_stage) cudaFree(sim->d_stage);
+    if (sim->d_mom) cudaFree(sim->d_mom);
+    if (sim->d_trace) cudaFree(sim->d_trace);
+    for (int k = 0; k < 2; ++k) {
+        if (sim->h_tables[k]) cudaFreeHost(sim->h_tables[k]);
+        if (sim->table_ev[k]) cudaEventDestroy(sim->table_ev[k]);
+    }
+    if (sim->h_EM) cudaFreeHost(sim->h_EM);
     delete sim;
 }
 
@@ -325,7 +372,19 @@ static int create_impl(spin_sim* sim, void* device_buffer, size_t buffer_bytes) 
         CUDA_TRY(cudaMalloc(&sim->d_hist, sizeof(unsigned int) * 128 * B));
         CUDA_TRY(cudaMemsetAsync(sim->d_hist, 0, sizeof(unsigned int) * 128 * B, sim->stream));
     }
-    CUDA_TRY(cudaMallocHost(&sim->h_tables, sizeof(uint32_t) * kTableStride * B));
+    for (int k = 0; k < 2; ++k) {
+        CUDA_TRY(cudaMallocHost(&sim->h_tables[k], sizeof(uint32_t) * kTableStride * B));
+        CUDA_TRY(cudaEventCreateWithFlags(&sim->table_ev[k], cudaEventDisableTiming));
+    }
+    CUDA_TRY(cudaMallocHost(&sim->h_EM, sizeof(long long) * 2 * B));
+    CUDA_TRY(cudaMalloc(&sim->d_mom, sizeof(long long) * 8 * B));
+    // per-device kernel state lives in the handle (a handle belongs to the device current at creation)
+    if (sim->layout == SPIN_LAYOUT_BITPACKED) {
+        sim->d_aux = ising_bits_make_aux_table();
+        if (!sim->d_aux) return fail(SPIN_ERR_CUDA, "could not allocate the bit-packed kernel's lookup table");
+    }
+    if (sim->model == SPIN_MODEL_ISING && sim->layout == SPIN_LAYOUT_INT8 && ising_int8_resident_fits(sim->L))
+        CUDA_TRY(ising_int8_resident_configure());
     CUDA_TRY(cudaMemcpyAsync(sim->d_q, sim->q.data(), sizeof(int32_t) * B, cudaMemcpyHostToDevice, sim->stream));
     // row a0: initial lattice
     InitArgs ia;
@@ -354,6 +413,7 @@ spin_sim* spin_create_ex(int32_t batch, int32_t L, int32_t model, const int32_t*
     if (layout == SPIN_LAYOUT_BITPACKED && L % 64 != 0) { fail(SPIN_ERR_UNSUPPORTED, "spin_create: the bit-packed layout needs L %% 64 == 0"); return nullptr; }
     spin_sim* sim = new (std::nothrow) spin_sim;
     if (!sim) { fail(SPIN_ERR_NOMEM, "spin_create: out of host memory"); return nullptr; }
+    try {
     sim->batch = batch; sim->L = L; sim->model = model; sim->layout = layout; sim->seed = seed;
     sim->replica_offset = (uint32_t)replica_offset;
     sim->stream = (cudaStream_t)cuda_stream;
@@ -364,15 +424,24 @@ spin_sim* spin_create_ex(int32_t batch, int32_t L, int32_t model, const int32_t*
         if (qb < 2 || qb > 127) {
             fail(SPIN_ERR_INVALID, "spin_create: q[%d] = %d outside 2..127", b, qb);
             delete sim;
+            sim = nullptr;
             return nullptr;
         }
         sim->q[b] = qb;
     }
-    if (create_impl(sim, device_buffer, buffer_bytes) != SPIN_OK) {
-        const std::string keep = g_last_error;
+    const int rc = create_impl(sim, device_buffer, buffer_bytes);
+    if (rc != SPIN_OK) {
+        char keep[512];
+        snprintf(keep, sizeof keep, "%s", g_last_error.c_str());
         spin_destroy(sim);
+        sim = nullptr;
         cudaGetLastError();
-        g_last_error = keep;
+        fail(rc, "%s", keep);
+        return nullptr;
+    }
+    } catch (...) {   // std::bad_alloc from the host-side containers
+        if (sim) spin_destroy(sim);
+        fail(SPIN_ERR_NOMEM, "spin_create: out of host memory");
         return nullptr;
     }
     return sim;
@@ -425,19 +494,17 @@ int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv) {
     }
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_BITPACKED)
         return fail(SPIN_ERR_UNSUPPORTED, "spin_set_bonds: +-J couplings are implemented for the bit-packed Ising layout only");
-    // natural-layout signs -> device -> per-colour bit planes (validated on the device; a rejected call leaves the
-    // handle's couplings as they were)
+    // natural-layout signs -> device staging -> per-colour bit planes (validated on the device; a rejected call leaves
+    // the handle's couplings as they were)
     const int L = sim->L;
     const size_t nat = (size_t)sim->batch * L * L;
     const size_t words = (size_t)sim->batch * 2 * 4 * L * (size_t)(L >> 6);
-    int8_t* d_nat = nullptr;
+    const int rs = ensure_stage(sim, 2 * nat);
+    if (rs != SPIN_OK) return rs;
+    int8_t* d_nat = sim->d_stage;
     uint32_t* d_new = nullptr;
-    cudaError_t e = cudaMalloc(&d_nat, 2 * nat);
-    if (e == cudaSuccess) e = cudaMalloc(&d_new, words * sizeof(uint32_t));
-    if (e != cudaSuccess) {
-        if (d_nat) cudaFree(d_nat);
-        return fail(SPIN_ERR_NOMEM, "spin_set_bonds: cudaMalloc: %s", cudaGetErrorString(e));
-    }
+    cudaError_t e = cudaMalloc(&d_new, words * sizeof(uint32_t));
+    if (e != cudaSuccess) return fail(SPIN_ERR_NOMEM, "spin_set_bonds: cudaMalloc: %s", cudaGetErrorString(e));
     unsigned int bad = 0;
     e = cudaMemcpyAsync(d_nat, Jh, nat, cudaMemcpyHostToDevice, sim->stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(d_nat + nat, Jv, nat, cudaMemcpyHostToDevice, sim->stream);
@@ -447,7 +514,6 @@ int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv) {
         e = cudaMemcpyAsync(&bad, sim->d_bad, sizeof bad, cudaMemcpyDeviceToHost, sim->stream);
     }
     if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
-    cudaFree(d_nat);
     if (e != cudaSuccess) { cudaFree(d_new); return cuda_fail(e, "spin_set_bonds"); }
     if (bad) { cudaFree(d_new); return fail(SPIN_ERR_INVALID, "spin_set_bonds: bond signs must be +1 or -1"); }
     if (sim->d_bonds) cudaFree(sim->d_bonds);
@@ -494,11 +560,10 @@ int spin_observables(spin_sim* sim, int64_t* E, int64_t* M) {
     const size_t B = (size_t)sim->batch;
     const int rc = enqueue_observe(sim, sim->d_EM, sim->d_EM + B);
     if (rc != SPIN_OK) return rc;
-    std::vector<long long> tmp(2 * B);
-    CUDA_TRY(cudaMemcpyAsync(tmp.data(), sim->d_EM, sizeof(long long) * 2 * B, cudaMemcpyDeviceToHost, sim->stream));
+    CUDA_TRY(cudaMemcpyAsync(sim->h_EM, sim->d_EM, sizeof(long long) * 2 * B, cudaMemcpyDeviceToHost, sim->stream));
     CUDA_TRY(cudaStreamSynchronize(sim->stream));
-    if (E) std::memcpy(E, tmp.data(), sizeof(long long) * B);
-    if (M) std::memcpy(M, tmp.data() + B, sizeof(long long) * B);
+    if (E) std::memcpy(E, sim->h_EM, sizeof(long long) * B);
+    if (M) std::memcpy(M, sim->h_EM + B, sizeof(long long) * B);
     return SPIN_OK;
 }
 
@@ -506,14 +571,11 @@ int spin_get_spins(spin_sim* sim, int8_t* out) {
     if (!sim || !out) return fail(SPIN_ERR_INVALID, "spin_get_spins: NULL argument");
     CUDA_TRY(cudaSetDevice(sim->device));
     const size_t n = (size_t)sim->batch * sim->L * sim->L;
-    int8_t* d_nat = nullptr;
-    cudaError_t e = cudaMalloc(&d_nat, n);
-    if (e != cudaSuccess) return fail(SPIN_ERR_NOMEM, "spin_get_spins: cudaMalloc(%zu): %s", n, cudaGetErrorString(e));
-    sim->launches += launch_to_natural(sim->lattice, d_nat, sim->batch, sim->L, sim->layout, sim->stream);
-    e = cudaMemcpyAsync(out, d_nat, n, cudaMemcpyDeviceToHost, sim->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
-    cudaFree(d_nat);
-    if (e != cudaSuccess) return cuda_fail(e, "spin_get_spins");
+    const int rs = ensure_stage(sim, n);
+    if (rs != SPIN_OK) return rs;
+    sim->launches += launch_to_natural(sim->lattice, sim->d_stage, sim->batch, sim->L, sim->layout, sim->stream);
+    CUDA_TRY(cudaMemcpyAsync(out, sim->d_stage, n, cudaMemcpyDeviceToHost, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
     return SPIN_OK;
 }
 
@@ -521,24 +583,18 @@ int spin_set_spins(spin_sim* sim, const int8_t* in) {
     if (!sim || !in) return fail(SPIN_ERR_INVALID, "spin_set_spins: NULL argument");
     CUDA_TRY(cudaSetDevice(sim->device));
     const size_t n = (size_t)sim->batch * sim->L * sim->L;
-    int8_t* d_nat = nullptr;
-    cudaError_t e = cudaMalloc(&d_nat, n);
-    if (e != cudaSuccess) return fail(SPIN_ERR_NOMEM, "spin_set_spins: cudaMalloc(%zu): %s", n, cudaGetErrorString(e));
+    const int rs = ensure_stage(sim, n);
+    if (rs != SPIN_OK) return rs;
     unsigned int bad = 0;
-    e = cudaMemcpyAsync(d_nat, in, n, cudaMemcpyHostToDevice, sim->stream);
-    if (e == cudaSuccess) e = cudaMemsetAsync(sim->d_bad, 0, sizeof(unsigned int), sim->stream);
-    if (e == cudaSuccess) {
-        sim->launches += launch_validate_natural(d_nat, sim->batch, sim->L, sim->model, sim->d_q, sim->d_bad, sim->stream);
-        e = cudaMemcpyAsync(&bad, sim->d_bad, sizeof bad, cudaMemcpyDeviceToHost, sim->stream);
-    }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
-    if (e == cudaSuccess && bad == 0) {
-        sim->launches += launch_from_natural(d_nat, sim->lattice, sim->batch, sim->L, sim->layout, sim->stream);
-        e = cudaStreamSynchronize(sim->stream);
-    }
-    cudaFree(d_nat);
-    if (e != cudaSuccess) return cuda_fail(e, "spin_set_spins");
+    CUDA_TRY(cudaMemcpyAsync(sim->d_stage, in, n, cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaMemsetAsync(sim->d_bad, 0, sizeof(unsigned int), sim->stream));
+    sim->launches += launch_validate_natural(sim->d_stage, sim->batch, sim->L, sim->model, sim->d_q, sim->d_bad, sim->stream);
+    CUDA_TRY(cudaMemcpyAsync(&bad, sim->d_bad, sizeof bad, cudaMemcpyDeviceToHost, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
     if (bad) return fail(SPIN_ERR_INVALID, "spin_set_spins: %u values are not valid states", bad);
+    sim->launches += launch_from_natural(sim->d_stage, sim->lattice, sim->batch, sim->L, sim->layout, sim->stream);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));   // the caller may reuse `in`; the staging buffer may be reused
     return SPIN_OK;
 }
 
@@ -549,47 +605,59 @@ int spin_sweep_measure(spin_sim* sim, const double* beta, double J, double h, in
     if (n_sweeps == 0) return SPIN_OK;
     CUDA_TRY(cudaSetDevice(sim->device));
     const size_t B = (size_t)sim->batch;
-    if (n_sweeps > (int64_t)((size_t)1 << 40) / (int64_t)(B * 16))
-        return fail(SPIN_ERR_INVALID, "spin_sweep_measure: n_sweeps * batch too large for one call; chunk it");
+    const bool want_trace = E_trace || M_trace;
+    if (want_trace && n_sweeps > (int64_t)((size_t)1 << 40) / (int64_t)(B * 16))
+        return fail(SPIN_ERR_INVALID, "spin_sweep_measure: n_sweeps * batch too large for one traced call; chunk it");
+    if (moments) {
+        // sum M^2 and sum E*M are plain int64: |M| <= N, |E_int| <= 2N, so n samples stay below 2^63 iff n * 2 N^2 < 2^63
+        // (sum E^2 has two limbs).  Reject rather than wrap (documented in spin.h).
+        const long double N = (long double)sim->L * (long double)sim->L;
+        long double nmax = 0;
+        for (size_t b = 0; b < B; ++b) {
+            if (moments[8 * b] < 0) return fail(SPIN_ERR_INVALID, "spin_sweep_measure: moments[%zu][0] (sample count) is negative", b);
+            if ((long double)moments[8 * b] > nmax) nmax = (long double)moments[8 * b];
+        }
+        if ((nmax + (long double)n_sweeps) * 2.0L * N * N >= 9223372036854775807.0L)
+            return fail(SPIN_ERR_INVALID, "spin_sweep_measure: %lld more samples on L = %d could overflow the 64-bit "
+                        "sums of M^2 and E*M (limit: samples * 2 L^4 < 2^63); accumulate in shorter runs",
+                        (long long)n_sweeps, sim->L);
+    }
+    const bool resident = use_resident(sim, true);
+    // traces wanted: device trace [2][n_sweeps][B].  Otherwise the streaming path reuses one [2][B] sample slot every
+    // sweep, and the resident kernel keeps its sums in registers and takes null trace pointers.
+    const size_t trace_elems = want_trace ? (size_t)n_sweeps * B : (resident ? 0 : B);
+    if (trace_elems) {
+        const int rs = ensure_trace(sim, sizeof(long long) * 2 * trace_elems);
+        if (rs != SPIN_OK) return rs;
+    }
+    long long* d_trace = trace_elems ? sim->d_trace : nullptr;
+    long long* d_mom = moments ? sim->d_mom : nullptr;
     const int rt = upload_tables(sim, beta, J, h);
     if (rt != SPIN_OK) return rt;
-    // device trace [2][n_sweeps][B] + moments [B][8]
-    long long* d_trace = nullptr;
-    long long* d_mom = nullptr;
-    const size_t trace_elems = (size_t)n_sweeps * B;
-    cudaError_t e = cudaMalloc(&d_trace, sizeof(long long) * 2 * trace_elems);
-    if (e != cudaSuccess) return fail(SPIN_ERR_NOMEM, "spin_sweep_measure: cudaMalloc trace: %s", cudaGetErrorString(e));
-    int result = SPIN_OK;
-    do {
-        if (moments) {
-            e = cudaMalloc(&d_mom, sizeof(long long) * 8 * B);
-            if (e != cudaSuccess) { result = fail(SPIN_ERR_NOMEM, "spin_sweep_measure: cudaMalloc moments: %s", cudaGetErrorString(e)); break; }
-            e = cudaMemcpyAsync(d_mom, moments, sizeof(long long) * 8 * B, cudaMemcpyHostToDevice, sim->stream);
-            if (e != cudaSuccess) { result = cuda_fail(e, "copy moments"); break; }
-        }
-        if (use_resident(sim, true))
-            enqueue_resident(sim, sweep_offset, n_sweeps, true, d_trace, d_trace + trace_elems, d_mom);
-        else for (int64_t local = 0; local < n_sweeps && result == SPIN_OK; ++local) {
+    if (moments) CUDA_TRY(cudaMemcpyAsync(d_mom, moments, sizeof(long long) * 8 * B, cudaMemcpyHostToDevice, sim->stream));
+    if (resident) {
+        enqueue_resident(sim, sweep_offset, n_sweeps, true, want_trace ? d_trace : nullptr,
+                         want_trace ? d_trace + trace_elems : nullptr, d_mom);
+    } else {
+        for (int64_t local = 0; local < n_sweeps; ++local) {
             const int64_t t = sweep_offset + local;
             enqueue_half_sweep(sim, t, 0);
             enqueue_half_sweep(sim, t, 1);
-            long long* Et = d_trace + (size_t)local * B;
-            long long* Mt = d_trace + trace_elems + (size_t)local * B;
-            result = enqueue_observe(sim, Et, Mt);
-            if (result == SPIN_OK && moments) sim->launches += launch_accumulate_moments(d_mom, Et, Mt, sim->batch, sim->stream);
+            long long* Et = d_trace + (want_trace ? (size_t)local * B : 0);
+            long long* Mt = d_trace + trace_elems + (want_trace ? (size_t)local * B : 0);
+            const int ro = enqueue_observe(sim, Et, Mt);
+            if (ro != SPIN_OK) { cudaStreamSynchronize(sim->stream); return ro; }
+            if (moments) sim->launches += launch_accumulate_moments(d_mom, Et, Mt, sim->batch, sim->stream);
         }
-        if (result != SPIN_OK) break;
-        e = cudaGetLastError();
-        if (e == cudaSuccess && E_trace) e = cudaMemcpyAsync(E_trace, d_trace, sizeof(long long) * trace_elems, cudaMemcpyDeviceToHost, sim->stream);
-        if (e == cudaSuccess && M_trace) e = cudaMemcpyAsync(M_trace, d_trace + trace_elems, sizeof(long long) * trace_elems, cudaMemcpyDeviceToHost, sim->stream);
-        if (e == cudaSuccess && moments) e = cudaMemcpyAsync(moments, d_mom, sizeof(long long) * 8 * B, cudaMemcpyDeviceToHost, sim->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
-        if (e != cudaSuccess) result = cuda_fail(e, "spin_sweep_measure");
-    } while (0);
-    cudaStreamSynchronize(sim->stream);
-    cudaFree(d_trace);
-    if (d_mom) cudaFree(d_mom);
-    return result;
+    }
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && E_trace) e = cudaMemcpyAsync(E_trace, d_trace, sizeof(long long) * trace_elems, cudaMemcpyDeviceToHost, sim->stream);
+    if (e == cudaSuccess && M_trace) e = cudaMemcpyAsync(M_trace, d_trace + trace_elems, sizeof(long long) * trace_elems, cudaMemcpyDeviceToHost, sim->stream);
+    if (e == cudaSuccess && moments) e = cudaMemcpyAsync(moments, d_mom, sizeof(long long) * 8 * B, cudaMemcpyDeviceToHost, sim->stream);
+    const cudaError_t es = cudaStreamSynchronize(sim->stream);
+    if (e == cudaSuccess) e = es;
+    if (e != cudaSuccess) return cuda_fail(e, "spin_sweep_measure");
+    return SPIN_OK;
 }
 
 }  // extern "C"

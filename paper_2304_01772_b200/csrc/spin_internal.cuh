@@ -58,7 +58,7 @@ struct SweepArgs {
     uint32_t c2;              // low 32 bits of the sweep index t
     uint32_t c3;              // (t >> 32) & 0xFFFFFF | colour << 24 | domain << 28
     int32_t colour;
-    const uint8_t* aux;       // bit-packed kernel: nibble-pair -> 4 * class byte table (ising_bits_aux_table), else nullptr
+    const uint8_t* aux;       // bit-packed kernel: nibble-pair -> 4 * class byte table (spin_sim::d_aux), else nullptr
     const uint32_t* bonds;    // bit-packed +-J couplings: [B][2][4][L][L/64] words (bit = bond is -1; planes up, down,
                               // centre, side of the colour's sites), or nullptr for uniform couplings
     RoundKeys rk;
@@ -132,9 +132,10 @@ int launch_init(const InitArgs& a, int model, int layout, cudaStream_t s);
 int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s);      // picks generic / vectorised
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s);
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s);
-const uint8_t* ising_bits_aux_table();     // device pointer to the constant 2 KiB lookup table (uploaded on first use)
+uint8_t* ising_bits_make_aux_table();      // allocates + fills the constant 2 KiB lookup table on the current device (owned by the caller)
 const char* ising_int8_variant(int L);
 bool ising_int8_resident_fits(int L);                                       // a replica fits one CTA's shared memory
+cudaError_t ising_int8_resident_configure();                                // per device: allow > 48 KiB dynamic shared memory
 int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s);      // all n_sweeps in one launch
 const char* potts_int8_variant(int L);
 
