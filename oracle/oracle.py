@@ -11,20 +11,22 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "spin_oracle.cpp")
+_SRCS = [_SRC, os.path.join(_HERE, "dmc_oracle.cpp")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 __all__ = [
     "build", "philox4x32_10", "ising_table", "potts_table", "init", "ising_half_sweep",
     "potts_half_sweep", "ising_observables", "potts_observables", "accumulate_moments", "sweep",
     "sweep_bonds", "ising_bonds_observables", "ising_bonds_half_sweep",
+    "dmc_half_sweep", "dmc_forward", "dmc_discretise", "dmc_backward",
 ]
 
 
 def build(force=False):
     """Compile the oracle with ``g++ -O2 -ffp-contract=off`` (no FMA contraction)."""
-    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < max(os.path.getmtime(p) for p in _SRCS):
         tmp = _LIB + ".%d.tmp" % os.getpid()
-        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-o", tmp, _SRC])
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fPIC", "-shared", "-o", tmp] + _SRCS)
         os.replace(tmp, _LIB)
     return _LIB
 
@@ -56,6 +58,14 @@ def _l():
                                                       c.c_uint64, c.c_int64, c.c_int64, c.c_int32]
         lib.oracle_sweep_bonds.argtypes = [p, p, p, c.c_int32, c.c_int32, p, c.c_double, c.c_double, c.c_uint64,
                                            c.c_int64, c.c_int64, c.c_int64, p, p]
+        d = c.c_double
+        lib.oracle_dmc_half_sweep.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
+                                              c.c_int32, p]
+        lib.oracle_dmc_forward.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
+                                           c.c_int64, p]
+        lib.oracle_dmc_discretise.argtypes = [p, c.c_int64]
+        lib.oracle_dmc_backward.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
+                                            c.c_int64, p, p, p, p, p, p]
         _lib = lib
     return _lib
 
@@ -207,3 +217,55 @@ def ising_bonds_half_sweep(spins, Jh, Jv, beta, J, h, seed, t, colour, replica_o
     jh, jv = _bonds(Jh, B, L), _bonds(Jv, B, L)
     _l().oracle_ising_bonds_half_sweep(_ptr(spins), _ptr(jh), _ptr(jv), B, L, _ptr(ba), float(J), float(h),
                                        int(seed), int(replica_offset), int(t), int(colour))
+
+
+# ---- Differentiable Monte Carlo (dmc_oracle.cpp; Algorithm 2, Eq. 4) ------------------------------------------
+def _f64(a, shape):
+    a = np.ascontiguousarray(np.broadcast_to(np.asarray(a, dtype=np.float64), shape))
+    return a
+
+
+def _dmc_lattice(s):
+    assert s.dtype == np.float64 and s.ndim == 3 and s.shape[1] == s.shape[2] and s.flags["C_CONTIGUOUS"]
+    return s.shape[0], s.shape[1]
+
+
+def dmc_half_sweep(s, Jh, Jv, h, beta, alpha, seed, t, colour, replica_offset=0, want_q=False):
+    """One DMC half-sweep in place on the float64 lattice s [B][L][L]; returns q [B][L][L] (NaN elsewhere) if want_q."""
+    B, L = _dmc_lattice(s)
+    jh, jv, ba = _f64(Jh, (B, L, L)), _f64(Jv, (B, L, L)), _beta_array(beta, B)
+    q = np.full((B, L, L), np.nan) if want_q else None
+    _l().oracle_dmc_half_sweep(_ptr(s), _ptr(jh), _ptr(jv), B, L, float(h), _ptr(ba), float(alpha), int(seed),
+                               int(replica_offset), int(t), int(colour), _ptr(q))
+    return q
+
+
+def dmc_forward(s, Jh, Jv, h, beta, alpha, seed, n_sweeps, sweep_offset=0, replica_offset=0, want_traj=False):
+    """n_sweeps DMC sweeps in place; returns the trajectory [2 n_sweeps + 1][B][L][L] if want_traj."""
+    B, L = _dmc_lattice(s)
+    jh, jv, ba = _f64(Jh, (B, L, L)), _f64(Jv, (B, L, L)), _beta_array(beta, B)
+    traj = np.zeros((2 * n_sweeps + 1, B, L, L)) if want_traj else None
+    _l().oracle_dmc_forward(_ptr(s), _ptr(jh), _ptr(jv), B, L, float(h), _ptr(ba), float(alpha), int(seed),
+                            int(replica_offset), int(n_sweeps), int(sweep_offset), _ptr(traj))
+    return traj
+
+
+def dmc_discretise(s):
+    assert s.dtype == np.float64 and s.flags["C_CONTIGUOUS"]
+    _l().oracle_dmc_discretise(_ptr(s), s.size)
+    return s
+
+
+def dmc_backward(traj, Jh, Jv, h, beta, alpha, seed, grad_out, sweep_offset=0, replica_offset=0):
+    """-> (grad_s0, grad_Jh, grad_Jv [B][L][L], grad_beta [B], grad_h [B]) of a loss whose gradient with respect to the
+    final lattice is grad_out; traj from dmc_forward(..., want_traj=True)."""
+    assert traj.dtype == np.float64 and traj.ndim == 4 and traj.flags["C_CONTIGUOUS"]
+    n_sweeps, B, L = (traj.shape[0] - 1) // 2, traj.shape[1], traj.shape[2]
+    jh, jv, ba = _f64(Jh, (B, L, L)), _f64(Jv, (B, L, L)), _beta_array(beta, B)
+    go = _f64(grad_out, (B, L, L))
+    gs, gjh, gjv = np.zeros((B, L, L)), np.zeros((B, L, L)), np.zeros((B, L, L))
+    gb, gh = np.zeros(B), np.zeros(B)
+    _l().oracle_dmc_backward(_ptr(traj), _ptr(jh), _ptr(jv), B, L, float(h), _ptr(ba), float(alpha), int(seed),
+                             int(replica_offset), int(n_sweeps), int(sweep_offset), _ptr(go), _ptr(gs), _ptr(gjh),
+                             _ptr(gjv), _ptr(gb), _ptr(gh))
+    return gs, gjh, gjv, gb, gh
