@@ -354,6 +354,70 @@ def per_config_block(runner, sp, args, peaks, measured):
     return out
 
 
+def dmc_entries(runner, sp, args, peaks):
+    """Differentiable Monte Carlo (Algorithm 2): forward only, and forward + backward (one training
+    step of PAPER.md:308-332 without the optimiser), fp32, on a C2-shaped batch.  HBM-bound: the roofline is the
+    algorithmic bytes per site per sweep over the measured copy bandwidth."""
+    torch = runner.torch
+    B, L, n_sweeps, seed, alpha, h = 64, 1024, 4, 7, 6.0, 0.0
+    if args.sweeps:
+        n_sweeps = max(1, min(n_sweeps, args.sweeps))
+    gen = torch.Generator(device="cuda").manual_seed(seed)
+    s0 = torch.rand((B, L, L), device="cuda", generator=gen) * 2 - 1
+    Jh = torch.randn((B, L, L), device="cuda", generator=gen)
+    Jv = torch.randn((B, L, L), device="cuda", generator=gen)
+    target = torch.sign(torch.randn((B, L, L), device="cuda", generator=gen))
+    beta = np.array([0.5 + 0.5 * b / (B - 1) for b in range(B)])
+    out = torch.empty_like(s0)
+    traj = torch.empty((2 * n_sweeps + 1, B, L, L), device="cuda")
+    go, gs, gjh, gjv = (torch.empty_like(s0) for _ in range(4))
+    stream = runner.stream
+    F32 = sp.SPIN_DTYPE_F32
+
+    def fwd(k):
+        sp.spin_dmc_forward(B, L, F32, s0.data_ptr(), Jh.data_ptr(), Jv.data_ptr(), h, beta, alpha, seed, n_sweeps,
+                            sweep_offset=k * n_sweeps, s_out_ptr=out.data_ptr(), cuda_stream=stream.cuda_stream)
+
+    def train(k):
+        sp.spin_dmc_forward(B, L, F32, s0.data_ptr(), Jh.data_ptr(), Jv.data_ptr(), h, beta, alpha, seed, n_sweeps,
+                            sweep_offset=k * n_sweeps, s_out_ptr=out.data_ptr(), traj_ptr=traj.data_ptr(),
+                            cuda_stream=stream.cuda_stream)
+        with torch.cuda.stream(stream):
+            torch.sub(out, target, out=go).mul_(2.0)                     # dLoss/ds of Eq. 8 (plumbing, not the product)
+        sp.spin_dmc_backward(B, L, F32, traj.data_ptr(), Jh.data_ptr(), Jv.data_ptr(), h, beta, alpha, seed, n_sweeps,
+                             go.data_ptr(), gs.data_ptr(), gjh.data_ptr(), gjv.data_ptr(), sweep_offset=k * n_sweeps,
+                             cuda_stream=stream.cuda_stream, want_host=False)
+
+    res = {}
+    updates = float(B) * L * L * n_sweeps
+    for key, fn, bytes_per_site_sweep, launches in (("DMC-forward", fwd, 32.0, 2 * n_sweeps),
+                                                    ("DMC-forward+backward", train, 32.0 + 128.0, 6 * n_sweeps)):
+        with torch.cuda.stream(stream):
+            for k in range(args.warmup):
+                fn(k)
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        for k in range(args.steps):
+            with torch.cuda.stream(stream):
+                runner.flush.fill_(k)
+            ev[k][0].record(stream)
+            fn(args.warmup + k)
+            ev[k][1].record(stream)
+        torch.cuda.synchronize()
+        ms = np.array([a.elapsed_time(b) for a, b in ev])
+        vals = updates / (ms * 1e6)
+        gbs = bytes_per_site_sweep * updates / (float(ms.mean()) * 1e-3) / 1e9
+        res[key] = {"workload": "DMC: Ising +-J-glass couplings (normal), fp32, %dx%d^2, %d sweeps, alpha=%g" % (B, L, n_sweeps, alpha),
+                    "value": float(updates * len(ms) / (ms.sum() * 1e6)), "unit": UNIT, "best": float(vals.max()),
+                    "median": float(np.median(vals)), "ms_per_step": float(ms.mean()),
+                    "kernel": "dmc_forward_kernel<float,4>" + ("" if key == "DMC-forward" else " + dmc_backward1/2_kernel<float,4>"),
+                    "gpu_launches_per_step": launches, "dtype": "f32",
+                    "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                                 "frac": gbs / peaks["hbm_gbs"], "bytes_per_site_per_sweep": bytes_per_site_sweep,
+                                 "peak_source": peaks["source"]}}
+    return res
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -458,6 +522,7 @@ def main():
         sim.spin_destroy()
         if world == 1 and not args.no_per_config:
             line["per_config"] = per_config_block(runner, sp, args, peaks, measured)
+            line["per_config"].update(dmc_entries(runner, sp, args, peaks))
         if not args.no_cpu_baseline and world == 1:
             v, threads, sample, _ = oracle_throughput(w, 12.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,

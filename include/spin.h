@@ -180,6 +180,41 @@ SPIN_API int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv);
 enum { SPIN_POLICY_AUTO = 0, SPIN_POLICY_STREAMING = 1, SPIN_POLICY_RESIDENT = 2 };
 SPIN_API int spin_set_policy(spin_sim* sim, int32_t policy);
 
+/* ---------------------------------------------------------------------------------------------
+ * Differentiable Monte Carlo: Algorithm 2 and Eq. 4 of the paper,
+ * forward and backward, for the 2D Ising model with a coupling per bond (Eq. 1).  Stateless calls on
+ * DEVICE arrays in the natural layout [batch][L][L], element type float (SPIN_DTYPE_F32) or double (SPIN_DTYPE_F64).
+ * Jh[b][i][j] couples (i, j)-(i, (j+1) mod L), Jv[b][i][j] couples (i, j)-((i+1) mod L, j) (as in spin_set_bonds, but
+ * real-valued); H = -sum_bonds J_ij s_i s_j - h sum_i s_i.  Per site x of the current colour (colour 0, then 1):
+ *   F = sum_n J_xn s_n + h,  dE = 2 s F,  p = exp(-beta dE),  r = (w >> 8) / 2^24 with w the Philox word the Ising sweep
+ *   uses for that (seed, replica, site, t, colour),  q = 1 / (1 + exp(-alpha (p - r))),  s <- q (-s) + (1 - q) s
+ * (Alg. 2 lines 1-9 with the minus signs of PAPER.md:154; readings D1-D8 in DESIGN.md section 12).  alpha -> infinity
+ * followed by spin_dmc_discretise reproduces spin_sweep.  beta: HOST, [batch], finite, >= 0.  alpha >= 0, h finite.
+ * Inputs must keep beta |dE| below ~80 (fp32) so that p stays finite.  All work is enqueued on cuda_stream (NULL =
+ * default stream); temporaries come from the stream-ordered allocator.  SPIN_ERR_INVALID: NULL pointers, bad shapes
+ * (batch < 1, L odd or < 2), unknown dtype, bad sweep range; nothing is written in that case.
+ * ------------------------------------------------------------------------------------------- */
+enum { SPIN_DTYPE_F32 = 0, SPIN_DTYPE_F64 = 1 };
+
+/* n_sweeps DMC sweeps t = sweep_offset .. from the lattice s0.  s_out: device, receives the final lattice (may equal s0).
+ * traj: device, NULL or [(2 n_sweeps + 1)][batch][L][L]: traj[0] = s0 and traj[2k + 1 + c] = the lattice after the
+ * colour-c half-sweep of sweep k (what spin_dmc_backward needs).  Asynchronous. */
+SPIN_API int spin_dmc_forward(int32_t batch, int32_t L, int32_t dtype, const void* s0, const void* Jh, const void* Jv,
+                              double h, const double* beta, double alpha, uint64_t seed, int64_t replica_offset,
+                              int64_t n_sweeps, int64_t sweep_offset, void* s_out, void* traj, void* cuda_stream);
+
+/* Reverse-mode derivative of a scalar loss through spin_dmc_forward (same arguments, traj as written by it).
+ * grad_out: device [batch][L][L] = dLoss / d(final lattice).  Outputs, all overwritten: grad_s0, grad_Jh, grad_Jv: device
+ * [batch][L][L] (same dtype); grad_beta, grad_h: HOST double [batch] (either may be NULL; per replica, h is one scalar so
+ * its gradient is the sum over replicas).  Synchronises the stream when a host output is requested. */
+SPIN_API int spin_dmc_backward(int32_t batch, int32_t L, int32_t dtype, const void* traj, const void* Jh, const void* Jv,
+                               double h, const double* beta, double alpha, uint64_t seed, int64_t replica_offset,
+                               int64_t n_sweeps, int64_t sweep_offset, const void* grad_out, void* grad_s0, void* grad_Jh,
+                               void* grad_Jv, double* grad_beta, double* grad_h, void* cuda_stream);
+
+/* Eq. 4 (Alg. 2 line 11): s <- -1 if s < 0 else +1 on n device elements.  Asynchronous. */
+SPIN_API int spin_dmc_discretise(int32_t dtype, void* s, int64_t n, void* cuda_stream);
+
 /* Measurement aid ("second, tighter denominator"): runs a register-only kernel on the current
  * device that does nothing but the algorithmic work of the sweep - Philox-4x32-10 calls (precomputed round keys) whose
  * four output words are each compared with a threshold - and returns the best-of-5 rate in random words per

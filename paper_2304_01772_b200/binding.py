@@ -12,12 +12,14 @@ SPIN_OK, SPIN_ERR_INVALID, SPIN_ERR_NOMEM, SPIN_ERR_CUDA, SPIN_ERR_UNSUPPORTED =
 SPIN_MODEL_ISING, SPIN_MODEL_POTTS = 0, 1
 SPIN_LAYOUT_INT8, SPIN_LAYOUT_BITPACKED = 0, 1
 SPIN_POLICY_AUTO, SPIN_POLICY_STREAMING, SPIN_POLICY_RESIDENT = 0, 1, 2
+SPIN_DTYPE_F32, SPIN_DTYPE_F64 = 0, 1
 
 __all__ = [
     "SPIN_OK", "SPIN_ERR_INVALID", "SPIN_ERR_NOMEM", "SPIN_ERR_CUDA", "SPIN_ERR_UNSUPPORTED",
     "SPIN_MODEL_ISING", "SPIN_MODEL_POTTS", "SPIN_LAYOUT_INT8", "SPIN_LAYOUT_BITPACKED",
     "SPIN_POLICY_AUTO", "SPIN_POLICY_STREAMING", "SPIN_POLICY_RESIDENT",
     "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim", "spin_measure_philox_compare_rate",
+    "SPIN_DTYPE_F32", "SPIN_DTYPE_F64", "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
     "spin_create", "spin_create_ex",
 ]
 
@@ -61,6 +63,9 @@ def load_library():
         "spin_set_policy": (c.c_int, [vp, i32]),
         "spin_set_bonds": (c.c_int, [vp, vp, vp]),
         "spin_measure_philox_compare_rate": (c.c_int, [vp]),
+        "spin_dmc_forward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp]),
+        "spin_dmc_backward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp, vp, vp, vp, vp]),
+        "spin_dmc_discretise": (c.c_int, [i32, vp, i64, vp]),
     }
     for name, (res, args) in protos.items():
         fn = getattr(lib, name)
@@ -75,6 +80,7 @@ EXPORTED_SYMBOLS = (
     "spin_create_ex", "spin_set_stream", "spin_get_spins", "spin_set_spins", "spin_sweep_measure",
     "spin_observables_dev", "spin_synchronize", "spin_threshold_table", "spin_kernel_launches",
     "spin_kernel_variant", "spin_set_policy", "spin_set_bonds", "spin_measure_philox_compare_rate",
+    "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
 )
 
 
@@ -110,6 +116,35 @@ def spin_measure_philox_compare_rate():
     v = ctypes.c_double(0.0)
     _check(load_library().spin_measure_philox_compare_rate(ctypes.byref(v)))
     return float(v.value)
+
+
+def _beta64(beta, batch):
+    return np.ascontiguousarray(np.broadcast_to(np.asarray(beta, dtype=np.float64), (batch,)))
+
+
+def spin_dmc_forward(batch, L, dtype, s0_ptr, Jh_ptr, Jv_ptr, h, beta, alpha, seed, n_sweeps, sweep_offset=0,
+                     replica_offset=0, s_out_ptr=None, traj_ptr=None, cuda_stream=None):
+    """Device pointers (ints) in, device results out; see include/spin.h."""
+    b = _beta64(beta, batch)
+    _check(load_library().spin_dmc_forward(batch, L, dtype, s0_ptr, Jh_ptr, Jv_ptr, float(h), _np_ptr(b), float(alpha),
+                                           int(seed), int(replica_offset), int(n_sweeps), int(sweep_offset), s_out_ptr,
+                                           traj_ptr, cuda_stream))
+
+
+def spin_dmc_backward(batch, L, dtype, traj_ptr, Jh_ptr, Jv_ptr, h, beta, alpha, seed, n_sweeps, grad_out_ptr, grad_s0_ptr,
+                      grad_Jh_ptr, grad_Jv_ptr, sweep_offset=0, replica_offset=0, cuda_stream=None, want_host=True):
+    """-> (grad_beta, grad_h) float64[batch] on the host (None, None if not want_host: fully asynchronous)."""
+    b = _beta64(beta, batch)
+    gb = np.zeros(batch) if want_host else None
+    gh = np.zeros(batch) if want_host else None
+    _check(load_library().spin_dmc_backward(batch, L, dtype, traj_ptr, Jh_ptr, Jv_ptr, float(h), _np_ptr(b), float(alpha),
+                                            int(seed), int(replica_offset), int(n_sweeps), int(sweep_offset), grad_out_ptr,
+                                            grad_s0_ptr, grad_Jh_ptr, grad_Jv_ptr, _np_ptr(gb), _np_ptr(gh), cuda_stream))
+    return gb, gh
+
+
+def spin_dmc_discretise(dtype, s_ptr, n, cuda_stream=None):
+    _check(load_library().spin_dmc_discretise(dtype, s_ptr, int(n), cuda_stream))
 
 
 class SpinSim:

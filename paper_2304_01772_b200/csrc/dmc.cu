@@ -1,0 +1,407 @@
+// dmc.cu — SURVEY.md section 8(f) #1: the paper's Differentiable Monte Carlo step (Algorithm 2 and Eq. 4,
+// PAPER.md:125, 140-158) for the 2D Ising model with per-bond couplings (Eq. 1), forward and
+// hand-written backward (dLoss/dJ_ij, dLoss/dbeta, dLoss/dh, dLoss/ds_0; the training use is PAPER.md:308-332).
+//
+// Per site x of the current colour (readings D1-D8):
+//   F = sum_n J_xn s_n + h,  dE = 2 s F,  p = exp(-beta dE),  r = (w >> 8) 2^-24 (w: the Ising sweep's Philox word),
+//   q = 1 / (1 + exp(-alpha (p - r))),  s <- q (-s) + (1 - q) s.
+// Float lattices in the NATURAL layout [B][L][L] (fp32, or fp64 for tight parity), couplings Jh / Jv [B][L][L] as in
+// spin_set_bonds.  The path is HBM-bound (a few dozen flops and two exponentials per 16-32 bytes), so the kernels are
+// plain streaming kernels: one thread per V consecutive sites of a row (one 16-byte vector of the lattice and of every
+// operand row), coalesced vector loads / stores, the three lattice rows and the two coupling arrays read once per
+// half-sweep, grids of whole rows.  A half-sweep is out of place (state k -> state k+1), which is what the backward
+// pass needs anyway (it re-reads the state every half-sweep started from).
+//
+// Backward of one half-sweep, with A = alpha q (1-q) p at the updated sites (0 elsewhere):
+//   pass 1 (updated sites):  G_x = g_x 4 beta A s^2  (= dLoss/dF_x),  D_x = g_x ((1-2q) + 4 beta A s F);  D_y = g_y elsewhere;
+//                            dLoss/dbeta += g_x 4 A s^2 F,  dLoss/dh += G_x          (block reduction + one atomic)
+//   pass 2 (all sites):      g_prev_x = D_x + sum_n G_n J_xn;  dJh[i][j] += G[i][j] s[i][j+1] + G[i][j+1] s[i][j],
+//                            dJv[i][j] += G[i][j] s[i+1][j] + G[i+1][j] s[i][j]      (every bond has one updated end)
+// No atomics on the lattice-sized arrays, no scattered accesses.
+#include "../../include/spin.h"
+#include "spin_internal.cuh"
+
+#include <cmath>
+#include <cstdio>
+
+namespace spin {
+namespace {
+
+template <typename T, int V>
+struct alignas(sizeof(T) * V) Vec {
+    T v[V];
+};
+
+template <typename T> __device__ __forceinline__ T exp_t(T x);
+template <> __device__ __forceinline__ float exp_t<float>(float x) { return expf(x); }
+template <> __device__ __forceinline__ double exp_t<double>(double x) { return exp(x); }
+
+struct DmcArgs {
+    int32_t batch, L;
+    uint32_t replica_offset;
+    uint32_t c2, c3;          // Philox counter words of (t, colour), domain ISING (reading D4)
+    int32_t colour;
+    double h, alpha;
+    const double* beta;       // device [B]
+    RoundKeys rk;
+};
+
+// Everything Algorithm 2 computes for the V sites a thread owns.  upd[e]: the site has the current colour.
+template <typename T, int V>
+struct Sites {
+    T s[V], F[V], p[V], q[V];
+    bool upd[V];
+};
+
+// Loads the thread's neighbourhood from the state `src` and evaluates lines 2-8 of Algorithm 2 for its updated sites.
+template <typename T, int V>
+__device__ __forceinline__ void eval_sites(const DmcArgs& a, const T* __restrict__ src, const T* __restrict__ Jh,
+                                           const T* __restrict__ Jv, int b, int i, int j0, Sites<T, V>& o) {
+    const int L = a.L;
+    const size_t base = (size_t)b * L * L;
+    const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+    const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + V == L ? 0 : j0 + V;
+    const Vec<T, V> sc = *(const Vec<T, V>*)(src + base + (size_t)i * L + j0);
+    const Vec<T, V> su = *(const Vec<T, V>*)(src + base + (size_t)iu * L + j0);
+    const Vec<T, V> sd = *(const Vec<T, V>*)(src + base + (size_t)id * L + j0);
+    const Vec<T, V> jh = *(const Vec<T, V>*)(Jh + base + (size_t)i * L + j0);
+    const Vec<T, V> jvu = *(const Vec<T, V>*)(Jv + base + (size_t)iu * L + j0);
+    const Vec<T, V> jvc = *(const Vec<T, V>*)(Jv + base + (size_t)i * L + j0);
+    const T sl = src[base + (size_t)i * L + jl], sr = src[base + (size_t)i * L + jr];
+    const T jhl = Jh[base + (size_t)i * L + jl];
+    // one Philox call covers the thread's updated sites when V == 4 (L % 4 == 0: n and n+1 share a group); with V == 2
+    // there is one updated site
+    const T beta = (T)a.beta[b];
+    uint32_t r[4];
+    uint32_t have = 0xFFFFFFFFu;
+#pragma unroll
+    for (int e = 0; e < V; ++e) {
+        const int j = j0 + e;
+        o.s[e] = sc.v[e];
+        o.upd[e] = ((i + j) & 1) == a.colour;
+        o.F[e] = o.p[e] = o.q[e] = (T)0;
+        if (!o.upd[e]) continue;
+        const uint32_t n = (uint32_t)i * (uint32_t)(L >> 1) + (uint32_t)(j >> 1);
+        if ((n >> 2) != have) {
+            have = n >> 2;
+            philox4x32_10(a.rk, have, (uint32_t)b + a.replica_offset, a.c2, a.c3, r);
+        }
+        const uint32_t w = (n & 3u) == 0u ? r[0] : (n & 3u) == 1u ? r[1] : (n & 3u) == 2u ? r[2] : r[3];
+        const T rr = (T)(w >> 8) * (T)(1.0 / 16777216.0);
+        const T left = e == 0 ? sl : sc.v[e > 0 ? e - 1 : 0];
+        const T right = e == V - 1 ? sr : sc.v[e < V - 1 ? e + 1 : V - 1];
+        const T jleft = e == 0 ? jhl : jh.v[e > 0 ? e - 1 : 0];
+        // same association order as the oracle: up, down, left, right, then h
+        const T F = jvu.v[e] * su.v[e] + jvc.v[e] * sd.v[e] + jleft * left + jh.v[e] * right + (T)a.h;
+        const T dE = (T)2 * o.s[e] * F;
+        const T p = exp_t<T>(-beta * dE);
+        o.F[e] = F;
+        o.p[e] = p;
+        o.q[e] = (T)1 / ((T)1 + exp_t<T>(-(T)a.alpha * (p - rr)));
+    }
+}
+
+template <typename T, int V>
+__global__ void __launch_bounds__(256) dmc_forward_kernel(DmcArgs a, const T* __restrict__ src, T* __restrict__ dst,
+                                                          const T* __restrict__ Jh, const T* __restrict__ Jv) {
+    const int vpr = a.L / V;                                   // vectors per row
+    const long long total = (long long)a.batch * a.L * vpr;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= total) return;
+    const int x = (int)(gid % vpr);
+    const long long bi = gid / vpr;
+    const int i = (int)(bi % a.L), b = (int)(bi / a.L);
+    Sites<T, V> st;
+    eval_sites<T, V>(a, src, Jh, Jv, b, i, x * V, st);
+    Vec<T, V> out;
+#pragma unroll
+    for (int e = 0; e < V; ++e)
+        out.v[e] = st.upd[e] ? st.q[e] * (-st.s[e]) + ((T)1 - st.q[e]) * st.s[e] : st.s[e];      // line 9
+    *(Vec<T, V>*)(dst + (size_t)b * a.L * a.L + (size_t)i * a.L + x * V) = out;
+}
+
+// Backward pass 1: blocks never straddle replicas (grid = blocks per replica x batch), so the beta / h sums reduce per block.
+template <typename T, int V>
+__global__ void __launch_bounds__(256) dmc_backward1_kernel(DmcArgs a, const T* __restrict__ src, const T* __restrict__ Jh,
+                                                            const T* __restrict__ Jv, const T* __restrict__ gnew,
+                                                            T* __restrict__ D, T* __restrict__ G, double* gbeta, double* gh,
+                                                            int bpr) {
+    __shared__ double red[2][8];
+    const int vpr = a.L / V;
+    const int per = a.L * vpr;
+    const int b = blockIdx.x / bpr, blk = blockIdx.x - b * bpr;
+    const int u = blk * blockDim.x + threadIdx.x;
+    double sb = 0.0, sh = 0.0;
+    if (u < per) {
+        const int i = u / vpr, x = u - i * vpr;
+        Sites<T, V> st;
+        eval_sites<T, V>(a, src, Jh, Jv, b, i, x * V, st);
+        const size_t off = (size_t)b * a.L * a.L + (size_t)i * a.L + x * V;
+        const Vec<T, V> g = *(const Vec<T, V>*)(gnew + off);
+        const T beta = (T)a.beta[b];
+        Vec<T, V> d, gg;
+#pragma unroll
+        for (int e = 0; e < V; ++e) {
+            if (!st.upd[e]) { d.v[e] = g.v[e]; gg.v[e] = (T)0; continue; }
+            const T A = (T)a.alpha * st.q[e] * ((T)1 - st.q[e]) * st.p[e];
+            const T s = st.s[e];
+            d.v[e] = g.v[e] * (((T)1 - (T)2 * st.q[e]) + (T)4 * beta * A * s * st.F[e]);
+            gg.v[e] = g.v[e] * ((T)4 * beta * A * s * s);
+            sb += (double)(g.v[e] * ((T)4 * A * s * s * st.F[e]));
+            sh += (double)gg.v[e];
+        }
+        *(Vec<T, V>*)(D + off) = d;
+        *(Vec<T, V>*)(G + off) = gg;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sb += __shfl_xor_sync(0xFFFFFFFFu, sb, o);
+        sh += __shfl_xor_sync(0xFFFFFFFFu, sh, o);
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) { red[0][w] = sb; red[1][w] = sh; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tb = 0.0, th = 0.0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) { tb += red[0][k]; th += red[1][k]; }
+        atomicAdd(gbeta + b, tb);
+        atomicAdd(gh + b, th);
+    }
+}
+
+// Backward pass 2, all sites: g_prev = D + sum_n G_n J_xn (in place in D), and the coupling gradients.
+template <typename T, int V>
+__global__ void __launch_bounds__(256) dmc_backward2_kernel(int batch, int L, const T* __restrict__ src,
+                                                            const T* __restrict__ Jh, const T* __restrict__ Jv,
+                                                            const T* __restrict__ G, T* __restrict__ D, T* __restrict__ gJh,
+                                                            T* __restrict__ gJv) {
+    const int vpr = L / V;
+    const long long total = (long long)batch * L * vpr;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= total) return;
+    const int x = (int)(gid % vpr);
+    const long long bi = gid / vpr;
+    const int i = (int)(bi % L), b = (int)(bi / L);
+    const int j0 = x * V;
+    const size_t base = (size_t)b * L * L;
+    const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+    const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + V == L ? 0 : j0 + V;
+    const size_t off = base + (size_t)i * L + j0, offu = base + (size_t)iu * L + j0, offd = base + (size_t)id * L + j0;
+    const Vec<T, V> gc = *(const Vec<T, V>*)(G + off), gu = *(const Vec<T, V>*)(G + offu), gd = *(const Vec<T, V>*)(G + offd);
+    const Vec<T, V> sc = *(const Vec<T, V>*)(src + off), sd = *(const Vec<T, V>*)(src + offd);
+    const Vec<T, V> jh = *(const Vec<T, V>*)(Jh + off), jvu = *(const Vec<T, V>*)(Jv + offu), jvc = *(const Vec<T, V>*)(Jv + off);
+    const T gl = G[base + (size_t)i * L + jl], gr = G[base + (size_t)i * L + jr];
+    const T jhl = Jh[base + (size_t)i * L + jl], sr = src[base + (size_t)i * L + jr];
+    Vec<T, V> d = *(const Vec<T, V>*)(D + off);
+    Vec<T, V> ah = *(const Vec<T, V>*)(gJh + off), av = *(const Vec<T, V>*)(gJv + off);
+#pragma unroll
+    for (int e = 0; e < V; ++e) {
+        const T gleft = e == 0 ? gl : gc.v[e > 0 ? e - 1 : 0];
+        const T gright = e == V - 1 ? gr : gc.v[e < V - 1 ? e + 1 : V - 1];
+        const T jleft = e == 0 ? jhl : jh.v[e > 0 ? e - 1 : 0];
+        const T sright = e == V - 1 ? sr : sc.v[e < V - 1 ? e + 1 : V - 1];
+        d.v[e] += gu.v[e] * jvu.v[e] + gd.v[e] * jvc.v[e] + gleft * jleft + gright * jh.v[e];
+        ah.v[e] += gc.v[e] * sright + gright * sc.v[e];
+        av.v[e] += gc.v[e] * sd.v[e] + gd.v[e] * sc.v[e];
+    }
+    *(Vec<T, V>*)(D + off) = d;
+    *(Vec<T, V>*)(gJh + off) = ah;
+    *(Vec<T, V>*)(gJv + off) = av;
+}
+
+template <typename T>
+__global__ void dmc_discretise_kernel(T* s, long long n) {
+    const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k < n) s[k] = s[k] < (T)0 ? (T)-1 : (T)1;             // Eq. 4
+}
+
+}  // namespace
+}  // namespace spin
+
+// ---- host side ---------------------------------------------------------------------------------------------------
+namespace {
+
+using namespace spin;
+
+int dmc_fail(int code, const char* msg) { return spin::set_error(code, msg); }   // thread-local spin_last_error (spin_api.cu)
+
+struct DmcShape {
+    int32_t batch, L, dtype;
+    size_t elems() const { return (size_t)batch * L * L; }
+    size_t bytes() const { return elems() * (dtype == SPIN_DTYPE_F64 ? 8 : 4); }
+};
+
+int check_common(int32_t batch, int32_t L, int32_t dtype, const double* beta, double h, double alpha, int64_t replica_offset,
+                 int64_t n_sweeps, int64_t sweep_offset) {
+    if (batch < 1 || L < 2 || (L & 1) || L > 65536) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc: batch >= 1 and even L in 2..65536 required");
+    if (dtype != SPIN_DTYPE_F32 && dtype != SPIN_DTYPE_F64) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc: dtype must be SPIN_DTYPE_F32 or SPIN_DTYPE_F64");
+    if (!beta) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc: beta is NULL");
+    for (int b = 0; b < batch; ++b)
+        if (!std::isfinite(beta[b]) || beta[b] < 0.0) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc: beta must be finite and >= 0");
+    if (!std::isfinite(h) || !std::isfinite(alpha) || alpha < 0.0) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc: h finite and alpha finite, >= 0 required");
+    if (replica_offset < 0 || replica_offset + (int64_t)batch > (1ll << 32)) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc: replica_offset + batch must stay within [0, 2^32]");
+    if (n_sweeps < 0 || sweep_offset < 0 || sweep_offset > (1ll << 56) || n_sweeps > (1ll << 56) || sweep_offset + n_sweeps > (1ll << 56))
+        return dmc_fail(SPIN_ERR_INVALID, "spin_dmc: sweep range must lie in [0, 2^56]");
+    return SPIN_OK;
+}
+
+// The temporaries come from the device's default stream-ordered pool; keep freed blocks cached in the pool (the default
+// release threshold of 0 returns them to the driver at every synchronisation, which costs milliseconds per call).
+void keep_pool_memory() {
+    int dev = 0;
+    cudaMemPool_t pool;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetDefaultMemPool(&pool, dev) != cudaSuccess) { cudaGetLastError(); return; }
+    unsigned long long keep = ~0ull;
+    cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    cudaGetLastError();
+}
+
+DmcArgs make_args(int32_t batch, int32_t L, double h, double alpha, const double* d_beta, uint64_t seed,
+                  int64_t replica_offset, int64_t t, int colour) {
+    DmcArgs a;
+    a.batch = batch; a.L = L; a.replica_offset = (uint32_t)replica_offset;
+    a.c2 = (uint32_t)((uint64_t)t & 0xFFFFFFFFull);
+    a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)colour << 24) | ((uint32_t)kDomainIsing << 28);
+    a.colour = colour; a.h = h; a.alpha = alpha; a.beta = d_beta;
+    uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) { a.rk.k0[r] = k0; a.rk.k1[r] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+    return a;
+}
+
+template <typename T, int V>
+void launch_forward(const DmcArgs& a, const void* src, void* dst, const void* Jh, const void* Jv, cudaStream_t s) {
+    const long long total = (long long)a.batch * a.L * (a.L / V);
+    dmc_forward_kernel<T, V><<<(unsigned)((total + 255) / 256), 256, 0, s>>>(a, (const T*)src, (T*)dst, (const T*)Jh, (const T*)Jv);
+}
+
+void forward_half(int dtype, const DmcArgs& a, const void* src, void* dst, const void* Jh, const void* Jv, cudaStream_t s) {
+    if (dtype == SPIN_DTYPE_F64) launch_forward<double, 2>(a, src, dst, Jh, Jv, s);
+    else if (a.L % 4 == 0) launch_forward<float, 4>(a, src, dst, Jh, Jv, s);
+    else launch_forward<float, 2>(a, src, dst, Jh, Jv, s);
+}
+
+template <typename T, int V>
+void launch_backward(const DmcArgs& a, const void* src, const void* Jh, const void* Jv, const void* gnew, void* D, void* G,
+                     double* gbeta, double* gh, void* gJh, void* gJv, cudaStream_t s) {
+    const int per = a.L * (a.L / V);
+    const int bpr = (per + 255) / 256;
+    dmc_backward1_kernel<T, V><<<(unsigned)((long long)bpr * a.batch), 256, 0, s>>>(a, (const T*)src, (const T*)Jh, (const T*)Jv,
+                                                                                  (const T*)gnew, (T*)D, (T*)G, gbeta, gh, bpr);
+    const long long total = (long long)a.batch * per;
+    dmc_backward2_kernel<T, V><<<(unsigned)((total + 255) / 256), 256, 0, s>>>(a.batch, a.L, (const T*)src, (const T*)Jh,
+                                                                              (const T*)Jv, (const T*)G, (T*)D, (T*)gJh, (T*)gJv);
+}
+
+void backward_half(int dtype, const DmcArgs& a, const void* src, const void* Jh, const void* Jv, const void* gnew, void* D,
+                   void* G, double* gbeta, double* gh, void* gJh, void* gJv, cudaStream_t s) {
+    if (dtype == SPIN_DTYPE_F64) launch_backward<double, 2>(a, src, Jh, Jv, gnew, D, G, gbeta, gh, gJh, gJv, s);
+    else if (a.L % 4 == 0) launch_backward<float, 4>(a, src, Jh, Jv, gnew, D, G, gbeta, gh, gJh, gJv, s);
+    else launch_backward<float, 2>(a, src, Jh, Jv, gnew, D, G, gbeta, gh, gJh, gJv, s);
+}
+
+#define DMC_TRY(expr)                                                                             \
+    do {                                                                                          \
+        cudaError_t e_ = (expr);                                                                  \
+        if (e_ != cudaSuccess) { rc = dmc_fail(SPIN_ERR_CUDA, cudaGetErrorString(e_)); goto done; } \
+    } while (0)
+
+}  // namespace
+
+extern "C" {
+
+int spin_dmc_forward(int32_t batch, int32_t L, int32_t dtype, const void* s0, const void* Jh, const void* Jv, double h,
+                     const double* beta, double alpha, uint64_t seed, int64_t replica_offset, int64_t n_sweeps,
+                     int64_t sweep_offset, void* s_out, void* traj, void* cuda_stream) {
+    int rc = check_common(batch, L, dtype, beta, h, alpha, replica_offset, n_sweeps, sweep_offset);
+    if (rc != SPIN_OK) return rc;
+    if (!s0 || !Jh || !Jv || !s_out) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc_forward: NULL device pointer");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const DmcShape sh{batch, L, dtype};
+    const size_t bytes = sh.bytes();
+    double* d_beta = nullptr;
+    void* tmp = nullptr;
+    keep_pool_memory();
+    DMC_TRY(cudaMallocAsync(&d_beta, sizeof(double) * batch, s));
+    DMC_TRY(cudaMemcpyAsync(d_beta, beta, sizeof(double) * batch, cudaMemcpyHostToDevice, s));
+    if (traj) DMC_TRY(cudaMemcpyAsync(traj, s0, bytes, cudaMemcpyDeviceToDevice, s));
+    else if (n_sweeps > 0) DMC_TRY(cudaMallocAsync(&tmp, bytes, s));
+    {
+        const void* cur = s0;
+        for (int64_t k = 0; k < n_sweeps; ++k)
+            for (int c = 0; c < 2; ++c) {
+                // with a trajectory: state 2k+c -> state 2k+c+1; without: ping-pong so that the last state lands in s_out
+                void* dst = traj ? (void*)((char*)traj + (size_t)(2 * k + c + 1) * bytes) : (c == 0 ? tmp : s_out);
+                const DmcArgs a = make_args(batch, L, h, alpha, d_beta, seed, replica_offset, sweep_offset + k, c);
+                forward_half(dtype, a, cur, dst, Jh, Jv, s);
+                cur = dst;
+            }
+        if (cur != s_out) DMC_TRY(cudaMemcpyAsync(s_out, cur, bytes, cudaMemcpyDeviceToDevice, s));
+    }
+    DMC_TRY(cudaGetLastError());
+done:
+    if (tmp) cudaFreeAsync(tmp, s);
+    if (d_beta) cudaFreeAsync(d_beta, s);
+    return rc;
+}
+
+int spin_dmc_backward(int32_t batch, int32_t L, int32_t dtype, const void* traj, const void* Jh, const void* Jv, double h,
+                      const double* beta, double alpha, uint64_t seed, int64_t replica_offset, int64_t n_sweeps,
+                      int64_t sweep_offset, const void* grad_out, void* grad_s0, void* grad_Jh, void* grad_Jv,
+                      double* grad_beta, double* grad_h, void* cuda_stream) {
+    int rc = check_common(batch, L, dtype, beta, h, alpha, replica_offset, n_sweeps, sweep_offset);
+    if (rc != SPIN_OK) return rc;
+    if (!traj || !Jh || !Jv || !grad_out || !grad_s0 || !grad_Jh || !grad_Jv)
+        return dmc_fail(SPIN_ERR_INVALID, "spin_dmc_backward: NULL device pointer");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    const DmcShape sh{batch, L, dtype};
+    const size_t bytes = sh.bytes();
+    double* d_small = nullptr;     // [beta | grad_beta | grad_h]
+    void* ws = nullptr;            // [g ping | g pong | G]
+    keep_pool_memory();
+    DMC_TRY(cudaMallocAsync(&d_small, sizeof(double) * 3 * batch, s));
+    DMC_TRY(cudaMemcpyAsync(d_small, beta, sizeof(double) * batch, cudaMemcpyHostToDevice, s));
+    DMC_TRY(cudaMemsetAsync(d_small + batch, 0, sizeof(double) * 2 * batch, s));
+    DMC_TRY(cudaMallocAsync(&ws, 3 * bytes, s));
+    DMC_TRY(cudaMemsetAsync(grad_Jh, 0, bytes, s));
+    DMC_TRY(cudaMemsetAsync(grad_Jv, 0, bytes, s));
+    {
+        char* g0 = (char*)ws;
+        char* g1 = g0 + bytes;
+        void* G = g1 + bytes;
+        const void* gnew = grad_out;
+        int flip = 0;
+        for (int64_t k = n_sweeps - 1; k >= 0; --k)
+            for (int c = 1; c >= 0; --c) {
+                const void* before = (const char*)traj + (size_t)(2 * k + c) * bytes;
+                void* D = flip ? g1 : g0;
+                const DmcArgs a = make_args(batch, L, h, alpha, d_small, seed, replica_offset, sweep_offset + k, c);
+                backward_half(dtype, a, before, Jh, Jv, gnew, D, G, d_small + batch, d_small + 2 * batch, grad_Jh, grad_Jv, s);
+                gnew = D;
+                flip ^= 1;
+            }
+        DMC_TRY(cudaMemcpyAsync(grad_s0, gnew, bytes, cudaMemcpyDeviceToDevice, s));
+    }
+    DMC_TRY(cudaGetLastError());
+    if (grad_beta) DMC_TRY(cudaMemcpyAsync(grad_beta, d_small + batch, sizeof(double) * batch, cudaMemcpyDeviceToHost, s));
+    if (grad_h) DMC_TRY(cudaMemcpyAsync(grad_h, d_small + 2 * batch, sizeof(double) * batch, cudaMemcpyDeviceToHost, s));
+    if (grad_beta || grad_h) DMC_TRY(cudaStreamSynchronize(s));
+done:
+    if (ws) cudaFreeAsync(ws, s);
+    if (d_small) cudaFreeAsync(d_small, s);
+    return rc;
+}
+
+int spin_dmc_discretise(int32_t dtype, void* s, int64_t n, void* cuda_stream) {
+    if (!s || n < 0) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc_discretise: NULL pointer or negative count");
+    if (dtype != SPIN_DTYPE_F32 && dtype != SPIN_DTYPE_F64) return dmc_fail(SPIN_ERR_INVALID, "spin_dmc_discretise: unknown dtype");
+    if (n == 0) return SPIN_OK;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    if (dtype == SPIN_DTYPE_F64) spin::dmc_discretise_kernel<double><<<grid, 256, 0, st>>>((double*)s, n);
+    else spin::dmc_discretise_kernel<float><<<grid, 256, 0, st>>>((float*)s, n);
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return dmc_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+    return SPIN_OK;
+}
+
+}  // extern "C"

@@ -81,6 +81,10 @@ void encode(const ClassAccept& c, int idx, uint32_t* rec) {
 
 }  // namespace
 
+namespace spin {
+int set_error(int code, const char* msg) { return fail(code, "%s", msg); }
+}  // namespace spin
+
 struct spin_sim {
     int32_t batch = 0, L = 0, model = 0, layout = 0;
     uint64_t seed = 0;

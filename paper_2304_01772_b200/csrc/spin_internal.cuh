@@ -126,6 +126,9 @@ inline int pick_block(int units) {
     return best;
 }
 
+// Records the thread-local spin_last_error() text and returns `code` (spin_api.cu).
+int set_error(int code, const char* msg);
+
 // ---- launchers (each returns the number of kernels it launched; errors via cudaGetLastError) --------
 int launch_init(const InitArgs& a, int model, int layout, cudaStream_t s);
 
