@@ -11,7 +11,7 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "spin_oracle.cpp")
-_SRCS = [_SRC, os.path.join(_HERE, "dmc_oracle.cpp")]
+_SRCS = [_SRC, os.path.join(_HERE, "dmc_oracle.cpp"), os.path.join(_HERE, "general_oracle.cpp")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 __all__ = [
@@ -19,6 +19,8 @@ __all__ = [
     "potts_half_sweep", "ising_observables", "potts_observables", "accumulate_moments", "sweep",
     "sweep_bonds", "ising_bonds_observables", "ising_bonds_half_sweep",
     "dmc_half_sweep", "dmc_forward", "dmc_discretise", "dmc_backward",
+    "ising_general_half_sweep", "sweep_general", "ising_general_observables", "potts_general_half_sweep",
+    "sweep_potts_general", "potts_general_observables", "sweep_schedule",
 ]
 
 
@@ -59,6 +61,12 @@ def _l():
         lib.oracle_sweep_bonds.argtypes = [p, p, p, c.c_int32, c.c_int32, p, c.c_double, c.c_double, c.c_uint64,
                                            c.c_int64, c.c_int64, c.c_int64, p, p]
         d = c.c_double
+        lib.oracle_ising_general_half_sweep.argtypes = [p, p, p, p, c.c_int32, c.c_int32, p, c.c_uint64, c.c_int64,
+                                                        c.c_int64, c.c_int32]
+        lib.oracle_ising_general_observables.argtypes = [p, p, p, p, c.c_int32, c.c_int32, p, p]
+        lib.oracle_potts_general_half_sweep.argtypes = [p, p, p, c.c_int32, c.c_int32, p, p, d, d, c.c_uint64, c.c_int64,
+                                                        c.c_int64, c.c_int32]
+        lib.oracle_potts_general_observables.argtypes = [p, p, p, c.c_int32, c.c_int32, p, p, p, p]
         lib.oracle_dmc_half_sweep.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
                                               c.c_int32, p]
         lib.oracle_dmc_forward.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
@@ -269,3 +277,70 @@ def dmc_backward(traj, Jh, Jv, h, beta, alpha, seed, grad_out, sweep_offset=0, r
                              int(replica_offset), int(n_sweeps), int(sweep_offset), _ptr(go), _ptr(gs), _ptr(gjh),
                              _ptr(gjv), _ptr(gb), _ptr(gh))
     return gs, gjh, gjv, gb, gh
+
+
+# ---- general couplings and fields (general_oracle.cpp; Eq. 1 and Eq. 5 as the paper writes them) ---------------------
+def ising_general_half_sweep(spins, Jh, Jv, B, beta, seed, t, colour, replica_offset=0):
+    Bn, L = _lattice(spins)
+    jh, jv, fb, ba = _f64(Jh, (Bn, L, L)), _f64(Jv, (Bn, L, L)), _f64(B, (Bn, L, L)), _beta_array(beta, Bn)
+    _l().oracle_ising_general_half_sweep(_ptr(spins), _ptr(jh), _ptr(jv), _ptr(fb), Bn, L, _ptr(ba), int(seed),
+                                         int(replica_offset), int(t), int(colour))
+
+
+def sweep_general(spins, Jh, Jv, B, beta, seed, n_sweeps, sweep_offset=0, replica_offset=0):
+    """Ising sweeps with real couplings Jh, Jv and per-site fields B (natural [batch][L][L], broadcastable), in place."""
+    for t in range(sweep_offset, sweep_offset + n_sweeps):
+        for colour in (0, 1):
+            ising_general_half_sweep(spins, Jh, Jv, B, beta, seed, t, colour, replica_offset)
+
+
+def ising_general_observables(spins, Jh, Jv, B):
+    """-> (E float64[batch] = -sum J s s - sum B s, M int64[batch])."""
+    Bn, L = _lattice(spins)
+    jh, jv, fb = _f64(Jh, (Bn, L, L)), _f64(Jv, (Bn, L, L)), _f64(B, (Bn, L, L))
+    E = np.zeros(Bn)
+    M = np.zeros(Bn, dtype=np.int64)
+    _l().oracle_ising_general_observables(_ptr(spins), _ptr(jh), _ptr(jv), _ptr(fb), Bn, L, _ptr(E), _ptr(M))
+    return E, M
+
+
+def _opt_bonds(J, Bn, L):
+    return None if J is None else _bonds(J, Bn, L)
+
+
+def potts_general_half_sweep(spins, q, beta, J, h, seed, t, colour, Jh=None, Jv=None, replica_offset=0):
+    Bn, L = _lattice(spins)
+    assert (Jh is None) == (Jv is None)
+    jh, jv, ba, qa = _opt_bonds(Jh, Bn, L), _opt_bonds(Jv, Bn, L), _beta_array(beta, Bn), _q_array(q, Bn)
+    _l().oracle_potts_general_half_sweep(_ptr(spins), _ptr(jh), _ptr(jv), Bn, L, _ptr(qa), _ptr(ba), float(J), float(h),
+                                         int(seed), int(replica_offset), int(t), int(colour))
+
+
+def sweep_potts_general(spins, q, beta, J, h, seed, n_sweeps, Jh=None, Jv=None, sweep_offset=0, replica_offset=0):
+    """Potts sweeps with a field h on the state label and optional +-1 bond signs, in place."""
+    for t in range(sweep_offset, sweep_offset + n_sweeps):
+        for colour in (0, 1):
+            potts_general_half_sweep(spins, q, beta, J, h, seed, t, colour, Jh, Jv, replica_offset)
+
+
+def potts_general_observables(spins, q, Jh=None, Jv=None):
+    """-> (E_int = -sum_bonds J_ij delta, S = sum of state labels, M = max_k N_k), int64[batch] each."""
+    Bn, L = _lattice(spins)
+    jh, jv, qa = _opt_bonds(Jh, Bn, L), _opt_bonds(Jv, Bn, L), _q_array(q, Bn)
+    E, S, M = (np.zeros(Bn, dtype=np.int64) for _ in range(3))
+    _l().oracle_potts_general_observables(_ptr(spins), _ptr(jh), _ptr(jv), Bn, L, _ptr(qa), _ptr(E), _ptr(S), _ptr(M))
+    return E, S, M
+
+
+def sweep_schedule(spins, beta_steps, J, h, seed, sweeps_per_step, sweep_offset=0, q=None, replica_offset=0, Jh=None,
+                   Jv=None):
+    """Annealing schedule (Fig. 9's Monte Carlo arm): step k runs sweeps_per_step sweeps at beta_steps[k]
+    ([n_steps][batch]); the sweep index keeps counting across steps."""
+    beta_steps = np.asarray(beta_steps, dtype=np.float64)
+    t = sweep_offset
+    for k in range(beta_steps.shape[0]):
+        if Jh is not None and q is None:
+            sweep_bonds(spins, Jh, Jv, beta_steps[k], J, h, seed, sweeps_per_step, sweep_offset=t, replica_offset=replica_offset)
+        else:
+            sweep(spins, beta_steps[k], J, h, seed, sweeps_per_step, sweep_offset=t, q=q, replica_offset=replica_offset)
+        t += sweeps_per_step

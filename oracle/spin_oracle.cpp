@@ -111,6 +111,13 @@ void oracle_philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t
     philox4x32_10(ctr, key, out);
 }
 
+// O2 counter assembly and O4 acceptance of one class, exported unchanged for the other oracle files (general_oracle.cpp).
+void oracle_draw(uint64_t seed, uint32_t group, uint32_t replica, uint64_t t, uint32_t colour, uint32_t domain,
+                 uint32_t out[4]) {
+    draw(seed, group, replica, t, colour, domain, out);
+}
+void oracle_threshold(double beta, double dE, uint32_t* T, uint8_t* always) { threshold(beta, dE, T, always); }
+
 // O4, Ising.  Class index = 5*(s+1)/2 + (nn+4)/2; dE of flipping s with neighbour sum nn is
 // H(-s) - H(s) = 2 s (J nn + h) (Eq. 1 with reading P1; local energy = spin x neighbour sum,
 // PAPER.md:123).
