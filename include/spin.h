@@ -73,7 +73,8 @@ SPIN_API spin_sim* spin_create(int32_t batch, int32_t L, int32_t q, uint64_t see
 /* Run Metropolis sweeps t = sweep_offset .. sweep_offset + n_sweeps - 1; each sweep updates colour 0
  * ((i+j) even) and then colour 1 (Alg. 1 + checkerboard).
  * beta: host, [batch], inverse temperature of each replica (finite, >= 0); copied before return.
- * J, h: coupling and field (finite).  h must be 0 for Potts (SPIN_ERR_UNSUPPORTED otherwise).
+ * J, h: coupling and field (finite).  Potts: the field acts on the state label, H = -J sum delta - h sum_i s_i (Eq. 5,
+ * PAPER.md:166; reading P7); h != 0 (or bond signs) selects the general Potts kernel.
  * n_sweeps >= 0, sweep_offset >= 0, sweep_offset + n_sweeps <= 2^56.
  * Asynchronous on the handle's stream: the call builds the acceptance tables (O(batch) host work), enqueues their
  * upload and the sweep kernels, and returns without waiting for earlier work of the stream (the two pinned table
@@ -167,9 +168,41 @@ SPIN_API const char* spin_kernel_variant(const spin_sim* sim);
  * ((i+1) mod L, j).  From then on spin_sweep* use H = -J sum_bonds J_ij s_i s_j - h sum_i s_i (the local field is the
  * bond-weighted neighbour sum; thresholds, random words and acceptance are unchanged) and spin_observables* return
  * E_int = -sum_bonds J_ij s_i s_j.  Both NULL: back to uniform couplings.  The arrays are copied before return.
- * Implemented for the Ising model in the bit-packed layout (SPIN_ERR_UNSUPPORTED otherwise); SPIN_ERR_INVALID for a
- * NULL handle, exactly one NULL array, or a value that is not +-1 (the handle is left unchanged). */
+ * Bit-packed Ising layout: sign planes XORed into the multi-spin kernel (the fast path).  int8 layout, Ising and Potts
+ * (Potts: H = -J sum_bonds J_ij delta(s_i, s_j) - h sum s_i, E_int = -sum_bonds J_ij delta): general one-thread-per-
+ * group kernels.  SPIN_ERR_INVALID for a NULL handle, exactly one NULL array, a value that is not +-1, or a handle
+ * with real couplings (the handle is left unchanged). */
 SPIN_API int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv);
+
+/* Real-valued couplings and per-site fields (Eq. 1 as the paper writes it):
+ * H = -sum_bonds J_ij s_i s_j - sum_i B_i s_i.  Jh, Jv, B: HOST double arrays, natural layout [batch][L][L] (bond
+ * orientation as in spin_set_bonds), finite; copied before return.  From then on spin_sweep* ignore their J and h
+ * arguments: the acceptance of each of the 32 (own spin, neighbour configuration) classes of every site is evaluated
+ * on the host in IEEE double with the arithmetic of spin_threshold_table (dE = 2 s F, F = Jv[i-1][j] s_up + Jv[i][j]
+ * s_down + Jh[i][j-1] s_left + Jh[i][j] s_right + B[i][j], summed in this order) whenever beta changes, uploaded
+ * (132 bytes per site and replica) and looked up by the sweep kernel: bit-exact against the oracle by construction.
+ * spin_observables keeps returning the uniform-model integers (E_int = -sum_bonds s_i s_j, M); the energy of the
+ * general model comes from spin_energy_general.  All three NULL: back to uniform couplings.
+ * Ising, int8 layout only (SPIN_ERR_UNSUPPORTED otherwise); SPIN_ERR_INVALID for a NULL handle, a partial set of
+ * arrays, non-finite values, or a handle that has +-J bond signs; SPIN_ERR_NOMEM when the tables do not fit. */
+SPIN_API int spin_set_couplings(spin_sim* sim, const double* Jh, const double* Jv, const double* B);
+
+/* E[b] = -sum_bonds J_ij s_i s_j - sum_i B_i s_i of the current lattices for the couplings of spin_set_couplings, summed
+ * in double on the device (agrees with a sequential double sum to ~1e-13 relative).  E: host [batch].  Synchronises. */
+SPIN_API int spin_energy_general(spin_sim* sim, double* E);
+
+/* Potts: S[b] = sum_i s_i, the sum of the state labels the field term of Eq. 5 couples to (reading P7).
+ * With a field, spin_sweep samples H = J E_int - h S.  S: host [batch].  Synchronises. */
+SPIN_API int spin_potts_label_sum(spin_sim* sim, int64_t* S);
+
+/* Annealing schedule in one call (the Monte Carlo arm of the paper's Fig. 9): step k = 0 .. n_steps-1
+ * runs sweeps_per_step sweeps at beta_steps[k][0..batch-1] (HOST, [n_steps][batch]), sweep indices
+ * sweep_offset + k sweeps_per_step + 0 .. sweeps_per_step-1, exactly as n_steps consecutive spin_sweep calls would.
+ * The tables of ALL steps are built first and uploaded in one copy; no host synchronisation between steps.
+ * Asynchronous.  Class-table models only (uniform or +-J couplings; Potts without field): SPIN_ERR_UNSUPPORTED for
+ * handles with real couplings or for Potts with h != 0 / bond signs.  Argument rules as for spin_sweep. */
+SPIN_API int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps, double J, double h,
+                                 int64_t sweeps_per_step, int64_t sweep_offset);
 
 /* Kernel selection policy (diagnostics / tests; the results never depend on it: every path computes the same
  * lattice).  SPIN_POLICY_AUTO picks per shape; SPIN_POLICY_STREAMING forces the two-launches-

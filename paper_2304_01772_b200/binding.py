@@ -63,6 +63,10 @@ def load_library():
         "spin_set_policy": (c.c_int, [vp, i32]),
         "spin_set_bonds": (c.c_int, [vp, vp, vp]),
         "spin_measure_philox_compare_rate": (c.c_int, [vp]),
+        "spin_set_couplings": (c.c_int, [vp, vp, vp, vp]),
+        "spin_energy_general": (c.c_int, [vp, vp]),
+        "spin_potts_label_sum": (c.c_int, [vp, vp]),
+        "spin_sweep_schedule": (c.c_int, [vp, vp, i64, dbl, dbl, i64, i64]),
         "spin_dmc_forward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp]),
         "spin_dmc_backward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp, vp, vp, vp, vp]),
         "spin_dmc_discretise": (c.c_int, [i32, vp, i64, vp]),
@@ -81,6 +85,7 @@ EXPORTED_SYMBOLS = (
     "spin_observables_dev", "spin_synchronize", "spin_threshold_table", "spin_kernel_launches",
     "spin_kernel_variant", "spin_set_policy", "spin_set_bonds", "spin_measure_philox_compare_rate",
     "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
+    "spin_set_couplings", "spin_energy_general", "spin_potts_label_sum", "spin_sweep_schedule",
 )
 
 
@@ -218,6 +223,31 @@ class SpinSim:
         jh = np.ascontiguousarray(np.broadcast_to(np.asarray(Jh, dtype=np.int8), shape))
         jv = np.ascontiguousarray(np.broadcast_to(np.asarray(Jv, dtype=np.int8), shape))
         _check(load_library().spin_set_bonds(self._h, _np_ptr(jh), _np_ptr(jv)))
+
+    def spin_set_couplings(self, Jh, Jv, B):
+        """Real couplings / per-site fields, natural [batch][L][L] (broadcastable); (None, None, None) removes them."""
+        if Jh is None and Jv is None and B is None:
+            _check(load_library().spin_set_couplings(self._h, None, None, None))
+            return
+        shape = (self.batch, self.L, self.L)
+        a = [np.ascontiguousarray(np.broadcast_to(np.asarray(x, dtype=np.float64), shape)) for x in (Jh, Jv, B)]
+        _check(load_library().spin_set_couplings(self._h, _np_ptr(a[0]), _np_ptr(a[1]), _np_ptr(a[2])))
+
+    def spin_energy_general(self):
+        E = np.zeros(self.batch, dtype=np.float64)
+        _check(load_library().spin_energy_general(self._h, _np_ptr(E)))
+        return E
+
+    def spin_potts_label_sum(self):
+        S = np.zeros(self.batch, dtype=np.int64)
+        _check(load_library().spin_potts_label_sum(self._h, _np_ptr(S)))
+        return S
+
+    def spin_sweep_schedule(self, beta_steps, J, h, sweeps_per_step, sweep_offset=0):
+        bs = np.ascontiguousarray(np.asarray(beta_steps, dtype=np.float64))
+        assert bs.ndim == 2 and bs.shape[1] == self.batch
+        _check(load_library().spin_sweep_schedule(self._h, _np_ptr(bs), bs.shape[0], float(J), float(h), int(sweeps_per_step),
+                                                  int(sweep_offset)))
 
     def spin_set_policy(self, policy):
         _check(load_library().spin_set_policy(self._h, int(policy)))

@@ -102,6 +102,20 @@ struct spin_sim {
     unsigned int* d_hist = nullptr;  // [B][128] (Potts)
     unsigned int* d_bad = nullptr;   // validation counter
     uint32_t* d_bonds = nullptr;     // +-J sign planes [B][2][4][L][L/64] (bit-packed layout) or nullptr
+    int8_t* d_bond_nat = nullptr;    // +-J signs in the natural layout [2][B][L][L] (Jh then Jv): int8 Ising and Potts
+    // real couplings and per-site fields (Ising, int8 layout): host copies for the threshold build, device copies for
+    // the energy, the per-site thresholds [B][N][32] + always masks [B][N], and the beta they were built for
+    std::vector<double> g_Jh, g_Jv, g_B, g_beta;
+    double* d_gen = nullptr;         // [3][B][N] doubles: Jh, Jv, B
+    uint32_t* d_thr = nullptr;
+    uint32_t* d_alw = nullptr;
+    bool general = false;
+    unsigned long long* d_tab2 = nullptr;   // Potts with a field / bond signs: [B][9][255] (always << 32) | T
+    bool potts_general = false;             // the current tables were built for the general Potts kernel
+    uint32_t* d_sched = nullptr;            // tables of spin_sweep_schedule [n_steps][B][kTableStride] (grow-only)
+    size_t sched_bytes = 0;
+    uint32_t* h_sched = nullptr;            // pinned staging of the same size, guarded by sched_ev (recorded after its upload)
+    cudaEvent_t sched_ev = nullptr;
     uint8_t* d_aux = nullptr;        // bit-packed kernel's constant 2 KiB lookup table, on this handle's device
     int8_t* d_stage = nullptr;       // natural-layout staging for spin_get_spins / spin_set_spins / spin_set_bonds (grow-only)
     size_t stage_bytes = 0;
@@ -145,8 +159,75 @@ int check_sweep_args(const spin_sim* sim, const double* beta, double J, double h
     for (int b = 0; b < sim->batch; ++b)
         if (!std::isfinite(beta[b]) || beta[b] < 0.0)
             return fail(SPIN_ERR_INVALID, "spin_sweep: beta[%d] must be finite and >= 0", b);
-    if (sim->model == SPIN_MODEL_POTTS && h != 0.0)
-        return fail(SPIN_ERR_UNSUPPORTED, "spin_sweep: a field term is not supported for the Potts model (h must be 0)");
+    return SPIN_OK;
+}
+
+// One replica's device record for (beta, J, h).
+void build_record(const spin_sim* sim, int b, double beta, double J, double h, uint32_t* rec) {
+    std::memset(rec, 0, sizeof(uint32_t) * kTableStride);
+    if (sim->model == SPIN_MODEL_ISING) {
+        for (int d = 0; d < 2; ++d)
+            for (int nd = 0; nd <= 4; ++nd) {
+                const int s = d ? -1 : 1, nn = 4 - 2 * nd;
+                encode(ising_class(beta, J, h, s, nn), d * 8 + nd, rec);
+            }
+    } else {
+        for (int dn = -4; dn <= 4; ++dn) encode(potts_class(beta, J, dn), dn + 4, rec);
+    }
+    rec[kTabQ] = (uint32_t)sim->q[b];
+}
+
+// Real couplings and per-site fields: Alg. 1's acceptance for each of the 32 (own spin, neighbour configuration) classes
+// of every site, evaluated on the host in IEEE double in the order the oracle uses (general_oracle.cpp): local field
+// F = Jv[i-1][j] s_up + Jv[i][j] s_down + Jh[i][j-1] s_left + Jh[i][j] s_right + B[i][j], dE = 2 s F, then O4.
+int upload_general_thresholds(spin_sim* sim, const double* beta) {
+    const int L = sim->L;
+    const size_t N = (size_t)L * L, B = (size_t)sim->batch;
+    bool same = sim->g_beta.size() == B;
+    for (size_t b = 0; same && b < B; ++b) same = sim->g_beta[b] == beta[b];
+    if (same) return SPIN_OK;                               // thresholds on the device are current
+    std::vector<uint32_t> thr(B * N * 32), alw(B * N);
+    for (size_t b = 0; b < B; ++b)
+        for (int i = 0; i < L; ++i)
+            for (int j = 0; j < L; ++j) {
+                const int iu = i == 0 ? L - 1 : i - 1, jl = j == 0 ? L - 1 : j - 1;
+                const size_t x = b * N + (size_t)i * L + j;
+                const double ju = sim->g_Jv[b * N + (size_t)iu * L + j], jd = sim->g_Jv[x];
+                const double jlft = sim->g_Jh[b * N + (size_t)i * L + jl], jrgt = sim->g_Jh[x], fb = sim->g_B[x];
+                uint32_t mask = 0u;
+                for (int k = 0; k < 32; ++k) {
+                    const double s = (k & 16) ? -1.0 : 1.0;
+                    const double su = (k & 1) ? -1.0 : 1.0, sd = (k & 2) ? -1.0 : 1.0, sl = (k & 4) ? -1.0 : 1.0, sr = (k & 8) ? -1.0 : 1.0;
+                    const double F = ju * su + jd * sd + jlft * sl + jrgt * sr + fb;
+                    const ClassAccept c = class_accept(beta[b], 2.0 * s * F);
+                    thr[x * 32 + k] = c.T;
+                    if (c.always) mask |= 1u << k;
+                }
+                alw[x] = mask;
+            }
+    CUDA_TRY(cudaMemcpyAsync(sim->d_thr, thr.data(), thr.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaMemcpyAsync(sim->d_alw, alw.data(), alw.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));           // the host vectors go out of scope
+    sim->g_beta.assign(beta, beta + B);
+    return SPIN_OK;
+}
+
+// Potts with a field on the state label and / or bond signs: class (dn, dl = new - old), dE = -(J dn) - h dl.
+int upload_potts_general(spin_sim* sim, const double* beta, double J, double h) {
+    const size_t B = (size_t)sim->batch;
+    if (!sim->d_tab2) CUDA_TRY(cudaMalloc(&sim->d_tab2, sizeof(unsigned long long) * 9 * 255 * B));
+    std::vector<unsigned long long> tab(B * 9 * 255, 0ull);
+    for (size_t b = 0; b < B; ++b) {
+        const int q = sim->q[b];
+        for (int dn = -4; dn <= 4; ++dn)
+            for (int dl = -(q - 1); dl <= q - 1; ++dl) {
+                const double dE = -(J * (double)dn) - h * (double)dl;
+                const ClassAccept c = class_accept(beta[b], dE);
+                tab[(b * 9 + (size_t)(dn + 4)) * 255 + (size_t)(dl + 127)] = ((unsigned long long)(c.always ? 1 : 0) << 32) | c.T;
+            }
+    }
+    CUDA_TRY(cudaMemcpyAsync(sim->d_tab2, tab.data(), tab.size() * sizeof(unsigned long long), cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
     return SPIN_OK;
 }
 
@@ -157,23 +238,19 @@ int upload_tables(spin_sim* sim, const double* beta, double J, double h) {
     sim->table_slot ^= 1;
     uint32_t* h_tab = sim->h_tables[slot];
     CUDA_TRY(cudaEventSynchronize(sim->table_ev[slot]));
-    std::memset(h_tab, 0, sizeof(uint32_t) * kTableStride * (size_t)sim->batch);
-    for (int b = 0; b < sim->batch; ++b) {
-        uint32_t* rec = h_tab + (size_t)b * kTableStride;
-        if (sim->model == SPIN_MODEL_ISING) {
-            for (int d = 0; d < 2; ++d)
-                for (int nd = 0; nd <= 4; ++nd) {
-                    const int s = d ? -1 : 1, nn = 4 - 2 * nd;
-                    encode(ising_class(beta[b], J, h, s, nn), d * 8 + nd, rec);
-                }
-        } else {
-            for (int dn = -4; dn <= 4; ++dn) encode(potts_class(beta[b], J, dn), dn + 4, rec);
-        }
-        rec[kTabQ] = (uint32_t)sim->q[b];
-    }
+    for (int b = 0; b < sim->batch; ++b) build_record(sim, b, beta[b], J, h, h_tab + (size_t)b * kTableStride);
     CUDA_TRY(cudaMemcpyAsync(sim->d_tables, h_tab, sizeof(uint32_t) * kTableStride * (size_t)sim->batch,
                              cudaMemcpyHostToDevice, sim->stream));
     CUDA_TRY(cudaEventRecord(sim->table_ev[slot], sim->stream));
+    if (sim->general) {
+        const int rg = upload_general_thresholds(sim, beta);
+        if (rg != SPIN_OK) return rg;
+    }
+    sim->potts_general = sim->model == SPIN_MODEL_POTTS && (h != 0.0 || sim->d_bond_nat != nullptr);
+    if (sim->potts_general) {
+        const int rp = upload_potts_general(sim, beta, J, h);
+        if (rp != SPIN_OK) return rp;
+    }
     return SPIN_OK;
 }
 
@@ -198,6 +275,7 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
 // batch gives every SM work (or when the lattice is so small that the streaming kernels are launch-bound anyway).
 bool use_resident(const spin_sim* sim, bool measure) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || !ising_int8_resident_fits(sim->L)) return false;
+    if (sim->general || sim->d_bond_nat) return false;            // per-bond couplings run on the general kernels
     if (sim->policy == SPIN_POLICY_STREAMING) return false;
     if (sim->policy == SPIN_POLICY_RESIDENT) return true;
     const long long sites = (long long)sim->batch * sim->L * sim->L;
@@ -212,10 +290,10 @@ bool use_resident(const spin_sim* sim, bool measure) {
 }
 
 void enqueue_resident(spin_sim* sim, int64_t t0, int64_t n_sweeps, bool measure, long long* E_trace, long long* M_trace,
-                      long long* moments) {
+                      long long* moments, const uint32_t* tables = nullptr) {
     ResidentArgs a;
     a.lattice = sim->lattice;
-    a.tables = sim->d_tables;
+    a.tables = tables ? tables : sim->d_tables;
     a.batch = sim->batch;
     a.L = sim->L;
     a.replica_offset = sim->replica_offset;
@@ -229,10 +307,18 @@ void enqueue_resident(spin_sim* sim, int64_t t0, int64_t n_sweeps, bool measure,
     sim->launches += launch_ising_int8_resident(a, sim->stream);
 }
 
-void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour) {
-    const SweepArgs a = sweep_args(sim, t, colour);
-    if (sim->model == SPIN_MODEL_POTTS) sim->launches += launch_potts_int8_half_sweep(a, sim->stream);
-    else if (sim->layout == SPIN_LAYOUT_BITPACKED) sim->launches += launch_ising_bits_half_sweep(a, sim->stream);
+void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour, const uint32_t* tables = nullptr) {
+    SweepArgs a = sweep_args(sim, t, colour);
+    if (tables) a.tables = tables;                          // a step of spin_sweep_schedule
+    const size_t nat = (size_t)sim->batch * sim->L * sim->L;
+    if (sim->model == SPIN_MODEL_POTTS) {
+        if (sim->potts_general)
+            sim->launches += launch_potts_int8_general_half_sweep(a, sim->d_tab2, sim->d_bond_nat,
+                                                                  sim->d_bond_nat ? sim->d_bond_nat + nat : nullptr, sim->stream);
+        else sim->launches += launch_potts_int8_half_sweep(a, sim->stream);
+    } else if (sim->layout == SPIN_LAYOUT_BITPACKED) sim->launches += launch_ising_bits_half_sweep(a, sim->stream);
+    else if (sim->general) sim->launches += launch_ising_int8_general_half_sweep(a, sim->d_thr, sim->d_alw, sim->stream);
+    else if (sim->d_bond_nat) sim->launches += launch_ising_int8_bonds_half_sweep(a, sim->d_bond_nat, sim->d_bond_nat + nat, sim->stream);
     else sim->launches += launch_ising_int8_half_sweep(a, sim->stream);
 }
 
@@ -241,12 +327,22 @@ void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour) {
 int enqueue_observe(spin_sim* sim, long long* E_out, long long* M_out) {
     const size_t nb = sizeof(long long) * (size_t)sim->batch;
     if (E_out) CUDA_TRY(cudaMemsetAsync(E_out, 0, nb, sim->stream));
+    const size_t nat = (size_t)sim->batch * sim->L * sim->L;
     if (sim->model == SPIN_MODEL_POTTS) {
-        sim->launches += launch_potts_int8_observe(sim->lattice, sim->batch, sim->L, sim->d_q, E_out, M_out ? sim->d_hist : nullptr, sim->stream);
+        // with bond signs the energy comes from the general reduction; the histogram (M) from the regular one
+        const bool signs = sim->d_bond_nat != nullptr;
+        if (signs && E_out) sim->launches += launch_potts_general_observe(sim->lattice, sim->d_bond_nat, sim->d_bond_nat + nat, sim->batch,
+                                                                          sim->L, E_out, nullptr, sim->stream);
+        if (!signs || M_out)
+            sim->launches += launch_potts_int8_observe(sim->lattice, sim->batch, sim->L, sim->d_q, signs ? nullptr : E_out,
+                                                       M_out ? sim->d_hist : nullptr, sim->stream);
         if (M_out) sim->launches += launch_potts_finalize(sim->d_hist, sim->d_q, sim->batch, M_out, sim->stream);
     } else {
         if (M_out) CUDA_TRY(cudaMemsetAsync(M_out, 0, nb, sim->stream));
-        if (sim->layout == SPIN_LAYOUT_BITPACKED)
+        if (sim->layout == SPIN_LAYOUT_INT8 && sim->d_bond_nat)
+            sim->launches += launch_ising_int8_bonds_observe(sim->lattice, sim->d_bond_nat, sim->d_bond_nat + nat, sim->batch, sim->L,
+                                                             E_out, M_out, sim->stream);
+        else if (sim->layout == SPIN_LAYOUT_BITPACKED)
             sim->launches += launch_ising_bits_observe(sim->lattice, sim->d_bonds, sim->batch, sim->L, E_out, M_out, sim->stream);
         else
             sim->launches += launch_ising_int8_observe(sim->lattice, sim->batch, sim->L, E_out, M_out, sim->stream);
@@ -332,6 +428,14 @@ void spin_destroy(spin_sim* sim) {
     if (sim->d_EM) cudaFree(sim->d_EM);
     if (sim->d_hist) cudaFree(sim->d_hist);
     if (sim->d_bad) cudaFree(sim->d_bad);
+    if (sim->d_bond_nat) cudaFree(sim->d_bond_nat);
+    if (sim->d_gen) cudaFree(sim->d_gen);
+    if (sim->d_thr) cudaFree(sim->d_thr);
+    if (sim->d_alw) cudaFree(sim->d_alw);
+    if (sim->d_tab2) cudaFree(sim->d_tab2);
+    if (sim->d_sched) cudaFree(sim->d_sched);
+    if (sim->h_sched) cudaFreeHost(sim->h_sched);
+    if (sim->sched_ev) cudaEventDestroy(sim->sched_ev);
     if (sim->d_aux) cudaFree(sim->d_aux);
     if (sim->d_stage) cudaFree(sim->d_stage);
     if (sim->d_mom) cudaFree(sim->d_mom);
@@ -494,10 +598,33 @@ int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv) {
         CUDA_TRY(cudaStreamSynchronize(sim->stream));
         if (sim->d_bonds) cudaFree(sim->d_bonds);
         sim->d_bonds = nullptr;
+        if (sim->d_bond_nat) cudaFree(sim->d_bond_nat);
+        sim->d_bond_nat = nullptr;
         return SPIN_OK;
     }
-    if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_BITPACKED)
-        return fail(SPIN_ERR_UNSUPPORTED, "spin_set_bonds: +-J couplings are implemented for the bit-packed Ising layout only");
+    if (sim->general) return fail(SPIN_ERR_INVALID, "spin_set_bonds: the handle has real couplings (spin_set_couplings); remove them first");
+    if (sim->layout == SPIN_LAYOUT_INT8) {
+        // int8 layout (Ising and Potts): the signs stay in the natural layout on the device, read by the general kernels
+        const size_t n = (size_t)sim->batch * sim->L * sim->L;
+        int8_t* d_new = nullptr;
+        cudaError_t e = cudaMalloc(&d_new, 2 * n);
+        if (e != cudaSuccess) return fail(SPIN_ERR_NOMEM, "spin_set_bonds: cudaMalloc: %s", cudaGetErrorString(e));
+        unsigned int bad = 0;
+        e = cudaMemcpyAsync(d_new, Jh, n, cudaMemcpyHostToDevice, sim->stream);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(d_new + n, Jv, n, cudaMemcpyHostToDevice, sim->stream);
+        if (e == cudaSuccess) e = cudaMemsetAsync(sim->d_bad, 0, sizeof(unsigned int), sim->stream);
+        if (e == cudaSuccess) {
+            // +-1 validation = the Ising-spin validation over the two arrays
+            sim->launches += launch_validate_natural(d_new, 2 * sim->batch, sim->L, SPIN_MODEL_ISING, nullptr, sim->d_bad, sim->stream);
+            e = cudaMemcpyAsync(&bad, sim->d_bad, sizeof bad, cudaMemcpyDeviceToHost, sim->stream);
+        }
+        if (e == cudaSuccess) e = cudaStreamSynchronize(sim->stream);
+        if (e != cudaSuccess) { cudaFree(d_new); return cuda_fail(e, "spin_set_bonds"); }
+        if (bad) { cudaFree(d_new); return fail(SPIN_ERR_INVALID, "spin_set_bonds: bond signs must be +1 or -1"); }
+        if (sim->d_bond_nat) cudaFree(sim->d_bond_nat);
+        sim->d_bond_nat = d_new;
+        return SPIN_OK;
+    }
     // natural-layout signs -> device staging -> per-colour bit planes (validated on the device; a rejected call leaves
     // the handle's couplings as they were)
     const int L = sim->L;
@@ -522,6 +649,139 @@ int spin_set_bonds(spin_sim* sim, const int8_t* Jh, const int8_t* Jv) {
     if (bad) { cudaFree(d_new); return fail(SPIN_ERR_INVALID, "spin_set_bonds: bond signs must be +1 or -1"); }
     if (sim->d_bonds) cudaFree(sim->d_bonds);
     sim->d_bonds = d_new;
+    return SPIN_OK;
+}
+
+int spin_set_couplings(spin_sim* sim, const double* Jh, const double* Jv, const double* Bf) {
+    if (!sim) return fail(SPIN_ERR_INVALID, "spin_set_couplings: NULL handle");
+    const bool none = !Jh && !Jv && !Bf;
+    if (!none && (!Jh || !Jv || !Bf)) return fail(SPIN_ERR_INVALID, "spin_set_couplings: Jh, Jv and B must all be given or all be NULL");
+    CUDA_TRY(cudaSetDevice(sim->device));
+    if (none) {
+        CUDA_TRY(cudaStreamSynchronize(sim->stream));
+        if (sim->d_gen) cudaFree(sim->d_gen);
+        if (sim->d_thr) cudaFree(sim->d_thr);
+        if (sim->d_alw) cudaFree(sim->d_alw);
+        sim->d_gen = nullptr; sim->d_thr = nullptr; sim->d_alw = nullptr;
+        sim->general = false;
+        try { sim->g_Jh.clear(); sim->g_Jv.clear(); sim->g_B.clear(); sim->g_beta.clear(); } catch (...) {}
+        return SPIN_OK;
+    }
+    if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8)
+        return fail(SPIN_ERR_UNSUPPORTED, "spin_set_couplings: real couplings are implemented for the Ising model in the int8 layout");
+    if (sim->d_bond_nat) return fail(SPIN_ERR_INVALID, "spin_set_couplings: the handle has +-J bond signs (spin_set_bonds); remove them first");
+    const size_t n = (size_t)sim->batch * sim->L * sim->L;
+    for (size_t k = 0; k < n; ++k)
+        if (!std::isfinite(Jh[k]) || !std::isfinite(Jv[k]) || !std::isfinite(Bf[k]))
+            return fail(SPIN_ERR_INVALID, "spin_set_couplings: couplings and fields must be finite");
+    try {
+        sim->g_Jh.assign(Jh, Jh + n); sim->g_Jv.assign(Jv, Jv + n); sim->g_B.assign(Bf, Bf + n);
+        sim->g_beta.clear();
+    } catch (...) { sim->general = false; return fail(SPIN_ERR_NOMEM, "spin_set_couplings: out of host memory"); }
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    if (!sim->d_gen) {
+        cudaError_t e = cudaMalloc(&sim->d_gen, 3 * n * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc(&sim->d_thr, n * 32 * sizeof(uint32_t));
+        if (e == cudaSuccess) e = cudaMalloc(&sim->d_alw, n * sizeof(uint32_t));
+        if (e != cudaSuccess) {
+            if (sim->d_gen) cudaFree(sim->d_gen);
+            if (sim->d_thr) cudaFree(sim->d_thr);
+            sim->d_gen = nullptr; sim->d_thr = nullptr; sim->d_alw = nullptr; sim->general = false;
+            return fail(SPIN_ERR_NOMEM, "spin_set_couplings: cudaMalloc (132 bytes of thresholds per site): %s", cudaGetErrorString(e));
+        }
+    }
+    CUDA_TRY(cudaMemcpyAsync(sim->d_gen, Jh, n * sizeof(double), cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaMemcpyAsync(sim->d_gen + n, Jv, n * sizeof(double), cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaMemcpyAsync(sim->d_gen + 2 * n, Bf, n * sizeof(double), cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    sim->general = true;
+    return SPIN_OK;
+}
+
+int spin_energy_general(spin_sim* sim, double* E) {
+    if (!sim || !E) return fail(SPIN_ERR_INVALID, "spin_energy_general: NULL argument");
+    if (!sim->general) return fail(SPIN_ERR_INVALID, "spin_energy_general: the handle has no real couplings (spin_set_couplings)");
+    CUDA_TRY(cudaSetDevice(sim->device));
+    const size_t B = (size_t)sim->batch, n = B * sim->L * sim->L;
+    double* d_E = (double*)sim->d_EM;                       // [2][B] int64 scratch, reused as B doubles
+    CUDA_TRY(cudaMemsetAsync(d_E, 0, sizeof(double) * B, sim->stream));
+    sim->launches += launch_ising_general_energy(sim->lattice, sim->d_gen, sim->d_gen + n, sim->d_gen + 2 * n, sim->batch, sim->L, d_E, sim->stream);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(sim->h_EM, d_E, sizeof(double) * B, cudaMemcpyDeviceToHost, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    std::memcpy(E, sim->h_EM, sizeof(double) * B);
+    return SPIN_OK;
+}
+
+int spin_potts_label_sum(spin_sim* sim, int64_t* S) {
+    if (!sim || !S) return fail(SPIN_ERR_INVALID, "spin_potts_label_sum: NULL argument");
+    if (sim->model != SPIN_MODEL_POTTS) return fail(SPIN_ERR_INVALID, "spin_potts_label_sum: Potts handles only");
+    CUDA_TRY(cudaSetDevice(sim->device));
+    const size_t B = (size_t)sim->batch;
+    CUDA_TRY(cudaMemsetAsync(sim->d_EM, 0, sizeof(long long) * B, sim->stream));
+    sim->launches += launch_potts_general_observe(sim->lattice, nullptr, nullptr, sim->batch, sim->L, nullptr, sim->d_EM, sim->stream);
+    CUDA_TRY(cudaGetLastError());
+    CUDA_TRY(cudaMemcpyAsync(sim->h_EM, sim->d_EM, sizeof(long long) * B, cudaMemcpyDeviceToHost, sim->stream));
+    CUDA_TRY(cudaStreamSynchronize(sim->stream));
+    std::memcpy(S, sim->h_EM, sizeof(long long) * B);
+    return SPIN_OK;
+}
+
+int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps, double J, double h, int64_t sweeps_per_step,
+                        int64_t sweep_offset) {
+    if (!sim || !beta_steps) return fail(SPIN_ERR_INVALID, "spin_sweep_schedule: NULL argument");
+    if (n_steps < 0 || sweeps_per_step < 0 || n_steps > (1ll << 24)) return fail(SPIN_ERR_INVALID, "spin_sweep_schedule: n_steps in 0..2^24 and sweeps_per_step >= 0 required");
+    if (sweeps_per_step > 0 && n_steps > (1ll << 56) / sweeps_per_step) return fail(SPIN_ERR_INVALID, "spin_sweep_schedule: sweep range exceeds 2^56");
+    const size_t B = (size_t)sim->batch;
+    for (int64_t k = 0; k < n_steps; ++k) {
+        const int rc = check_sweep_args(sim, beta_steps + (size_t)k * B, J, h, sweeps_per_step, sweep_offset + k * sweeps_per_step);
+        if (rc != SPIN_OK) return rc;
+    }
+    if (n_steps == 0 || sweeps_per_step == 0) return SPIN_OK;
+    if (sim->general || (sim->model == SPIN_MODEL_POTTS && (h != 0.0 || sim->d_bond_nat)))
+        return fail(SPIN_ERR_UNSUPPORTED, "spin_sweep_schedule: class-table models only (uniform or +-J couplings, Potts without field); "
+                    "call spin_sweep per step for real couplings");
+    CUDA_TRY(cudaSetDevice(sim->device));
+    // every step's records are built now and uploaded in ONE copy; the kernels of step k read their own slice, so the
+    // whole schedule is enqueued without a host synchronisation between steps
+    const size_t bytes = sizeof(uint32_t) * kTableStride * B * (size_t)n_steps;
+    if (!sim->sched_ev) CUDA_TRY(cudaEventCreateWithFlags(&sim->sched_ev, cudaEventDisableTiming));
+    if (sim->sched_bytes < bytes) {
+        CUDA_TRY(cudaStreamSynchronize(sim->stream));
+        if (sim->d_sched) cudaFree(sim->d_sched);
+        if (sim->h_sched) cudaFreeHost(sim->h_sched);
+        sim->d_sched = nullptr; sim->h_sched = nullptr; sim->sched_bytes = 0;
+        cudaError_t e = cudaMalloc(&sim->d_sched, bytes);
+        if (e == cudaSuccess) e = cudaMallocHost(&sim->h_sched, bytes);
+        if (e != cudaSuccess) {
+            if (sim->d_sched) cudaFree(sim->d_sched);
+            sim->d_sched = nullptr; sim->h_sched = nullptr;
+            return fail(SPIN_ERR_NOMEM, "spin_sweep_schedule: allocating %zu bytes of tables: %s", bytes, cudaGetErrorString(e));
+        }
+        sim->sched_bytes = bytes;
+    }
+    CUDA_TRY(cudaEventSynchronize(sim->sched_ev));          // the previous schedule's upload has left the pinned buffer
+    for (int64_t k = 0; k < n_steps; ++k)
+        for (size_t b = 0; b < B; ++b)
+            build_record(sim, (int)b, beta_steps[(size_t)k * B + b], J, h, sim->h_sched + ((size_t)k * B + b) * kTableStride);
+    // NOTE: earlier sweeps of this stream that still read d_sched (a previous schedule) are ordered before this copy
+    CUDA_TRY(cudaMemcpyAsync(sim->d_sched, sim->h_sched, bytes, cudaMemcpyHostToDevice, sim->stream));
+    CUDA_TRY(cudaEventRecord(sim->sched_ev, sim->stream));
+    sim->potts_general = false;
+    const bool resident = use_resident(sim, false);
+    for (int64_t k = 0; k < n_steps; ++k) {
+        const uint32_t* tab = sim->d_sched + (size_t)k * B * kTableStride;
+        const int64_t t0 = sweep_offset + k * sweeps_per_step;
+        if (resident) {
+            enqueue_resident(sim, t0, sweeps_per_step, false, nullptr, nullptr, nullptr, tab);
+        } else {
+            for (int64_t t = t0; t < t0 + sweeps_per_step; ++t) {
+                enqueue_half_sweep(sim, t, 0, tab);
+                enqueue_half_sweep(sim, t, 1, tab);
+            }
+        }
+    }
+    CUDA_TRY(cudaGetLastError());
     return SPIN_OK;
 }
 

@@ -142,6 +142,18 @@ cudaError_t ising_int8_resident_configure();                                // p
 int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s);      // all n_sweeps in one launch
 const char* potts_int8_variant(int L);
 
+// General couplings (general.cu): natural-layout device arrays.
+int launch_ising_int8_bonds_half_sweep(const SweepArgs& a, const int8_t* Jh, const int8_t* Jv, cudaStream_t s);
+int launch_ising_int8_general_half_sweep(const SweepArgs& a, const uint32_t* thr, const uint32_t* alw, cudaStream_t s);
+int launch_potts_int8_general_half_sweep(const SweepArgs& a, const unsigned long long* tab2, const int8_t* Jh, const int8_t* Jv,
+                                         cudaStream_t s);
+int launch_ising_general_energy(const void* lattice, const double* Jh, const double* Jv, const double* B, int batch, int L,
+                                double* E, cudaStream_t s);                  // E[b] += ..., zero on entry
+int launch_potts_general_observe(const void* lattice, const int8_t* Jh, const int8_t* Jv, int batch, int L, long long* E_acc,
+                                 long long* S_acc, cudaStream_t s);
+int launch_ising_int8_bonds_observe(const void* lattice, const int8_t* Jh, const int8_t* Jv, int batch, int L, long long* E_acc,
+                                    long long* M_acc, cudaStream_t s);
+
 // Observables: accumulate into E_acc[b], M_acc[b] (int64, must be zero on entry; Potts uses hist).
 int launch_ising_int8_observe(const void* lattice, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);
 int launch_ising_bits_observe(const void* lattice, const uint32_t* bonds, int batch, int L, long long* E_acc, long long* M_acc, cudaStream_t s);

@@ -83,9 +83,9 @@ def test_set_bonds_argument_checks():
             sim.spin_set_bonds(bad, Jv)
         sim.spin_sweep([0.5, 0.5], 1.0, 0.0, 1, 0)          # still the uniform model
         assert not np.array_equal(sim.spin_get_spins(), before)
-    with _mk(2, 64, 1, layout=sp.SPIN_LAYOUT_INT8) as sim:
+    with _mk(2, 64, 1, layout=sp.SPIN_LAYOUT_INT8) as sim:       # int8 layout: accepted (general kernels), still validated
         with pytest.raises(sp.SpinError):
-            sim.spin_set_bonds(Jh, Jv)
-    with sp.spin_create_ex(2, 64, sp.SPIN_MODEL_POTTS, q_per_replica=np.array([3, 3], dtype=np.int32), seed=1) as sim:
-        with pytest.raises(sp.SpinError):
-            sim.spin_set_bonds(Jh, Jv)
+            sim.spin_set_bonds(bad, Jv)
+        sim.spin_set_bonds(Jh, Jv)
+        with pytest.raises(sp.SpinError):                          # bond signs and real couplings exclude each other
+            sim.spin_set_couplings(Jh.astype(float), Jv.astype(float), np.zeros((2, 64, 64)))
