@@ -211,11 +211,13 @@ class Runner:
             sim.spin_set_policy(policy)
         return sim
 
-    def run(self, w, mode, steps, warmup, policy=None, e2e_steps=None, barrier=lambda: None):
+    def run(self, w, mode, steps, warmup, policy=None, e2e_steps=None, barrier=lambda: None, prepare=None):
         """mode: 'sweep' (spin_sweep + spin_observables_dev), 'trace' (spin_sweep_measure with per-sweep E, M traces),
         'moments' (w.therm plain sweeps, then spin_sweep_measure with moments and no trace)."""
         torch, stream = self.torch, self.stream
         sim = self.create(w, policy)
+        if prepare:
+            prepare(sim)
         E_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
         M_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
         state = {"offset": 0, "per_call": None}
@@ -227,6 +229,13 @@ class Runner:
             if mode == "sweep":
                 l0 = sim.spin_kernel_launches()
                 sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, off)
+                state["per_call"] = sim.spin_kernel_launches() - l0
+                if events:
+                    events[1].record(stream)
+                sim.spin_observables_dev(E_dev.data_ptr(), M_dev.data_ptr())
+            elif mode == "schedule":
+                l0 = sim.spin_kernel_launches()
+                sim.spin_sweep_schedule(w.beta_steps, w.J, w.h, w.n_sweeps // len(w.beta_steps), off)
                 state["per_call"] = sim.spin_kernel_launches() - l0
                 if events:
                     events[1].record(stream)
@@ -418,6 +427,47 @@ def dmc_entries(runner, sp, args, peaks):
     return res
 
 
+def general_entries(runner, sp, args, peaks, measured):
+    """SURVEY.md 8(f) #2 shapes: real couplings + site fields (per-site thresholds, HBM-bound), the Potts field term
+    (general kernel), and a +-J glass annealed by spin_sweep_schedule in one call (Fig. 9's Monte Carlo arm)."""
+    from paper_2304_01772_b200.workloads import Workload
+    out = {}
+    n = args.sweeps or 40
+    rng = np.random.default_rng(11)
+    B, L = 16, 512
+    w = Workload("F2-real-couplings", "ising", B, L, 8, np.full(B, 0.6), 1.0, 0.0, n)
+    Jh, Jv, Bf = rng.normal(size=(B, L, L)), rng.normal(size=(B, L, L)), 0.3 * rng.normal(size=(B, L, L))
+    res = runner.run(w, "sweep", args.steps, args.warmup, prepare=lambda sim: sim.spin_set_couplings(Jh, Jv, Bf))
+    d = summarise(w, res, peaks, measured)
+    rate = d["roofline"]["sweep_only_flips_per_ns"]
+    # per site and sweep: one 4-byte threshold + the 4-byte always mask (each fetched as a 32-byte sector: 64 bytes of
+    # DRAM traffic) + 3 bytes of spins
+    d["kernel"] = "ising_int8_general_kernel"
+    d["roofline"] = {"bound": "hbm", "achieved": 67.0 * rate, "peak": peaks["hbm_gbs"], "unit": "GB/s",
+                     "frac": 67.0 * rate / peaks["hbm_gbs"], "bytes_per_site_per_sweep": 67.0,
+                     "note": "sector-granular bytes (2 x 32 B table sectors + 3 B of spins); useful bytes are 11 per site"}
+    out[w.name] = d
+    res["sim"].spin_destroy()
+    q = np.array([3] * (B // 2) + [8] * (B // 2), dtype=np.int32)
+    w = Workload("F2-potts-field", "potts", B, L, 9, np.full(B, 1.0), 1.0, 0.1, n, q=q)
+    res = runner.run(w, "sweep", args.steps, args.warmup)
+    d = summarise(w, res, peaks, measured)
+    d["kernel"] = "potts_int8_general_kernel"
+    out[w.name] = d
+    res["sim"].spin_destroy()
+    B, L, n_steps, per = 4, 1024, 50, 4
+    w = Workload("F2-anneal-schedule", "ising", B, L, 10, np.full(B, 1.0), 1.0, 0.0, n_steps * per, layout="bits")
+    w.beta_steps = np.array([[0.1 + 2.9 * k / (n_steps - 1)] * B for k in range(n_steps)])
+    sg = lambda: (2 * rng.integers(0, 2, size=(B, L, L)) - 1).astype(np.int8)
+    Jh8, Jv8 = sg(), sg()
+    res = runner.run(w, "schedule", args.steps, args.warmup, prepare=lambda sim: sim.spin_set_bonds(Jh8, Jv8))
+    d = summarise(w, res, peaks, measured)
+    d["mode"] = "spin_sweep_schedule: %d beta steps x %d sweeps in one call, +-J glass" % (n_steps, per)
+    out[w.name] = d
+    res["sim"].spin_destroy()
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -523,6 +573,7 @@ def main():
         if world == 1 and not args.no_per_config:
             line["per_config"] = per_config_block(runner, sp, args, peaks, measured)
             line["per_config"].update(dmc_entries(runner, sp, args, peaks))
+            line["per_config"].update(general_entries(runner, sp, args, peaks, measured))
         if not args.no_cpu_baseline and world == 1:
             v, threads, sample, _ = oracle_throughput(w, 12.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,

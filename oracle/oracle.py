@@ -11,7 +11,8 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "spin_oracle.cpp")
-_SRCS = [_SRC, os.path.join(_HERE, "dmc_oracle.cpp"), os.path.join(_HERE, "general_oracle.cpp")]
+_SRCS = [_SRC, os.path.join(_HERE, "dmc_oracle.cpp"), os.path.join(_HERE, "general_oracle.cpp"),
+         os.path.join(_HERE, "stencil_oracle.cpp")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 __all__ = [
@@ -21,6 +22,8 @@ __all__ = [
     "dmc_half_sweep", "dmc_forward", "dmc_discretise", "dmc_backward",
     "ising_general_half_sweep", "sweep_general", "ising_general_observables", "potts_general_half_sweep",
     "sweep_potts_general", "potts_general_observables", "sweep_schedule",
+    "STENCIL_TRIANGULAR", "STENCIL_CUBIC", "STENCIL_SQUARE_NNN", "stencil_shape", "stencil_init", "stencil_colour_pass",
+    "stencil_sweep", "stencil_observables",
 ]
 
 
@@ -67,6 +70,14 @@ def _l():
         lib.oracle_potts_general_half_sweep.argtypes = [p, p, p, c.c_int32, c.c_int32, p, p, d, d, c.c_uint64, c.c_int64,
                                                         c.c_int64, c.c_int32]
         lib.oracle_potts_general_observables.argtypes = [p, p, p, c.c_int32, c.c_int32, p, p, p, p]
+        lib.oracle_stencil_sites.argtypes = [c.c_int32, c.c_int32]
+        lib.oracle_stencil_sites.restype = c.c_int64
+        lib.oracle_stencil_init.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, c.c_uint64, c.c_int64]
+        lib.oracle_stencil_colour_pass.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, d, d, d, c.c_uint64, c.c_int64,
+                                                   c.c_int64, c.c_int32]
+        lib.oracle_stencil_sweep.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, d, d, d, c.c_uint64, c.c_int64,
+                                             c.c_int64, c.c_int64]
+        lib.oracle_stencil_observables.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, p, p]
         lib.oracle_dmc_half_sweep.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
                                               c.c_int32, p]
         lib.oracle_dmc_forward.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
@@ -344,3 +355,44 @@ def sweep_schedule(spins, beta_steps, J, h, seed, sweeps_per_step, sweep_offset=
         else:
             sweep(spins, beta_steps[k], J, h, seed, sweeps_per_step, sweep_offset=t, q=q, replica_offset=replica_offset)
         t += sweeps_per_step
+
+
+# ---- other lattice geometries (stencil_oracle.cpp) -----------------------------------------
+STENCIL_TRIANGULAR, STENCIL_CUBIC, STENCIL_SQUARE_NNN = 0, 1, 2
+
+
+def stencil_shape(stencil, batch, L):
+    return (batch, L, L, L) if stencil == STENCIL_CUBIC else (batch, L, L)
+
+
+def stencil_init(stencil, batch, L, seed, replica_offset=0):
+    spins = np.zeros(stencil_shape(stencil, batch, L), dtype=np.int8)
+    _l().oracle_stencil_init(_ptr(spins), stencil, batch, L, int(seed), int(replica_offset))
+    return spins
+
+
+def _stencil_lattice(stencil, spins):
+    assert spins.dtype == np.int8 and spins.flags["C_CONTIGUOUS"] and spins.ndim == (5 if False else (4 if stencil == STENCIL_CUBIC else 3))
+    return spins.shape[0], spins.shape[1]
+
+
+def stencil_colour_pass(stencil, spins, beta, J1, J2, h, seed, t, colour, replica_offset=0):
+    B, L = _stencil_lattice(stencil, spins)
+    ba = _beta_array(beta, B)
+    _l().oracle_stencil_colour_pass(_ptr(spins), stencil, B, L, _ptr(ba), float(J1), float(J2), float(h), int(seed),
+                                    int(replica_offset), int(t), int(colour))
+
+
+def stencil_sweep(stencil, spins, beta, J1, J2, h, seed, n_sweeps, sweep_offset=0, replica_offset=0):
+    B, L = _stencil_lattice(stencil, spins)
+    ba = _beta_array(beta, B)
+    _l().oracle_stencil_sweep(_ptr(spins), stencil, B, L, _ptr(ba), float(J1), float(J2), float(h), int(seed),
+                              int(replica_offset), int(n_sweeps), int(sweep_offset))
+
+
+def stencil_observables(stencil, spins):
+    """-> (E1, E2, M) int64[batch]: minus the first- / second-neighbour bond sums, and sum s."""
+    B, L = _stencil_lattice(stencil, spins)
+    E1, E2, M = (np.zeros(B, dtype=np.int64) for _ in range(3))
+    _l().oracle_stencil_observables(_ptr(spins), stencil, B, L, _ptr(E1), _ptr(E2), _ptr(M))
+    return E1, E2, M
