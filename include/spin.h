@@ -248,6 +248,36 @@ SPIN_API int spin_dmc_backward(int32_t batch, int32_t L, int32_t dtype, const vo
 /* Eq. 4 (Alg. 2 line 11): s <- -1 if s < 0 else +1 on n device elements.  Asynchronous. */
 SPIN_API int spin_dmc_discretise(int32_t dtype, void* s, int64_t n, void* cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Other lattice geometries: Algorithm 1 on the triangular lattice (Eq. 3),
+ * the 3D cubic lattice and the square lattice with second neighbours ("more colors").
+ * Stateless calls on a DEVICE int8 lattice of +-1 spins in the natural row-major layout, [batch][L][L] or
+ * [batch][L][L][L].  H = -J1 sum_<first> s s' - J2 sum_<second> s s' - h sum s (J2 is used by SQUARE_NNN only).
+ *   SPIN_STENCIL_TRIANGULAR: L % 3 == 0; neighbours (i+-1, j), (i, j+-1), (i+1, j+1), (i-1, j-1); colours (i + j) mod 3.
+ *   SPIN_STENCIL_CUBIC:      L even; neighbours +-1 along each axis; colours (i + j + k) & 1.
+ *   SPIN_STENCIL_SQUARE_NNN: L even; 4 first + 4 diagonal second neighbours; colours 2 (i & 1) + (j & 1).
+ * A sweep visits the colours in order 0, 1, ...; the random word of a site is Philox group n >> 2, word n & 3, with n the
+ * index of the site among the sites of its colour in row-major order (counter as in DESIGN.md O2, domain 3); acceptance
+ * as in spin_threshold_table with dE = 2 s (J1 nn1 + J2 nn2 + h).  Readings S1-S6, DESIGN.md section 13.
+ * beta: HOST [batch].  Work is enqueued on cuda_stream (NULL = default).  SPIN_ERR_INVALID for bad shapes / arguments.
+ * ------------------------------------------------------------------------------------------- */
+enum { SPIN_STENCIL_TRIANGULAR = 0, SPIN_STENCIL_CUBIC = 1, SPIN_STENCIL_SQUARE_NNN = 2 };
+
+/* Sites (= bytes) per replica: L*L or L*L*L; 0 if the shape is invalid for the stencil. */
+SPIN_API size_t spin_stencil_sites(int32_t stencil, int32_t L);
+/* Uniform random +-1 lattice from Philox(seed): natural site index p, group p >> 2, word p & 3, +1 iff bit 31. */
+SPIN_API int spin_stencil_init(int32_t stencil, int32_t batch, int32_t L, int8_t* lattice, uint64_t seed, int64_t replica_offset,
+                               void* cuda_stream);
+/* Sweeps t = sweep_offset .. sweep_offset + n_sweeps - 1, in place.  Asynchronous. */
+SPIN_API int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_t* lattice, const double* beta, double J1,
+                                double J2, double h, uint64_t seed, int64_t replica_offset, int64_t n_sweeps,
+                                int64_t sweep_offset, void* cuda_stream);
+/* E1[b] = -(sum over first-neighbour bonds of s s'), E2[b] = the same over second-neighbour bonds, M[b] = sum s; every bond
+ * once, with multiplicity on tiny lattices.  HOST int64 [batch], any may be NULL.  Energy = J1 E1 + J2 E2 - h M.
+ * Synchronises the stream. */
+SPIN_API int spin_stencil_observables(int32_t stencil, int32_t batch, int32_t L, const int8_t* lattice, int64_t* E1,
+                                      int64_t* E2, int64_t* M, void* cuda_stream);
+
 /* Measurement aid ("second, tighter denominator"): runs a register-only kernel on the current
  * device that does nothing but the algorithmic work of the sweep - Philox-4x32-10 calls (precomputed round keys) whose
  * four output words are each compared with a threshold - and returns the best-of-5 rate in random words per

@@ -13,13 +13,15 @@ SPIN_MODEL_ISING, SPIN_MODEL_POTTS = 0, 1
 SPIN_LAYOUT_INT8, SPIN_LAYOUT_BITPACKED = 0, 1
 SPIN_POLICY_AUTO, SPIN_POLICY_STREAMING, SPIN_POLICY_RESIDENT = 0, 1, 2
 SPIN_DTYPE_F32, SPIN_DTYPE_F64 = 0, 1
+SPIN_STENCIL_TRIANGULAR, SPIN_STENCIL_CUBIC, SPIN_STENCIL_SQUARE_NNN = 0, 1, 2
 
 __all__ = [
     "SPIN_OK", "SPIN_ERR_INVALID", "SPIN_ERR_NOMEM", "SPIN_ERR_CUDA", "SPIN_ERR_UNSUPPORTED",
     "SPIN_MODEL_ISING", "SPIN_MODEL_POTTS", "SPIN_LAYOUT_INT8", "SPIN_LAYOUT_BITPACKED",
     "SPIN_POLICY_AUTO", "SPIN_POLICY_STREAMING", "SPIN_POLICY_RESIDENT",
     "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim", "spin_measure_philox_compare_rate",
-    "SPIN_DTYPE_F32", "SPIN_DTYPE_F64", "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
+    "SPIN_DTYPE_F32", "SPIN_DTYPE_F64", "SPIN_STENCIL_TRIANGULAR", "SPIN_STENCIL_CUBIC", "SPIN_STENCIL_SQUARE_NNN",
+    "spin_stencil_sites", "spin_stencil_init", "spin_stencil_sweep", "spin_stencil_observables", "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
     "spin_create", "spin_create_ex",
 ]
 
@@ -67,6 +69,10 @@ def load_library():
         "spin_energy_general": (c.c_int, [vp, vp]),
         "spin_potts_label_sum": (c.c_int, [vp, vp]),
         "spin_sweep_schedule": (c.c_int, [vp, vp, i64, dbl, dbl, i64, i64]),
+        "spin_stencil_sites": (sz, [i32, i32]),
+        "spin_stencil_init": (c.c_int, [i32, i32, i32, vp, u64, i64, vp]),
+        "spin_stencil_sweep": (c.c_int, [i32, i32, i32, vp, vp, dbl, dbl, dbl, u64, i64, i64, i64, vp]),
+        "spin_stencil_observables": (c.c_int, [i32, i32, i32, vp, vp, vp, vp, vp]),
         "spin_dmc_forward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp]),
         "spin_dmc_backward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp, vp, vp, vp, vp]),
         "spin_dmc_discretise": (c.c_int, [i32, vp, i64, vp]),
@@ -86,6 +92,7 @@ EXPORTED_SYMBOLS = (
     "spin_kernel_variant", "spin_set_policy", "spin_set_bonds", "spin_measure_philox_compare_rate",
     "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
     "spin_set_couplings", "spin_energy_general", "spin_potts_label_sum", "spin_sweep_schedule",
+    "spin_stencil_sites", "spin_stencil_init", "spin_stencil_sweep", "spin_stencil_observables",
 )
 
 
@@ -146,6 +153,28 @@ def spin_dmc_backward(batch, L, dtype, traj_ptr, Jh_ptr, Jv_ptr, h, beta, alpha,
                                             int(seed), int(replica_offset), int(n_sweeps), int(sweep_offset), grad_out_ptr,
                                             grad_s0_ptr, grad_Jh_ptr, grad_Jv_ptr, _np_ptr(gb), _np_ptr(gh), cuda_stream))
     return gb, gh
+
+
+def spin_stencil_sites(stencil, L):
+    return int(load_library().spin_stencil_sites(stencil, L))
+
+
+def spin_stencil_init(stencil, batch, L, lattice_ptr, seed, replica_offset=0, cuda_stream=None):
+    _check(load_library().spin_stencil_init(stencil, batch, L, lattice_ptr, int(seed), int(replica_offset), cuda_stream))
+
+
+def spin_stencil_sweep(stencil, batch, L, lattice_ptr, beta, J1, J2, h, seed, n_sweeps, sweep_offset=0, replica_offset=0,
+                       cuda_stream=None):
+    b = _beta64(beta, batch)
+    _check(load_library().spin_stencil_sweep(stencil, batch, L, lattice_ptr, _np_ptr(b), float(J1), float(J2), float(h),
+                                             int(seed), int(replica_offset), int(n_sweeps), int(sweep_offset), cuda_stream))
+
+
+def spin_stencil_observables(stencil, batch, L, lattice_ptr, cuda_stream=None):
+    E1, E2, M = (np.zeros(batch, dtype=np.int64) for _ in range(3))
+    _check(load_library().spin_stencil_observables(stencil, batch, L, lattice_ptr, _np_ptr(E1), _np_ptr(E2), _np_ptr(M),
+                                                   cuda_stream))
+    return E1, E2, M
 
 
 def spin_dmc_discretise(dtype, s_ptr, n, cuda_stream=None):

@@ -1,0 +1,304 @@
+// stencil.cu — SURVEY.md section 8(f) #4: Algorithm 1 on the other geometries the paper names:
+// the triangular lattice (Eq. 3), the 3D cubic lattice and the square lattice with
+// second neighbours, which needs "more colors".  Readings S1-S6 in DESIGN.md section 13:
+//   TRIANGULAR: L x L, L % 3 == 0, neighbours (i+-1, j), (i, j+-1), (i+1, j+1), (i-1, j-1), colours (i + j) mod 3;
+//   CUBIC:      L^3, L even, neighbours +-1 along each axis, colours (i + j + k) & 1;
+//   SQUARE_NNN: L x L, L even, 4 first (J1) + 4 diagonal second (J2) neighbours, colours 2 (i & 1) + (j & 1).
+// Natural row-major int8 lattices (no colour split: with 2, 3 or 4 colours and two dimensionalities one layout serves
+// all), H = -J1 sum_<1> s s' - J2 sum_<2> s s' - h sum s, dE = 2 s (J1 nn1 + J2 nn2 + h), per-replica class table
+// T[d][nd1][nd2] built on the host in IEEE double (the arithmetic of spin_threshold_table).  Random word of a site:
+// Philox group n >> 2, word n & 3, n = index of the site among the sites of its colour in row-major order, domain 3.
+// One thread per Philox group = 4 consecutive same-colour sites of one row (a row holds a multiple of ... sites of a
+// colour only when L allows; groups may straddle rows, handled per site).
+#include "../../include/spin.h"
+#include "spin_internal.cuh"
+
+#include <cmath>
+#include <vector>
+
+namespace spin {
+namespace {
+
+constexpr uint32_t kDomainStencil = 3;
+constexpr int kStencilRec = 64;            // uint32 per replica: T[0..49], always mask at [62] (low) and [63] (high)
+
+struct StencilArgs {
+    int8_t* lattice;
+    const uint32_t* tables;                // [B][kStencilRec]
+    int32_t stencil, batch, L, colour;
+    uint32_t replica_offset, c2, c3;
+    RoundKeys rk;
+};
+
+__device__ __forceinline__ int wrap_inc(int a, int L) { return a == L - 1 ? 0 : a + 1; }
+__device__ __forceinline__ int wrap_dec(int a, int L) { return a == 0 ? L - 1 : a - 1; }
+
+// Number of sites of one colour, and coordinates of same-colour site n (row-major order among that colour).
+__device__ __host__ __forceinline__ long long colour_sites(int stencil, int L) {
+    if (stencil == SPIN_STENCIL_TRIANGULAR) return (long long)L * (L / 3);
+    if (stencil == SPIN_STENCIL_CUBIC) return (long long)L * L * (L / 2);
+    return (long long)(L / 2) * (L / 2);
+}
+
+template <int kStencil>
+__global__ void __launch_bounds__(128) stencil_pass_kernel(StencilArgs a) {
+    const int L = a.L;
+    const long long per = colour_sites(kStencil, L);
+    const long long groups = (per + 3) >> 2;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= groups * a.batch) return;
+    const int b = (int)(gid / groups);
+    const uint32_t g = (uint32_t)(gid % groups);
+    const long long N = kStencil == SPIN_STENCIL_CUBIC ? (long long)L * L * L : (long long)L * L;
+    int8_t* lat = a.lattice + (size_t)b * N;
+    const uint32_t* tab = a.tables + (size_t)b * kStencilRec;
+    const unsigned long long always = (unsigned long long)tab[62] | ((unsigned long long)tab[63] << 32);
+    uint32_t r[4];
+    philox4x32_10(a.rk, g, (uint32_t)b + a.replica_offset, a.c2, a.c3, r);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const long long n = 4ll * g + e;
+        if (n >= per) break;
+        int idx;
+        size_t x;
+        int s;
+        if (kStencil == SPIN_STENCIL_TRIANGULAR) {
+            const int W = L / 3;
+            const int i = (int)(n / W), m = (int)(n % W);
+            const int j = 3 * m + ((a.colour - i) % 3 + 3) % 3;
+            const int iu = wrap_dec(i, L), id = wrap_inc(i, L), jl = wrap_dec(j, L), jr = wrap_inc(j, L);
+            x = (size_t)i * L + j;
+            s = lat[x];
+            const int nd = (lat[(size_t)iu * L + j] < 0) + (lat[(size_t)id * L + j] < 0) + (lat[(size_t)i * L + jl] < 0) +
+                           (lat[(size_t)i * L + jr] < 0) + (lat[(size_t)id * L + jr] < 0) + (lat[(size_t)iu * L + jl] < 0);
+            idx = (s < 0 ? 7 : 0) + nd;
+        } else if (kStencil == SPIN_STENCIL_CUBIC) {
+            const int W = L / 2;
+            const long long ij = n / W;
+            const int m = (int)(n % W);
+            const int i = (int)(ij / L), j = (int)(ij % L);
+            const int k = 2 * m + ((i + j + a.colour) & 1);
+            const int iu = wrap_dec(i, L), id = wrap_inc(i, L), jl = wrap_dec(j, L), jr = wrap_inc(j, L), kl = wrap_dec(k, L), kr = wrap_inc(k, L);
+            x = ((size_t)i * L + j) * L + k;
+            s = lat[x];
+            const int nd = (lat[((size_t)iu * L + j) * L + k] < 0) + (lat[((size_t)id * L + j) * L + k] < 0) +
+                           (lat[((size_t)i * L + jl) * L + k] < 0) + (lat[((size_t)i * L + jr) * L + k] < 0) +
+                           (lat[((size_t)i * L + j) * L + kl] < 0) + (lat[((size_t)i * L + j) * L + kr] < 0);
+            idx = (s < 0 ? 7 : 0) + nd;
+        } else {
+            const int W = L / 2;
+            const int ai = (int)(n / W), m = (int)(n % W);
+            const int i = 2 * ai + (a.colour >> 1), j = 2 * m + (a.colour & 1);
+            const int iu = wrap_dec(i, L), id = wrap_inc(i, L), jl = wrap_dec(j, L), jr = wrap_inc(j, L);
+            x = (size_t)i * L + j;
+            s = lat[x];
+            const int nd1 = (lat[(size_t)iu * L + j] < 0) + (lat[(size_t)id * L + j] < 0) + (lat[(size_t)i * L + jl] < 0) +
+                            (lat[(size_t)i * L + jr] < 0);
+            const int nd2 = (lat[(size_t)iu * L + jl] < 0) + (lat[(size_t)iu * L + jr] < 0) + (lat[(size_t)id * L + jl] < 0) +
+                            (lat[(size_t)id * L + jr] < 0);
+            idx = (s < 0 ? 25 : 0) + nd1 * 5 + nd2;
+        }
+        if (((always >> idx) & 1ull) || r[e] < tab[idx]) lat[x] = (int8_t)(-s);
+    }
+}
+
+__global__ void stencil_init_kernel(int8_t* lattice, long long N, int batch, uint32_t replica_offset, RoundKeys rk) {
+    const long long groups = (N + 3) >> 2;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= groups * batch) return;
+    const int b = (int)(gid / groups);
+    const uint32_t g = (uint32_t)(gid % groups);
+    uint32_t out[4];
+    philox4x32_10(rk, g, (uint32_t)b + replica_offset, 0u, (uint32_t)kDomainInit << 28, out);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        const long long p = 4ll * g + e;
+        if (p < N) lattice[(size_t)b * N + p] = (out[e] & 0x80000000u) ? (int8_t)1 : (int8_t)-1;
+    }
+}
+
+// acc[b][0..2] += (E1, E2, M) partial sums; blocks never straddle replicas.
+template <int kStencil>
+__global__ void __launch_bounds__(256) stencil_observe_kernel(const int8_t* __restrict__ lattice, int L, int bpr, long long* acc) {
+    __shared__ long long sh[3][8];
+    const int b = blockIdx.x / bpr, blk = blockIdx.x - b * bpr;
+    const long long N = kStencil == SPIN_STENCIL_CUBIC ? (long long)L * L * L : (long long)L * L;
+    const int8_t* lat = lattice + (size_t)b * N;
+    long long e1 = 0, e2 = 0, m = 0;
+    for (long long x = (long long)blk * blockDim.x + threadIdx.x; x < N; x += (long long)bpr * blockDim.x) {
+        const int s = lat[x];
+        m += s;
+        if (kStencil == SPIN_STENCIL_CUBIC) {
+            const int k = (int)(x % L), j = (int)((x / L) % L), i = (int)(x / ((long long)L * L));
+            e1 -= s * (lat[((size_t)wrap_inc(i, L) * L + j) * L + k] + lat[((size_t)i * L + wrap_inc(j, L)) * L + k] +
+                       lat[((size_t)i * L + j) * L + wrap_inc(k, L)]);
+        } else {
+            const int i = (int)(x / L), j = (int)(x % L);
+            const int id = wrap_inc(i, L), jr = wrap_inc(j, L), jl = wrap_dec(j, L);
+            e1 -= s * (lat[(size_t)id * L + j] + lat[(size_t)i * L + jr]);
+            if (kStencil == SPIN_STENCIL_TRIANGULAR) e1 -= s * lat[(size_t)id * L + jr];
+            else e2 -= s * (lat[(size_t)id * L + jl] + lat[(size_t)id * L + jr]);
+        }
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        e1 += __shfl_xor_sync(0xFFFFFFFFu, e1, o);
+        e2 += __shfl_xor_sync(0xFFFFFFFFu, e2, o);
+        m += __shfl_xor_sync(0xFFFFFFFFu, m, o);
+    }
+    if ((threadIdx.x & 31) == 0) { sh[0][threadIdx.x >> 5] = e1; sh[1][threadIdx.x >> 5] = e2; sh[2][threadIdx.x >> 5] = m; }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        long long t = 0;
+        for (int k = 0; k < (int)(blockDim.x >> 5); ++k) t += sh[threadIdx.x][k];
+        atomicAdd((unsigned long long*)acc + 3 * b + threadIdx.x, (unsigned long long)t);
+    }
+}
+
+int stencil_fail(int code, const char* msg) { return set_error(code, msg); }
+
+int check_shape(int32_t stencil, int32_t batch, int32_t L) {
+    if (batch < 1) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil: batch must be >= 1");
+    if (stencil == SPIN_STENCIL_TRIANGULAR) {
+        if (L < 3 || L % 3 != 0 || L > 65535) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil: the triangular lattice needs L % 3 == 0 (three colours on a periodic lattice), 3 <= L <= 65535");
+    } else if (stencil == SPIN_STENCIL_CUBIC) {
+        if (L < 2 || (L & 1) || L > 1624) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil: the cubic lattice needs even L, 2 <= L <= 1624");
+    } else if (stencil == SPIN_STENCIL_SQUARE_NNN) {
+        if (L < 2 || (L & 1) || L > 65536) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil: the second-neighbour square lattice needs even L, 2 <= L <= 65536");
+    } else return stencil_fail(SPIN_ERR_INVALID, "spin_stencil: unknown stencil");
+    return SPIN_OK;
+}
+
+long long total_sites(int stencil, int L) { return stencil == SPIN_STENCIL_CUBIC ? (long long)L * L * L : (long long)L * L; }
+int n_colours(int stencil) { return stencil == SPIN_STENCIL_TRIANGULAR ? 3 : stencil == SPIN_STENCIL_CUBIC ? 2 : 4; }
+
+RoundKeys keys_for(uint64_t seed) {
+    RoundKeys rk;
+    uint32_t k0 = (uint32_t)(seed & 0xFFFFFFFFull), k1 = (uint32_t)(seed >> 32);
+    for (int r = 0; r < 10; ++r) { rk.k0[r] = k0; rk.k1[r] = k1; k0 += kPhiloxW0; k1 += kPhiloxW1; }
+    return rk;
+}
+
+}  // namespace
+}  // namespace spin
+
+using namespace spin;
+
+extern "C" {
+
+size_t spin_stencil_sites(int32_t stencil, int32_t L) {
+    if (check_shape(stencil, 1, L) != SPIN_OK) return 0;
+    return (size_t)total_sites(stencil, L);
+}
+
+int spin_stencil_init(int32_t stencil, int32_t batch, int32_t L, int8_t* lattice, uint64_t seed, int64_t replica_offset,
+                      void* cuda_stream) {
+    const int rc = check_shape(stencil, batch, L);
+    if (rc != SPIN_OK) return rc;
+    if (!lattice) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil_init: NULL lattice");
+    if (replica_offset < 0 || replica_offset + (int64_t)batch > (1ll << 32)) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil: replica_offset + batch must stay within [0, 2^32]");
+    const long long N = total_sites(stencil, L), total = ((N + 3) >> 2) * batch;
+    stencil_init_kernel<<<(unsigned)((total + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(lattice, N, batch, (uint32_t)replica_offset, keys_for(seed));
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? SPIN_OK : stencil_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+}
+
+int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_t* lattice, const double* beta, double J1, double J2,
+                       double h, uint64_t seed, int64_t replica_offset, int64_t n_sweeps, int64_t sweep_offset, void* cuda_stream) {
+    const int rc = check_shape(stencil, batch, L);
+    if (rc != SPIN_OK) return rc;
+    if (!lattice || !beta) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil_sweep: NULL argument");
+    if (!std::isfinite(J1) || !std::isfinite(J2) || !std::isfinite(h)) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil_sweep: J1, J2 and h must be finite");
+    for (int b = 0; b < batch; ++b)
+        if (!std::isfinite(beta[b]) || beta[b] < 0.0) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil_sweep: beta must be finite and >= 0");
+    if (replica_offset < 0 || replica_offset + (int64_t)batch > (1ll << 32)) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil: replica_offset + batch must stay within [0, 2^32]");
+    if (n_sweeps < 0 || sweep_offset < 0 || sweep_offset > (1ll << 56) || n_sweeps > (1ll << 56) || sweep_offset + n_sweeps > (1ll << 56))
+        return stencil_fail(SPIN_ERR_INVALID, "spin_stencil_sweep: sweep range must lie in [0, 2^56]");
+    if (n_sweeps == 0) return SPIN_OK;
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    // class table per replica: dE = 2 s (J1 nn1 + J2 nn2 + h), nn = (number of neighbours) - 2 (number of -1 neighbours)
+    const int n1 = stencil == SPIN_STENCIL_SQUARE_NNN ? 4 : 6, n2 = stencil == SPIN_STENCIL_SQUARE_NNN ? 4 : 0;
+    std::vector<uint32_t> rec;
+    try { rec.assign((size_t)batch * kStencilRec, 0u); } catch (...) { return stencil_fail(SPIN_ERR_NOMEM, "spin_stencil_sweep: out of host memory"); }
+    for (int b = 0; b < batch; ++b) {
+        uint32_t* r = rec.data() + (size_t)b * kStencilRec;
+        unsigned long long always = 0ull;
+        for (int d = 0; d < 2; ++d)
+            for (int nd1 = 0; nd1 <= n1; ++nd1)
+                for (int nd2 = 0; nd2 <= n2; ++nd2) {
+                    const int idx = d * (n1 + 1) * (n2 + 1) + nd1 * (n2 + 1) + nd2;
+                    const double sgn = d ? -1.0 : 1.0;
+                    const double dE = 2.0 * sgn * (J1 * (double)(n1 - 2 * nd1) + J2 * (double)(n2 - 2 * nd2) + h);
+                    uint32_t T[1];
+                    uint8_t al[1];
+                    // the arithmetic of row a1 (spin_threshold_table): a one-class "Potts table" with dn = -dE, J = 1
+                    const double x = beta[b] * dE;
+                    if (x <= 0.0) { al[0] = 1; T[0] = 0xFFFFFFFFu; }
+                    else {
+                        const double v = std::floor(std::exp(-x) * 4294967296.0);
+                        al[0] = 0;
+                        T[0] = v >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)v;
+                    }
+                    r[idx] = T[0];
+                    if (al[0]) always |= 1ull << idx;
+                }
+        r[62] = (uint32_t)always;
+        r[63] = (uint32_t)(always >> 32);
+    }
+    uint32_t* d_tab = nullptr;
+    cudaError_t e = cudaMallocAsync(&d_tab, rec.size() * sizeof(uint32_t), s);
+    if (e != cudaSuccess) return stencil_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+    e = cudaMemcpyAsync(d_tab, rec.data(), rec.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, s);   // pageable: staged before return
+    StencilArgs a;
+    a.lattice = lattice; a.tables = d_tab; a.stencil = stencil; a.batch = batch; a.L = L;
+    a.replica_offset = (uint32_t)replica_offset; a.rk = keys_for(seed);
+    const long long total = ((colour_sites(stencil, L) + 3) >> 2) * batch;
+    const unsigned grid = (unsigned)((total + 127) / 128);
+    const int nc = n_colours(stencil);
+    for (int64_t t = sweep_offset; t < sweep_offset + n_sweeps && e == cudaSuccess; ++t)
+        for (int c = 0; c < nc; ++c) {
+            a.colour = c;
+            a.c2 = (uint32_t)((uint64_t)t & 0xFFFFFFFFull);
+            a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)c << 24) | (kDomainStencil << 28);
+            if (stencil == SPIN_STENCIL_TRIANGULAR) stencil_pass_kernel<SPIN_STENCIL_TRIANGULAR><<<grid, 128, 0, s>>>(a);
+            else if (stencil == SPIN_STENCIL_CUBIC) stencil_pass_kernel<SPIN_STENCIL_CUBIC><<<grid, 128, 0, s>>>(a);
+            else stencil_pass_kernel<SPIN_STENCIL_SQUARE_NNN><<<grid, 128, 0, s>>>(a);
+        }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    cudaFreeAsync(d_tab, s);
+    return e == cudaSuccess ? SPIN_OK : stencil_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+}
+
+int spin_stencil_observables(int32_t stencil, int32_t batch, int32_t L, const int8_t* lattice, int64_t* E1, int64_t* E2,
+                             int64_t* M, void* cuda_stream) {
+    const int rc = check_shape(stencil, batch, L);
+    if (rc != SPIN_OK) return rc;
+    if (!lattice) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil_observables: NULL lattice");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    long long* d_acc = nullptr;
+    std::vector<long long> host;
+    try { host.assign((size_t)batch * 3, 0); } catch (...) { return stencil_fail(SPIN_ERR_NOMEM, "spin_stencil_observables: out of host memory"); }
+    cudaError_t e = cudaMallocAsync(&d_acc, sizeof(long long) * 3 * batch, s);
+    if (e != cudaSuccess) return stencil_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+    e = cudaMemsetAsync(d_acc, 0, sizeof(long long) * 3 * batch, s);
+    const long long N = total_sites(stencil, L);
+    long long want = (N + 255) / 256, cap = (148ll * 16 + batch - 1) / batch;
+    const int bpr = (int)(want < cap ? want : (cap < 1 ? 1 : cap));
+    const unsigned grid = (unsigned)((long long)bpr * batch);
+    if (stencil == SPIN_STENCIL_TRIANGULAR) stencil_observe_kernel<SPIN_STENCIL_TRIANGULAR><<<grid, 256, 0, s>>>(lattice, L, bpr, d_acc);
+    else if (stencil == SPIN_STENCIL_CUBIC) stencil_observe_kernel<SPIN_STENCIL_CUBIC><<<grid, 256, 0, s>>>(lattice, L, bpr, d_acc);
+    else stencil_observe_kernel<SPIN_STENCIL_SQUARE_NNN><<<grid, 256, 0, s>>>(lattice, L, bpr, d_acc);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaMemcpyAsync(host.data(), d_acc, sizeof(long long) * 3 * batch, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    cudaFreeAsync(d_acc, s);
+    if (e != cudaSuccess) return stencil_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+    for (int b = 0; b < batch; ++b) {
+        if (E1) E1[b] = host[3 * b];
+        if (E2) E2[b] = host[3 * b + 1];
+        if (M) M[b] = host[3 * b + 2];
+    }
+    return SPIN_OK;
+}
+
+}  // extern "C"
