@@ -12,7 +12,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "spin_oracle.cpp")
 _SRCS = [_SRC, os.path.join(_HERE, "dmc_oracle.cpp"), os.path.join(_HERE, "general_oracle.cpp"),
-         os.path.join(_HERE, "stencil_oracle.cpp")]
+         os.path.join(_HERE, "stencil_oracle.cpp"), os.path.join(_HERE, "cpm_oracle.cpp")]
 _LIB = os.path.join(_HERE, "liboracle.so")
 
 __all__ = [
@@ -24,6 +24,7 @@ __all__ = [
     "sweep_potts_general", "potts_general_observables", "sweep_schedule",
     "STENCIL_TRIANGULAR", "STENCIL_CUBIC", "STENCIL_SQUARE_NNN", "stencil_shape", "stencil_init", "stencil_colour_pass",
     "stencil_sweep", "stencil_observables",
+    "cpm_delta", "cpm_colour_pass", "cpm_sweep", "cpm_observables",
 ]
 
 
@@ -78,6 +79,13 @@ def _l():
         lib.oracle_stencil_sweep.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, d, d, d, c.c_uint64, c.c_int64,
                                              c.c_int64, c.c_int64]
         lib.oracle_stencil_observables.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, p, p]
+        lib.oracle_cpm_delta.argtypes = [p, c.c_int32, c.c_int32, p, p, c.c_int32, c.c_int64, p, c.c_int32, c.c_int32, c.c_int32]
+        lib.oracle_cpm_delta.restype = c.c_int64
+        lib.oracle_cpm_colour_pass.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, p, c.c_int32, c.c_int64, p, p,
+                                               c.c_uint64, c.c_int64, c.c_int64, c.c_int32]
+        lib.oracle_cpm_sweep.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, p, c.c_int32, c.c_int64, p, p, c.c_uint64,
+                                         c.c_int64, c.c_int64, c.c_int64]
+        lib.oracle_cpm_observables.argtypes = [p, c.c_int32, c.c_int32, c.c_int32, p, p, c.c_int32, c.c_int64, p, p, p, p, p]
         lib.oracle_dmc_half_sweep.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
                                               c.c_int32, p]
         lib.oracle_dmc_forward.argtypes = [p, p, p, c.c_int32, c.c_int32, d, p, d, c.c_uint64, c.c_int64, c.c_int64,
@@ -396,3 +404,47 @@ def stencil_observables(stencil, spins):
     E1, E2, M = (np.zeros(B, dtype=np.int64) for _ in range(3))
     _l().oracle_stencil_observables(_ptr(spins), stencil, B, L, _ptr(E1), _ptr(E2), _ptr(M))
     return E1, E2, M
+
+
+# ---- Cellular Potts model (cpm_oracle.cpp; Eq. 7, Table II) ----------------------------------------
+def _cpm_params(tau, Jtab, A):
+    tau = np.ascontiguousarray(tau, dtype=np.int32)
+    Jtab = np.ascontiguousarray(Jtab, dtype=np.int32)
+    A = np.ascontiguousarray(A, dtype=np.int32)
+    q, nt = tau.shape[0], Jtab.shape[0]
+    assert Jtab.shape == (nt, nt) and A.shape == (q,) and tau.min() >= 0 and tau.max() < nt
+    return tau, Jtab, A, q, nt
+
+
+def cpm_delta(lat, tau, Jtab, lam, A, i, j, new):
+    """dH of the proposal lat[i][j] -> new on one lattice [L][L] (areas counted from lat)."""
+    tau, Jtab, A, q, nt = _cpm_params(tau, Jtab, A)
+    assert lat.dtype == np.int8 and lat.ndim == 2 and lat.flags["C_CONTIGUOUS"]
+    return int(_l().oracle_cpm_delta(_ptr(lat), lat.shape[0], q, _ptr(tau), _ptr(Jtab), nt, int(lam), _ptr(A), int(i), int(j), int(new)))
+
+
+def cpm_colour_pass(spins, tau, Jtab, lam, A, beta, seed, t, colour, replica_offset=0):
+    B, L = _lattice(spins)
+    tau, Jtab, A, q, nt = _cpm_params(tau, Jtab, A)
+    ba = _beta_array(beta, B)
+    _l().oracle_cpm_colour_pass(_ptr(spins), B, L, q, _ptr(tau), _ptr(Jtab), nt, int(lam), _ptr(A), _ptr(ba), int(seed),
+                                int(replica_offset), int(t), int(colour))
+
+
+def cpm_sweep(spins, tau, Jtab, lam, A, beta, seed, n_sweeps, sweep_offset=0, replica_offset=0):
+    B, L = _lattice(spins)
+    tau, Jtab, A, q, nt = _cpm_params(tau, Jtab, A)
+    ba = _beta_array(beta, B)
+    _l().oracle_cpm_sweep(_ptr(spins), B, L, q, _ptr(tau), _ptr(Jtab), nt, int(lam), _ptr(A), _ptr(ba), int(seed),
+                          int(replica_offset), int(n_sweeps), int(sweep_offset))
+
+
+def cpm_observables(spins, tau, Jtab, lam, A):
+    """-> (H_adh [B], H_area [B], areas [B][q], boundary [B][ntypes][ntypes]) int64."""
+    B, L = _lattice(spins)
+    tau, Jtab, A, q, nt = _cpm_params(tau, Jtab, A)
+    Ha, Hr = np.zeros(B, dtype=np.int64), np.zeros(B, dtype=np.int64)
+    ar, bl = np.zeros((B, q), dtype=np.int64), np.zeros((B, nt, nt), dtype=np.int64)
+    _l().oracle_cpm_observables(_ptr(spins), B, L, q, _ptr(tau), _ptr(Jtab), nt, int(lam), _ptr(A), _ptr(Ha), _ptr(Hr),
+                                _ptr(ar), _ptr(bl))
+    return Ha, Hr, ar, bl

@@ -72,3 +72,24 @@ def random_potts_lattice(batch, L, q, seed):
     for b in range(batch):
         out[b] = rng.integers(0, int(q[b]), size=(L, L), dtype=np.int8)
     return out
+
+
+# ---- Cellular Potts model inputs (three cell types, 37 identifiers, Table II, k_B T = 8, A = 25, lambda = 1)
+CPM_TABLE_II = np.array([[0, 16, 16], [16, 2, 11], [16, 11, 14]], dtype=np.int32)   # medium, light, dark (symmetric)
+
+
+def cpm_initial(batch, L, cells_per_side=6, cell_size=5, seed=0):
+    """'An arbitrary aggregate of square-shaped cells': cells_per_side^2 square cells of cell_size^2 sites
+    in the middle of an L x L medium, identifiers 1.., types light (1) / dark (2) drawn with a numpy generator.
+    -> (lattice int8 [batch][L][L], tau int32 [q], target areas int32 [q])."""
+    n = cells_per_side * cells_per_side
+    assert n + 1 <= 127 and cells_per_side * cell_size <= L and L % 2 == 0
+    rng = np.random.default_rng(seed)
+    tau = np.concatenate([[0], rng.integers(1, 3, size=n)]).astype(np.int32)
+    A = np.concatenate([[0], np.full(n, cell_size * cell_size)]).astype(np.int32)
+    lat = np.zeros((L, L), dtype=np.int8)
+    o = (L - cells_per_side * cell_size) // 2
+    for a in range(cells_per_side):
+        for b in range(cells_per_side):
+            lat[o + a * cell_size:o + (a + 1) * cell_size, o + b * cell_size:o + (b + 1) * cell_size] = 1 + a * cells_per_side + b
+    return np.ascontiguousarray(np.broadcast_to(lat, (batch, L, L))), tau, A
