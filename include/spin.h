@@ -278,6 +278,28 @@ SPIN_API int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_
 SPIN_API int spin_stencil_observables(int32_t stencil, int32_t batch, int32_t L, const int8_t* lattice, int64_t* E1,
                                       int64_t* E2, int64_t* M, void* cuda_stream);
 
+/* ---------------------------------------------------------------------------------------------
+ * Cellular Potts model (Eq. 7 and Table II of the paper):
+ *   H = 1/2 sum_x sum_{y in Moore(x)} J[tau(s_x)][tau(s_y)] (1 - delta(s_x, s_y)) + lambda sum_{cells s >= 1} (a_s - A_s)^2
+ * on a DEVICE int8 lattice [batch][L][L] of cell identifiers 0..q-1 (0 = the medium, whose area is unconstrained), L even,
+ * periodic.  tau: HOST int32 [q], type of each identifier (0..ntypes-1, ntypes <= 4); Jtab: HOST int32 [ntypes][ntypes],
+ * symmetric; A: HOST int32 [q] target areas; lambda: integer >= 0 (readings C1-C9: integer
+ * parameters make dH an exact integer).  A sweep = four colour passes (colour 2 (i & 1) + (j & 1)); in a pass every
+ * site of the colour copies one of its eight Moore neighbours (chosen by r_prop >> 29) with the acceptance of Alg. 1
+ * on dH = adhesion change + lambda [(new != 0)(2 (a_new - A_new) + 1) + (old != 0)(-2 (a_old - A_old) + 1)], the areas
+ * counted at the start of the pass.  beta: HOST [batch] (= 1 / k_B T; the paper runs k_B T = 8).  Asynchronous.
+ * SPIN_ERR_UNSUPPORTED when 0 < beta is so small that exp(-beta dH) 2^32 >= 1 beyond dH = 65536.
+ * ------------------------------------------------------------------------------------------- */
+SPIN_API int spin_cpm_sweep(int32_t batch, int32_t L, int32_t q, int8_t* lattice, const int32_t* tau, const int32_t* Jtab,
+                            int32_t ntypes, int64_t lambda, const int32_t* A, const double* beta, uint64_t seed,
+                            int64_t replica_offset, int64_t n_sweeps, int64_t sweep_offset, void* cuda_stream);
+/* H_adh[b] = first term of Eq. 7 (every unordered Moore pair once), H_area[b] = second term, areas: [batch][q],
+ * boundary: [batch][ntypes][ntypes], number of unordered Moore pairs with different identifiers and types (t, t'), stored
+ * at [min][max] (the boundary lengths of the paper's Fig. 6).  HOST int64 arrays, any may be NULL.  Synchronises. */
+SPIN_API int spin_cpm_observables(int32_t batch, int32_t L, int32_t q, const int8_t* lattice, const int32_t* tau,
+                                  const int32_t* Jtab, int32_t ntypes, int64_t lambda, const int32_t* A, int64_t* H_adh,
+                                  int64_t* H_area, int64_t* areas, int64_t* boundary, void* cuda_stream);
+
 /* Measurement aid ("second, tighter denominator"): runs a register-only kernel on the current
  * device that does nothing but the algorithmic work of the sweep - Philox-4x32-10 calls (precomputed round keys) whose
  * four output words are each compared with a threshold - and returns the best-of-5 rate in random words per

@@ -21,7 +21,8 @@ __all__ = [
     "SPIN_POLICY_AUTO", "SPIN_POLICY_STREAMING", "SPIN_POLICY_RESIDENT",
     "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim", "spin_measure_philox_compare_rate",
     "SPIN_DTYPE_F32", "SPIN_DTYPE_F64", "SPIN_STENCIL_TRIANGULAR", "SPIN_STENCIL_CUBIC", "SPIN_STENCIL_SQUARE_NNN",
-    "spin_stencil_sites", "spin_stencil_init", "spin_stencil_sweep", "spin_stencil_observables", "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
+    "spin_stencil_sites", "spin_stencil_init", "spin_stencil_sweep", "spin_stencil_observables",
+    "spin_cpm_sweep", "spin_cpm_observables", "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
     "spin_create", "spin_create_ex",
 ]
 
@@ -73,6 +74,8 @@ def load_library():
         "spin_stencil_init": (c.c_int, [i32, i32, i32, vp, u64, i64, vp]),
         "spin_stencil_sweep": (c.c_int, [i32, i32, i32, vp, vp, dbl, dbl, dbl, u64, i64, i64, i64, vp]),
         "spin_stencil_observables": (c.c_int, [i32, i32, i32, vp, vp, vp, vp, vp]),
+        "spin_cpm_sweep": (c.c_int, [i32, i32, i32, vp, vp, vp, i32, i64, vp, vp, u64, i64, i64, i64, vp]),
+        "spin_cpm_observables": (c.c_int, [i32, i32, i32, vp, vp, vp, i32, i64, vp, vp, vp, vp, vp, vp]),
         "spin_dmc_forward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp]),
         "spin_dmc_backward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp, vp, vp, vp, vp]),
         "spin_dmc_discretise": (c.c_int, [i32, vp, i64, vp]),
@@ -93,6 +96,7 @@ EXPORTED_SYMBOLS = (
     "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
     "spin_set_couplings", "spin_energy_general", "spin_potts_label_sum", "spin_sweep_schedule",
     "spin_stencil_sites", "spin_stencil_init", "spin_stencil_sweep", "spin_stencil_observables",
+    "spin_cpm_sweep", "spin_cpm_observables",
 )
 
 
@@ -175,6 +179,34 @@ def spin_stencil_observables(stencil, batch, L, lattice_ptr, cuda_stream=None):
     _check(load_library().spin_stencil_observables(stencil, batch, L, lattice_ptr, _np_ptr(E1), _np_ptr(E2), _np_ptr(M),
                                                    cuda_stream))
     return E1, E2, M
+
+
+def _cpm_arrays(tau, Jtab, A):
+    tau = np.ascontiguousarray(tau, dtype=np.int32)
+    Jtab = np.ascontiguousarray(Jtab, dtype=np.int32)
+    A = np.ascontiguousarray(A, dtype=np.int32)
+    assert Jtab.ndim == 2 and Jtab.shape[0] == Jtab.shape[1] and A.shape == tau.shape
+    return tau, Jtab, A
+
+
+def spin_cpm_sweep(batch, L, lattice_ptr, tau, Jtab, lam, A, beta, seed, n_sweeps, sweep_offset=0, replica_offset=0,
+                   cuda_stream=None):
+    tau, Jtab, A = _cpm_arrays(tau, Jtab, A)
+    b = _beta64(beta, batch)
+    _check(load_library().spin_cpm_sweep(batch, L, tau.shape[0], lattice_ptr, _np_ptr(tau), _np_ptr(Jtab), Jtab.shape[0],
+                                         int(lam), _np_ptr(A), _np_ptr(b), int(seed), int(replica_offset), int(n_sweeps),
+                                         int(sweep_offset), cuda_stream))
+
+
+def spin_cpm_observables(batch, L, lattice_ptr, tau, Jtab, lam, A, cuda_stream=None):
+    """-> (H_adh [B], H_area [B], areas [B][q], boundary [B][ntypes][ntypes]) int64."""
+    tau, Jtab, A = _cpm_arrays(tau, Jtab, A)
+    q, nt = tau.shape[0], Jtab.shape[0]
+    Ha, Hr = np.zeros(batch, dtype=np.int64), np.zeros(batch, dtype=np.int64)
+    ar, bl = np.zeros((batch, q), dtype=np.int64), np.zeros((batch, nt, nt), dtype=np.int64)
+    _check(load_library().spin_cpm_observables(batch, L, q, lattice_ptr, _np_ptr(tau), _np_ptr(Jtab), nt, int(lam), _np_ptr(A),
+                                               _np_ptr(Ha), _np_ptr(Hr), _np_ptr(ar), _np_ptr(bl), cuda_stream))
+    return Ha, Hr, ar, bl
 
 
 def spin_dmc_discretise(dtype, s_ptr, n, cuda_stream=None):
