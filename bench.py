@@ -468,6 +468,61 @@ def general_entries(runner, sp, args, peaks, measured):
     return out
 
 
+def _time_calls(runner, args, fn):
+    """warm-up + timed steps of fn(k) on the runner's stream -> ms per step (numpy array)."""
+    torch, stream = runner.torch, runner.stream
+    for k in range(args.warmup):
+        fn(k)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    for k in range(args.steps):
+        with torch.cuda.stream(stream):
+            runner.flush.fill_(k)
+        ev[k][0].record(stream)
+        fn(args.warmup + k)
+        ev[k][1].record(stream)
+    torch.cuda.synchronize()
+    return np.array([a.elapsed_time(b) for a, b in ev])
+
+
+def _alu_entry(name, workload, updates, ms, ops, words, kernel, launches, peaks, measured):
+    vals = updates / (ms * 1e6)
+    rate = updates / (float(ms.mean()) * 1e6)
+    return {"workload": workload, "value": float(updates * len(ms) / (ms.sum() * 1e6)), "unit": UNIT, "best": float(vals.max()),
+            "median": float(np.median(vals)), "ms_per_step": float(ms.mean()), "kernel": kernel, "gpu_launches_per_step": launches,
+            "roofline": {"bound": "alu", "frac": float(ops * rate * 1e9 / 1e12 / alu_peak(peaks)), "ops_per_update": ops,
+                         "frac_of_measured": float(rate * words / measured) if measured else None}}
+
+
+def stencil_cpm_entries(runner, sp, args, peaks, measured):
+    """SURVEY.md 8(f) #4 (triangular, cubic, second-neighbour lattices) and #3 (cellular Potts, the paper's set-up)."""
+    torch, stream = runner.torch, runner.stream
+    out = {}
+    n = args.sweeps or 20
+    for key, stencil, B, L in (("F4-triangular", sp.SPIN_STENCIL_TRIANGULAR, 16, 768), ("F4-cubic", sp.SPIN_STENCIL_CUBIC, 8, 128),
+                               ("F4-square-nnn", sp.SPIN_STENCIL_SQUARE_NNN, 16, 1024)):
+        sites = sp.spin_stencil_sites(stencil, L)
+        lat = torch.empty(B * sites, dtype=torch.int8, device="cuda")
+        sp.spin_stencil_init(stencil, B, L, lat.data_ptr(), 21, cuda_stream=stream.cuda_stream)
+        beta = np.full(B, 0.25 if stencil != sp.SPIN_STENCIL_SQUARE_NNN else 0.35)
+        ms = _time_calls(runner, args, lambda k: sp.spin_stencil_sweep(stencil, B, L, lat.data_ptr(), beta, 1.0, 0.2, 0.0, 21, n,
+                                                                       sweep_offset=k * n, cuda_stream=stream.cuda_stream))
+        ncol = {sp.SPIN_STENCIL_TRIANGULAR: 3, sp.SPIN_STENCIL_CUBIC: 2, sp.SPIN_STENCIL_SQUARE_NNN: 4}[stencil]
+        out[key] = _alu_entry(key, "%s: Ising, batch %d, L = %d (%d sites per replica), %d sweeps" % (key, B, L, sites, n),
+                              float(B) * sites * n, ms, 11.0, 1.0, "stencil_pass_kernel", ncol * n, peaks, measured)
+    B, L = 256, 64
+    spins, tau, A = sp.workloads.cpm_initial(B, L, 6, 5, seed=5)
+    lat = torch.from_numpy(spins.copy()).cuda()
+    beta = np.full(B, 1.0 / 8.0)
+    nc = args.sweeps or 50
+    ms = _time_calls(runner, args, lambda k: sp.spin_cpm_sweep(B, L, lat.data_ptr(), tau, sp.workloads.CPM_TABLE_II, 1, A, beta, 5, nc,
+                                                               sweep_offset=k * nc, cuda_stream=stream.cuda_stream))
+    out["F3-cpm"] = _alu_entry("F3-cpm", "CPM: Table II, 36 cells + medium, k_B T = 8, A = 25, lambda = 1, batch %d x %d^2, %d sweeps "
+                               "(copy attempts)" % (B, L, nc), float(B) * L * L * nc, ms, 21.0, 2.0,
+                               "cpm_area_kernel + cpm_pass_kernel", 8 * nc, peaks, measured)
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -574,6 +629,7 @@ def main():
             line["per_config"] = per_config_block(runner, sp, args, peaks, measured)
             line["per_config"].update(dmc_entries(runner, sp, args, peaks))
             line["per_config"].update(general_entries(runner, sp, args, peaks, measured))
+            line["per_config"].update(stencil_cpm_entries(runner, sp, args, peaks, measured))
         if not args.no_cpu_baseline and world == 1:
             v, threads, sample, _ = oracle_throughput(w, 12.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,
