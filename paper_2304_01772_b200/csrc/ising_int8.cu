@@ -151,12 +151,19 @@ __device__ __forceinline__ uint4 update_row(const RoundKeys& rk, uint32_t c2, ui
     return res;
 }
 
+// Loads of lattice words.  The two-launches-per-sweep kernels read the other colour through the read-only path (it is
+// constant during a launch); the persistent kernel below runs many half-sweeps in one launch, so everything another
+// SM may have written since this SM last read it must bypass the (non-coherent) L1: ld.global.cg.
+template <bool kCoherent> __device__ __forceinline__ uint4 ld4(const uint4* p) { return kCoherent ? __ldcg(p) : __ldg(p); }
+template <bool kCoherent> __device__ __forceinline__ uint32_t ld1(const uint32_t* p) { return kCoherent ? __ldcg(p) : __ldg(p); }
+template <bool kCoherent> __device__ __forceinline__ uint4 ldown(const uint4* p) { return kCoherent ? __ldcg(p) : *p; }
+
 __device__ __forceinline__ uint4 mask4(const uint4& v) {
     const uint32_t m = 0x04040404u;      // 4 per -1 spin
     return make_uint4(v.x & m, v.y & m, v.z & m, v.w & m);
 }
 
-template <int kColour, bool kHasNever, int kRows>
+template <int kColour, bool kHasNever, int kRows, bool kPersist = false>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, uint32_t slot, int b, int rb,
                                            int x) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
@@ -180,31 +187,31 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     // even rows of the block have parity kColour, odd rows 1 - kColour (i0 is even)
     const uint32_t* pEdgeEven = oth1 + (size_t)i0 * W4 + (kColour ? eNext : ePrev);
     const uint32_t* pEdgeOdd = oth1 + (size_t)(i0 + 1) * W4 + (kColour ? ePrev : eNext);
-    uint4 wU = mask4(__ldg(oth4 + (size_t)iu * W16 + x));     // masked other-colour rows i-1, i, i+1
-    uint4 wC = mask4(__ldg(pOth - 2 * rowStride));
-    uint4 wD = mask4(__ldg(pOth - rowStride));
-    uint4 own = *pOwn;
-    uint32_t edge = __ldg(pEdgeEven) & 0x04040404u;
+    uint4 wU = mask4(ld4<kPersist>(oth4 + (size_t)iu * W16 + x));     // masked other-colour rows i-1, i, i+1
+    uint4 wC = mask4(ld4<kPersist>(pOth - 2 * rowStride));
+    uint4 wD = mask4(ld4<kPersist>(pOth - rowStride));
+    uint4 own = ldown<kPersist>(pOwn);
+    uint32_t edge = ld1<kPersist>(pEdgeEven) & 0x04040404u;
     uint32_t g0 = (uint32_t)i0 * (uint32_t)W4 + 4u * (uint32_t)x;
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
-    __syncthreads();    // the block's threshold table (filled by the caller) is first read below: the loads above
-                        // are already in flight while the block waits for it
+    if (!kPersist) __syncthreads();   // the block's threshold table (filled by the caller) is first read below: the loads
+                                      // above are already in flight while the block waits for it
     // Two rows per iteration (the side-neighbour parity alternates); the four iterations of an 8-row thread are
     // unrolled so that the register window rotates by renaming instead of moves (measured: +2.5 % over the rolled loop).
 #pragma unroll 4
     for (int rr = 0; rr < kRows; rr += 2) {
         const bool more = rr + 2 < kRows;
         // inputs of the odd row i+1: other-colour row i+2 (the only one that can wrap), own row i+1, its edge word
-        const uint4 n1 = __ldg(more ? pOth : pOthLast);
-        const uint4 own1 = *(pOwn + rowStride);
-        const uint32_t edge1 = __ldg(pEdgeOdd);
+        const uint4 n1 = ld4<kPersist>(more ? pOth : pOthLast);
+        const uint4 own1 = ldown<kPersist>(pOwn + rowStride);
+        const uint32_t edge1 = ld1<kPersist>(pEdgeOdd);
         // inputs of the next even row i+2: other-colour row i+3, own row i+2, its edge word
         uint4 n2 = n1, own2 = own1;
         uint32_t edge2 = edge1;
         if (more) {
-            n2 = __ldg(pOth + rowStride);
-            own2 = *(pOwn + 2 * rowStride);
-            edge2 = __ldg(pEdgeEven + edgeStride2);
+            n2 = ld4<kPersist>(pOth + rowStride);
+            own2 = ldown<kPersist>(pOwn + 2 * rowStride);
+            edge2 = ld1<kPersist>(pEdgeEven + edgeStride2);
         }
         uint4 res = update_row<kHasNever, kColour>(a.rk, a.c2, a.c3, own, wU, wC, wD, edge, g0, c1, stab, slot);
         *pOwn = res;
@@ -245,6 +252,65 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_kern
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
     if (never) march_rows<kColour, true, kRows>(a, stab, slot, b, rb, x);
     else march_rows<kColour, false, kRows>(a, stab, slot, b, rb, x);
+}
+
+// ---- persistent kernel for launch-bound shapes (lattices too big for one CTA's shared memory, too small for a
+// half-sweep to hide a kernel launch: the paper's own Table III sizes).  All sweeps of a call run in
+// ONE cooperative launch: the grid is what fits on the GPU at once, every block loops over its share of the
+// (replica, row block, strip) work items with the same march_rows code, and the half-sweeps are separated by a grid-wide
+// barrier (one atomic arrive + an acquire spin per block, ~1 us) instead of a kernel boundary (~2.7 us with PDL).  The
+// lattice stays in L2.  Work items are assigned statically (item v -> block v % gridDim), so a word is always written
+// by the same block.  Only tables without never-classes take this path (the host falls back to streaming otherwise).
+__device__ __forceinline__ void grid_barrier(unsigned int* counter, unsigned int& target) {
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        target += gridDim.x;
+        __threadfence();                                   // this block's lattice writes are visible before it arrives
+        atomicAdd(counter, 1u);
+        unsigned int seen;
+        do {
+            asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(seen) : "l"(counter) : "memory");
+        } while ((int)(seen - target) < 0);
+    }
+    __syncthreads();
+}
+
+template <int kRows>
+__global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_persistent_kernel(SweepArgs a, int bpr, int items,
+                                                                                         unsigned long long t0,
+                                                                                         long long n_sweeps,
+                                                                                         unsigned int* counter) {
+    __shared__ uint32_t stab[kTableStride];
+    __shared__ uint32_t sidx[4 * kRowsThreads];
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
+    const int W16 = a.L >> 5;
+    const int perReplica = (a.L / kRows) * W16;
+    unsigned int target = 0u;
+    int loaded = -1;                                        // replica whose table is in stab
+    for (long long s = 0; s < n_sweeps; ++s) {
+        const unsigned long long t = t0 + (unsigned long long)s;
+        a.c2 = (uint32_t)(t & 0xFFFFFFFFull);
+#pragma unroll 1
+        for (int colour = 0; colour < 2; ++colour) {
+            a.c3 = (uint32_t)((t >> 32) & 0xFFFFFFull) | ((uint32_t)colour << 24) | (kDomainIsing << 28);
+            for (int v = blockIdx.x; v < items; v += gridDim.x) {
+                const int b = v / bpr, blk = v - b * bpr;
+                if (b != loaded) {                          // block-uniform
+                    __syncthreads();
+                    for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
+                    __syncthreads();
+                    loaded = b;
+                }
+                const int u = blk * blockDim.x + threadIdx.x;
+                if (u < perReplica) {
+                    const int rb = u / W16, x = u - rb * W16;
+                    if (colour == 0) march_rows<0, false, kRows, true>(a, stab, slot, b, rb, x);
+                    else march_rows<1, false, kRows, true>(a, stab, slot, b, rb, x);
+                }
+            }
+            grid_barrier(counter, target);
+        }
+    }
 }
 
 // ---- shared-memory-resident kernel: L % 32 == 0 and the replica (L^2 bytes) fits one CTA's shared memory.
@@ -475,6 +541,39 @@ static size_t resident_smem_bytes(int L) {
 }
 
 bool ising_int8_resident_fits(int L) { return L % 32 == 0 && (size_t)L * L <= kResMaxLatticeBytes; }
+
+// Cooperative launch of the persistent kernel: n_sweeps sweeps from t0 in one launch.  counter: one zeroed device
+// word.  Returns the number of kernels launched (1), or 0 when the shape does not qualify / the launch is refused (the
+// caller then uses the streaming path).
+int launch_ising_int8_persistent(const SweepArgs& a, unsigned long long t0, long long n_sweeps, unsigned int* counter,
+                                 cudaStream_t s) {
+    if (a.L % 32 != 0) return 0;
+    const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 5) * a.batch;
+    const bool shortRows = longThreads < 148ll * 4 * kRowsThreads || (a.L / kRowsLong) * (a.L >> 5) < kRowsThreads / 2;
+    const int rows = shortRows ? kRowsShort : kRowsLong;
+    const int perReplica = (a.L / rows) * (a.L >> 5);
+    const int tpb = pick_block(perReplica);
+    int bpr = (perReplica + tpb - 1) / tpb;
+    int items = bpr * a.batch;
+    void (*kern)(SweepArgs, int, int, unsigned long long, long long, unsigned int*) =
+        shortRows ? ising_int8_persistent_kernel<kRowsShort> : ising_int8_persistent_kernel<kRowsLong>;
+    int dev = 0, sms = 0, perSm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&perSm, kern, tpb, 0) != cudaSuccess || perSm < 1) {
+        cudaGetLastError();
+        return 0;
+    }
+    int grid = sms * perSm;
+    if (grid > items) grid = items;
+    SweepArgs args = a;
+    void* params[] = {&args, &bpr, &items, &t0, &n_sweeps, &counter};
+    if (cudaMemsetAsync(counter, 0, sizeof(unsigned int), s) != cudaSuccess ||
+        cudaLaunchCooperativeKernel((void*)kern, dim3((unsigned)grid), dim3((unsigned)tpb), params, 0, s) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    return 1;
+}
 
 // Opt the resident kernel in to more than 48 KiB of dynamic shared memory on the CURRENT device (called once per
 // handle at creation: the attribute is per device, and cheap to set again).

@@ -121,14 +121,23 @@ __device__ __forceinline__ void site_step(uint32_t& acc_mask, uint32_t o, uint32
 }
 
 // One 4-site word: r0 feeds sites 0, 1 (proposal words r0[0], r0[2]; acceptance words r0[1], r0[3]), r1 sites 2, 3.
-template <bool kHasNever, bool kSmallQ, int kJ>
+// kPow2: q - 1 is a power of two 2^k <= 8 (q = 2, 3, 5, 9): floor(r (q-1) / 2^32) is the top k bits of r, so the four
+// proposal offsets of a word come from the top bytes of the four words with three PRMT, a shift and a mask
+// (dshift = 8 - k, dmask = (2^k - 1) per byte) instead of four IMAD.HI (half-rate) and three merges.
+template <bool kHasNever, bool kSmallQ, bool kPow2, int kJ>
 __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t ct, uint32_t sd,
                                                 const uint32_t r0[4], const uint32_t r1[4], uint32_t q, uint32_t geAdd,
+                                                uint32_t dshift, uint32_t dmask,
                                                 const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
     // proposal (O6): new = old + 1 + floor(r_prop (q-1) / 2^32), minus q if >= q
     const uint32_t qm1 = q - 1u;
-    const uint32_t d = __umulhi(r0[0], qm1) | (__umulhi(r0[2], qm1) << 8) | (__umulhi(r1[0], qm1) << 16) |
-                       (__umulhi(r1[2], qm1) << 24);
+    uint32_t d;
+    if (kPow2) {
+        const uint32_t t01 = __byte_perm(r0[0], r0[2], 0x0073), t23 = __byte_perm(r1[0], r1[2], 0x0073);
+        d = (__byte_perm(t01, t23, 0x5410) >> dshift) & dmask;
+    } else {
+        d = __umulhi(r0[0], qm1) | (__umulhi(r0[2], qm1) << 8) | (__umulhi(r1[0], qm1) << 16) | (__umulhi(r1[2], qm1) << 24);
+    }
     uint32_t nw = own + 0x01010101u + d;                              // <= 2q-2 per byte
     const uint32_t ge = ((nw + geAdd) >> 7) & 0x01010101u;            // 1 where nw >= q (geAdd = (0x80 - q) per byte)
     nw -= ge * q;
@@ -150,10 +159,11 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
 
 // One row of one strip.  up / ct / dn: other-colour words of rows i-1, i, i+1; kParity = 1: the side neighbour of
 // site k is other[i][k+1], else other[i][k-1]; `edge` is the 32-bit word holding the 17th byte.
-template <bool kHasNever, bool kSmallQ, int kParity>
+template <bool kHasNever, bool kSmallQ, bool kPow2, int kParity>
 __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const uint4& up, const uint4& ct,
                                             const uint4& dn, uint32_t edge, uint32_t g0, uint32_t c1, uint32_t q,
-                                            uint32_t geAdd, const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
+                                            uint32_t geAdd, uint32_t dshift, uint32_t dmask, const uint32_t* stab,
+                                            const uint32_t* snever, uint32_t slot) {
     uint32_t s0, s1, s2, s3;
     if (kParity) {
         s0 = __byte_perm(ct.x, ct.y, 0x4321);
@@ -170,20 +180,20 @@ __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const
     uint32_t r0[4], r1[4];
     philox4x32_10(a.rk, g0 + 0, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 1, c1, a.c2, a.c3, r1);
-    res.x = update_word<kHasNever, kSmallQ, 0>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, geAdd, stab, snever, slot);
+    res.x = update_word<kHasNever, kSmallQ, kPow2, 0>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 2, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 3, c1, a.c2, a.c3, r1);
-    res.y = update_word<kHasNever, kSmallQ, 1>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, geAdd, stab, snever, slot);
+    res.y = update_word<kHasNever, kSmallQ, kPow2, 1>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 4, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 5, c1, a.c2, a.c3, r1);
-    res.z = update_word<kHasNever, kSmallQ, 2>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, geAdd, stab, snever, slot);
+    res.z = update_word<kHasNever, kSmallQ, kPow2, 2>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot);
     philox4x32_10(a.rk, g0 + 6, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 7, c1, a.c2, a.c3, r1);
-    res.w = update_word<kHasNever, kSmallQ, 3>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, geAdd, stab, snever, slot);
+    res.w = update_word<kHasNever, kSmallQ, kPow2, 3>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot);
     return res;
 }
 
-template <int kColour, bool kHasNever, bool kSmallQ, int kRows>
+template <int kColour, bool kHasNever, bool kSmallQ, bool kPow2, int kRows>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint32_t* snever, uint32_t q,
                                            uint32_t slot, int b, int rb, int x) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
@@ -213,13 +223,18 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     uint32_t g0 = (uint32_t)i0 * (uint32_t)(W >> 1) + 8u * (uint32_t)x;   // Philox group = n >> 1
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
     const uint32_t geAdd = (0x80u - q) * 0x01010101u;
-#pragma unroll 2
+    // q - 1 = 2^k: offsets are the top k bits of the proposal words
+    const uint32_t kbits = 31u - (uint32_t)__clz((int)(q - 1u));
+    const uint32_t dshift = 8u - kbits, dmask = ((1u << kbits) - 1u) * 0x01010101u;
+    // rolled: with the q - 1 = 2^k variant next to the general small-q one, two unrolled bodies no longer fit the
+    // instruction cache when replicas with different q share a launch (C4: 529 unrolled vs 538 rolled updates/ns)
+#pragma unroll 1
     for (int rr = 0; rr < kRows; rr += 2) {
         const bool more = rr + 2 < kRows;
         const uint4 n1 = __ldg(more ? pOth : pOthLast);
         const uint4 own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
-        uint4 res = update_row<kHasNever, kSmallQ, kColour>(a, own, wU, wC, wD, edge, g0, c1, q, geAdd, stab, snever, slot);
+        uint4 res = update_row<kHasNever, kSmallQ, kPow2, kColour>(a, own, wU, wC, wD, edge, g0, c1, q, geAdd, dshift, dmask, stab, snever, slot);
         *pOwn = res;
         uint4 n2 = n1, own2 = own1;
         uint32_t edge2 = edge1;
@@ -228,8 +243,8 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             own2 = *(pOwn + 2 * rowStride);
             edge2 = __ldg(pEdgeEven + edgeStride2);
         }
-        res = update_row<kHasNever, kSmallQ, 1 - kColour>(a, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd,
-                                                          stab, snever, slot);
+        res = update_row<kHasNever, kSmallQ, kPow2, 1 - kColour>(a, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd,
+                                                                 dshift, dmask, stab, snever, slot);
         *(pOwn + rowStride) = res;
         wU = wD;
         wC = n1;
@@ -271,9 +286,10 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) potts_int8_rows_kern
     if (u >= (a.L / kRows) * W16) return;                  // ragged last block of a replica (after the barrier)
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
-    if (never) march_rows<kColour, true, false, kRows>(a, stab, snever, q, slot, b, rb, x);
-    else if (q <= 16u) march_rows<kColour, false, true, kRows>(a, stab, snever, q, slot, b, rb, x);   // shift-free indicators
-    else march_rows<kColour, false, false, kRows>(a, stab, snever, q, slot, b, rb, x);
+    if (never) march_rows<kColour, true, false, false, kRows>(a, stab, snever, q, slot, b, rb, x);
+    else if (q <= 16u && ((q - 1u) & (q - 2u)) == 0u) march_rows<kColour, false, true, true, kRows>(a, stab, snever, q, slot, b, rb, x);
+    else if (q <= 16u) march_rows<kColour, false, true, false, kRows>(a, stab, snever, q, slot, b, rb, x);   // shift-free indicators
+    else march_rows<kColour, false, false, false, kRows>(a, stab, snever, q, slot, b, rb, x);
 }
 
 }  // namespace

@@ -116,6 +116,8 @@ struct spin_sim {
     size_t sched_bytes = 0;
     uint32_t* h_sched = nullptr;            // pinned staging of the same size, guarded by sched_ev (recorded after its upload)
     cudaEvent_t sched_ev = nullptr;
+    unsigned int* d_counter = nullptr;      // grid-barrier word of the persistent kernel
+    bool any_never = false;                 // some replica's current table has a never-accepted class
     uint8_t* d_aux = nullptr;        // bit-packed kernel's constant 2 KiB lookup table, on this handle's device
     int8_t* d_stage = nullptr;       // natural-layout staging for spin_get_spins / spin_set_spins / spin_set_bonds (grow-only)
     size_t stage_bytes = 0;
@@ -238,7 +240,11 @@ int upload_tables(spin_sim* sim, const double* beta, double J, double h) {
     sim->table_slot ^= 1;
     uint32_t* h_tab = sim->h_tables[slot];
     CUDA_TRY(cudaEventSynchronize(sim->table_ev[slot]));
-    for (int b = 0; b < sim->batch; ++b) build_record(sim, b, beta[b], J, h, h_tab + (size_t)b * kTableStride);
+    sim->any_never = false;
+    for (int b = 0; b < sim->batch; ++b) {
+        build_record(sim, b, beta[b], J, h, h_tab + (size_t)b * kTableStride);
+        if (h_tab[(size_t)b * kTableStride + kTabNever]) sim->any_never = true;
+    }
     CUDA_TRY(cudaMemcpyAsync(sim->d_tables, h_tab, sizeof(uint32_t) * kTableStride * (size_t)sim->batch,
                              cudaMemcpyHostToDevice, sim->stream));
     CUDA_TRY(cudaEventRecord(sim->table_ev[slot], sim->stream));
@@ -276,17 +282,58 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
 bool use_resident(const spin_sim* sim, bool measure) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || !ising_int8_resident_fits(sim->L)) return false;
     if (sim->general || sim->d_bond_nat) return false;            // per-bond couplings run on the general kernels
-    if (sim->policy == SPIN_POLICY_STREAMING) return false;
+    if (sim->policy == SPIN_POLICY_STREAMING || sim->policy == SPIN_POLICY_PERSISTENT) return false;
     if (sim->policy == SPIN_POLICY_RESIDENT) return true;
-    const long long sites = (long long)sim->batch * sim->L * sim->L;
-    if (sites <= (1ll << 20)) return true;                         // launch-latency-bound shapes
-    // the streaming kernel's blocks cover (L/8) x (L/32) thread strips of ONE replica: below 64 of them (L = 64, 96,
-    // 160, ...) its blocks are a fraction of a warp and the resident kernel is faster (L = 64: 922 vs 576 flips/ns)
+    // Measured on B200 (profiles/r2_policy_grid.md): one CTA per replica wins for every batch size while a half-sweep of
+    // a replica is a handful of warps (L <= 128: 3.1 vs 0.9 flips/ns at 1 x 64^2, 767 vs 500 at 256 x 128^2); for larger
+    // replicas a CTA needs tens of microseconds per sweep, so it only pays when the batch fills the GPU (>= 1 CTA per SM)
+    // AND the streaming kernel's blocks would be ragged (L = 160, 224: 766 vs 655 flips/ns at 256 x 224^2); small batches
+    // of large resident-eligible replicas (4 x 416^2: 23 vs 112 flips/ns) go to the persistent / streaming kernels.
+    if (sim->L <= 128) return true;
     int tpb = 128;
     const int perReplica = (sim->L / 8) * (sim->L / 32);
     while (perReplica % tpb) tpb >>= 1;
+    if (sim->L > 256) return false;                                // one CTA per SM only: 256 x 416^2 runs 692 resident vs 1020 streaming
     if (tpb < 64 && sim->batch >= 148) return true;
     return measure && sim->batch >= 296;                           // fused per-sweep reductions, >= 2 CTAs per SM
+}
+
+// Persistent cooperative kernel (ising_int8.cu): uniform Ising model, int8 layout, L % 32 == 0, no never-classes in the
+// current tables.  AUTO takes it for launch-bound shapes: measured (profiles/r2_policy_grid.md) it beats the streaming
+// path up to about 2 M sites per sweep (1 x 1024^2: 213 vs 134 flips/ns, 4 x 640^2: 282 vs 202) and loses above
+// (4 x 1024^2: 473 vs 513): a grid barrier costs ~2.3 us here, the same as a programmatic dependent launch, and the
+// streaming kernels overlap their launch with the previous kernel's tail.
+bool use_persistent(const spin_sim* sim) {
+    if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || sim->L % 32 != 0) return false;
+    if (sim->general || sim->d_bond_nat || sim->any_never) return false;
+    if (sim->policy == SPIN_POLICY_PERSISTENT) return true;
+    if (sim->policy != SPIN_POLICY_AUTO) return false;
+    return (long long)sim->batch * sim->L * sim->L <= (1ll << 21);
+}
+
+SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour);
+
+// Returns false when the cooperative launch was not possible (the caller streams instead).
+bool enqueue_persistent(spin_sim* sim, int64_t t0, int64_t n_sweeps, const uint32_t* tables = nullptr) {
+    SweepArgs a = sweep_args(sim, t0, 0);
+    if (tables) a.tables = tables;
+    for (int64_t done = 0; done < n_sweeps;) {
+        const int64_t chunk = n_sweeps - done < (1ll << 20) ? n_sweeps - done : (1ll << 20);   // barrier counter stays below 2^31
+        const int n = launch_ising_int8_persistent(a, (unsigned long long)(t0 + done), chunk, sim->d_counter, sim->stream);
+        if (n == 0) {
+            if (done == 0) return false;
+            for (int64_t t = t0 + done; t < t0 + n_sweeps; ++t) {      // finish on the streaming path
+                SweepArgs h0 = sweep_args(sim, t, 0), h1 = sweep_args(sim, t, 1);
+                if (tables) { h0.tables = tables; h1.tables = tables; }
+                sim->launches += launch_ising_int8_half_sweep(h0, sim->stream);
+                sim->launches += launch_ising_int8_half_sweep(h1, sim->stream);
+            }
+            return true;
+        }
+        sim->launches += n;
+        done += chunk;
+    }
+    return true;
 }
 
 void enqueue_resident(spin_sim* sim, int64_t t0, int64_t n_sweeps, bool measure, long long* E_trace, long long* M_trace,
@@ -436,6 +483,7 @@ void spin_destroy(spin_sim* sim) {
     if (sim->d_sched) cudaFree(sim->d_sched);
     if (sim->h_sched) cudaFreeHost(sim->h_sched);
     if (sim->sched_ev) cudaEventDestroy(sim->sched_ev);
+    if (sim->d_counter) cudaFree(sim->d_counter);
     if (sim->d_aux) cudaFree(sim->d_aux);
     if (sim->d_stage) cudaFree(sim->d_stage);
     if (sim->d_mom) cudaFree(sim->d_mom);
@@ -476,6 +524,7 @@ static int create_impl(spin_sim* sim, void* device_buffer, size_t buffer_bytes) 
     CUDA_TRY(cudaMalloc(&sim->d_q, sizeof(int32_t) * B));
     CUDA_TRY(cudaMalloc(&sim->d_EM, sizeof(long long) * 2 * B));
     CUDA_TRY(cudaMalloc(&sim->d_bad, sizeof(unsigned int)));
+    CUDA_TRY(cudaMalloc(&sim->d_counter, sizeof(unsigned int)));
     if (sim->model == SPIN_MODEL_POTTS) {
         CUDA_TRY(cudaMalloc(&sim->d_hist, sizeof(unsigned int) * 128 * B));
         CUDA_TRY(cudaMemsetAsync(sim->d_hist, 0, sizeof(unsigned int) * 128 * B, sim->stream));
@@ -581,6 +630,7 @@ const char* spin_kernel_variant(const spin_sim* sim) {
     if (sim->model == SPIN_MODEL_POTTS) return potts_int8_variant(sim->L);
     if (sim->layout == SPIN_LAYOUT_BITPACKED) return "ising_bits_rows32";
     if (use_resident(sim, false)) return "ising_int8_resident";
+    if (use_persistent(sim)) return "ising_int8_persistent";
     return ising_int8_variant(sim->L);
 }
 
@@ -769,11 +819,16 @@ int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps
     CUDA_TRY(cudaEventRecord(sim->sched_ev, sim->stream));
     sim->potts_general = false;
     const bool resident = use_resident(sim, false);
+    bool sched_never = false;
+    for (size_t k = 0; k < (size_t)n_steps * B; ++k) sched_never = sched_never || sim->h_sched[k * kTableStride + kTabNever] != 0u;
+    sim->any_never = sched_never;
+    const bool persistent = !resident && use_persistent(sim);
     for (int64_t k = 0; k < n_steps; ++k) {
         const uint32_t* tab = sim->d_sched + (size_t)k * B * kTableStride;
         const int64_t t0 = sweep_offset + k * sweeps_per_step;
         if (resident) {
             enqueue_resident(sim, t0, sweeps_per_step, false, nullptr, nullptr, nullptr, tab);
+        } else if (persistent && enqueue_persistent(sim, t0, sweeps_per_step, tab)) {
         } else {
             for (int64_t t = t0; t < t0 + sweeps_per_step; ++t) {
                 enqueue_half_sweep(sim, t, 0, tab);
@@ -787,7 +842,8 @@ int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps
 
 int spin_set_policy(spin_sim* sim, int32_t policy) {
     if (!sim) return fail(SPIN_ERR_INVALID, "spin_set_policy: NULL handle");
-    if (policy != SPIN_POLICY_AUTO && policy != SPIN_POLICY_STREAMING && policy != SPIN_POLICY_RESIDENT)
+    if (policy != SPIN_POLICY_AUTO && policy != SPIN_POLICY_STREAMING && policy != SPIN_POLICY_RESIDENT &&
+        policy != SPIN_POLICY_PERSISTENT)
         return fail(SPIN_ERR_INVALID, "spin_set_policy: unknown policy %d", (int)policy);
     sim->policy = policy;
     return SPIN_OK;
@@ -802,7 +858,7 @@ int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_
     if (rt != SPIN_OK) return rt;
     if (use_resident(sim, false)) {
         enqueue_resident(sim, sweep_offset, n_sweeps, false, nullptr, nullptr, nullptr);
-    } else {
+    } else if (!(use_persistent(sim) && enqueue_persistent(sim, sweep_offset, n_sweeps))) {
         for (int64_t t = sweep_offset; t < sweep_offset + n_sweeps; ++t) {
             enqueue_half_sweep(sim, t, 0);
             enqueue_half_sweep(sim, t, 1);

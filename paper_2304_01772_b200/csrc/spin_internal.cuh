@@ -138,6 +138,8 @@ int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s);
 uint8_t* ising_bits_make_aux_table();      // allocates + fills the constant 2 KiB lookup table on the current device (owned by the caller)
 const char* ising_int8_variant(int L);
 bool ising_int8_resident_fits(int L);                                       // a replica fits one CTA's shared memory
+int launch_ising_int8_persistent(const SweepArgs& a, unsigned long long t0, long long n_sweeps, unsigned int* counter,
+                                 cudaStream_t s);                           // 0: not launched, use the streaming path
 cudaError_t ising_int8_resident_configure();                                // per device: allow > 48 KiB dynamic shared memory
 int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s);      // all n_sweeps in one launch
 const char* potts_int8_variant(int L);

@@ -84,9 +84,10 @@ def test_config2_sampled_replicas(oracle_mod):
 
 
 @pytest.mark.parametrize("layout", ["int8", "bits"])
-def test_config3_sampled_replica(oracle_mod, layout):
-    # 8192^2 = 6.7e7 sites per replica: one replica, 2 sweeps (about 20 s of oracle time per layout)
-    _compare_sampled_replicas(oracle_mod, sp.workloads.config(3), [3], n_sweeps=2, layout=layout)
+def test_config3_all_replicas(oracle_mod, layout):
+    # 8192^2 = 6.7e7 sites per replica: all four replicas, 3 sweeps, lattice and (E, M) after every sweep
+    # (8e8 oracle updates per layout)
+    _compare_sampled_replicas(oracle_mod, sp.workloads.config(3), [0, 1, 2, 3], n_sweeps=3, layout=layout)
 
 
 def test_config4_sampled_replicas(oracle_mod):

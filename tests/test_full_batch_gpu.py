@@ -1,4 +1,4 @@
-"""Whole-batch parity at the BASELINE.json shapes: EVERY replica of C2, C4 and C5 after a multi-sweep call, the
+"""Whole-batch parity at the BASELINE.json shapes: EVERY replica of C2, C3 (both layouts), C4 and C5 after a multi-sweep call, the
 oracle running one replica per host thread (ctypes releases the GIL; the oracle itself stays single-threaded).
 Sized for about a minute on a 16-core host."""
 import os
@@ -44,6 +44,11 @@ def _check_all_replicas(oracle_mod, cfg, n_sweeps, layout="int8"):
 
 def test_config2_every_replica(oracle_mod):
     _check_all_replicas(oracle_mod, 2, n_sweeps=60)     # 64 x 1024^2 x 60 = 4.0e9 updates on the host
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+def test_config3_every_replica(oracle_mod, layout):
+    _check_all_replicas(oracle_mod, 3, n_sweeps=5, layout=layout)   # 4 x 8192^2 x 5 = 1.3e9 updates per layout
 
 
 def test_config4_every_replica(oracle_mod):

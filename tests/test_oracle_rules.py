@@ -180,6 +180,32 @@ def test_sweep_uses_time_colour_and_seed(oracle_mod):
             assert not np.array_equal(outs[a], outs[b])
 
 
+def test_high_sweep_index_field_by_hand(oracle_mod):
+    """Pins the placement of bits 32..55 of t in counter word 3 (O2): at t = 2^32 + 5 and t = (0xABCDEF << 32) + 7 every
+    site of a half-sweep is recomputed here from the exported Philox with c3 = (t >> 32) & 0xFFFFFF | colour << 24 |
+    1 << 28 written out; a wrong shift or mask in the oracle's counter assembly fails it."""
+    L, seed, beta, J, h = 8, 0x5DEECE66D1234567, 0.37, 1.0, 0.05
+    T, always = oracle_mod.ising_table(beta, J, h)
+    for t in ((1 << 32) + 5, (0xABCDEF << 32) + 7):
+        for colour in (0, 1):
+            lat = oracle_mod.init(1, L, seed=3)
+            expect = lat[0].copy()
+            for i in range(L):
+                for j in range(L):
+                    if (i + j) & 1 != colour:
+                        continue
+                    n = i * (L // 2) + (j >> 1)
+                    ctr = [n >> 2, 0, t & 0xFFFFFFFF, ((t >> 32) & 0xFFFFFF) | (colour << 24) | (1 << 28)]
+                    r = int(oracle_mod.philox4x32_10(ctr, [seed & 0xFFFFFFFF, seed >> 32])[n & 3])
+                    s0 = int(lat[0, i, j])
+                    nn = int(lat[0, (i - 1) % L, j]) + int(lat[0, (i + 1) % L, j]) + int(lat[0, i, (j - 1) % L]) + int(lat[0, i, (j + 1) % L])
+                    cls = 5 * ((s0 + 1) // 2) + (nn + 4) // 2
+                    if always[cls] or r < int(T[cls]):
+                        expect[i, j] = -s0
+            oracle_mod.ising_half_sweep(lat, beta, J, h, seed, t, colour)
+            assert np.array_equal(lat[0], expect), (t, colour)
+
+
 # ---------------------------------------------------------------- Q6: observables
 def _numpy_ising_obs(s):
     s = s.astype(np.int64)

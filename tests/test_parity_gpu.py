@@ -25,9 +25,10 @@ def _mk_ising(batch, L, seed, layout="int8", replica_offset=0, policy=None):
     return sim
 
 
-# every int8 Ising case runs through both kernel families: the two-launches-per-sweep HBM kernels and the
-# shared-memory-resident multi-sweep kernel (used when the shape allows it, else it falls back to streaming)
-POLICIES = [sp.SPIN_POLICY_STREAMING, sp.SPIN_POLICY_RESIDENT]
+# every int8 Ising case runs through the three kernel families: the two-launches-per-sweep HBM kernels, the
+# shared-memory-resident multi-sweep kernel and the persistent cooperative kernel (each used when the shape allows it,
+# else the call falls back to streaming)
+POLICIES = [sp.SPIN_POLICY_STREAMING, sp.SPIN_POLICY_RESIDENT, sp.SPIN_POLICY_PERSISTENT]
 
 
 def _mk_potts(batch, L, q, seed, replica_offset=0):
@@ -286,3 +287,29 @@ def test_caller_owned_buffer_and_stream(oracle_mod):
     Eo, Mo = oracle_mod.ising_observables(ref)
     assert np.array_equal(Ed.cpu().numpy(), Eo) and np.array_equal(Md.cpu().numpy(), Mo)
     sim.spin_destroy()
+
+
+# ------------------------------------------------------------- persistent cooperative kernel (launch-bound shapes)
+@pytest.mark.parametrize("batch,L,n", [(1, 640, 12), (3, 128, 20), (2, 1024, 6), (5, 96, 15), (1, 2560, 3)])
+def test_persistent_kernel_many_sweeps_in_one_launch(oracle_mod, batch, L, n):
+    """All sweeps of a call in one cooperative launch, grid barrier between half-sweeps (the paper's Table III shapes,
+    PAPER.md:252-276): lattice, E and M equal the oracle's; chunked calls continue the same trajectory."""
+    seed, beta = 60 + L, np.linspace(0.3, 0.6, batch)
+    ref = oracle_mod.init(batch, L, seed=seed)
+    with _mk_ising(batch, L, seed, policy=sp.SPIN_POLICY_PERSISTENT) as sim:
+        assert sim.spin_kernel_variant() == "ising_int8_persistent"
+        l0 = sim.spin_kernel_launches()
+        sim.spin_sweep(beta, 1.0, 0.02, n, 3)
+        assert sim.spin_kernel_launches() - l0 == 1
+        oracle_mod.sweep(ref, beta, 1.0, 0.02, seed=seed, n_sweeps=n, sweep_offset=3)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        sim.spin_sweep(beta, 1.0, 0.02, 2, 3 + n)
+        oracle_mod.sweep(ref, beta, 1.0, 0.02, seed=seed, n_sweeps=2, sweep_offset=3 + n)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        E, M = sim.spin_observables()
+        Eo, Mo = oracle_mod.ising_observables(ref)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+        # a never-accepted class (beta = 20) cannot use the kernel: the call streams, results unchanged
+        sim.spin_sweep(np.full(batch, 20.0), 1.0, 0.0, 2, 100)
+        oracle_mod.sweep(ref, np.full(batch, 20.0), 1.0, 0.0, seed=seed, n_sweeps=2, sweep_offset=100)
+        assert np.array_equal(sim.spin_get_spins(), ref)
