@@ -399,8 +399,10 @@ def dmc_entries(runner, sp, args, peaks):
 
     res = {}
     updates = float(B) * L * L * n_sweeps
-    for key, fn, bytes_per_site_sweep, launches in (("DMC-forward", fwd, 32.0, 2 * n_sweeps),
-                                                    ("DMC-forward+backward", train, 32.0 + 128.0, 6 * n_sweeps)):
+    # algorithmic bytes per site and sweep, fp32: forward = read the lattice, write it, read both
+    # coupling arrays once (16); with a stored trajectory the colour-0 state is written too (20); backward 128
+    for key, fn, bytes_per_site_sweep, launches in (("DMC-forward", fwd, 16.0, n_sweeps),
+                                                    ("DMC-forward+backward", train, 20.0 + 128.0, 5 * n_sweeps)):
         with torch.cuda.stream(stream):
             for k in range(args.warmup):
                 fn(k)
@@ -419,7 +421,7 @@ def dmc_entries(runner, sp, args, peaks):
         res[key] = {"workload": "DMC: Ising +-J-glass couplings (normal), fp32, %dx%d^2, %d sweeps, alpha=%g" % (B, L, n_sweeps, alpha),
                     "value": float(updates * len(ms) / (ms.sum() * 1e6)), "unit": UNIT, "best": float(vals.max()),
                     "median": float(np.median(vals)), "ms_per_step": float(ms.mean()),
-                    "kernel": "dmc_forward_kernel<float,4>" + ("" if key == "DMC-forward" else " + dmc_backward1/2_kernel<float,4>"),
+                    "kernel": "dmc_fused_sweep_kernel" + ("" if key == "DMC-forward" else " + dmc_backward1/2_kernel<float,4>"),
                     "gpu_launches_per_step": launches, "dtype": "f32",
                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                  "frac": gbs / peaks["hbm_gbs"], "bytes_per_site_per_sweep": bytes_per_site_sweep,
@@ -508,8 +510,10 @@ def stencil_cpm_entries(runner, sp, args, peaks, measured):
         ms = _time_calls(runner, args, lambda k: sp.spin_stencil_sweep(stencil, B, L, lat.data_ptr(), beta, 1.0, 0.2, 0.0, 21, n,
                                                                        sweep_offset=k * n, cuda_stream=stream.cuda_stream))
         ncol = {sp.SPIN_STENCIL_TRIANGULAR: 3, sp.SPIN_STENCIL_CUBIC: 2, sp.SPIN_STENCIL_SQUARE_NNN: 4}[stencil]
+        kern = {sp.SPIN_STENCIL_TRIANGULAR: "stencil_pass_kernel<triangular>", sp.SPIN_STENCIL_CUBIC: "cubic_pass_vec_kernel",
+                sp.SPIN_STENCIL_SQUARE_NNN: "nnn_pass_vec_kernel"}[stencil]
         out[key] = _alu_entry(key, "%s: Ising, batch %d, L = %d (%d sites per replica), %d sweeps" % (key, B, L, sites, n),
-                              float(B) * sites * n, ms, 11.0, 1.0, "stencil_pass_kernel", ncol * n, peaks, measured)
+                              float(B) * sites * n, ms, 11.0, 1.0, kern, ncol * n, peaks, measured)
     B, L = 256, 64
     spins, tau, A = sp.workloads.cpm_initial(B, L, 6, 5, seed=5)
     lat = torch.from_numpy(spins.copy()).cuda()
@@ -519,7 +523,7 @@ def stencil_cpm_entries(runner, sp, args, peaks, measured):
                                                                sweep_offset=k * nc, cuda_stream=stream.cuda_stream))
     out["F3-cpm"] = _alu_entry("F3-cpm", "CPM: Table II, 36 cells + medium, k_B T = 8, A = 25, lambda = 1, batch %d x %d^2, %d sweeps "
                                "(copy attempts)" % (B, L, nc), float(B) * L * L * nc, ms, 21.0, 2.0,
-                               "cpm_area_kernel + cpm_pass_kernel", 8 * nc, peaks, measured)
+                               "cpm_resident_kernel", 1, peaks, measured)
     return out
 
 

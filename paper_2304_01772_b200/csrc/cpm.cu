@@ -51,6 +51,33 @@ __global__ void __launch_bounds__(256) cpm_area_kernel(const int8_t* __restrict_
         if (sh[k]) atomicAdd(&areas[b * 128 + k], sh[k]);
 }
 
+// One proposal (readings C1, C3-C6): returns the new identifier of site (i, j), or -1 if it keeps its value.
+__device__ __forceinline__ int cpm_site(const int8_t* lat, int L, int i, int j, uint32_t r_prop, uint32_t r_acc,
+                                        const int32_t* areas, const CpmParams& p, const uint32_t* T, int dmax, bool beta_zero) {
+    const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1, jl = j == 0 ? L - 1 : j - 1, jr = j == L - 1 ? 0 : j + 1;
+    const int old = lat[(size_t)i * L + j];
+    const int nb[8] = {lat[(size_t)iu * L + jl], lat[(size_t)iu * L + j], lat[(size_t)iu * L + jr], lat[(size_t)i * L + jl],
+                       lat[(size_t)i * L + jr], lat[(size_t)id * L + jl], lat[(size_t)id * L + j], lat[(size_t)id * L + jr]};
+    const uint32_t dir = r_prop >> 29;
+    int nw = nb[0];
+#pragma unroll
+    for (int k = 1; k < 8; ++k) nw = dir == (uint32_t)k ? nb[k] : nw;
+    if (nw == old) return -1;
+    const int tn = p.tau[nw], to = p.tau[old];
+    long long dH = 0;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+        const int ty = p.tau[nb[k]];
+        if (nw != nb[k]) dH += p.J[tn * p.ntypes + ty];
+        if (old != nb[k]) dH -= p.J[to * p.ntypes + ty];
+    }
+    if (nw != 0) dH += p.lambda * (2ll * ((long long)areas[nw] - p.A[nw]) + 1);
+    if (old != 0) dH += p.lambda * (-2ll * ((long long)areas[old] - p.A[old]) + 1);
+    bool acc = dH <= 0 || beta_zero;
+    if (!acc && dH <= (long long)dmax) acc = r_acc < T[dH];
+    return acc ? nw : -1;
+}
+
 __global__ void __launch_bounds__(128) cpm_pass_kernel(CpmArgs a, CpmParams p) {
     const int L = a.L, W = L >> 1;
     const long long per = (long long)W * W, groups = (per + 1) >> 1;
@@ -59,7 +86,6 @@ __global__ void __launch_bounds__(128) cpm_pass_kernel(CpmArgs a, CpmParams p) {
     const int b = (int)(gid / groups);
     const uint32_t g = (uint32_t)(gid % groups);
     int8_t* lat = a.lattice + (size_t)b * L * L;
-    const int32_t* areas = a.areas + b * 128;
     uint32_t r[4];
     philox4x32_10(a.rk, g, (uint32_t)b + a.replica_offset, a.c2, a.c3, r);
 #pragma unroll
@@ -67,29 +93,67 @@ __global__ void __launch_bounds__(128) cpm_pass_kernel(CpmArgs a, CpmParams p) {
         const long long n = 2ll * g + e;
         if (n >= per) break;
         const int i = 2 * (int)(n / W) + (a.colour >> 1), j = 2 * (int)(n % W) + (a.colour & 1);
-        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1, jl = j == 0 ? L - 1 : j - 1, jr = j == L - 1 ? 0 : j + 1;
-        const int old = lat[(size_t)i * L + j];
-        const int nb[8] = {lat[(size_t)iu * L + jl], lat[(size_t)iu * L + j], lat[(size_t)iu * L + jr], lat[(size_t)i * L + jl],
-                           lat[(size_t)i * L + jr], lat[(size_t)id * L + jl], lat[(size_t)id * L + j], lat[(size_t)id * L + jr]};
-        const uint32_t dir = r[2 * e] >> 29;
-        int nw = nb[0];
-#pragma unroll
-        for (int k = 1; k < 8; ++k) nw = dir == (uint32_t)k ? nb[k] : nw;
-        if (nw == old) continue;
-        const int tn = p.tau[nw], to = p.tau[old];
-        long long dH = 0;
-#pragma unroll
-        for (int k = 0; k < 8; ++k) {
-            const int ty = p.tau[nb[k]];
-            if (nw != nb[k]) dH += p.J[tn * p.ntypes + ty];
-            if (old != nb[k]) dH -= p.J[to * p.ntypes + ty];
-        }
-        if (nw != 0) dH += p.lambda * (2ll * ((long long)areas[nw] - p.A[nw]) + 1);
-        if (old != 0) dH += p.lambda * (-2ll * ((long long)areas[old] - p.A[old]) + 1);
-        bool acc = dH <= 0 || a.beta_zero[b] != 0;
-        if (!acc && dH <= (long long)a.dmax) acc = r[2 * e + 1] < a.T[(size_t)b * (a.dmax + 1) + (size_t)dH];
-        if (acc) lat[(size_t)i * L + j] = (int8_t)nw;
+        const int nw = cpm_site(lat, L, i, j, r[2 * e], r[2 * e + 1], a.areas + b * 128, p, a.T + (size_t)b * (a.dmax + 1), a.dmax,
+                                a.beta_zero[b] != 0);
+        if (nw >= 0) lat[(size_t)i * L + j] = (int8_t)nw;
     }
+}
+
+// Resident variant for small lattices (the paper's set-up is 36 cells of 25 sites: a few thousand sites): one CTA per
+// replica keeps the lattice and the area counters in shared memory and runs every sweep of the call in one launch.  The
+// areas are counted once; during a colour pass accepted copies add to a separate delta array, which is folded into the
+// areas after the pass - so every proposal of a pass still sees the counts of the start of that pass (reading C3).
+__global__ void __launch_bounds__(256) cpm_resident_kernel(CpmArgs a, CpmParams p, unsigned long long t0, long long n_sweeps) {
+    extern __shared__ __align__(16) int8_t slat[];
+    __shared__ int32_t sarea[128], sdelta[128];
+    const int L = a.L, W = L >> 1, b = blockIdx.x;
+    const int N = L * L;
+    int8_t* glat = a.lattice + (size_t)b * N;
+    for (int k = threadIdx.x; k < 128; k += blockDim.x) { sarea[k] = 0; sdelta[k] = 0; }
+    for (int k = threadIdx.x; k < (N >> 2); k += blockDim.x) ((uint32_t*)slat)[k] = ((const uint32_t*)glat)[k];
+    __syncthreads();
+    {   // initial count: the medium (0) usually dominates, so it is counted in a register and reduced per warp
+        int zeros = 0;
+        for (int x = threadIdx.x; x < N; x += blockDim.x) {
+            const int s = slat[x];
+            if (s == 0) ++zeros; else atomicAdd(&sarea[s], 1);
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) zeros += __shfl_xor_sync(0xFFFFFFFFu, zeros, o);
+        if ((threadIdx.x & 31) == 0 && zeros) atomicAdd(&sarea[0], zeros);
+    }
+    __syncthreads();
+    const int per = W * W, groups = (per + 1) >> 1;
+    const uint32_t* T = a.T + (size_t)b * (a.dmax + 1);
+    const bool bz = a.beta_zero[b] != 0;
+    for (long long s = 0; s < n_sweeps; ++s) {
+        const unsigned long long t = t0 + (unsigned long long)s;
+        const uint32_t c2 = (uint32_t)(t & 0xFFFFFFFFull);
+        for (int colour = 0; colour < 4; ++colour) {
+            const uint32_t c3 = (uint32_t)((t >> 32) & 0xFFFFFFull) | ((uint32_t)colour << 24) | (kDomainCpm << 28);
+            for (int g = threadIdx.x; g < groups; g += blockDim.x) {
+                uint32_t r[4];
+                philox4x32_10(a.rk, (uint32_t)g, (uint32_t)b + a.replica_offset, c2, c3, r);
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    const int n = 2 * g + e;
+                    if (n >= per) break;
+                    const int i = 2 * (n / W) + (colour >> 1), j = 2 * (n % W) + (colour & 1);
+                    const int nw = cpm_site(slat, L, i, j, r[2 * e], r[2 * e + 1], sarea, p, T, a.dmax, bz);
+                    if (nw >= 0) {
+                        const int old = slat[i * L + j];
+                        slat[i * L + j] = (int8_t)nw;         // only this thread touches a site of the current colour
+                        atomicAdd(&sdelta[nw], 1);
+                        atomicAdd(&sdelta[old], -1);
+                    }
+                }
+            }
+            __syncthreads();
+            if (threadIdx.x < 128) { sarea[threadIdx.x] += sdelta[threadIdx.x]; sdelta[threadIdx.x] = 0; }
+            __syncthreads();
+        }
+    }
+    for (int k = threadIdx.x; k < (N >> 2); k += blockDim.x) ((uint32_t*)glat)[k] = ((const uint32_t*)slat)[k];
 }
 
 // acc[b][0] += adhesion energy, acc[b][1 + lo * ntypes + hi] += boundary pairs, per forward Moore pair.
@@ -204,7 +268,14 @@ int spin_cpm_sweep(int32_t batch, int32_t L, int32_t q, int8_t* lattice, const i
         long long want = (N + 255) / 256, cap = (148ll * 8 + batch - 1) / batch;
         const int bpr = (int)(want < cap ? want : (cap < 1 ? 1 : cap));
         const long long groups = (((long long)(L / 2) * (L / 2) + 1) >> 1) * batch;
-        for (int64_t t = sweep_offset; t < sweep_offset + n_sweeps && e == cudaSuccess; ++t)
+        // small lattices: one CTA per replica, everything in shared memory, all sweeps in one launch
+        const bool resident = N <= 65536 && (N & 3) == 0 && (L <= 128 || batch >= 148);
+        if (resident) {
+            a.colour = 0; a.c2 = 0; a.c3 = 0;
+            if (N > 32768) e = cudaFuncSetAttribute(cpm_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
+            if (e == cudaSuccess) cpm_resident_kernel<<<(unsigned)batch, 256, (size_t)N, s>>>(a, p, (unsigned long long)sweep_offset, (long long)n_sweeps);
+        }
+        for (int64_t t = sweep_offset; !resident && t < sweep_offset + n_sweeps && e == cudaSuccess; ++t)
             for (int c = 0; c < 4; ++c) {
                 e = cudaMemsetAsync(d_areas, 0, sizeof(int32_t) * 128 * batch, s);
                 cpm_area_kernel<<<(unsigned)((long long)bpr * batch), 256, 0, s>>>(lattice, L, bpr, d_areas);

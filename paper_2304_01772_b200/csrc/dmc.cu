@@ -120,6 +120,108 @@ __global__ void __launch_bounds__(256) dmc_forward_kernel(DmcArgs a, const T* __
     *(Vec<T, V>*)(dst + (size_t)b * a.L * a.L + (size_t)i * a.L + x * V) = out;
 }
 
+// ---- fused forward sweep (fp32, L % 8 == 0, L <= 2048): both colours of a sweep in ONE pass.  A block owns a tile of R
+// whole rows.  Phase A applies the colour-0 half-sweep to rows i0-1 .. i0+R (one halo row on each side, recomputed by the
+// neighbouring tile as well: the counter-based random numbers make the redundant updates identical) and keeps the result
+// in shared memory; phase B applies the colour-1 half-sweep to rows i0 .. i0+R-1 from shared memory and writes the final
+// rows.  The lattice and the couplings are read from HBM once per SWEEP instead of once per half-sweep (the second
+// read of the couplings hits L1/L2): about (R+4)/R * 4 + 4 + (R+2)/R * 8 = 18 B/site/sweep at R = 14 instead of 32.
+// A thread's unit of work is 8 consecutive sites of a row = the 4 sites of one colour = one Philox call (all 4 words).
+// The arithmetic per site is the two-pass kernels' expression for expression (same rounding: results are bit-identical).
+__device__ __forceinline__ float dmc_site(float s, float su, float sd, float sl, float sr, float jvu, float jvc, float jl,
+                                          float jr, float h, float beta, float alpha, uint32_t w) {
+    const float rr = (float)(w >> 8) * (float)(1.0 / 16777216.0);
+    const float F = jvu * su + jvc * sd + jl * sl + jr * sr + h;
+    const float dE = 2.0f * s * F;
+    const float p = expf(-beta * dE);
+    const float q = 1.0f / (1.0f + expf(-alpha * (p - rr)));
+    return q * (-s) + (1.0f - q) * s;
+}
+
+// Updates the 4 sites of parity kPar (columns j0 + kPar + 2m) among 8 consecutive sites c[0..7] of row i.
+template <int kPar>
+__device__ __forceinline__ void dmc_chunk_par(const DmcArgs& a, const uint32_t r[4], const float c[8], const float u[8],
+                                              const float d[8], float left, float right, const float jh[8], float jhl,
+                                              const float jvu[8], const float jvc[8], float beta, float out[8]) {
+#pragma unroll
+    for (int e = 0; e < 8; ++e) out[e] = c[e];
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        const int e = 2 * m + kPar;
+        const float sl = e == 0 ? left : c[e > 0 ? e - 1 : 0];
+        const float sr = e == 7 ? right : c[e < 7 ? e + 1 : 7];
+        const float jl = e == 0 ? jhl : jh[e > 0 ? e - 1 : 0];
+        out[e] = dmc_site(c[e], u[e], d[e], sl, sr, jvu[e], jvc[e], jl, jh[e], (float)a.h, beta, (float)a.alpha, r[m]);
+    }
+}
+
+__device__ __forceinline__ void dmc_chunk(const DmcArgs& a, int b, int i, int cidx, int par, uint32_t c3, const float c[8],
+                                          const float u[8], const float d[8], float left, float right, const float jh[8],
+                                          float jhl, const float jvu[8], const float jvc[8], float beta, float out[8]) {
+    uint32_t r[4];
+    philox4x32_10(a.rk, (uint32_t)i * (uint32_t)(a.L >> 3) + (uint32_t)cidx, (uint32_t)b + a.replica_offset, a.c2, c3, r);
+    if (par == 0) dmc_chunk_par<0>(a, r, c, u, d, left, right, jh, jhl, jvu, jvc, beta, out);
+    else dmc_chunk_par<1>(a, r, c, u, d, left, right, jh, jhl, jvu, jvc, beta, out);
+}
+
+__device__ __forceinline__ void load8(const float* p, float v[8]) {
+    const float4 x = *(const float4*)p, y = *(const float4*)(p + 4);
+    v[0] = x.x; v[1] = x.y; v[2] = x.z; v[3] = x.w; v[4] = y.x; v[5] = y.y; v[6] = y.z; v[7] = y.w;
+}
+__device__ __forceinline__ void store8(float* p, const float v[8]) {
+    *(float4*)p = make_float4(v[0], v[1], v[2], v[3]);
+    *(float4*)(p + 4) = make_float4(v[4], v[5], v[6], v[7]);
+}
+
+__global__ void __launch_bounds__(256) dmc_fused_sweep_kernel(DmcArgs a, const float* __restrict__ src, float* __restrict__ mid,
+                                                              float* __restrict__ dst, const float* __restrict__ Jh,
+                                                              const float* __restrict__ Jv, int R, int tiles) {
+    extern __shared__ __align__(16) float sA[];               // (R + 2) rows of L floats: the state after colour 0
+    const int L = a.L, cpr = L >> 3;
+    const int b = blockIdx.x / tiles, tile = blockIdx.x - b * tiles;
+    const int i0 = tile * R, rows = min(R, L - i0);
+    const size_t base = (size_t)b * L * L;
+    const float beta = (float)a.beta[b];
+    const uint32_t c3lo = a.c3 & ~(0xFu << 24);               // colour field cleared
+    // phase A: colour 0 on rows i0 - 1 .. i0 + rows
+    for (int task = threadIdx.x; task < (rows + 2) * cpr; task += blockDim.x) {
+        const int ra = task / cpr, cidx = task - ra * cpr;
+        int i = i0 - 1 + ra;
+        i = i < 0 ? L - 1 : (i >= L ? i - L : i);
+        const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1, j0 = cidx << 3;
+        const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 8 == L ? 0 : j0 + 8;
+        float c[8], u[8], d[8], jh[8], jvu[8], jvc[8], out[8];
+        load8(src + base + (size_t)i * L + j0, c);
+        load8(src + base + (size_t)iu * L + j0, u);
+        load8(src + base + (size_t)id * L + j0, d);
+        load8(Jh + base + (size_t)i * L + j0, jh);
+        load8(Jv + base + (size_t)iu * L + j0, jvu);
+        load8(Jv + base + (size_t)i * L + j0, jvc);
+        dmc_chunk(a, b, i, cidx, i & 1, c3lo, c, u, d, src[base + (size_t)i * L + jl], src[base + (size_t)i * L + jr], jh,
+                  Jh[base + (size_t)i * L + jl], jvu, jvc, beta, out);
+        store8(sA + (size_t)ra * L + j0, out);
+        if (mid && ra >= 1 && ra <= rows) store8(mid + base + (size_t)i * L + j0, out);
+    }
+    __syncthreads();
+    // phase B: colour 1 on rows i0 .. i0 + rows - 1, neighbours from shared memory
+    for (int task = threadIdx.x; task < rows * cpr; task += blockDim.x) {
+        const int rb = task / cpr, cidx = task - rb * cpr;
+        const int ra = rb + 1, i = i0 + rb, j0 = cidx << 3;
+        const int iu = i == 0 ? L - 1 : i - 1;
+        const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 8 == L ? 0 : j0 + 8;
+        float c[8], u[8], d[8], jh[8], jvu[8], jvc[8], out[8];
+        load8(sA + (size_t)ra * L + j0, c);
+        load8(sA + (size_t)(ra - 1) * L + j0, u);
+        load8(sA + (size_t)(ra + 1) * L + j0, d);
+        load8(Jh + base + (size_t)i * L + j0, jh);
+        load8(Jv + base + (size_t)iu * L + j0, jvu);
+        load8(Jv + base + (size_t)i * L + j0, jvc);
+        dmc_chunk(a, b, i, cidx, 1 - (i & 1), c3lo | (1u << 24), c, u, d, sA[(size_t)ra * L + jl], sA[(size_t)ra * L + jr], jh,
+                  Jh[base + (size_t)i * L + jl], jvu, jvc, beta, out);
+        store8(dst + base + (size_t)i * L + j0, out);
+    }
+}
+
 // Backward pass 1: blocks never straddle replicas (grid = blocks per replica x batch), so the beta / h sums reduce per block.
 template <typename T, int V>
 __global__ void __launch_bounds__(256) dmc_backward1_kernel(DmcArgs a, const T* __restrict__ src, const T* __restrict__ Jh,
@@ -274,6 +376,27 @@ void launch_forward(const DmcArgs& a, const void* src, void* dst, const void* Jh
     dmc_forward_kernel<T, V><<<(unsigned)((total + 255) / 256), 256, 0, s>>>(a, (const T*)src, (T*)dst, (const T*)Jh, (const T*)Jv);
 }
 
+// Rows per tile of the fused sweep: (R + 2) rows of L floats in at most 64 KiB (96 KiB for L > 1024) of shared memory.
+int fused_tile_rows(int L) {
+    const int budget = L > 1024 ? 96 * 1024 : 64 * 1024;
+    int R = budget / (4 * L) - 2;
+    if (R > 64) R = 64;
+    if (R > L) R = L;
+    return R;
+}
+bool fused_ok(int dtype, int L) { return dtype == SPIN_DTYPE_F32 && L % 8 == 0 && L <= 2048 && fused_tile_rows(L) >= 4; }
+
+cudaError_t forward_sweep_fused(const DmcArgs& a, const void* src, void* mid, void* dst, const void* Jh, const void* Jv,
+                                cudaStream_t s) {
+    const int R = fused_tile_rows(a.L), tiles = (a.L + R - 1) / R;
+    const size_t smem = (size_t)(R + 2) * a.L * sizeof(float);
+    cudaError_t e = cudaFuncSetAttribute(dmc_fused_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    if (e != cudaSuccess) return e;
+    dmc_fused_sweep_kernel<<<(unsigned)((long long)tiles * a.batch), 256, smem, s>>>(a, (const float*)src, (float*)mid, (float*)dst,
+                                                                                   (const float*)Jh, (const float*)Jv, R, tiles);
+    return cudaGetLastError();
+}
+
 void forward_half(int dtype, const DmcArgs& a, const void* src, void* dst, const void* Jh, const void* Jv, cudaStream_t s) {
     if (dtype == SPIN_DTYPE_F64) launch_forward<double, 2>(a, src, dst, Jh, Jv, s);
     else if (a.L % 4 == 0) launch_forward<float, 4>(a, src, dst, Jh, Jv, s);
@@ -325,7 +448,20 @@ int spin_dmc_forward(int32_t batch, int32_t L, int32_t dtype, const void* s0, co
     DMC_TRY(cudaMemcpyAsync(d_beta, beta, sizeof(double) * batch, cudaMemcpyHostToDevice, s));
     if (traj) DMC_TRY(cudaMemcpyAsync(traj, s0, bytes, cudaMemcpyDeviceToDevice, s));
     else if (n_sweeps > 0) DMC_TRY(cudaMallocAsync(&tmp, bytes, s));
-    {
+    if (fused_ok(dtype, L)) {
+        // one kernel per sweep: state 2k -> (state 2k+1 into the trajectory, if any) -> state 2k+2.  Out of place, so
+        // without a trajectory the sweeps ping-pong between tmp and s_out, ending in s_out.
+        const void* cur = s0;
+        for (int64_t k = 0; k < n_sweeps; ++k) {
+            void* mid = traj ? (void*)((char*)traj + (size_t)(2 * k + 1) * bytes) : nullptr;
+            void* dst = traj ? (void*)((char*)traj + (size_t)(2 * k + 2) * bytes) : (((n_sweeps - k) & 1) ? s_out : tmp);
+            if (!traj && dst == cur) dst = (dst == s_out) ? tmp : s_out;      // s0 == s_out on the first sweep
+            const DmcArgs a = make_args(batch, L, h, alpha, d_beta, seed, replica_offset, sweep_offset + k, 0);
+            DMC_TRY(forward_sweep_fused(a, cur, mid, dst, Jh, Jv, s));
+            cur = dst;
+        }
+        if (cur != s_out) DMC_TRY(cudaMemcpyAsync(s_out, cur, bytes, cudaMemcpyDeviceToDevice, s));
+    } else {
         const void* cur = s0;
         for (int64_t k = 0; k < n_sweeps; ++k)
             for (int c = 0; c < 2; ++c) {

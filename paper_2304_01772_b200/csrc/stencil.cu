@@ -102,6 +102,166 @@ __global__ void __launch_bounds__(128) stencil_pass_kernel(StencilArgs a) {
     }
 }
 
+// ---- cubic lattice, L % 16 == 0: byte-SIMD kernel.  One thread owns 16 consecutive sites along k of one (i, j) line
+// (one 128-bit word of the natural layout): 8 of them have the current colour = two Philox groups.  The four
+// neighbour lines (i+-1, j), (i, j+-1) are 128-bit loads of the same k range; the k+-1 neighbours are the other-colour
+// bytes of the own word (plus one edge byte on each side).  As in the int8 Ising kernel the spins are masked to "4 per
+// -1 spin" per byte, the six neighbours are added per byte, and 4 nd + 32 d is the byte offset of the class threshold
+// in a shared-memory table laid out [d][8].  The whole word is written back: its other-colour bytes are rewritten with
+// the values they already have (no thread changes them during this pass).
+__global__ void __launch_bounds__(128) cubic_pass_vec_kernel(StencilArgs a) {
+    __shared__ uint32_t stab[16];
+    __shared__ uint32_t salways;
+    const int L = a.L, V = L >> 4;                             // 16-site words per line
+    const long long lines = (long long)L * L;
+    const long long total = lines * V * a.batch;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    // a block never straddles replicas when (L^2 * V) % 128 == 0; otherwise the table is re-read per thread below
+    const int b0 = (int)(((long long)blockIdx.x * blockDim.x) / (lines * V));
+    if (threadIdx.x < 16) {
+        const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
+        const int d = threadIdx.x >> 3, nd = threadIdx.x & 7;
+        stab[threadIdx.x] = nd <= 6 ? tab[d * 7 + nd] : 0u;
+        if (threadIdx.x == 0) {
+            // always-accept bits re-indexed to d * 8 + nd
+            const uint32_t al = tab[62];
+            salways = (al & 0x7Fu) | (((al >> 7) & 0x7Fu) << 8);
+        }
+    }
+    __syncthreads();
+    if (gid >= total) return;
+    const int b = (int)(gid / (lines * V));
+    const long long rem = gid - (long long)b * lines * V;
+    const int v = (int)(rem % V);
+    const long long ij = rem / V;
+    const int i = (int)(ij / L), j = (int)(ij % L);
+    const int iu = wrap_dec(i, L), id = wrap_inc(i, L), jl = wrap_dec(j, L), jr = wrap_inc(j, L);
+    int8_t* lat = a.lattice + (size_t)b * lines * L;
+    const int k0 = v << 4;
+    const uint4 c = *(const uint4*)(lat + ((size_t)i * L + j) * L + k0);
+    const uint4 u = *(const uint4*)(lat + ((size_t)iu * L + j) * L + k0), d = *(const uint4*)(lat + ((size_t)id * L + j) * L + k0);
+    const uint4 f = *(const uint4*)(lat + ((size_t)i * L + jl) * L + k0), g = *(const uint4*)(lat + ((size_t)i * L + jr) * L + k0);
+    const uint32_t eL = (uint32_t)(uint8_t)lat[((size_t)i * L + j) * L + (k0 == 0 ? L - 1 : k0 - 1)];
+    const uint32_t eR = (uint32_t)(uint8_t)lat[((size_t)i * L + j) * L + (k0 + 16 == L ? 0 : k0 + 16)];
+    const uint32_t m = 0x04040404u;
+    const uint32_t cw[4] = {c.x, c.y, c.z, c.w};
+    const uint32_t cm[4] = {c.x & m, c.y & m, c.z & m, c.w & m};
+    const uint32_t sum4[4] = {(u.x & m) + (d.x & m) + (f.x & m) + (g.x & m), (u.y & m) + (d.y & m) + (f.y & m) + (g.y & m),
+                              (u.z & m) + (d.z & m) + (f.z & m) + (g.z & m), (u.w & m) + (d.w & m) + (f.w & m) + (g.w & m)};
+    const uint32_t par = (uint32_t)((i + j + a.colour) & 1);   // k parity of the updated sites (k0 is even)
+    // Philox groups: n = (i L + j)(L/2) + k/2, the 8 updated sites are n0 .. n0+7 with n0 = (i L + j)(L/2) + 8 v
+    const uint32_t g0 = (uint32_t)(((long long)i * L + j) * (L >> 3) + 2 * v);
+    uint32_t r[8];
+    philox4x32_10(a.rk, g0, (uint32_t)b + a.replica_offset, a.c2, a.c3, r);
+    philox4x32_10(a.rk, g0 + 1u, (uint32_t)b + a.replica_offset, a.c2, a.c3, r + 4);
+    const uint32_t* tabp = stab;
+    uint32_t always = salways;
+    if (b != b0) {                                             // ragged: this thread's replica differs from the block's first
+        tabp = nullptr;
+    }
+    uint32_t out[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t prevm = w == 0 ? ((eL & 4u) << 24) : (cm[w - 1] & 0xFF000000u);     // masked byte k-1 of byte 0, in byte 3
+        const uint32_t nextm = w == 3 ? (eR & 4u) : (cm[w + 1] & 0xFFu);                   // masked byte k+1 of byte 3, in byte 0
+        const uint32_t left = (cm[w] << 8) | (prevm >> 24);
+        const uint32_t right = (cm[w] >> 8) | (nextm << 24);
+        const uint32_t t = sum4[w] + left + right + (cw[w] & 0x20202020u);                  // bytes: 4 nd + 32 d
+        uint32_t flip = 0u;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const uint32_t pos = 2u * (uint32_t)e + par;                                    // byte of the updated site
+            const uint32_t off = (t >> (8u * pos)) & 0xFFu;
+            const uint32_t idx = off >> 2;                                                  // d * 8 + nd
+            uint32_t T;
+            bool al;
+            if (tabp) { T = tabp[idx]; al = (always >> idx) & 1u; }
+            else {
+                const uint32_t* tab = a.tables + (size_t)b * kStencilRec;
+                const uint32_t k7 = (idx >> 3) * 7u + (idx & 7u);
+                T = tab[k7];
+                al = (tab[62] >> k7) & 1u;
+            }
+            if (al || r[2 * w + e] < T) flip |= 0xFEu << (8u * pos);
+        }
+        out[w] = cw[w] ^ flip;
+    }
+    *(uint4*)(lat + ((size_t)i * L + j) * L + k0) = make_uint4(out[0], out[1], out[2], out[3]);
+}
+
+// ---- square lattice with second neighbours, L % 16 == 0: the same byte-SIMD scheme.  A thread owns 16 consecutive sites
+// of a row of the colour's row parity; 8 of them (column parity of the colour) are updated.  With every spin masked to
+// "4 per -1 spin", 5 (N + S + W + E) + (NW + NE + SW + SE) + 25 own is 4 (25 d + 5 nd1 + nd2): the byte offset of the class
+// threshold in the 50-entry table.
+__device__ __forceinline__ void shifted_words(const uint32_t x[4], uint32_t edgeL, uint32_t edgeR, uint32_t left[4], uint32_t right[4]) {
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t prev = w == 0 ? edgeL : (x[w - 1] >> 24);
+        const uint32_t next = w == 3 ? edgeR : (x[w + 1] & 0xFFu);
+        left[w] = (x[w] << 8) | prev;          // byte e holds the site at column - 1
+        right[w] = (x[w] >> 8) | (next << 24); // byte e holds the site at column + 1
+    }
+}
+
+__global__ void __launch_bounds__(128) nnn_pass_vec_kernel(StencilArgs a) {
+    __shared__ uint32_t stab[50];
+    __shared__ uint32_t salw[2];
+    const int L = a.L, V = L >> 4, H = L >> 1;
+    const long long per = (long long)H * V;                    // words of the colour's rows per replica
+    const long long total = per * a.batch;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int b0 = (int)(((long long)blockIdx.x * blockDim.x) / per);
+    const bool uniform = (per % blockDim.x) == 0;              // then a block never straddles replicas
+    if (uniform) {
+        const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
+        if (threadIdx.x < 50) stab[threadIdx.x] = tab[threadIdx.x];
+        if (threadIdx.x < 2) salw[threadIdx.x] = tab[62 + threadIdx.x];
+        __syncthreads();
+    }
+    if (gid >= total) return;
+    const int b = (int)(gid / per);
+    const long long rem = gid - (long long)b * per;
+    const int v = (int)(rem % V), ar = (int)(rem / V);
+    const int i = 2 * ar + (a.colour >> 1);
+    const uint32_t pj = (uint32_t)(a.colour & 1);
+    const int iu = wrap_dec(i, L), id = wrap_inc(i, L), j0 = v << 4;
+    const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 16 == L ? 0 : j0 + 16;
+    int8_t* lat = a.lattice + (size_t)b * L * L;
+    const uint32_t m = 0x04040404u;
+    const uint4 c4 = *(const uint4*)(lat + (size_t)i * L + j0), u4 = *(const uint4*)(lat + (size_t)iu * L + j0),
+                d4 = *(const uint4*)(lat + (size_t)id * L + j0);
+    const uint32_t cw[4] = {c4.x, c4.y, c4.z, c4.w};
+    const uint32_t cm[4] = {c4.x & m, c4.y & m, c4.z & m, c4.w & m}, um[4] = {u4.x & m, u4.y & m, u4.z & m, u4.w & m},
+                   dm[4] = {d4.x & m, d4.y & m, d4.z & m, d4.w & m};
+    uint32_t cl[4], cr[4], ul[4], ur[4], dl[4], dr[4];
+    shifted_words(cm, (uint32_t)(uint8_t)lat[(size_t)i * L + jl] & 4u, (uint32_t)(uint8_t)lat[(size_t)i * L + jr] & 4u, cl, cr);
+    shifted_words(um, (uint32_t)(uint8_t)lat[(size_t)iu * L + jl] & 4u, (uint32_t)(uint8_t)lat[(size_t)iu * L + jr] & 4u, ul, ur);
+    shifted_words(dm, (uint32_t)(uint8_t)lat[(size_t)id * L + jl] & 4u, (uint32_t)(uint8_t)lat[(size_t)id * L + jr] & 4u, dl, dr);
+    const uint32_t g0 = (uint32_t)((long long)ar * (L >> 3) + 2 * v);
+    uint32_t r[8];
+    philox4x32_10(a.rk, g0, (uint32_t)b + a.replica_offset, a.c2, a.c3, r);
+    philox4x32_10(a.rk, g0 + 1u, (uint32_t)b + a.replica_offset, a.c2, a.c3, r + 4);
+    const uint32_t* tab = uniform ? stab : a.tables + (size_t)b * kStencilRec;
+    const unsigned long long always = uniform ? ((unsigned long long)salw[0] | ((unsigned long long)salw[1] << 32))
+                                              : ((unsigned long long)tab[62] | ((unsigned long long)tab[63] << 32));
+    uint32_t out[4];
+#pragma unroll
+    for (int w = 0; w < 4; ++w) {
+        const uint32_t first = um[w] + dm[w] + cl[w] + cr[w];             // 4 nd1 per byte
+        const uint32_t second = ul[w] + ur[w] + dl[w] + dr[w];            // 4 nd2 per byte
+        const uint32_t t = first * 5u + second + cm[w] * 25u;             // 4 (25 d + 5 nd1 + nd2), < 256 per byte
+        uint32_t flip = 0u;
+#pragma unroll
+        for (int e = 0; e < 2; ++e) {
+            const uint32_t pos = 2u * (uint32_t)e + pj;
+            const uint32_t idx = ((t >> (8u * pos)) & 0xFFu) >> 2;
+            if (((always >> idx) & 1ull) || r[2 * w + e] < tab[idx]) flip |= 0xFEu << (8u * pos);
+        }
+        out[w] = cw[w] ^ flip;
+    }
+    *(uint4*)(lat + (size_t)i * L + j0) = make_uint4(out[0], out[1], out[2], out[3]);
+}
+
 __global__ void stencil_init_kernel(int8_t* lattice, long long N, int batch, uint32_t replica_offset, RoundKeys rk) {
     const long long groups = (N + 3) >> 2;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -261,8 +421,14 @@ int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_t* lattic
             a.c2 = (uint32_t)((uint64_t)t & 0xFFFFFFFFull);
             a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)c << 24) | (kDomainStencil << 28);
             if (stencil == SPIN_STENCIL_TRIANGULAR) stencil_pass_kernel<SPIN_STENCIL_TRIANGULAR><<<grid, 128, 0, s>>>(a);
-            else if (stencil == SPIN_STENCIL_CUBIC) stencil_pass_kernel<SPIN_STENCIL_CUBIC><<<grid, 128, 0, s>>>(a);
-            else stencil_pass_kernel<SPIN_STENCIL_SQUARE_NNN><<<grid, 128, 0, s>>>(a);
+            else if (stencil == SPIN_STENCIL_CUBIC && L % 16 == 0) {
+                const long long words = (long long)L * L * (L >> 4) * batch;
+                cubic_pass_vec_kernel<<<(unsigned)((words + 127) / 128), 128, 0, s>>>(a);
+            } else if (stencil == SPIN_STENCIL_CUBIC) stencil_pass_kernel<SPIN_STENCIL_CUBIC><<<grid, 128, 0, s>>>(a);
+            else if (L % 16 == 0) {
+                const long long words = (long long)(L >> 1) * (L >> 4) * batch;
+                nnn_pass_vec_kernel<<<(unsigned)((words + 127) / 128), 128, 0, s>>>(a);
+            } else stencil_pass_kernel<SPIN_STENCIL_SQUARE_NNN><<<grid, 128, 0, s>>>(a);
         }
     if (e == cudaSuccess) e = cudaGetLastError();
     cudaFreeAsync(d_tab, s);

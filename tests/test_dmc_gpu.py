@@ -115,6 +115,35 @@ def test_without_trajectory_and_in_place_give_the_same_final_lattice():
     assert np.array_equal(ds2.cpu().numpy(), ref)
 
 
+@pytest.mark.parametrize("L", [8, 24, 64, 256, 1024, 2048])
+def test_fused_sweep_kernel_matches_oracle_and_its_own_trajectory(L):
+    """fp32 with L % 8 == 0 runs the fused two-colour sweep kernel (one launch per sweep, tiles of rows with a recomputed
+    halo row): final state with and without a stored trajectory is bit-identical (odd and even sweep counts, in place),
+    the stored intermediate states chain correctly, and everything stays within the fp32 tolerance of the oracle."""
+    B, seed, h, alpha = 2, 41, 0.02, 6.0
+    s, Jh, Jv, beta = _inputs(B, L, 300 + L, sp.SPIN_DTYPE_F32)
+    st = torch.cuda.current_stream().cuda_stream
+    for n in (1, 2, 3):
+        g = _run_gpu(sp.SPIN_DTYPE_F32, s, Jh, Jv, h, beta, alpha, seed, n)
+        ds, dJh, dJv = _dev(s), _dev(Jh), _dev(Jv)
+        out = torch.empty_like(ds)
+        sp.spin_dmc_forward(B, L, sp.SPIN_DTYPE_F32, ds.data_ptr(), dJh.data_ptr(), dJv.data_ptr(), h, beta, alpha, seed, n,
+                            s_out_ptr=out.data_ptr(), cuda_stream=st)
+        assert np.array_equal(out.cpu().numpy(), g["out"]), n
+        sp.spin_dmc_forward(B, L, sp.SPIN_DTYPE_F32, ds.data_ptr(), dJh.data_ptr(), dJv.data_ptr(), h, beta, alpha, seed, n,
+                            s_out_ptr=ds.data_ptr(), cuda_stream=st)
+        assert np.array_equal(ds.cpu().numpy(), g["out"]), n
+        if L <= 256 and n == 2:
+            o = _run_oracle(s, Jh, Jv, h, beta, alpha, seed, n)
+            err = [float(np.max(np.abs(g["traj"][k] - o["traj"][k]))) for k in range(2 * n + 1)]
+            assert max(err) <= 2e-5, err
+        # every stored state is one half-sweep of the previous one: colour c sites of state k+1 differ, the others not
+        ii, jj = np.indices((L, L))
+        for k in range(2 * n):
+            other = ((ii + jj) & 1) != (k & 1)
+            assert np.array_equal(g["traj"][k + 1][:, other], g["traj"][k][:, other]), k
+
+
 def test_alpha_to_infinity_then_eq4_reproduces_the_discrete_sweep():
     """'at the limit alpha -> infinity becomes the standard Metropolis algorithm'.  fp32 kernel, +-J glass,
     against the discrete Algorithm-1 oracle (the two acceptance tests differ with probability ~2^-24 per site)."""
