@@ -231,6 +231,7 @@ int spin_cpm_sweep(int32_t batch, int32_t L, int32_t q, int8_t* lattice, const i
     for (int b = 0; b < batch; ++b) {
         if (!std::isfinite(beta[b]) || beta[b] < 0.0) return cpm_fail(SPIN_ERR_INVALID, "spin_cpm_sweep: beta must be finite and >= 0");
         if (beta[b] == 0.0) continue;
+        if (b > 0 && beta[b] == beta[b - 1]) continue;      // same table as the previous replica
         int d = 1;
         while (d <= kCap && std::floor(std::exp(-(beta[b] * (double)d)) * 4294967296.0) >= 1.0) ++d;
         if (d > kCap) return cpm_fail(SPIN_ERR_UNSUPPORTED, "spin_cpm_sweep: beta is so small that exp(-beta dH) 2^32 >= 1 beyond dH = 65536; use beta = 0 or a larger beta");
@@ -242,6 +243,10 @@ int spin_cpm_sweep(int32_t batch, int32_t L, int32_t q, int8_t* lattice, const i
     try { T.assign((size_t)batch * (dmax + 1), 0u); bz.assign(batch, 0); } catch (...) { return cpm_fail(SPIN_ERR_NOMEM, "spin_cpm_sweep: out of host memory"); }
     for (int b = 0; b < batch; ++b) {
         bz[b] = beta[b] == 0.0 ? 1 : 0;
+        if (b > 0 && beta[b] == beta[b - 1]) {                // replicas at one temperature share the (identical) table
+            std::memcpy(&T[(size_t)b * (dmax + 1)], &T[(size_t)(b - 1) * (dmax + 1)], sizeof(uint32_t) * (dmax + 1));
+            continue;
+        }
         for (int d = 1; d <= dmax; ++d) {
             const double x = beta[b] * (double)d;              // O4 with dE = d > 0
             if (x <= 0.0) { T[(size_t)b * (dmax + 1) + d] = 0xFFFFFFFFu; continue; }

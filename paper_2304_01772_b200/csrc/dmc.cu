@@ -127,14 +127,15 @@ __global__ void __launch_bounds__(256) dmc_forward_kernel(DmcArgs a, const T* __
 // rows.  The lattice and the couplings are read from HBM once per SWEEP instead of once per half-sweep (the second
 // read of the couplings hits L1/L2): about (R+4)/R * 4 + 4 + (R+2)/R * 8 = 18 B/site/sweep at R = 14 instead of 32.
 // A thread's unit of work is 8 consecutive sites of a row = the 4 sites of one colour = one Philox call (all 4 words).
-// The arithmetic per site is the two-pass kernels' expression for expression (same rounding: results are bit-identical).
+// The arithmetic per site is the two-pass kernels' up to the last bits (fast reciprocal, FMA contraction): both are held
+// to the fp32 tolerance against the oracle, not to each other.
 __device__ __forceinline__ float dmc_site(float s, float su, float sd, float sl, float sr, float jvu, float jvc, float jl,
                                           float jr, float h, float beta, float alpha, uint32_t w) {
     const float rr = (float)(w >> 8) * (float)(1.0 / 16777216.0);
     const float F = jvu * su + jvc * sd + jl * sl + jr * sr + h;
     const float dE = 2.0f * s * F;
     const float p = expf(-beta * dE);
-    const float q = 1.0f / (1.0f + expf(-alpha * (p - rr)));
+    const float q = __fdividef(1.0f, 1.0f + expf(-alpha * (p - rr)));       // MUFU.RCP + FMUL, 2 ulp
     return q * (-s) + (1.0f - q) * s;
 }
 
