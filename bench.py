@@ -97,8 +97,8 @@ class ClockSampler:
 
 def _ncu_traffic(kernel_variant, w):
     """DRAM bytes per launch of the dominant kernel from the committed `ncu --set full` capture summary
-    (profiles/r1_traffic.csv: kernel variant, workload, dram read + write bytes per launch), or None."""
-    p = os.path.join(ROOT, "profiles", "r1_traffic.csv")
+    (profiles/r2_traffic.csv: kernel variant, workload, dram read + write bytes per launch), or None."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.csv")
     if not os.path.exists(p):
         return None
     for line in open(p):

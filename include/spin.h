@@ -211,9 +211,13 @@ SPIN_API int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_
  * layout, L a multiple of 32, L*L <= 192 KiB) and falls back to streaming otherwise.  SPIN_POLICY_PERSISTENT uses the
  * persistent cooperative kernel (all sweeps of a call in one launch, the lattice in L2, a grid-wide barrier between
  * half-sweeps) whenever the shape allows it (Ising, int8 layout, L a multiple of 32, uniform couplings, no class whose
- * acceptance threshold is 0); AUTO takes it for batches of at most 2^21 sites that do not go to the resident kernel.
+ * acceptance threshold is 0); AUTO takes it for batches of at most 2^21 sites that do not go to the resident kernel.  SPIN_POLICY_TILED uses the temporally blocked tile kernel (a CTA advances
+ * a tile with a halo by several sweeps per launch in shared memory, about one tile per SM; needs a second lattice
+ * buffer, allocated by the library on first use) whenever the shape allows it (Ising, int8 layout, L % 8 == 0, L >= 16,
+ * uniform couplings).
  * Returns SPIN_OK or SPIN_ERR_INVALID (NULL handle, unknown policy). */
-enum { SPIN_POLICY_AUTO = 0, SPIN_POLICY_STREAMING = 1, SPIN_POLICY_RESIDENT = 2, SPIN_POLICY_PERSISTENT = 3 };
+enum { SPIN_POLICY_AUTO = 0, SPIN_POLICY_STREAMING = 1, SPIN_POLICY_RESIDENT = 2, SPIN_POLICY_PERSISTENT = 3,
+       SPIN_POLICY_TILED = 4 };
 SPIN_API int spin_set_policy(spin_sim* sim, int32_t policy);
 
 /* ---------------------------------------------------------------------------------------------

@@ -4,6 +4,8 @@
 // consecutive same-colour sites), one unsigned compare against the replica's threshold table, flip.
 #include "spin_internal.cuh"
 
+#include <cmath>
+
 namespace spin {
 
 namespace {
@@ -313,6 +315,110 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_persisten
     }
 }
 
+// ---- temporally blocked tile kernel (launch-bound shapes, L % 8 == 0).  The counter-based random numbers make every
+// update a pure function of (seed, replica, site, sweep, colour) and of the neighbouring spins, so a CTA can advance a
+// TILE of one replica by several sweeps on its own if it also carries a halo: each half-sweep the outermost valid ring
+// of the halo becomes stale (its outside neighbours are not there), so 2 * sweeps halo rows / columns keep the interior
+// exact.  The halo sites are updated redundantly by the neighbouring tiles with identical results.  One launch =
+// `sweeps` full sweeps for every tile: the launch gap (~2.7 us per half-sweep on the streaming path) is paid once per
+// `sweeps` sweeps, and a one-replica lattice is spread over all SMs instead of one.
+// Region in shared memory: rows r <-> global row (i0 - HR + r) mod L, words wx <-> global k = (k0 - HK + 4 wx) mod (L/2),
+// both colours.  One thread per 4-site word (= one Philox group) per half-sweep; region-edge words use clamped
+// neighbours (their results are stale by construction and never reach the interior).
+template <bool kHasNever>
+__device__ __forceinline__ void tiled_half_sweep(const TiledArgs& a, int colour, uint32_t c2, uint32_t c3, uint32_t* own1,
+                                                 const uint32_t* oth1, int SR, int SWX, int iBase, int kBase,
+                                                 const uint32_t* stab, uint32_t slot, uint32_t c1) {
+    const int L = a.L, W = L >> 1, W4 = W >> 2;
+    const uint32_t m = 0x04040404u;
+    for (int task = threadIdx.x; task < SR * SWX; task += blockDim.x) {
+        const int r = task / SWX, wx = task - r * SWX;
+        int gi = iBase + r;                                    // iBase in [0, L): at most two wraps for regions <= 2 L
+        gi = gi >= L ? gi - L : gi;
+        gi = gi >= L ? gi - L : gi;
+        int gk = kBase + 4 * wx;
+        gk = gk >= W ? gk - W : gk;
+        gk = gk >= W ? gk - W : gk;
+        const bool par = ((gi + colour) & 1) != 0;             // side neighbour of site k: k+1 if par else k-1
+        const int ru = r == 0 ? 0 : r - 1, rd = r == SR - 1 ? r : r + 1;
+        const int xs = par ? (wx == SWX - 1 ? wx : wx + 1) : (wx == 0 ? 0 : wx - 1);
+        const uint32_t um = oth1[ru * SWX + wx] & m, cm = oth1[task] & m, dm = oth1[rd * SWX + wx] & m;
+        const uint32_t nb = oth1[r * SWX + xs] & m;
+        const uint32_t sd = __byte_perm(par ? cm : nb, par ? nb : cm, par ? 0x4321u : 0x6543u);
+        const uint32_t own = own1[task];
+        const uint32_t n4 = um + cm + dm + sd;                  // 4 x number of -1 neighbours per byte
+        uint32_t rw[4];
+        philox4x32_10(a.rk, (uint32_t)gi * (uint32_t)W4 + (uint32_t)(gk >> 2), c1, c2, c3, rw);
+        own1[task] = update_word<kHasNever, 0>(own, n4 + (own & 0x20202020u), rw, stab, slot);
+    }
+}
+
+constexpr int kTiledThreads = 512;
+
+__global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledArgs a) {
+    extern __shared__ __align__(16) uint32_t tsm[];
+    __shared__ uint32_t stab[kTableStride];
+    __shared__ uint32_t sidx[kTiledThreads];
+    pdl_launch_dependents();
+    const int L = a.L, W = L >> 1;
+    const int SR = a.TR + 2 * a.HR, SWX = (a.TK + 2 * a.HK) >> 2;
+    const int perReplica = a.tilesR * a.tilesK;
+    const int b = blockIdx.x / perReplica, tile = blockIdx.x - b * perReplica;
+    const int tr = tile / a.tilesK, tk = tile - tr * a.tilesK;
+    const int i0 = tr * a.TR, k0 = tk * a.TK;
+    int iBase = (i0 - a.HR) % L, kBase = (k0 - a.HK) % W;
+    iBase = iBase < 0 ? iBase + L : iBase;
+    kBase = kBase < 0 ? kBase + W : kBase;
+    uint32_t* reg0 = tsm;                                      // colour 0: [SR][SWX] words
+    uint32_t* reg1 = tsm + SR * SWX;
+    const size_t half = (size_t)L * W;
+    const uint32_t* g0 = (const uint32_t*)((const int8_t*)a.src + (size_t)b * 2 * half);
+    const uint32_t* g1 = (const uint32_t*)((const int8_t*)a.src + (size_t)b * 2 * half + half);
+    const int W4 = W >> 2;
+    pdl_wait();
+    for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
+    for (int task = threadIdx.x; task < SR * SWX; task += blockDim.x) {
+        const int r = task / SWX, wx = task - r * SWX;
+        int gi = iBase + r;
+        gi = gi >= L ? gi - L : gi;
+        gi = gi >= L ? gi - L : gi;
+        int gk = kBase + 4 * wx;
+        gk = gk >= W ? gk - W : gk;
+        gk = gk >= W ? gk - W : gk;
+        const size_t gw = (size_t)gi * W4 + (gk >> 2);
+        reg0[task] = __ldcg(g0 + gw);
+        reg1[task] = __ldcg(g1 + gw);
+    }
+    __syncthreads();
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
+    const uint32_t c1 = (uint32_t)b + a.replica_offset;
+    const bool never = stab[kTabNever] != 0u;
+    for (int s = 0; s < a.sweeps; ++s) {
+        const unsigned long long t = a.t0 + (unsigned long long)s;
+        const uint32_t c2 = (uint32_t)(t & 0xFFFFFFFFull);
+        const uint32_t c3lo = (uint32_t)((t >> 32) & 0xFFFFFFull) | (kDomainIsing << 28);
+        for (int colour = 0; colour < 2; ++colour) {
+            const uint32_t c3 = c3lo | ((uint32_t)colour << 24);
+            uint32_t* own1 = colour ? reg1 : reg0;
+            const uint32_t* oth1 = colour ? reg0 : reg1;
+            if (never) tiled_half_sweep<true>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1);
+            else tiled_half_sweep<false>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1);
+            __syncthreads();
+        }
+    }
+    // write back the interior (clipped at the lattice edge for the last tile row / column)
+    const int rows = min(a.TR, L - i0), wcols = min(a.TK, W - k0) >> 2;
+    uint32_t* o0 = (uint32_t*)((int8_t*)a.dst + (size_t)b * 2 * half);
+    uint32_t* o1 = (uint32_t*)((int8_t*)a.dst + (size_t)b * 2 * half + half);
+    for (int task = threadIdx.x; task < rows * wcols; task += blockDim.x) {
+        const int rr = task / wcols, ww = task - rr * wcols;
+        const int sidxw = (a.HR + rr) * SWX + (a.HK >> 2) + ww;
+        const size_t gw = (size_t)(i0 + rr) * W4 + ((k0 >> 2) + ww);
+        o0[gw] = reg0[sidxw];
+        o1[gw] = reg1[sidxw];
+    }
+}
+
 // ---- shared-memory-resident kernel: L % 32 == 0 and the replica (L^2 bytes) fits one CTA's shared memory.
 // One CTA per replica runs every sweep of the call: both colours stay in shared memory, the half-sweeps are
 // separated by __syncthreads() (a colour only reads the other colour), the Philox counter words of sweep t are
@@ -573,6 +679,84 @@ int launch_ising_int8_persistent(const SweepArgs& a, unsigned long long t0, long
         return 0;
     }
     return 1;
+}
+
+// Tile geometry for the tiled kernel: about one tile per SM (148 on a B200) over the whole batch, tiles as square as
+// the word granularity allows, 4 sweeps per launch (halo 8) when a tile has at least 32 rows, else 2 (halo 4).
+struct TileGeom {
+    int TR, TK, HR, HK, tilesR, tilesK, sweeps;
+    size_t smem;
+};
+
+static bool tile_geometry(int batch, int L, TileGeom& g) {
+    if (L % 8 != 0 || L < 16) return false;
+    const int W = L >> 1;
+    const long long N = (long long)L * L;
+    int perReplica = (148 + batch - 1) / batch;                 // tiles wanted per replica
+    if (perReplica < 1) perReplica = 1;
+    const double target = (double)N / perReplica;               // sites per tile (both colours)
+    int TK = (int)(sqrt(target / 2.0) / 4.0 + 0.5) * 4;          // same-colour columns: the tile is TR x 2 TK sites
+    if (TK < 16) TK = 16;
+    if (TK > W) TK = W;
+    int tilesK = (W + TK - 1) / TK;
+    TK = ((W + tilesK - 1) / tilesK + 3) / 4 * 4;                // even out, keep a multiple of 4
+    tilesK = (W + TK - 1) / TK;
+    int tilesR = (perReplica + tilesK - 1) / tilesK;
+    if (tilesR < 1) tilesR = 1;
+    int TR = (L + tilesR - 1) / tilesR;
+    if (TR < 8) TR = 8;
+    tilesR = (L + TR - 1) / TR;
+    g.TR = TR; g.TK = TK; g.tilesR = tilesR; g.tilesK = tilesK;
+    g.sweeps = TR >= 32 && TK >= 32 ? 4 : 2;
+    g.HR = 2 * g.sweeps;
+    g.HK = 2 * g.sweeps < 4 ? 4 : (2 * g.sweeps + 3) / 4 * 4;
+    g.smem = (size_t)2 * (TR + 2 * g.HR) * (TK + 2 * g.HK);
+    // the region may wrap around the lattice at most once (two conditional subtractions in the kernel)
+    if (TR + 2 * g.HR > 2 * L || TK + 2 * g.HK > 2 * W) return false;
+    return g.smem <= 200 * 1024;
+}
+
+bool ising_int8_tiled_fits(int batch, int L) {
+    TileGeom g;
+    return tile_geometry(batch, L, g);
+}
+
+int launch_ising_int8_tiled(const SweepArgs& a, void* shadow, unsigned long long t0, long long n_sweeps, cudaStream_t s) {
+    TileGeom g;
+    if (!tile_geometry(a.batch, a.L, g) || !shadow) return 0;
+    if (cudaFuncSetAttribute(ising_int8_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    TiledArgs t;
+    t.tables = a.tables; t.batch = a.batch; t.L = a.L; t.replica_offset = a.replica_offset;
+    t.TR = g.TR; t.TK = g.TK; t.HR = g.HR; t.HK = g.HK; t.tilesR = g.tilesR; t.tilesK = g.tilesK; t.rk = a.rk;
+    const unsigned grid = (unsigned)((long long)g.tilesR * g.tilesK * a.batch);
+    const long long words = (long long)(g.TR + 2 * g.HR) * ((g.TK + 2 * g.HK) >> 2);
+    const unsigned tpb = words >= 1024 ? kTiledThreads : 256;
+    void* cur = a.lattice;
+    void* other = shadow;
+    int launches = 0;
+    for (long long done = 0; done < n_sweeps; done += g.sweeps) {
+        t.src = cur; t.dst = other; t.t0 = t0 + (unsigned long long)done;
+        t.sweeps = (int)(n_sweeps - done < g.sweeps ? n_sweeps - done : g.sweeps);
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid, 1, 1);
+        cfg.blockDim = dim3(tpb, 1, 1);
+        cfg.dynamicSmemBytes = g.smem;
+        cfg.stream = s;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+        attr[0].val.programmaticStreamSerializationAllowed = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        cudaLaunchKernelEx(&cfg, ising_int8_tiled_kernel, t);
+        ++launches;
+        void* tmp = cur; cur = other; other = tmp;
+    }
+    if (cur != a.lattice)                                       // an odd number of launches: the result is in the shadow
+        cudaMemcpyAsync(a.lattice, cur, (size_t)a.batch * a.L * a.L, cudaMemcpyDeviceToDevice, s);
+    return launches;
 }
 
 // Opt the resident kernel in to more than 48 KiB of dynamic shared memory on the CURRENT device (called once per

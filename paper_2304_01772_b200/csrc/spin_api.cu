@@ -116,6 +116,7 @@ struct spin_sim {
     size_t sched_bytes = 0;
     uint32_t* h_sched = nullptr;            // pinned staging of the same size, guarded by sched_ev (recorded after its upload)
     cudaEvent_t sched_ev = nullptr;
+    void* d_shadow = nullptr;               // second lattice of the tiled kernel (allocated on first use)
     unsigned int* d_counter = nullptr;      // grid-barrier word of the persistent kernel
     bool any_never = false;                 // some replica's current table has a never-accepted class
     uint8_t* d_aux = nullptr;        // bit-packed kernel's constant 2 KiB lookup table, on this handle's device
@@ -282,13 +283,15 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
 bool use_resident(const spin_sim* sim, bool measure) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || !ising_int8_resident_fits(sim->L)) return false;
     if (sim->general || sim->d_bond_nat) return false;            // per-bond couplings run on the general kernels
-    if (sim->policy == SPIN_POLICY_STREAMING || sim->policy == SPIN_POLICY_PERSISTENT) return false;
+    if (sim->policy == SPIN_POLICY_STREAMING || sim->policy == SPIN_POLICY_PERSISTENT || sim->policy == SPIN_POLICY_TILED) return false;
     if (sim->policy == SPIN_POLICY_RESIDENT) return true;
     // Measured on B200 (profiles/r2_policy_grid.md): one CTA per replica wins for every batch size while a half-sweep of
     // a replica is a handful of warps (L <= 128: 3.1 vs 0.9 flips/ns at 1 x 64^2, 767 vs 500 at 256 x 128^2); for larger
     // replicas a CTA needs tens of microseconds per sweep, so it only pays when the batch fills the GPU (>= 1 CTA per SM)
     // AND the streaming kernel's blocks would be ragged (L = 160, 224: 766 vs 655 flips/ns at 256 x 224^2); small batches
     // of large resident-eligible replicas (4 x 416^2: 23 vs 112 flips/ns) go to the persistent / streaming kernels.
+    if (sim->L == 128 && (long long)sim->batch * sim->L * sim->L <= (1ll << 16) && sim->policy == SPIN_POLICY_AUTO && !measure)
+        return false;                                              // 1-4 replicas of 128^2: the tiled kernel spreads them over the SMs
     if (sim->L <= 128) return true;
     int tpb = 128;
     const int perReplica = (sim->L / 8) * (sim->L / 32);
@@ -312,6 +315,33 @@ bool use_persistent(const spin_sim* sim) {
 }
 
 SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour);
+
+// Temporally blocked tile kernel (ising_int8.cu): uniform Ising model, int8 layout, L % 8 == 0; several sweeps per launch
+// on tiles with halos, one tile per SM.  Measured (profiles/r2_policy_grid.md) its one-thread-per-word shared-memory
+// update costs ~40 instructions per site (17 in the streaming kernel) on top of the halo redundancy, so it only wins
+// where everything else is latency-bound: one to four replicas of 128 <= L <= 256 (1 x 128^2: 7.8 vs 4.7 flips/ns
+// resident; 1 x 224^2: 16.7 vs 10.4 persistent).  AUTO takes it for at most 2^16 sites with L >= 128.
+bool use_tiled(const spin_sim* sim) {
+    if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8) return false;
+    if (sim->general || sim->d_bond_nat) return false;
+    if (!ising_int8_tiled_fits(sim->batch, sim->L)) return false;
+    if (sim->policy == SPIN_POLICY_TILED) return true;
+    if (sim->policy != SPIN_POLICY_AUTO) return false;
+    return sim->L >= 128 && (long long)sim->batch * sim->L * sim->L <= (1ll << 16);
+}
+
+bool enqueue_tiled(spin_sim* sim, int64_t t0, int64_t n_sweeps, const uint32_t* tables = nullptr) {
+    if (!sim->d_shadow && cudaMalloc(&sim->d_shadow, sim->lattice_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        sim->d_shadow = nullptr;
+        return false;
+    }
+    SweepArgs a = sweep_args(sim, t0, 0);
+    if (tables) a.tables = tables;
+    const int n = launch_ising_int8_tiled(a, sim->d_shadow, (unsigned long long)t0, n_sweeps, sim->stream);
+    sim->launches += n;
+    return n > 0;
+}
 
 // Returns false when the cooperative launch was not possible (the caller streams instead).
 bool enqueue_persistent(spin_sim* sim, int64_t t0, int64_t n_sweeps, const uint32_t* tables = nullptr) {
@@ -483,6 +513,7 @@ void spin_destroy(spin_sim* sim) {
     if (sim->d_sched) cudaFree(sim->d_sched);
     if (sim->h_sched) cudaFreeHost(sim->h_sched);
     if (sim->sched_ev) cudaEventDestroy(sim->sched_ev);
+    if (sim->d_shadow) cudaFree(sim->d_shadow);
     if (sim->d_counter) cudaFree(sim->d_counter);
     if (sim->d_aux) cudaFree(sim->d_aux);
     if (sim->d_stage) cudaFree(sim->d_stage);
@@ -630,6 +661,7 @@ const char* spin_kernel_variant(const spin_sim* sim) {
     if (sim->model == SPIN_MODEL_POTTS) return potts_int8_variant(sim->L);
     if (sim->layout == SPIN_LAYOUT_BITPACKED) return "ising_bits_rows32";
     if (use_resident(sim, false)) return "ising_int8_resident";
+    if (use_tiled(sim)) return "ising_int8_tiled";
     if (use_persistent(sim)) return "ising_int8_persistent";
     return ising_int8_variant(sim->L);
 }
@@ -822,12 +854,14 @@ int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps
     bool sched_never = false;
     for (size_t k = 0; k < (size_t)n_steps * B; ++k) sched_never = sched_never || sim->h_sched[k * kTableStride + kTabNever] != 0u;
     sim->any_never = sched_never;
-    const bool persistent = !resident && use_persistent(sim);
+    const bool tiled = !resident && use_tiled(sim);
+    const bool persistent = !resident && !tiled && use_persistent(sim);
     for (int64_t k = 0; k < n_steps; ++k) {
         const uint32_t* tab = sim->d_sched + (size_t)k * B * kTableStride;
         const int64_t t0 = sweep_offset + k * sweeps_per_step;
         if (resident) {
             enqueue_resident(sim, t0, sweeps_per_step, false, nullptr, nullptr, nullptr, tab);
+        } else if (tiled && enqueue_tiled(sim, t0, sweeps_per_step, tab)) {
         } else if (persistent && enqueue_persistent(sim, t0, sweeps_per_step, tab)) {
         } else {
             for (int64_t t = t0; t < t0 + sweeps_per_step; ++t) {
@@ -843,7 +877,7 @@ int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps
 int spin_set_policy(spin_sim* sim, int32_t policy) {
     if (!sim) return fail(SPIN_ERR_INVALID, "spin_set_policy: NULL handle");
     if (policy != SPIN_POLICY_AUTO && policy != SPIN_POLICY_STREAMING && policy != SPIN_POLICY_RESIDENT &&
-        policy != SPIN_POLICY_PERSISTENT)
+        policy != SPIN_POLICY_PERSISTENT && policy != SPIN_POLICY_TILED)
         return fail(SPIN_ERR_INVALID, "spin_set_policy: unknown policy %d", (int)policy);
     sim->policy = policy;
     return SPIN_OK;
@@ -858,6 +892,7 @@ int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_
     if (rt != SPIN_OK) return rt;
     if (use_resident(sim, false)) {
         enqueue_resident(sim, sweep_offset, n_sweeps, false, nullptr, nullptr, nullptr);
+    } else if (use_tiled(sim) && enqueue_tiled(sim, sweep_offset, n_sweeps)) {
     } else if (!(use_persistent(sim) && enqueue_persistent(sim, sweep_offset, n_sweeps))) {
         for (int64_t t = sweep_offset; t < sweep_offset + n_sweeps; ++t) {
             enqueue_half_sweep(sim, t, 0);

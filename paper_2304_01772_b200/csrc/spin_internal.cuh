@@ -81,6 +81,22 @@ struct ResidentArgs {
     RoundKeys rk;
 };
 
+// Temporally blocked tile kernel (launch-bound shapes): a CTA owns TR rows x TK same-colour columns of one replica plus a
+// halo of HR rows / HK columns on every side and advances `sweeps` full sweeps per launch in shared memory.
+struct TiledArgs {
+    const void* src;          // int8: [B][2][L][L/2], read by every tile (interior + halo)
+    void* dst;                // same shape, a DIFFERENT buffer: tiles of one launch read each other's interiors as halos,
+                              // so the advanced interiors go to a second lattice and the two swap roles per launch
+    const uint32_t* tables;   // [B][kTableStride]
+    int32_t batch, L;
+    uint32_t replica_offset;
+    unsigned long long t0;    // first sweep index of this launch
+    int32_t sweeps;           // sweeps in this launch (2 * sweeps <= HR and <= HK)
+    int32_t TR, TK, HR, HK;   // TK, HK multiples of 4 (k = same-colour column index)
+    int32_t tilesR, tilesK;
+    RoundKeys rk;
+};
+
 struct InitArgs {
     void* lattice;
     const int32_t* q;         // [B] (Potts) or nullptr
@@ -140,6 +156,10 @@ const char* ising_int8_variant(int L);
 bool ising_int8_resident_fits(int L);                                       // a replica fits one CTA's shared memory
 int launch_ising_int8_persistent(const SweepArgs& a, unsigned long long t0, long long n_sweeps, unsigned int* counter,
                                  cudaStream_t s);                           // 0: not launched, use the streaming path
+// Enqueues n_sweeps sweeps from t0 with the tiled kernel (ceil(n_sweeps / sweeps-per-launch) launches); returns the
+// number of kernels launched, 0 if the shape does not qualify.
+int launch_ising_int8_tiled(const SweepArgs& a, void* shadow, unsigned long long t0, long long n_sweeps, cudaStream_t s);
+bool ising_int8_tiled_fits(int batch, int L);
 cudaError_t ising_int8_resident_configure();                                // per device: allow > 48 KiB dynamic shared memory
 int launch_ising_int8_resident(const ResidentArgs& a, cudaStream_t s);      // all n_sweeps in one launch
 const char* potts_int8_variant(int L);

@@ -1,5 +1,5 @@
 """Measure the kernel-selection policies of the int8 Ising path on a (batch, L) grid: flips/ns of SPIN_POLICY_AUTO,
-STREAMING, RESIDENT and PERSISTENT (CUDA-event timing through the binding, best of 3).  Prints a markdown table; the
+STREAMING, RESIDENT, PERSISTENT and TILED (CUDA-event timing through the binding, best of 3).  Prints a markdown table; the
 crossovers it shows are what `use_resident` / `use_persistent` in csrc/spin_api.cu encode (profiles/r2_policy_grid.md).
 
     python -m paper_2304_01772_b200.policy_grid
@@ -14,10 +14,10 @@ def main():
 
     import paper_2304_01772_b200 as sp
     names = {sp.SPIN_POLICY_AUTO: "auto", sp.SPIN_POLICY_STREAMING: "streaming", sp.SPIN_POLICY_RESIDENT: "resident",
-             sp.SPIN_POLICY_PERSISTENT: "persistent"}
+             sp.SPIN_POLICY_PERSISTENT: "persistent", sp.SPIN_POLICY_TILED: "tiled"}
     stream = torch.cuda.Stream()
-    print("| batch | L | sites | auto picks | auto | streaming | resident | persistent |")
-    print("|---|---|---|---|---|---|---|---|")
+    print("| batch | L | sites | auto picks | auto | streaming | resident | persistent | tiled |")
+    print("|---|---|---|---|---|---|---|---|---|")
     for L in (64, 128, 224, 256, 416, 640, 1024, 2560):
         for batch in (1, 4, 16, 64, 256):
             sites = batch * L * L
@@ -26,7 +26,8 @@ def main():
             n = int(max(20, min(2000, 4e9 / sites / 4)))
             row = []
             picked = ""
-            for policy in (sp.SPIN_POLICY_AUTO, sp.SPIN_POLICY_STREAMING, sp.SPIN_POLICY_RESIDENT, sp.SPIN_POLICY_PERSISTENT):
+            for policy in (sp.SPIN_POLICY_AUTO, sp.SPIN_POLICY_STREAMING, sp.SPIN_POLICY_RESIDENT, sp.SPIN_POLICY_PERSISTENT,
+                           sp.SPIN_POLICY_TILED):
                 sim = sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=1, cuda_stream=stream.cuda_stream)
                 sim.spin_set_policy(policy)
                 variant = sim.spin_kernel_variant()

@@ -28,7 +28,7 @@ def _mk_ising(batch, L, seed, layout="int8", replica_offset=0, policy=None):
 # every int8 Ising case runs through the three kernel families: the two-launches-per-sweep HBM kernels, the
 # shared-memory-resident multi-sweep kernel and the persistent cooperative kernel (each used when the shape allows it,
 # else the call falls back to streaming)
-POLICIES = [sp.SPIN_POLICY_STREAMING, sp.SPIN_POLICY_RESIDENT, sp.SPIN_POLICY_PERSISTENT]
+POLICIES = [sp.SPIN_POLICY_STREAMING, sp.SPIN_POLICY_RESIDENT, sp.SPIN_POLICY_PERSISTENT, sp.SPIN_POLICY_TILED]
 
 
 def _mk_potts(batch, L, q, seed, replica_offset=0):
@@ -312,4 +312,30 @@ def test_persistent_kernel_many_sweeps_in_one_launch(oracle_mod, batch, L, n):
         # a never-accepted class (beta = 20) cannot use the kernel: the call streams, results unchanged
         sim.spin_sweep(np.full(batch, 20.0), 1.0, 0.0, 2, 100)
         oracle_mod.sweep(ref, np.full(batch, 20.0), 1.0, 0.0, seed=seed, n_sweeps=2, sweep_offset=100)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+
+
+# ------------------------------------------------------------- temporally blocked tile kernel (launch-bound shapes)
+@pytest.mark.parametrize("batch,L,n", [(1, 640, 13), (3, 128, 9), (2, 1024, 6), (5, 96, 7), (1, 2560, 5), (1, 16, 11),
+                                       (2, 40, 6), (7, 200, 5), (150, 64, 5)])
+def test_tiled_kernel_equals_oracle(oracle_mod, batch, L, n):
+    """Tiles with halos advance several sweeps per launch in shared memory: sweep counts that are not multiples of the
+    sweeps per launch, tile grids that do not divide the lattice, regions that wrap around small lattices, never-classes."""
+    seed = 80 + L
+    beta = np.linspace(0.25, 0.65, batch)
+    ref = oracle_mod.init(batch, L, seed=seed)
+    with _mk_ising(batch, L, seed, policy=sp.SPIN_POLICY_TILED) as sim:
+        assert sim.spin_kernel_variant() == "ising_int8_tiled"
+        sim.spin_sweep(beta, 1.0, 0.03, n, 2)
+        oracle_mod.sweep(ref, beta, 1.0, 0.03, seed=seed, n_sweeps=n, sweep_offset=2)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        sim.spin_sweep(beta, 1.0, 0.03, 1, 2 + n)
+        oracle_mod.sweep(ref, beta, 1.0, 0.03, seed=seed, n_sweeps=1, sweep_offset=2 + n)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        E, M = sim.spin_observables()
+        Eo, Mo = oracle_mod.ising_observables(ref)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+        cold = np.full(batch, 20.0)
+        sim.spin_sweep(cold, 1.0, 0.0, 3, (1 << 32) - 1)
+        oracle_mod.sweep(ref, cold, 1.0, 0.0, seed=seed, n_sweeps=3, sweep_offset=(1 << 32) - 1)
         assert np.array_equal(sim.spin_get_spins(), ref)
