@@ -400,9 +400,10 @@ def dmc_entries(runner, sp, args, peaks):
     res = {}
     updates = float(B) * L * L * n_sweeps
     # algorithmic bytes per site and sweep, fp32: forward = read the lattice, write it, read both
-    # coupling arrays once (16); with a stored trajectory the colour-0 state is written too (20); backward 128
+    # coupling arrays once (16); with a stored trajectory the colour-0 state is written too (20); backward per half-sweep:
+    # read s, Jh, Jv, g (16), write g_prev (4), read-modify-write dJh, dJv (16) = 36, i.e. 72 per sweep
     for key, fn, bytes_per_site_sweep, launches in (("DMC-forward", fwd, 16.0, n_sweeps),
-                                                    ("DMC-forward+backward", train, 20.0 + 128.0, 5 * n_sweeps)):
+                                                    ("DMC-forward+backward", train, 20.0 + 72.0, 3 * n_sweeps)):
         with torch.cuda.stream(stream):
             for k in range(args.warmup):
                 fn(k)
@@ -421,7 +422,7 @@ def dmc_entries(runner, sp, args, peaks):
         res[key] = {"workload": "DMC: Ising +-J-glass couplings (normal), fp32, %dx%d^2, %d sweeps, alpha=%g" % (B, L, n_sweeps, alpha),
                     "value": float(updates * len(ms) / (ms.sum() * 1e6)), "unit": UNIT, "best": float(vals.max()),
                     "median": float(np.median(vals)), "ms_per_step": float(ms.mean()),
-                    "kernel": "dmc_fused_sweep_kernel" + ("" if key == "DMC-forward" else " + dmc_backward1/2_kernel<float,4>"),
+                    "kernel": "dmc_march_sweep_kernel" + ("" if key == "DMC-forward" else " + dmc_march_backward_kernel"),
                     "gpu_launches_per_step": launches, "dtype": "f32",
                     "roofline": {"bound": "hbm", "achieved": gbs, "peak": peaks["hbm_gbs"], "unit": "GB/s",
                                  "frac": gbs / peaks["hbm_gbs"], "bytes_per_site_per_sweep": bytes_per_site_sweep,

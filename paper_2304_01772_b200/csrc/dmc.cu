@@ -223,6 +223,231 @@ __global__ void __launch_bounds__(256) dmc_fused_sweep_kernel(DmcArgs a, const f
     }
 }
 
+// ---- row-marching forward sweep (fp32, 256 <= L <= 2048, L % 8 == 0): the fused sweep above re-reads the couplings from
+// L2 for the second colour and pays a full memory latency per task; here a thread owns one 8-site chunk COLUMN and
+// marches down the R rows of its tile with everything it needs twice kept in registers: three source rows, three
+// colour-0 rows, the couplings of the current and the previous row.  Per row step: prefetch the next source row and the
+// next row's couplings, compute the colour-0 update A_i of row i, publish the two edge values of A_i to shared memory (the
+// neighbouring chunks need them for the colour-1 update), barrier, compute the colour-1 update of row i-1 from A_{i-2},
+// A_{i-1}, A_i and store it.  A block is one full row of chunks (L/8 threads), so the periodic wrap in the row stays in the
+// block; tiles overlap by one halo row at each end (recomputed, identical by construction).  Every source element and
+// every coupling is loaded from HBM exactly once per sweep (+ 4/R for the halo rows).
+__global__ void __launch_bounds__(256) dmc_march_sweep_kernel(DmcArgs a, const float* __restrict__ src, float* __restrict__ mid,
+                                                              float* __restrict__ dst, const float* __restrict__ Jh,
+                                                              const float* __restrict__ Jv, int R, int tiles) {
+    __shared__ float sEdge[3][256][2];                       // [row slot][chunk][first, last] of the colour-0 row
+    const int L = a.L, cpr = L >> 3, cidx = threadIdx.x;
+    const int b = blockIdx.x / tiles, tile = blockIdx.x - b * tiles;
+    const int i0 = tile * R, rows = min(R, L - i0);
+    const size_t base = (size_t)b * L * L;
+    const float beta = (float)a.beta[b];
+    const uint32_t c3lo = a.c3 & ~(0xFu << 24);
+    const int j0 = cidx << 3;
+    const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 8 == L ? 0 : j0 + 8;
+    const int cl = cidx == 0 ? cpr - 1 : cidx - 1, cr = cidx == cpr - 1 ? 0 : cidx + 1;
+    auto wrapi = [L](int i) { return i < 0 ? i + L : (i >= L ? i - L : i); };
+    // source rows i-1, i, i+1 of the first step (i = i0 - 1), couplings of row i and Jv of row i-1
+    float Sm[8], Sc[8], Sp[8], Sn[8];                         // rows i-1, i, i+1 and the prefetched i+2
+    float Am[8], Ac[8], An[8];                                // colour-0 rows i-2, i-1, i (An = newest)
+    float JhC[8], JhP[8], JhN[8], JvM[8], JvC[8], JvP2[8], JvN[8];
+    float jhlC, jhlP = 0.f, jhlN, slC, srC, slN, srN;
+    int i = wrapi(i0 - 1);
+    load8(src + base + (size_t)wrapi(i - 1) * L + j0, Sm);
+    load8(src + base + (size_t)i * L + j0, Sc);
+    load8(src + base + (size_t)wrapi(i + 1) * L + j0, Sp);
+    load8(Jh + base + (size_t)i * L + j0, JhC);
+    load8(Jv + base + (size_t)wrapi(i - 1) * L + j0, JvM);
+    load8(Jv + base + (size_t)i * L + j0, JvC);
+    jhlC = Jh[base + (size_t)i * L + jl];
+    slC = src[base + (size_t)i * L + jl];
+    srC = src[base + (size_t)i * L + jr];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) { Am[e] = 0.f; Ac[e] = 0.f; JhP[e] = 0.f; JvP2[e] = 0.f; }
+    for (int step = 0; step < rows + 2; ++step) {
+        // rows of this step: i (colour 0), i - 1 (colour 1, once step >= 2)
+        const int inext = i == L - 1 ? 0 : i + 1;             // row i + 1
+        const int inn = inext == L - 1 ? 0 : inext + 1;       // row i + 2
+        const bool more = step + 1 < rows + 2;
+        if (more) {                                           // prefetch what the next step needs
+            load8(src + base + (size_t)inn * L + j0, Sn);
+            load8(Jh + base + (size_t)inext * L + j0, JhN);
+            load8(Jv + base + (size_t)inext * L + j0, JvN);
+            jhlN = Jh[base + (size_t)inext * L + jl];
+            slN = src[base + (size_t)inext * L + jl];
+            srN = src[base + (size_t)inext * L + jr];
+        }
+        // colour 0 on row i
+        dmc_chunk(a, b, i, cidx, i & 1, c3lo, Sc, Sm, Sp, slC, srC, JhC, jhlC, JvM, JvC, beta, An);
+        const int slot = step % 3;
+        sEdge[slot][cidx][0] = An[0];
+        sEdge[slot][cidx][1] = An[7];
+        if (mid && step >= 1 && step <= rows) store8(mid + base + (size_t)i * L + j0, An);
+        __syncthreads();
+        if (step >= 2) {
+            // colour 1 on row i - 1: neighbours A_{i-2} (Am), A_i (An), own A_{i-1} (Ac); couplings of row i - 1
+            const int ip = i == 0 ? L - 1 : i - 1;
+            const int ps = (step + 2) % 3;                    // slot of step - 1
+            float out[8];
+            dmc_chunk(a, b, ip, cidx, 1 - (ip & 1), c3lo | (1u << 24), Ac, Am, An, sEdge[ps][cl][1], sEdge[ps][cr][0], JhP, jhlP,
+                      JvP2, JvM, beta, out);
+            store8(dst + base + (size_t)ip * L + j0, out);
+        }
+        // rotate the windows: rows move up by one
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            Am[e] = Ac[e]; Ac[e] = An[e];
+            JhP[e] = JhC[e]; JvP2[e] = JvM[e]; JvM[e] = JvC[e];
+            Sm[e] = Sc[e]; Sc[e] = Sp[e];
+            if (more) { Sp[e] = Sn[e]; JhC[e] = JhN[e]; JvC[e] = JvN[e]; }
+        }
+        jhlP = jhlC;
+        if (more) { jhlC = jhlN; slC = slN; srC = srN; }
+        i = inext;
+    }
+}
+
+// ---- row-marching backward half-sweep (fp32, 256 <= L <= 2048, L % 8 == 0): passes 1 and 2 below fused, so that G and D
+// never travel through HBM.  Same skeleton as dmc_march_sweep_kernel: a thread owns one 8-site chunk column; per step it
+// computes G_{i+1}, D_{i+1} of the next row (recomputing p, q from the stored state), publishes the edge values of G_{i+1},
+// and finishes row i, which needs G_{i-1}, G_i, G_{i+1}:
+//   g_prev_i[j] = D_i[j] + G_{i-1}[j] Jv_{i-1}[j] + G_{i+1}[j] Jv_i[j] + G_i[j-1] Jh_i[j-1] + G_i[j+1] Jh_i[j]
+//   dJh_i[j] += G_i[j] s_i[j+1] + G_i[j+1] s_i[j],   dJv_i[j] += G_i[j] s_{i+1}[j] + G_{i+1}[j] s_i[j]
+// Per site and half-sweep: read s, Jh, Jv, g (16 B), write g_prev (4), read-modify-write dJh, dJv (16) = 36 B instead of 64.
+template <int kPar>
+__device__ __forceinline__ void dmc_chunk_bwd_par(const DmcArgs& a, const uint32_t r[4], const float c[8], const float u[8],
+                                                  const float d[8], float left, float right, const float jh[8], float jhl,
+                                                  const float jvu[8], const float jvc[8], float beta, const float g[8],
+                                                  float G[8], float D[8], double& sb, double& sh) {
+#pragma unroll
+    for (int e = 0; e < 8; ++e) { G[e] = 0.f; D[e] = g[e]; }
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+        const int e = 2 * m + kPar;
+        const float sl = e == 0 ? left : c[e > 0 ? e - 1 : 0];
+        const float sr = e == 7 ? right : c[e < 7 ? e + 1 : 7];
+        const float jl = e == 0 ? jhl : jh[e > 0 ? e - 1 : 0];
+        const float sx = c[e];
+        const float rr = (float)(r[m] >> 8) * (float)(1.0 / 16777216.0);
+        const float F = jvu[e] * u[e] + jvc[e] * d[e] + jl * sl + jh[e] * sr + (float)a.h;
+        const float p = expf(-beta * (2.0f * sx * F));
+        const float q = __fdividef(1.0f, 1.0f + expf(-(float)a.alpha * (p - rr)));
+        const float A = (float)a.alpha * q * (1.0f - q) * p;
+        D[e] = g[e] * ((1.0f - 2.0f * q) + 4.0f * beta * A * sx * F);
+        G[e] = g[e] * (4.0f * beta * A * sx * sx);
+        sb += (double)(g[e] * (4.0f * A * sx * sx * F));
+        sh += (double)G[e];
+    }
+}
+
+__global__ void __launch_bounds__(256) dmc_march_backward_kernel(DmcArgs a, const float* __restrict__ src, const float* __restrict__ Jh,
+                                                                 const float* __restrict__ Jv, const float* __restrict__ gnew,
+                                                                 float* __restrict__ gprev, float* __restrict__ gJh,
+                                                                 float* __restrict__ gJv, double* gbeta, double* gh, int R, int tiles) {
+    __shared__ float sEdge[3][256][2];                       // [row slot][chunk][first, last] of G
+    __shared__ double red[2][8];
+    const int L = a.L, cpr = L >> 3, cidx = threadIdx.x;
+    const int b = blockIdx.x / tiles, tile = blockIdx.x - b * tiles;
+    const int i0 = tile * R, rows = min(R, L - i0);
+    const size_t base = (size_t)b * L * L;
+    const float beta = (float)a.beta[b];
+    const int j0 = cidx << 3;
+    const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 8 == L ? 0 : j0 + 8;
+    const int cl = cidx == 0 ? cpr - 1 : cidx - 1, cr = cidx == cpr - 1 ? 0 : cidx + 1;
+    auto wrapi = [L](int i) { return i < 0 ? i + L : (i >= L ? i - L : i); };
+    double sb = 0.0, sh = 0.0;
+    // the step for row i computes G_i, D_i (rows i0 - 1 .. i0 + rows) and finishes row i - 1 (rows i0 .. i0 + rows - 1)
+    float Sm[8], Sc[8], Sp[8], Sn[8];                         // state rows i-1, i, i+1, prefetched i+2
+    float Gm[8], Gc[8], Gn[8], Dc[8], Dn[8];                  // G rows i-2, i-1, i; D rows i-1, i
+    float JhC[8], JhP[8], JhN[8], JvM[8], JvC[8], JvP2[8], JvN[8], gC[8], gN[8];
+    float jhlC, jhlP = 0.f, jhlN, slC, srC, slN, srN, srP = 0.f;
+    int i = wrapi(i0 - 1);
+    load8(src + base + (size_t)wrapi(i - 1) * L + j0, Sm);
+    load8(src + base + (size_t)i * L + j0, Sc);
+    load8(src + base + (size_t)wrapi(i + 1) * L + j0, Sp);
+    load8(Jh + base + (size_t)i * L + j0, JhC);
+    load8(Jv + base + (size_t)wrapi(i - 1) * L + j0, JvM);
+    load8(Jv + base + (size_t)i * L + j0, JvC);
+    load8(gnew + base + (size_t)i * L + j0, gC);
+    jhlC = Jh[base + (size_t)i * L + jl];
+    slC = src[base + (size_t)i * L + jl];
+    srC = src[base + (size_t)i * L + jr];
+#pragma unroll
+    for (int e = 0; e < 8; ++e) { Gm[e] = 0.f; Gc[e] = 0.f; Dc[e] = 0.f; JhP[e] = 0.f; JvP2[e] = 0.f; }
+    for (int step = 0; step < rows + 2; ++step) {
+        const int inext = i == L - 1 ? 0 : i + 1;
+        const int inn = inext == L - 1 ? 0 : inext + 1;
+        const bool more = step + 1 < rows + 2;
+        if (more) {
+            load8(src + base + (size_t)inn * L + j0, Sn);
+            load8(Jh + base + (size_t)inext * L + j0, JhN);
+            load8(Jv + base + (size_t)inext * L + j0, JvN);
+            load8(gnew + base + (size_t)inext * L + j0, gN);
+            jhlN = Jh[base + (size_t)inext * L + jl];
+            slN = src[base + (size_t)inext * L + jl];
+            srN = src[base + (size_t)inext * L + jr];
+        }
+        {   // G_i, D_i; the beta / h sums count interior rows only (the halo rows belong to the neighbouring tiles)
+            uint32_t r[4];
+            philox4x32_10(a.rk, (uint32_t)i * (uint32_t)(L >> 3) + (uint32_t)cidx, (uint32_t)b + a.replica_offset, a.c2, a.c3, r);
+            double tb = 0.0, th = 0.0;
+            if (((i + a.colour) & 1) == 0) dmc_chunk_bwd_par<0>(a, r, Sc, Sm, Sp, slC, srC, JhC, jhlC, JvM, JvC, beta, gC, Gn, Dn, tb, th);
+            else dmc_chunk_bwd_par<1>(a, r, Sc, Sm, Sp, slC, srC, JhC, jhlC, JvM, JvC, beta, gC, Gn, Dn, tb, th);
+            if (step >= 1 && step <= rows) { sb += tb; sh += th; }
+        }
+        const int slot = step % 3;
+        sEdge[slot][cidx][0] = Gn[0];
+        sEdge[slot][cidx][1] = Gn[7];
+        __syncthreads();
+        if (step >= 2) {
+            // finish row ip = i - 1: G_{i-2} = Gm, G_{i-1} = Gc, G_i = Gn; state rows: s_{i-1} = Sm, s_i = Sc;
+            // couplings: Jh_{i-1} = JhP (left edge jhlP), Jv_{i-2} = JvP2, Jv_{i-1} = JvM
+            const int ip = i == 0 ? L - 1 : i - 1;
+            const int ps = (step + 2) % 3;
+            const float gl = sEdge[ps][cl][1], gr = sEdge[ps][cr][0];
+            const size_t off = base + (size_t)ip * L + j0;
+            float ah[8], av[8], out[8];
+            load8(gJh + off, ah);
+            load8(gJv + off, av);
+#pragma unroll
+            for (int e = 0; e < 8; ++e) {
+                const float gleft = e == 0 ? gl : Gc[e > 0 ? e - 1 : 0];
+                const float gright = e == 7 ? gr : Gc[e < 7 ? e + 1 : 7];
+                const float jleft = e == 0 ? jhlP : JhP[e > 0 ? e - 1 : 0];
+                const float sright = e == 7 ? srP : Sm[e < 7 ? e + 1 : 7];
+                out[e] = Dc[e] + (Gm[e] * JvP2[e] + Gn[e] * JvM[e] + gleft * jleft + gright * JhP[e]);
+                ah[e] += Gc[e] * sright + gright * Sm[e];
+                av[e] += Gc[e] * Sc[e] + Gn[e] * Sm[e];
+            }
+            store8(gprev + off, out);
+            store8(gJh + off, ah);
+            store8(gJv + off, av);
+        }
+#pragma unroll
+        for (int e = 0; e < 8; ++e) {
+            Gm[e] = Gc[e]; Gc[e] = Gn[e]; Dc[e] = Dn[e];
+            JhP[e] = JhC[e]; JvP2[e] = JvM[e]; JvM[e] = JvC[e];
+            Sm[e] = Sc[e]; Sc[e] = Sp[e];
+            if (more) { Sp[e] = Sn[e]; JhC[e] = JhN[e]; JvC[e] = JvN[e]; gC[e] = gN[e]; }
+        }
+        jhlP = jhlC; srP = srC;
+        if (more) { jhlC = jhlN; slC = slN; srC = srN; }
+        i = inext;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sb += __shfl_xor_sync(0xFFFFFFFFu, sb, o);
+        sh += __shfl_xor_sync(0xFFFFFFFFu, sh, o);
+    }
+    if ((threadIdx.x & 31) == 0) { red[0][threadIdx.x >> 5] = sb; red[1][threadIdx.x >> 5] = sh; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tb = 0.0, th = 0.0;
+        for (int k = 0; k < (int)((blockDim.x + 31) >> 5); ++k) { tb += red[0][k]; th += red[1][k]; }
+        atomicAdd(gbeta + b, tb);
+        atomicAdd(gh + b, th);
+    }
+}
+
 // Backward pass 1: blocks never straddle replicas (grid = blocks per replica x batch), so the beta / h sums reduce per block.
 template <typename T, int V>
 __global__ void __launch_bounds__(256) dmc_backward1_kernel(DmcArgs a, const T* __restrict__ src, const T* __restrict__ Jh,
@@ -389,6 +614,12 @@ bool fused_ok(int dtype, int L) { return dtype == SPIN_DTYPE_F32 && L % 8 == 0 &
 
 cudaError_t forward_sweep_fused(const DmcArgs& a, const void* src, void* mid, void* dst, const void* Jh, const void* Jv,
                                 cudaStream_t s) {
+    if (a.L >= 256) {                                         // row-marching kernel: one block = one row of chunks, R rows per tile
+        const int R = 32, tiles = (a.L + R - 1) / R;
+        dmc_march_sweep_kernel<<<(unsigned)((long long)tiles * a.batch), a.L >> 3, 0, s>>>(a, (const float*)src, (float*)mid, (float*)dst,
+                                                                                         (const float*)Jh, (const float*)Jv, R, tiles);
+        return cudaGetLastError();
+    }
     const int R = fused_tile_rows(a.L), tiles = (a.L + R - 1) / R;
     const size_t smem = (size_t)(R + 2) * a.L * sizeof(float);
     cudaError_t e = cudaFuncSetAttribute(dmc_fused_sweep_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
@@ -418,6 +649,13 @@ void launch_backward(const DmcArgs& a, const void* src, const void* Jh, const vo
 
 void backward_half(int dtype, const DmcArgs& a, const void* src, const void* Jh, const void* Jv, const void* gnew, void* D,
                    void* G, double* gbeta, double* gh, void* gJh, void* gJv, cudaStream_t s) {
+    if (dtype == SPIN_DTYPE_F32 && a.L % 8 == 0 && a.L >= 256 && a.L <= 2048) {
+        const int R = 32, tiles = (a.L + R - 1) / R;          // fused row-marching kernel: g_prev lands in D, G is unused
+        dmc_march_backward_kernel<<<(unsigned)((long long)tiles * a.batch), a.L >> 3, 0, s>>>(
+            a, (const float*)src, (const float*)Jh, (const float*)Jv, (const float*)gnew, (float*)D, (float*)gJh, (float*)gJv, gbeta, gh,
+            R, tiles);
+        return;
+    }
     if (dtype == SPIN_DTYPE_F64) launch_backward<double, 2>(a, src, Jh, Jv, gnew, D, G, gbeta, gh, gJh, gJv, s);
     else if (a.L % 4 == 0) launch_backward<float, 4>(a, src, Jh, Jv, gnew, D, G, gbeta, gh, gJh, gJv, s);
     else launch_backward<float, 2>(a, src, Jh, Jv, gnew, D, G, gbeta, gh, gJh, gJv, s);
