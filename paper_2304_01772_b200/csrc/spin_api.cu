@@ -189,7 +189,9 @@ int upload_general_thresholds(spin_sim* sim, const double* beta) {
     bool same = sim->g_beta.size() == B;
     for (size_t b = 0; same && b < B; ++b) same = sim->g_beta[b] == beta[b];
     if (same) return SPIN_OK;                               // thresholds on the device are current
-    std::vector<uint32_t> thr(B * N * 32), alw(B * N);
+    std::vector<uint32_t> thr, alw;
+    try { thr.resize(B * N * 32); alw.resize(B * N); }
+    catch (...) { return fail(SPIN_ERR_NOMEM, "spin_sweep: out of host memory for %zu per-site thresholds", B * N * 32); }
     for (size_t b = 0; b < B; ++b)
         for (int i = 0; i < L; ++i)
             for (int j = 0; j < L; ++j) {
@@ -211,7 +213,7 @@ int upload_general_thresholds(spin_sim* sim, const double* beta) {
     CUDA_TRY(cudaMemcpyAsync(sim->d_thr, thr.data(), thr.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, sim->stream));
     CUDA_TRY(cudaMemcpyAsync(sim->d_alw, alw.data(), alw.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, sim->stream));
     CUDA_TRY(cudaStreamSynchronize(sim->stream));           // the host vectors go out of scope
-    sim->g_beta.assign(beta, beta + B);
+    try { sim->g_beta.assign(beta, beta + B); } catch (...) { sim->g_beta.clear(); }   // no cache: rebuilt next call
     return SPIN_OK;
 }
 
@@ -219,7 +221,9 @@ int upload_general_thresholds(spin_sim* sim, const double* beta) {
 int upload_potts_general(spin_sim* sim, const double* beta, double J, double h) {
     const size_t B = (size_t)sim->batch;
     if (!sim->d_tab2) CUDA_TRY(cudaMalloc(&sim->d_tab2, sizeof(unsigned long long) * 9 * 255 * B));
-    std::vector<unsigned long long> tab(B * 9 * 255, 0ull);
+    std::vector<unsigned long long> tab;
+    try { tab.assign(B * 9 * 255, 0ull); }
+    catch (...) { return fail(SPIN_ERR_NOMEM, "spin_sweep: out of host memory for the Potts class tables"); }
     for (size_t b = 0; b < B; ++b) {
         const int q = sim->q[b];
         for (int dn = -4; dn <= 4; ++dn)
