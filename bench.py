@@ -248,7 +248,9 @@ class Runner:
                 mom = np.zeros((w.batch, 8), dtype=np.int64)
                 if w.therm:
                     sim.spin_sweep(w.beta, w.J, w.h, w.therm, off)
+                l0 = sim.spin_kernel_launches()
                 sim.spin_sweep_measure(w.beta, w.J, w.h, w.n_sweeps - w.therm, off + w.therm, trace=False, moments=mom)
+                state["measure_launches"] = sim.spin_kernel_launches() - l0
                 if events:
                     events[1].record(stream)
             if events:
@@ -273,8 +275,12 @@ class Runner:
         launches = sim.spin_kernel_launches() - launches0
         step_ms = [e[0].elapsed_time(e[2]) for e in ev]
         sweep_ms = [e[0].elapsed_time(e[1]) for e in ev]
+        kernel = sim.spin_kernel_variant()
+        if mode == "moments" and state.get("measure_launches") == 1:
+            # the measured sweeps ran in one launch: the shared-memory-resident kernel with fused E / M / moments
+            kernel += " (thermalisation) + ising_int8_resident (measured sweeps, reductions fused)"
         res = {"sim": sim, "step_ms": step_ms, "sweep_ms": sweep_ms, "launches": int(launches),
-               "launches_per_sweep_call": state["per_call"], "kernel": sim.spin_kernel_variant(), "state": state,
+               "launches_per_sweep_call": state["per_call"], "kernel": kernel, "state": state,
                "step_fn": step}
         if e2e_steps:
             host_lat = torch.empty((w.batch, w.L, w.L), dtype=torch.int8).pin_memory()
