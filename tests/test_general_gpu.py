@@ -160,3 +160,25 @@ def test_schedule_argument_checks():
         with pytest.raises(sp.SpinError) as e:
             sim.spin_sweep_schedule(np.array([[0.1, 0.2]]), 1.0, 0.0, 3)
         assert e.value.code == sp.SPIN_ERR_UNSUPPORTED
+
+
+def test_schedule_with_int8_bond_signs_and_for_potts():
+    """The schedule call on the remaining class-table models: +-J signs on the int8 layout, and the uniform Potts model."""
+    B, L, seed = 2, 32, 55
+    steps = np.array([[0.2, 0.3], [0.6, 0.7], [1.5, 2.0]])
+    Jh, Jv = _signs(3, B, L)
+    ref = oracle.init(B, L, seed=seed)
+    with sp.spin_create_ex(B, L, sp.SPIN_MODEL_ISING, seed=seed) as sim:
+        sim.spin_set_bonds(Jh, Jv)
+        sim.spin_sweep_schedule(steps, 1.0, 0.0, 3, sweep_offset=1)
+        oracle.sweep_schedule(ref, steps, 1.0, 0.0, seed, 3, sweep_offset=1, Jh=Jh, Jv=Jv)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+    q = [3, 8]
+    ref = oracle.init(B, L, seed=seed, q=q)
+    with sp.spin_create_ex(B, L, sp.SPIN_MODEL_POTTS, q_per_replica=np.array(q, dtype=np.int32), seed=seed) as sim:
+        sim.spin_sweep_schedule(steps, 1.0, 0.0, 3, sweep_offset=1)
+        oracle.sweep_schedule(ref, steps, 1.0, 0.0, seed, 3, sweep_offset=1, q=q)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        with pytest.raises(sp.SpinError) as e:                       # a Potts field needs the general kernel: per-call only
+            sim.spin_sweep_schedule(steps, 1.0, 0.1, 3)
+        assert e.value.code == sp.SPIN_ERR_UNSUPPORTED
