@@ -208,7 +208,8 @@ SPIN_API int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_
  * lattice).  SPIN_POLICY_AUTO picks per shape; SPIN_POLICY_STREAMING forces the two-launches-
  * per-sweep HBM kernels; SPIN_POLICY_RESIDENT uses the shared-memory-resident multi-sweep kernel (one CTA per
  * replica, all sweeps of a call in one launch, E / M reductions fused) whenever the shape allows it (Ising, int8
- * layout, L a multiple of 32, L*L <= 192 KiB) and falls back to streaming otherwise.  SPIN_POLICY_PERSISTENT uses the
+ * layout, L a multiple of 32, L*L <= 192 KiB; bit-packed layout with uniform couplings, L*L/8 <= 200 KiB, plain sweeps
+ * only) and falls back to streaming otherwise.  SPIN_POLICY_PERSISTENT uses the
  * persistent cooperative kernel (all sweeps of a call in one launch, the lattice in L2, a grid-wide barrier between
  * half-sweeps) whenever the shape allows it (Ising, int8 layout, L a multiple of 32, uniform couplings, no class whose
  * acceptance threshold is 0); AUTO takes it for batches of at most 2^21 sites that do not go to the resident kernel.  SPIN_POLICY_TILED uses the temporally blocked tile kernel (a CTA advances

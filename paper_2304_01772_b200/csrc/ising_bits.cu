@@ -187,7 +187,70 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) ising_bits_kernel(SweepA
     else march_rows<kColour, false, kRows, kBonds>(a, stab, sT, never, slot, b, rb, x);
 }
 
+// ---- shared-memory-resident kernel ("a 1024^2 replica is 128 KiB as bits and fits one CTA"): one CTA per
+// replica keeps both colours in shared memory and runs every sweep of a call in one launch, half-sweeps separated by
+// __syncthreads(): zero HBM traffic per sweep.  One thread per 32-site word per pass; the side of the horizontal
+// neighbour depends on the row parity and is handled with selects (no divergence).  The kernels are ALU-bound, so this
+// only removes launch gaps; with one CTA per replica it needs a batch of at least the SM count to match the streaming
+// kernels and is used on request (SPIN_POLICY_RESIDENT), not by AUTO.
+constexpr int kBitsResThreads = 256;
+
+__global__ void __launch_bounds__(kBitsResThreads) ising_bits_resident_kernel(ResidentArgs a, const uint8_t* __restrict__ aux) {
+    extern __shared__ __align__(16) uint32_t blat[];          // [2][L][L/64] words
+    __shared__ uint32_t stab[16];
+    __shared__ __align__(16) uint8_t sT[kAuxBytes];
+    __shared__ uint32_t sidx[4 * kBitsResThreads];            // word e of thread t at [(t >> 7) * 512 + e * 128 + (t & 127)]
+    const int L = a.L, WW = L >> 6, half = L * WW;
+    const int b = blockIdx.x;
+    uint32_t* g = (uint32_t*)a.lattice + (size_t)b * 2 * half;
+    for (int k = threadIdx.x; k < 2 * half; k += blockDim.x) blat[k] = g[k];
+    for (int k = threadIdx.x; k < kAuxBytes / 16; k += blockDim.x) ((uint4*)sT)[k] = ((const uint4*)aux)[k];
+    const uint32_t* tab = a.tables + (size_t)b * kTableStride;
+    if (threadIdx.x < 16) stab[threadIdx.x] = tab[threadIdx.x];
+    const uint32_t never = tab[kTabNever];
+    __syncthreads();
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[(threadIdx.x >> 7) * 512 + (threadIdx.x & 127)]);
+    const uint32_t c1 = (uint32_t)b + a.replica_offset;
+    SweepArgs sa;                                             // update_word reads rk, c2, c3 from here
+    sa.rk = a.rk;
+    for (long long s = 0; s < a.n_sweeps; ++s) {
+        const unsigned long long t = a.t0 + (unsigned long long)s;
+        sa.c2 = (uint32_t)(t & 0xFFFFFFFFull);
+        for (int colour = 0; colour < 2; ++colour) {
+            sa.c3 = (uint32_t)((t >> 32) & 0xFFFFFFull) | ((uint32_t)colour << 24) | (kDomainIsing << 28);
+            uint32_t* own1 = blat + colour * half;
+            const uint32_t* oth1 = blat + (1 - colour) * half;
+            for (int w = threadIdx.x; w < half; w += blockDim.x) {
+                const int i = w / WW, x = w - i * WW;
+                const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1;
+                const bool par = ((i + colour) & 1) != 0;     // side neighbour of site k: k+1 if par else k-1
+                const uint32_t ct = oth1[w];
+                const uint32_t ew = oth1[i * WW + (par ? (x == WW - 1 ? 0 : x + 1) : (x == 0 ? WW - 1 : x - 1))];
+                const uint32_t sd = par ? ((ct >> 1) | (ew << 31)) : ((ct << 1) | (ew >> 31));
+                const uint32_t g0 = (uint32_t)i * (uint32_t)(L >> 3) + 8u * (uint32_t)x;
+                uint32_t res;
+                if (never) res = update_word<true>(sa, own1[w], oth1[iu * WW + x], oth1[id * WW + x], ct, sd, g0, c1, stab, sT, never, slot);
+                else res = update_word<false>(sa, own1[w], oth1[iu * WW + x], oth1[id * WW + x], ct, sd, g0, c1, stab, sT, never, slot);
+                own1[w] = res;
+            }
+            __syncthreads();
+        }
+    }
+    for (int k = threadIdx.x; k < 2 * half; k += blockDim.x) g[k] = blat[k];
+}
+
 }  // namespace
+
+bool ising_bits_resident_fits(int L) { return L % 64 == 0 && (size_t)L * L / 8 <= 200 * 1024; }
+
+int launch_ising_bits_resident(const ResidentArgs& a, const uint8_t* aux, cudaStream_t s) {
+    if (cudaFuncSetAttribute(ising_bits_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
+        cudaGetLastError();
+        return 0;
+    }
+    ising_bits_resident_kernel<<<(unsigned)a.batch, kBitsResThreads, (size_t)a.L * a.L / 8, s>>>(a, aux);
+    return 1;
+}
 
 // Host side of the constant lookup table: entry [e][half][v] = 4 * class of the low (half 0) / high (half 1) nibble
 // of v, where the nibble of a site 4c+e holds (D, P2, P1, P0) rotated by e bits (see update_word).

@@ -305,6 +305,29 @@ bool use_resident(const spin_sim* sim, bool measure) {
     return measure && sim->batch >= 296;                           // fused per-sweep reductions, >= 2 CTAs per SM
 }
 
+// Bit-packed resident kernel (ising_bits.cu): uniform couplings, replica fits one CTA.  Measured:
+// 64 x 1024^2 406 vs 1123 flips/ns streaming (84 SMs idle), 148 x 1024^2 939 vs 1339, 296 x 512^2 1181 vs 1293,
+// 1024 x 256^2 1220 vs 1096: AUTO takes it only for many small replicas; SPIN_POLICY_RESIDENT forces it.
+bool use_bits_resident(const spin_sim* sim) {
+    if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_BITPACKED || sim->d_bonds) return false;
+    if (!ising_bits_resident_fits(sim->L)) return false;
+    if (sim->policy == SPIN_POLICY_RESIDENT) return true;
+    return sim->policy == SPIN_POLICY_AUTO && sim->L <= 256 && sim->batch >= 592;
+}
+
+bool enqueue_bits_resident(spin_sim* sim, int64_t t0, int64_t n_sweeps, const uint32_t* tables = nullptr) {
+    ResidentArgs a;
+    a.lattice = sim->lattice;
+    a.tables = tables ? tables : sim->d_tables;
+    a.batch = sim->batch; a.L = sim->L; a.replica_offset = sim->replica_offset; a.measure = 0u;
+    a.t0 = (unsigned long long)t0; a.n_sweeps = n_sweeps;
+    a.E_trace = nullptr; a.M_trace = nullptr; a.moments = nullptr;
+    a.rk = sim->rk;
+    const int n = launch_ising_bits_resident(a, sim->d_aux, sim->stream);
+    sim->launches += n;
+    return n > 0;
+}
+
 // Persistent cooperative kernel (ising_int8.cu): uniform Ising model, int8 layout, L % 32 == 0, no never-classes in the
 // current tables.  AUTO takes it for launch-bound shapes: measured (profiles/r2_policy_grid.md) it beats the streaming
 // path up to about 2 M sites per sweep (1 x 1024^2: 213 vs 134 flips/ns, 4 x 640^2: 282 vs 202) and loses above
@@ -663,6 +686,7 @@ int64_t spin_kernel_launches(const spin_sim* sim) { return sim ? sim->launches :
 const char* spin_kernel_variant(const spin_sim* sim) {
     if (!sim) return "";
     if (sim->model == SPIN_MODEL_POTTS) return potts_int8_variant(sim->L);
+    if (use_bits_resident(sim)) return "ising_bits_resident";
     if (sim->layout == SPIN_LAYOUT_BITPACKED) return "ising_bits_rows32";
     if (use_resident(sim, false)) return "ising_int8_resident";
     if (use_tiled(sim)) return "ising_int8_tiled";
@@ -865,6 +889,7 @@ int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps
         const int64_t t0 = sweep_offset + k * sweeps_per_step;
         if (resident) {
             enqueue_resident(sim, t0, sweeps_per_step, false, nullptr, nullptr, nullptr, tab);
+        } else if (use_bits_resident(sim) && enqueue_bits_resident(sim, t0, sweeps_per_step, tab)) {
         } else if (tiled && enqueue_tiled(sim, t0, sweeps_per_step, tab)) {
         } else if (persistent && enqueue_persistent(sim, t0, sweeps_per_step, tab)) {
         } else {
@@ -896,6 +921,7 @@ int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_
     if (rt != SPIN_OK) return rt;
     if (use_resident(sim, false)) {
         enqueue_resident(sim, sweep_offset, n_sweeps, false, nullptr, nullptr, nullptr);
+    } else if (use_bits_resident(sim) && enqueue_bits_resident(sim, sweep_offset, n_sweeps)) {
     } else if (use_tiled(sim) && enqueue_tiled(sim, sweep_offset, n_sweeps)) {
     } else if (!(use_persistent(sim) && enqueue_persistent(sim, sweep_offset, n_sweeps))) {
         for (int64_t t = sweep_offset; t < sweep_offset + n_sweeps; ++t) {

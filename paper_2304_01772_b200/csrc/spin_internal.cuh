@@ -151,6 +151,8 @@ int launch_init(const InitArgs& a, int model, int layout, cudaStream_t s);
 int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s);      // picks generic / vectorised
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s);
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s);
+bool ising_bits_resident_fits(int L);                                       // bit-packed replica fits one CTA's shared memory
+int launch_ising_bits_resident(const ResidentArgs& a, const uint8_t* aux, cudaStream_t s);   // 0: not launched
 uint8_t* ising_bits_make_aux_table();      // allocates + fills the constant 2 KiB lookup table on the current device (owned by the caller)
 const char* ising_int8_variant(int L);
 bool ising_int8_resident_fits(int L);                                       // a replica fits one CTA's shared memory

@@ -94,12 +94,12 @@ ISING_CASES = [
 @pytest.mark.parametrize("policy", POLICIES)
 @pytest.mark.parametrize("L,batch,layout,J,h,betas", ISING_CASES)
 def test_ising_sweeps_match_oracle_every_sweep(oracle_mod, L, batch, layout, J, h, betas, policy):
-    if layout == "bits" and policy == sp.SPIN_POLICY_RESIDENT:
-        pytest.skip("the resident kernel is int8 only; bits always stream")
     seed, n = 100 + L, 12
     ref = oracle_mod.init(batch, L, seed=seed)
     with _mk_ising(batch, L, seed=seed, layout=layout, policy=policy) as sim:
-        if policy == sp.SPIN_POLICY_RESIDENT and L % 32 == 0:
+        if policy == sp.SPIN_POLICY_RESIDENT and layout == "bits":
+            assert sim.spin_kernel_variant() == "ising_bits_resident"
+        elif policy == sp.SPIN_POLICY_RESIDENT and L % 32 == 0:
             assert sim.spin_kernel_variant() == "ising_int8_resident"
         for t in range(n):
             sim.spin_sweep(betas, J, h, 1, t)
@@ -339,3 +339,25 @@ def test_tiled_kernel_equals_oracle(oracle_mod, batch, L, n):
         sim.spin_sweep(cold, 1.0, 0.0, 3, (1 << 32) - 1)
         oracle_mod.sweep(ref, cold, 1.0, 0.0, seed=seed, n_sweeps=3, sweep_offset=(1 << 32) - 1)
         assert np.array_equal(sim.spin_get_spins(), ref)
+
+
+def test_bits_resident_kernel_many_sweeps_in_one_launch(oracle_mod):
+    """Bit-packed replica resident in one CTA: 1024^2 = 128 KiB of shared memory, all sweeps of a call in one
+    launch; equals the oracle, the streaming bit-packed kernel and continues across calls and a schedule."""
+    for batch, L, n in ((2, 1024, 5), (3, 256, 17), (1, 1280, 3)):
+        seed, beta = 70 + L, np.linspace(0.3, 0.6, batch)
+        ref = oracle_mod.init(batch, L, seed=seed)
+        with _mk_ising(batch, L, seed, layout="bits", policy=sp.SPIN_POLICY_RESIDENT) as sim:
+            assert sim.spin_kernel_variant() == "ising_bits_resident"
+            l0 = sim.spin_kernel_launches()
+            sim.spin_sweep(beta, 1.0, 0.02, n, 4)
+            assert sim.spin_kernel_launches() - l0 == 1
+            oracle_mod.sweep(ref, beta, 1.0, 0.02, seed=seed, n_sweeps=n, sweep_offset=4)
+            assert np.array_equal(sim.spin_get_spins(), ref)
+            steps = np.stack([beta * 0.5, beta * 2.0])
+            sim.spin_sweep_schedule(steps, 1.0, 0.0, 2, sweep_offset=4 + n)
+            oracle_mod.sweep_schedule(ref, steps, 1.0, 0.0, seed, 2, sweep_offset=4 + n)
+            assert np.array_equal(sim.spin_get_spins(), ref)
+            E, M = sim.spin_observables()
+            Eo, Mo = oracle_mod.ising_observables(ref)
+            assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
