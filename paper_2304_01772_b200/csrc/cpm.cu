@@ -52,8 +52,20 @@ __global__ void __launch_bounds__(256) cpm_area_kernel(const int8_t* __restrict_
 }
 
 // One proposal (readings C1, C3-C6): returns the new identifier of site (i, j), or -1 if it keeps its value.
+// The resident kernel reads tau / A / J from SHARED-memory copies of the parameters: indexing the kernel-parameter
+// (constant) bank with per-thread cell identifiers serialises a warp up to 32-fold.  The short-lived blocks of the
+// general pass kernel keep the parameter bank (filling shared tables per block costs more than it saves there).
+struct CpmTables {
+    const int8_t* tau;
+    const int32_t* A;
+    const int32_t* J;
+    long long lambda;
+    int ntypes;
+};
+
+template <typename P>   // CpmParams (kernel parameters) or CpmTables (shared-memory copies): same member names
 __device__ __forceinline__ int cpm_site(const int8_t* lat, int L, int i, int j, uint32_t r_prop, uint32_t r_acc,
-                                        const int32_t* areas, const CpmParams& p, const uint32_t* T, int dmax, bool beta_zero) {
+                                        const int32_t* areas, const P& p, const uint32_t* T, int dmax, bool beta_zero) {
     const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1, jl = j == 0 ? L - 1 : j - 1, jr = j == L - 1 ? 0 : j + 1;
     const int old = lat[(size_t)i * L + j];
     const int nb[8] = {lat[(size_t)iu * L + jl], lat[(size_t)iu * L + j], lat[(size_t)iu * L + jr], lat[(size_t)i * L + jl],
@@ -76,6 +88,14 @@ __device__ __forceinline__ int cpm_site(const int8_t* lat, int L, int i, int j, 
     bool acc = dH <= 0 || beta_zero;
     if (!acc && dH <= (long long)dmax) acc = r_acc < T[dH];
     return acc ? nw : -1;
+}
+
+__device__ __forceinline__ CpmTables load_tables(const CpmParams& p, int8_t* stau, int32_t* sA, int32_t* sJ) {
+    for (int k = threadIdx.x; k < 128; k += blockDim.x) { stau[k] = p.tau[k]; sA[k] = p.A[k]; }
+    if (threadIdx.x < kMaxTypes * kMaxTypes) sJ[threadIdx.x] = p.J[threadIdx.x];
+    CpmTables t;
+    t.tau = stau; t.A = sA; t.J = sJ; t.lambda = p.lambda; t.ntypes = p.ntypes;
+    return t;
 }
 
 __global__ void __launch_bounds__(128) cpm_pass_kernel(CpmArgs a, CpmParams p) {
@@ -103,9 +123,12 @@ __global__ void __launch_bounds__(128) cpm_pass_kernel(CpmArgs a, CpmParams p) {
 // replica keeps the lattice and the area counters in shared memory and runs every sweep of the call in one launch.  The
 // areas are counted once; during a colour pass accepted copies add to a separate delta array, which is folded into the
 // areas after the pass - so every proposal of a pass still sees the counts of the start of that pass (reading C3).
-__global__ void __launch_bounds__(256) cpm_resident_kernel(CpmArgs a, CpmParams p, unsigned long long t0, long long n_sweeps) {
+__global__ void __launch_bounds__(256) cpm_resident_kernel(CpmArgs a, CpmParams pp, unsigned long long t0, long long n_sweeps) {
     extern __shared__ __align__(16) int8_t slat[];
     __shared__ int32_t sarea[128], sdelta[128];
+    __shared__ int8_t stau[128];
+    __shared__ int32_t sA[128], sJ[kMaxTypes * kMaxTypes];
+    const CpmTables p = load_tables(pp, stau, sA, sJ);
     const int L = a.L, W = L >> 1, b = blockIdx.x;
     const int N = L * L;
     int8_t* glat = a.lattice + (size_t)b * N;
