@@ -386,6 +386,11 @@ __global__ void __launch_bounds__(256) dmc_march_backward_kernel(DmcArgs a, cons
             slN = src[base + (size_t)inext * L + jl];
             srN = src[base + (size_t)inext * L + jr];
         }
+        // the gradient rows this step will update (row i - 1): issue their loads now, use them after the barrier
+        const int ipre = i == 0 ? L - 1 : i - 1;
+        const size_t offpre = base + (size_t)ipre * L + j0;
+        float ah[8], av[8];
+        if (step >= 2) { load8(gJh + offpre, ah); load8(gJv + offpre, av); }
         {   // G_i, D_i; the beta / h sums count interior rows only (the halo rows belong to the neighbouring tiles)
             uint32_t r[4];
             philox4x32_10(a.rk, (uint32_t)i * (uint32_t)(L >> 3) + (uint32_t)cidx, (uint32_t)b + a.replica_offset, a.c2, a.c3, r);
@@ -404,10 +409,8 @@ __global__ void __launch_bounds__(256) dmc_march_backward_kernel(DmcArgs a, cons
             const int ip = i == 0 ? L - 1 : i - 1;
             const int ps = (step + 2) % 3;
             const float gl = sEdge[ps][cl][1], gr = sEdge[ps][cr][0];
-            const size_t off = base + (size_t)ip * L + j0;
-            float ah[8], av[8], out[8];
-            load8(gJh + off, ah);
-            load8(gJv + off, av);
+            const size_t off = offpre;
+            float out[8];
 #pragma unroll
             for (int e = 0; e < 8; ++e) {
                 const float gleft = e == 0 ? gl : Gc[e > 0 ? e - 1 : 0];
