@@ -135,3 +135,23 @@ def test_chunking_and_replica_offset():
     one = spins[1:2].copy()
     oracle.cpm_sweep(one, tau, JT, 1, A, 0.125, 9, 6, replica_offset=1)
     assert np.array_equal(one[0], a[1])
+
+
+def test_table_ii_and_parameters_are_the_papers():
+    """workloads.CPM_TABLE_II / cpm_initial against the values the paper prints (tests/golden/cpm_table_ii.txt)."""
+    import os
+    idx = {"medium": 0, "light": 1, "dark": 2}
+    want = np.full((3, 3), -1, dtype=np.int64)
+    params = {}
+    for line in open(os.path.join(os.path.dirname(__file__), "golden", "cpm_table_ii.txt")):
+        f = line.split()
+        if not f or f[0].startswith("#"):
+            continue
+        if f[0] in idx:
+            want[idx[f[0]], idx[f[1]]] = want[idx[f[1]], idx[f[0]]] = int(f[2])      # symmetric (PAPER.md:222)
+        else:
+            params[f[0]] = int(f[1])
+    assert np.array_equal(workloads.CPM_TABLE_II, want)
+    spins, tau, A = workloads.cpm_initial(1, 40)
+    assert len(tau) == params["identifiers"] and tau[0] == 0 and set(tau[1:]) <= {1, 2}
+    assert np.all(A[1:] == params["A"]) and np.all(np.bincount(spins.ravel(), minlength=37)[1:] == params["A"])
