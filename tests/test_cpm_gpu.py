@@ -65,3 +65,23 @@ def test_argument_checks():
         with pytest.raises(sp.SpinError):
             sp.spin_cpm_sweep(1, a["L"], d.data_ptr(), tau, a["Jtab"], a["lam"], A, a["beta"], 1, 1)
     assert np.array_equal(d.cpu().numpy(), spins)
+
+
+def test_cell_sorting_as_in_the_papers_figure_6():
+    """PAPER.md:288-294 (Fig. 5, 6): from the aggregate of square cells 'the interface between the blue cells and the medium
+    vanish[es], while the boundary length between red cells with medium and red cells with blue cells approaches a minimum':
+    with Table II one cell type ends up inside, wrapped by the other.  64 replicas, 2000 sweeps, through the public API."""
+    B, L = 64, 64
+    spins, tau, A = workloads.cpm_initial(B, L, 6, 5, seed=5)
+    d = torch.from_numpy(spins.copy()).cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    Ha0, _, ar0, bl0 = sp.spin_cpm_observables(B, L, d.data_ptr(), tau, JT, 1, A, cuda_stream=st)
+    sp.spin_cpm_sweep(B, L, d.data_ptr(), tau, JT, 1, A, np.full(B, 1.0 / 8.0), 5, 2000, cuda_stream=st)
+    Ha, Hr, ar, bl = sp.spin_cpm_observables(B, L, d.data_ptr(), tau, JT, 1, A, cuda_stream=st)
+    ml0, ml = bl0[:, 0, 1].mean(), bl[:, 0, 1].mean()          # medium-light boundary
+    assert ml < 0.4 * ml0, (ml0, ml)                           # 164 -> ~34: the light cells leave the surface
+    assert bl[:, 0, 2].mean() > bl0[:, 0, 2].mean()            # the dark cells take it over
+    assert bl[:, 1, 2].mean() < 0.7 * bl0[:, 1, 2].mean()      # light-dark contacts fall to a minimum (476 -> ~237)
+    assert Ha.mean() < Ha0.mean()                              # adhesion energy decreases
+    assert np.all((ar[:, 1:] > 0).sum(1) == 36)                # no cell disappears at lambda = 1, A = 25
+    assert np.all(np.abs(ar[:, 1:] - 25).mean(1) < 6)          # areas stay near the target
