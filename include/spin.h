@@ -205,17 +205,18 @@ SPIN_API int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_
                                  int64_t sweeps_per_step, int64_t sweep_offset);
 
 /* Kernel selection policy (diagnostics / tests; the results never depend on it: every path computes the same
- * lattice).  SPIN_POLICY_AUTO picks per shape; SPIN_POLICY_STREAMING forces the two-launches-
- * per-sweep HBM kernels; SPIN_POLICY_RESIDENT uses the shared-memory-resident multi-sweep kernel (one CTA per
- * replica, all sweeps of a call in one launch, E / M reductions fused) whenever the shape allows it (Ising, int8
- * layout, L a multiple of 32, L*L <= 192 KiB; bit-packed layout with uniform couplings, L*L/8 <= 200 KiB, plain sweeps
- * only) and falls back to streaming otherwise.  SPIN_POLICY_PERSISTENT uses the
- * persistent cooperative kernel (all sweeps of a call in one launch, the lattice in L2, a grid-wide barrier between
- * half-sweeps) whenever the shape allows it (Ising, int8 layout, L a multiple of 32, uniform couplings, no class whose
- * acceptance threshold is 0); AUTO takes it for batches of at most 2^21 sites that do not go to the resident kernel.  SPIN_POLICY_TILED uses the temporally blocked tile kernel (a CTA advances
- * a tile with a halo by several sweeps per launch in shared memory, about one tile per SM; needs a second lattice
- * buffer, allocated by the library on first use) whenever the shape allows it (Ising, int8 layout, L % 8 == 0, L >= 16,
- * uniform couplings).
+ * lattice).  A policy names a kernel family; whenever the handle's shape or couplings do not
+ * qualify for it the call falls back to the streaming kernels.
+ *   SPIN_POLICY_AUTO        picks per shape (rules derived from the measured grid profiles/r2_policy_grid.md).
+ *   SPIN_POLICY_STREAMING   two launches per sweep (one per colour), the HBM kernels.
+ *   SPIN_POLICY_RESIDENT    one CTA per replica keeps the lattice in shared memory and runs all sweeps of a call in one
+ *                           launch: Ising int8 with L % 32 == 0 and L*L <= 192 KiB (E / M reductions fused for
+ *                           spin_sweep_measure); bit-packed with uniform couplings and L*L/8 <= 200 KiB (plain sweeps).
+ *   SPIN_POLICY_PERSISTENT  one cooperative launch for all sweeps of a call, the lattice in L2, a grid-wide barrier between
+ *                           half-sweeps: Ising int8, L % 32 == 0, uniform couplings, no class whose threshold is 0.
+ *   SPIN_POLICY_TILED       temporal blocking: a CTA advances a tile with a halo by 2-4 sweeps per launch in shared memory,
+ *                           about one tile per SM; needs a second lattice buffer (allocated by the library on first use):
+ *                           Ising int8, L % 8 == 0, L >= 16, uniform couplings.
  * Returns SPIN_OK or SPIN_ERR_INVALID (NULL handle, unknown policy). */
 enum { SPIN_POLICY_AUTO = 0, SPIN_POLICY_STREAMING = 1, SPIN_POLICY_RESIDENT = 2, SPIN_POLICY_PERSISTENT = 3,
        SPIN_POLICY_TILED = 4 };
