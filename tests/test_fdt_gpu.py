@@ -28,7 +28,8 @@ def _run(stencil, B, L, beta, J1, J2, h, seed, n_therm, n_meas):
 
 
 @pytest.mark.parametrize("stencil,L,beta,J1,J2,h", [
-    (sp.SPIN_STENCIL_TRIANGULAR, 24, 0.18, 1.0, 0.0, 0.05),
+    (sp.SPIN_STENCIL_TRIANGULAR, 24, 0.18, 1.0, 0.0, 0.05),     # L % 12 == 0: byte-SIMD
+    (sp.SPIN_STENCIL_TRIANGULAR, 21, 0.18, 1.0, 0.0, 0.05),     # the general kernel
     (sp.SPIN_STENCIL_CUBIC, 16, 0.15, 1.0, 0.0, 0.0),           # L % 16 == 0: the byte-SIMD kernel
     (sp.SPIN_STENCIL_CUBIC, 10, 0.15, 1.0, 0.0, 0.1),           # the general kernel
     (sp.SPIN_STENCIL_SQUARE_NNN, 32, 0.22, 1.0, 0.4, 0.0),      # byte-SIMD

@@ -10,8 +10,9 @@ import paper_2304_01772_b200 as sp
 pytestmark = pytest.mark.gpu
 torch = pytest.importorskip("torch")
 
-# cubic and second-neighbour lattices with L % 16 == 0 run the byte-SIMD kernels, every other shape the general one
-CASES = ([(sp.SPIN_STENCIL_TRIANGULAR, L) for L in (3, 6, 9, 30, 96)]
+# cubic and second-neighbour lattices with L % 16 == 0 and triangular ones with L % 12 == 0 run the byte-SIMD kernels,
+# every other shape the general one
+CASES = ([(sp.SPIN_STENCIL_TRIANGULAR, L) for L in (3, 6, 9, 12, 30, 36, 96)]
          + [(sp.SPIN_STENCIL_CUBIC, L) for L in (2, 4, 6, 10, 16, 32, 48)]
          + [(sp.SPIN_STENCIL_SQUARE_NNN, L) for L in (2, 4, 6, 10, 16, 48, 64, 100)])
 
