@@ -214,6 +214,7 @@ SPIN_API int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_
  *                           spin_sweep_measure); bit-packed with uniform couplings and L*L/8 <= 200 KiB (plain sweeps).
  *   SPIN_POLICY_PERSISTENT  one cooperative launch for all sweeps of a call, the lattice in L2, a grid-wide barrier between
  *                           half-sweeps: Ising int8, L % 32 == 0, uniform couplings, no class whose threshold is 0.
+ *                           Never picked by AUTO (the streaming kernels are faster on every measured shape).
  *   SPIN_POLICY_TILED       temporal blocking: a CTA advances a tile with a halo by 2-4 sweeps per launch in shared memory,
  *                           about one tile per SM; needs a second lattice buffer (allocated by the library on first use):
  *                           Ising int8, L % 8 == 0, L >= 16, uniform couplings.

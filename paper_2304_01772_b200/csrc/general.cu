@@ -44,6 +44,7 @@ __device__ __forceinline__ void site_coords(int L, int colour, long long n, int&
 }
 
 __global__ void ising_int8_bonds_kernel(SweepArgs a, const int8_t* __restrict__ Jh, const int8_t* __restrict__ Jv) {
+    pdl_wait();   // launched with programmatic stream serialisation: the previous half-sweep must have completed
     const GroupPos p = group_pos(a, 4);
     if (!p.valid) return;
     const int L = a.L;
@@ -72,6 +73,7 @@ __global__ void ising_int8_bonds_kernel(SweepArgs a, const int8_t* __restrict__ 
 // thr: [B][L*L][32] uint32 T (accept iff r < T), alw: [B][L*L] bit k = class k always accepts; k = 16 d + cfg,
 // cfg bit 0 / 1 / 2 / 3 = the up / down / left / right neighbour is -1.
 __global__ void ising_int8_general_kernel(SweepArgs a, const uint32_t* __restrict__ thr, const uint32_t* __restrict__ alw) {
+    pdl_wait();   // launched with programmatic stream serialisation: the previous half-sweep must have completed
     const GroupPos p = group_pos(a, 4);
     if (!p.valid) return;
     const int L = a.L;
@@ -102,6 +104,7 @@ __global__ void ising_int8_general_kernel(SweepArgs a, const uint32_t* __restric
 // signs or nullptr.
 __global__ void potts_int8_general_kernel(SweepArgs a, const unsigned long long* __restrict__ tab2,
                                           const int8_t* __restrict__ Jh, const int8_t* __restrict__ Jv) {
+    pdl_wait();
     const GroupPos p = group_pos(a, 2);
     if (!p.valid) return;
     const int L = a.L;
@@ -240,20 +243,20 @@ inline int bpr_for(long long items, int batch) {
 
 int launch_ising_int8_bonds_half_sweep(const SweepArgs& a, const int8_t* Jh, const int8_t* Jv, cudaStream_t s) {
     const long long total = (((long long)a.L * (a.L >> 1) + 3) >> 2) * a.batch;
-    ising_int8_bonds_kernel<<<(unsigned)((total + 127) / 128), 128, 0, s>>>(a, Jh, Jv);
+    launch_pdl(ising_int8_bonds_kernel, (unsigned)((total + 127) / 128), 128u, s, a, Jh, Jv);
     return 1;
 }
 
 int launch_ising_int8_general_half_sweep(const SweepArgs& a, const uint32_t* thr, const uint32_t* alw, cudaStream_t s) {
     const long long total = (((long long)a.L * (a.L >> 1) + 3) >> 2) * a.batch;
-    ising_int8_general_kernel<<<(unsigned)((total + 127) / 128), 128, 0, s>>>(a, thr, alw);
+    launch_pdl(ising_int8_general_kernel, (unsigned)((total + 127) / 128), 128u, s, a, thr, alw);
     return 1;
 }
 
 int launch_potts_int8_general_half_sweep(const SweepArgs& a, const unsigned long long* tab2, const int8_t* Jh, const int8_t* Jv,
                                          cudaStream_t s) {
     const long long total = (((long long)a.L * (a.L >> 1) + 1) >> 1) * a.batch;
-    potts_int8_general_kernel<<<(unsigned)((total + 127) / 128), 128, 0, s>>>(a, tab2, Jh, Jv);
+    launch_pdl(potts_int8_general_kernel, (unsigned)((total + 127) / 128), 128u, s, a, tab2, Jh, Jv);
     return 1;
 }
 

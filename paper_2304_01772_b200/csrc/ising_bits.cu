@@ -13,6 +13,7 @@ namespace {
 __device__ __forceinline__ uint32_t sel(uint32_t m, uint32_t a, uint32_t b) { return (a & m) | (b & ~m); }
 
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
+constexpr int kRowsMid = 4;     // under about one wave of 8-row blocks
 constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
 constexpr int kThreads = 128;
 constexpr int kMinBlocks = 8;   // resident blocks per SM (64 registers)
@@ -130,6 +131,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 #pragma unroll 1
     for (int rr = 0; rr < kRows; rr += 2) {
         const bool more = rr + 2 < kRows;
+        if (!more && a.pdl_trigger == kPdlLastRows) pdl_launch_dependents();
         const uint32_t n1 = __ldg(more ? pOth : pOthLast);
         const uint32_t own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
@@ -169,7 +171,7 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) ising_bits_kernel(SweepA
     __shared__ uint32_t stab[16];                          // U[class], class = d * 8 + nd
     __shared__ __align__(16) uint8_t sT[kAuxBytes];        // [e][half][byte] -> 4 * class
     __shared__ uint32_t sidx[4 * kThreads];                // per-thread slot: word e of thread t at sidx[e * 128 + t]
-    pdl_launch_dependents();
+    if (a.pdl_trigger == kPdlAtStart) pdl_launch_dependents();
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
     for (int k = threadIdx.x; k < kAuxBytes / 16; k += blockDim.x) ((uint4*)sT)[k] = ((const uint4*)a.aux)[k];   // constant
@@ -279,23 +281,31 @@ uint8_t* ising_bits_make_aux_table() {
 }
 
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
-    const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 6) * a.batch;
-    const bool shortRows = longThreads < 148ll * 64;      // the per-block table set-up makes short threads pay off only for tiny launches
-    const int rows = shortRows ? kRowsShort : kRowsLong;
-    const int perReplica = (a.L / rows) * (a.L >> 6);
+    // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots); the
+    // smallest launches do best when the next one is released as soon as a thread has its first rows in registers
+    const int perReplica8 = (a.L / kRowsLong) * (a.L >> 6);
+    const long long threads8 = (long long)perReplica8 * a.batch;
+    RowsPlan plan = plan_rows(threads8, perReplica8, 148 * kMinBlocks, 0.3, 0.75, false);
+    if (plan.rows == kRowsShort && threads8 < 148ll * kMinBlocks * 128 / 10) plan.trigger = kPdlLastRows;
+    const int perReplica = (a.L / plan.rows) * (a.L >> 6);
     const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
     const int bpr = (perReplica + tpb - 1) / tpb;
     const unsigned grid = (unsigned)((long long)bpr * a.batch);
+    SweepArgs args = a;
+    args.pdl_trigger = plan.trigger;
     const bool bonds = a.bonds != nullptr;
     void (*k)(SweepArgs, int);
-    if (shortRows) {
+    if (plan.rows == kRowsShort) {
         if (bonds) k = a.colour == 0 ? ising_bits_kernel<0, kRowsShort, true> : ising_bits_kernel<1, kRowsShort, true>;
         else k = a.colour == 0 ? ising_bits_kernel<0, kRowsShort, false> : ising_bits_kernel<1, kRowsShort, false>;
+    } else if (plan.rows == kRowsMid) {
+        if (bonds) k = a.colour == 0 ? ising_bits_kernel<0, kRowsMid, true> : ising_bits_kernel<1, kRowsMid, true>;
+        else k = a.colour == 0 ? ising_bits_kernel<0, kRowsMid, false> : ising_bits_kernel<1, kRowsMid, false>;
     } else {
         if (bonds) k = a.colour == 0 ? ising_bits_kernel<0, kRowsLong, true> : ising_bits_kernel<1, kRowsLong, true>;
         else k = a.colour == 0 ? ising_bits_kernel<0, kRowsLong, false> : ising_bits_kernel<1, kRowsLong, false>;
     }
-    launch_pdl(k, grid, (unsigned)tpb, s, a, bpr);
+    launch_pdl(k, grid, (unsigned)tpb, s, args, bpr);
     return 1;
 }
 

@@ -64,7 +64,8 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 // (about 540 instructions) stays resident in the instruction caches.  Launched with programmatic dependent launch:
 // the next half-sweep's blocks are scheduled while this one drains.
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
-constexpr int kRowsShort = 2;   // ... and when it does not (latency-bound shapes): four times as many threads
+constexpr int kRowsMid = 4;     // ... about one wave of 8-row blocks or less: more, shorter blocks
+constexpr int kRowsShort = 2;   // ... and when even those leave SMs idle (latency-bound shapes)
 constexpr int kMinBlocks = 5;   // resident blocks per SM (96 registers)
 constexpr int kRowsThreads = 128;
 
@@ -239,7 +240,7 @@ template <int kColour, int kRows>
 __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[kTableStride];
     __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
-    pdl_launch_dependents();
+    if (a.pdl_trigger == kPdlAtStart) pdl_launch_dependents();
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
     pdl_wait();
@@ -614,22 +615,20 @@ const char* ising_int8_variant(int L) { return (L % 32 == 0) ? "ising_int8_rows1
 
 int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
-        // 8 rows per thread when that still gives every SM several blocks, else 2 rows (short threads, 4x as many)
-        const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 5) * a.batch;
-        const bool shortRows = longThreads < 148ll * 4 * kRowsThreads ||
-                               (a.L / kRowsLong) * (a.L >> 5) < kRowsThreads / 2;   // small L: keep the blocks full
-        const int rows = shortRows ? kRowsShort : kRowsLong;
-        const int perReplica = (a.L / rows) * (a.L >> 5);    // strips x row blocks of one colour
+        // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots)
+        const int perReplica8 = (a.L / kRowsLong) * (a.L >> 5);
+        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch, perReplica8, 148 * kMinBlocks, 0.25, 1.2, true);
+        const int perReplica = (a.L / plan.rows) * (a.L >> 5);    // strips x row blocks of one colour
         const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
         const int bpr = (perReplica + tpb - 1) / tpb;
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
-        if (shortRows) {
-            if (a.colour == 0) launch_pdl(ising_int8_rows_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
-            else launch_pdl(ising_int8_rows_kernel<1, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
-        } else {
-            if (a.colour == 0) launch_pdl(ising_int8_rows_kernel<0, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
-            else launch_pdl(ising_int8_rows_kernel<1, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
-        }
+        SweepArgs args = a;
+        args.pdl_trigger = plan.trigger;
+        void (*k)(SweepArgs, int);
+        if (plan.rows == kRowsShort) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsShort> : ising_int8_rows_kernel<1, kRowsShort>;
+        else if (plan.rows == kRowsMid) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsMid> : ising_int8_rows_kernel<1, kRowsMid>;
+        else k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsLong> : ising_int8_rows_kernel<1, kRowsLong>;
+        launch_pdl(k, grid, (unsigned)tpb, s, args, bpr);
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 3) >> 2) * a.batch;

@@ -54,6 +54,7 @@ __global__ void potts_int8_generic_kernel(SweepArgs a) {
 // indexes a 256-entry shared table holding U[dn + 4] (dn = n_new - n_old = #(!= old) - #(!= new)); the four index
 // bytes of a word go through a per-thread shared-memory slot (STS, then LDS.U8 straight into the table address).
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
+constexpr int kRowsMid = 4;     // under about one and a half waves of 8-row blocks
 constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
 constexpr int kRowsThreads = 128;
 constexpr int kMinBlocks = 4;   // resident blocks per SM (128 registers)
@@ -265,7 +266,7 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) potts_int8_rows_kern
     __shared__ uint32_t stab[16 + 64];            // U[dn + 4] in [0..8]; from word 16: 256-byte pattern -> 4 * class table
     __shared__ uint32_t snever[1];
     __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
-    pdl_launch_dependents();
+    if (a.pdl_trigger == kPdlAtStart) pdl_launch_dependents();
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
     pdl_wait();
@@ -298,21 +299,20 @@ const char* potts_int8_variant(int L) { return (L % 32 == 0) ? "potts_int8_rows1
 
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
-        const long long longThreads = (long long)(a.L / kRowsLong) * (a.L >> 5) * a.batch;
-        const bool shortRows = longThreads < 148ll * 4 * kRowsThreads ||
-                               (a.L / kRowsLong) * (a.L >> 5) < kRowsThreads / 2;   // small L: keep the blocks full
-        const int rows = shortRows ? kRowsShort : kRowsLong;
-        const int perReplica = (a.L / rows) * (a.L >> 5);    // strips x row blocks of one colour
+        // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots)
+        const int perReplica8 = (a.L / kRowsLong) * (a.L >> 5);
+        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch, perReplica8, 148 * kMinBlocks, 0.3, 1.5, false);
+        const int perReplica = (a.L / plan.rows) * (a.L >> 5);    // strips x row blocks of one colour
         const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
         const int bpr = (perReplica + tpb - 1) / tpb;
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
-        if (shortRows) {
-            if (a.colour == 0) launch_pdl(potts_int8_rows_kernel<0, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
-            else launch_pdl(potts_int8_rows_kernel<1, kRowsShort>, grid, (unsigned)tpb, s, a, bpr);
-        } else {
-            if (a.colour == 0) launch_pdl(potts_int8_rows_kernel<0, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
-            else launch_pdl(potts_int8_rows_kernel<1, kRowsLong>, grid, (unsigned)tpb, s, a, bpr);
-        }
+        SweepArgs args = a;
+        args.pdl_trigger = plan.trigger;
+        void (*k)(SweepArgs, int);
+        if (plan.rows == kRowsShort) k = a.colour == 0 ? potts_int8_rows_kernel<0, kRowsShort> : potts_int8_rows_kernel<1, kRowsShort>;
+        else if (plan.rows == kRowsMid) k = a.colour == 0 ? potts_int8_rows_kernel<0, kRowsMid> : potts_int8_rows_kernel<1, kRowsMid>;
+        else k = a.colour == 0 ? potts_int8_rows_kernel<0, kRowsLong> : potts_int8_rows_kernel<1, kRowsLong>;
+        launch_pdl(k, grid, (unsigned)tpb, s, args, bpr);
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 1) >> 1) * a.batch;

@@ -279,6 +279,7 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     a.aux = sim->d_aux;
     a.bonds = sim->d_bonds;
     a.rk = sim->rk;
+    a.pdl_trigger = kPdlAtExit;
     return a;
 }
 
@@ -329,16 +330,14 @@ bool enqueue_bits_resident(spin_sim* sim, int64_t t0, int64_t n_sweeps, const ui
 }
 
 // Persistent cooperative kernel (ising_int8.cu): uniform Ising model, int8 layout, L % 32 == 0, no never-classes in the
-// current tables.  AUTO takes it for launch-bound shapes: measured (profiles/r2_policy_grid.md) it beats the streaming
-// path up to about 2 M sites per sweep (1 x 1024^2: 213 vs 134 flips/ns, 4 x 640^2: 282 vs 202) and loses above
-// (4 x 1024^2: 473 vs 513): a grid barrier costs ~2.3 us here, the same as a programmatic dependent launch, and the
-// streaming kernels overlap their launch with the previous kernel's tail.
+// current tables.  On request only (SPIN_POLICY_PERSISTENT): a grid barrier costs ~2.3 us here, and since the streaming
+// kernels release the next launch where its blocks get a balanced placement (spin_internal.cuh, PdlTrigger) they are
+// faster on every shape of the measured grid (profiles/r2_policy_grid.md: 1 x 1024^2 224 vs 213 flips/ns, 4 x 640^2
+// 327 vs 279, 16 x 256^2 236 vs 214).
 bool use_persistent(const spin_sim* sim) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || sim->L % 32 != 0) return false;
     if (sim->general || sim->d_bond_nat || sim->any_never) return false;
-    if (sim->policy == SPIN_POLICY_PERSISTENT) return true;
-    if (sim->policy != SPIN_POLICY_AUTO) return false;
-    return (long long)sim->batch * sim->L * sim->L <= (1ll << 21);
+    return sim->policy == SPIN_POLICY_PERSISTENT;
 }
 
 SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour);
@@ -347,7 +346,7 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour);
 // on tiles with halos, one tile per SM.  Measured (profiles/r2_policy_grid.md) its one-thread-per-word shared-memory
 // update costs ~40 instructions per site (17 in the streaming kernel) on top of the halo redundancy, so it only wins
 // where everything else is latency-bound: one to four replicas of 128 <= L <= 256 (1 x 128^2: 7.8 vs 4.7 flips/ns
-// resident; 1 x 224^2: 16.7 vs 10.4 persistent).  AUTO takes it for at most 2^16 sites with L >= 128.
+// resident; 1 x 224^2: 16.0 vs 10.6 streaming).  AUTO takes it for at most 2^16 sites with L >= 128.
 bool use_tiled(const spin_sim* sim) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8) return false;
     if (sim->general || sim->d_bond_nat) return false;

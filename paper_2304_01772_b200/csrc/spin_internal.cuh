@@ -62,6 +62,7 @@ struct SweepArgs {
     const uint32_t* bonds;    // bit-packed +-J couplings: [B][2][4][L][L/64] words (bit = bond is -1; planes up, down,
                               // centre, side of the colour's sites), or nullptr for uniform couplings
     RoundKeys rk;
+    int32_t pdl_trigger;      // PdlTrigger: where the row-marching kernels release the next launch (set by the launchers)
 };
 
 // Shared-memory-resident multi-sweep kernel (small lattices: one CTA holds a whole replica and runs all sweeps of a
@@ -108,10 +109,20 @@ struct InitArgs {
 
 // ---- programmatic dependent launch -------------------------------------------------------------------
 // The sweep is a chain of short dependent kernels (two per sweep).  Launching them with the programmatic
-// stream-serialisation attribute lets the blocks of launch n+1 be scheduled, and run their index arithmetic, while
-// the last blocks of launch n drain; pdl_wait() then blocks until launch n has completed and its writes are
-// visible.  Every kernel launched this way calls pdl_launch_dependents() first and pdl_wait() before its first
-// global-memory access.
+// stream-serialisation attribute lets launch n+1 be staged while launch n runs; pdl_wait() then blocks until launch n
+// has completed and its writes are visible, and comes before the first access to the lattice.
+// WHERE launch n releases launch n+1 decides where the blocks of n+1 are placed (measured, profiles/r2_pdl_placement.md):
+// released at the start of n, the blocks of n+1 (and n+2, ..) become resident beside those of n, on whatever SMs have
+// room, and when a grid is around one wave or less that placement is lopsided for the whole launch (16 x 1024^2
+// bit-packed: 297 flips/ns, against 930-1030 with the same kernel released later).  Released when the blocks of n exit
+// (no explicit trigger), n+1 is placed on an empty GPU and is balanced.  With several waves the early release wins a
+// few percent (the next launch's blocks take the slots the last wave frees).  plan_rows() below picks the release
+// point together with the rows per thread.
+enum PdlTrigger : int32_t {
+    kPdlAtExit = 0,      // no explicit trigger: the dependent launch is released as this launch's blocks exit
+    kPdlAtStart = 1,     // first instruction of every block
+    kPdlLastRows = 2,    // when a thread starts its last two rows
+};
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
@@ -140,6 +151,25 @@ inline int pick_block(int units) {
         if (bestPad < 0 || pad < bestPad) { best = t; bestPad = pad; }
     }
     return best;
+}
+
+// Rows per thread (2, 4 or 8) and release point of a row-marching half-sweep launch.  w8 = waves the 8-row grid would
+// make (threads of 8 rows / (slots x 128), slots = 148 x resident blocks per SM of that kernel).  Long threads amortise
+// the per-thread set-up and the two halo rows; short threads fill the GPU when the launch is small.  The thresholds are
+// the crossovers of a measured (batch, L) grid per kernel (profiles/r2_pdl_placement.md); min8 = fewest 8-row threads
+// per replica for which 8 or 4 rows keep a block reasonably full.
+struct RowsPlan {
+    int rows;
+    int32_t trigger;
+};
+inline RowsPlan plan_rows(long long threads8, int perReplica8, int slots, double w_r2, double w_r8, bool early_r8) {
+    const double w8 = (double)threads8 / (128.0 * slots);
+    RowsPlan p;
+    if (perReplica8 < 64 || w8 < w_r2) p.rows = 2;
+    else if (w8 < w_r8) p.rows = 4;
+    else p.rows = 8;
+    p.trigger = (p.rows == 8 && early_r8) ? kPdlAtStart : kPdlAtExit;
+    return p;
 }
 
 // Records the thread-local spin_last_error() text and returns `code` (spin_api.cu).

@@ -42,6 +42,7 @@ __device__ __host__ __forceinline__ long long colour_sites(int stencil, int L) {
 
 template <int kStencil>
 __global__ void __launch_bounds__(128) stencil_pass_kernel(StencilArgs a) {
+    pdl_wait();   // launched with programmatic stream serialisation: the previous pass must have completed
     const int L = a.L;
     const long long per = colour_sites(kStencil, L);
     const long long groups = (per + 3) >> 2;
@@ -110,6 +111,7 @@ __global__ void __launch_bounds__(128) stencil_pass_kernel(StencilArgs a) {
 // in a shared-memory table laid out [d][8].  The whole word is written back: its other-colour bytes are rewritten with
 // the values they already have (no thread changes them during this pass).
 __global__ void __launch_bounds__(128) cubic_pass_vec_kernel(StencilArgs a) {
+    pdl_wait();   // launched with programmatic stream serialisation: the previous pass must have completed
     __shared__ uint32_t stab[16];
     __shared__ uint32_t salways;
     const int L = a.L, V = L >> 4;                             // 16-site words per line
@@ -204,6 +206,7 @@ __device__ __forceinline__ void shifted_words(const uint32_t x[4], uint32_t edge
 }
 
 __global__ void __launch_bounds__(128) nnn_pass_vec_kernel(StencilArgs a) {
+    pdl_wait();   // launched with programmatic stream serialisation: the previous pass must have completed
     __shared__ uint32_t stab[50];
     __shared__ uint32_t salw[2];
     const int L = a.L, V = L >> 4, H = L >> 1;
@@ -267,6 +270,7 @@ __global__ void __launch_bounds__(128) nnn_pass_vec_kernel(StencilArgs a) {
 // Philox group.  Neighbour sums per byte as in the kernels above: (i-1, j) + (i+1, j) + (i, j-1) + (i, j+1) + (i+1, j+1) +
 // (i-1, j-1), every spin masked to "4 per -1 spin"; 4 nd + 32 d indexes the [d][8] threshold table.
 __global__ void __launch_bounds__(128) triangular_pass_vec_kernel(StencilArgs a) {
+    pdl_wait();   // launched with programmatic stream serialisation: the previous pass must have completed
     __shared__ uint32_t stab[16];
     __shared__ uint32_t salways;
     const int L = a.L, V = L / 12;                             // 12-site chunks per row
@@ -499,16 +503,16 @@ int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_t* lattic
             a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)c << 24) | (kDomainStencil << 28);
             if (stencil == SPIN_STENCIL_TRIANGULAR && L % 12 == 0) {
                 const long long chunks = (long long)L * (L / 12) * batch;
-                triangular_pass_vec_kernel<<<(unsigned)((chunks + 127) / 128), 128, 0, s>>>(a);
-            } else if (stencil == SPIN_STENCIL_TRIANGULAR) stencil_pass_kernel<SPIN_STENCIL_TRIANGULAR><<<grid, 128, 0, s>>>(a);
+                launch_pdl(triangular_pass_vec_kernel, (unsigned)((chunks + 127) / 128), 128u, s, a);
+            } else if (stencil == SPIN_STENCIL_TRIANGULAR) launch_pdl(stencil_pass_kernel<SPIN_STENCIL_TRIANGULAR>, grid, 128u, s, a);
             else if (stencil == SPIN_STENCIL_CUBIC && L % 16 == 0) {
                 const long long words = (long long)L * L * (L >> 4) * batch;
-                cubic_pass_vec_kernel<<<(unsigned)((words + 127) / 128), 128, 0, s>>>(a);
-            } else if (stencil == SPIN_STENCIL_CUBIC) stencil_pass_kernel<SPIN_STENCIL_CUBIC><<<grid, 128, 0, s>>>(a);
+                launch_pdl(cubic_pass_vec_kernel, (unsigned)((words + 127) / 128), 128u, s, a);
+            } else if (stencil == SPIN_STENCIL_CUBIC) launch_pdl(stencil_pass_kernel<SPIN_STENCIL_CUBIC>, grid, 128u, s, a);
             else if (L % 16 == 0) {
                 const long long words = (long long)(L >> 1) * (L >> 4) * batch;
-                nnn_pass_vec_kernel<<<(unsigned)((words + 127) / 128), 128, 0, s>>>(a);
-            } else stencil_pass_kernel<SPIN_STENCIL_SQUARE_NNN><<<grid, 128, 0, s>>>(a);
+                launch_pdl(nnn_pass_vec_kernel, (unsigned)((words + 127) / 128), 128u, s, a);
+            } else launch_pdl(stencil_pass_kernel<SPIN_STENCIL_SQUARE_NNN>, grid, 128u, s, a);
         }
     if (e == cudaSuccess) e = cudaGetLastError();
     cudaFreeAsync(d_tab, s);
