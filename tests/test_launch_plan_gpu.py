@@ -1,0 +1,93 @@
+"""GPU parity over the launch plans of the row-marching kernels (csrc/spin_internal.cuh, plan_rows): 2, 4 or 8 rows per
+thread and the point where a half-sweep releases the next launch (at block exit, at the first instruction, at a thread's
+last rows) are chosen from the size of the launch.  The result may not depend on any of it: one shape per branch of each
+kernel's planner, streaming policy, lattice and observables against the oracle after every compared sweep.
+
+w8 = threads of the 8-row grid / (128 x 148 x resident blocks per SM) — int8 Ising: 5 blocks, < 0.25 -> 2 rows,
+< 1.2 -> 4 rows, else 8 rows released at the first instruction; bit-packed: 8 blocks, < 0.3 -> 2 rows (< 0.1: released
+at the last rows), < 0.75 -> 4, else 8; Potts: 4 blocks, < 0.3 -> 2, < 1.5 -> 4, else 8."""
+import numpy as np
+import pytest
+
+import paper_2304_01772_b200 as sp
+
+pytestmark = pytest.mark.gpu
+
+
+def _w8(batch, L, layout, slots_per_sm):
+    per = (L // 8) * (L >> (6 if layout == "bits" else 5))
+    return per * batch / (128.0 * 148 * slots_per_sm)
+
+
+ISING_PLANS = [
+    # batch, L, layout, expected rows, J, h
+    (2, 1024, "int8", 2, 1.0, 0.0),        # w8 0.09
+    (8, 1024, "int8", 4, 1.0, 0.01),       # w8 0.35
+    (100, 256, "int8", 4, -1.0, 0.2),      # w8 0.27, many replicas per wave
+    (30, 1024, "int8", 8, 1.0, 0.0),       # w8 1.30, released at the first instruction
+    (3, 64, "int8", 2, 1.0, 0.0),          # fewer than 64 eight-row threads per replica
+    (4, 1024, "bits", 2, 1.0, 0.01),       # w8 0.05, released at the last rows
+    (12, 1024, "bits", 2, 1.0, 0.0),       # w8 0.16, released at exit
+    (32, 1024, "bits", 4, -1.0, 0.2),      # w8 0.43
+    (60, 1024, "bits", 8, 1.0, 0.0),       # w8 0.81
+]
+
+
+@pytest.mark.parametrize("batch,L,layout,rows,J,h", ISING_PLANS)
+def test_ising_every_plan_equals_oracle(oracle_mod, batch, L, layout, rows, J, h):
+    w8 = _w8(batch, L, layout, 8 if layout == "bits" else 5)
+    lo, hi = (0.3, 0.75) if layout == "bits" else (0.25, 1.2)
+    per8 = (L // 8) * (L >> (6 if layout == "bits" else 5))
+    assert rows == (2 if per8 < 64 or w8 < lo else 4 if w8 < hi else 8), "the case no longer hits the branch it names"
+    seed = 300 + batch
+    beta = np.linspace(0.3, 0.6, batch)
+    beta[-1] = 20.0                                           # one replica with never-accepted classes
+    lay = sp.SPIN_LAYOUT_BITPACKED if layout == "bits" else sp.SPIN_LAYOUT_INT8
+    ref = oracle_mod.init(batch, L, seed=seed)
+    with sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed, layout=lay) as sim:
+        sim.spin_set_policy(sp.SPIN_POLICY_STREAMING)
+        for t0, n in ((0, 1), (1, 3)):
+            sim.spin_sweep(beta, J, h, n, t0)
+            oracle_mod.sweep(ref, beta, J, h, seed=seed, n_sweeps=n, sweep_offset=t0)
+            assert np.array_equal(sim.spin_get_spins(), ref), "lattice differs after sweep %d" % (t0 + n - 1)
+        E, M = sim.spin_observables()
+        Eo, Mo = oracle_mod.ising_observables(ref)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+
+
+@pytest.mark.parametrize("batch,L,rows", [(2, 512, 2), (32, 512, 4), (4, 1024, 2), (120, 512, 8)])
+def test_potts_every_plan_equals_oracle(oracle_mod, batch, L, rows):
+    w8 = _w8(batch, L, "int8", 4)
+    assert rows == (2 if w8 < 0.3 else 4 if w8 < 1.5 else 8), "the case no longer hits the branch it names"
+    seed = 400 + batch
+    q = np.array([3, 8, 5, 127][: min(batch, 4)] + [3 + (b % 6) for b in range(max(0, batch - 4))], dtype=np.int32)
+    beta = np.linspace(0.5, 1.6, batch)
+    beta[0] = 25.0                                            # never-accepted classes
+    ref = oracle_mod.init(batch, L, seed=seed, q=q)
+    with sp.spin_create_ex(batch, L, sp.SPIN_MODEL_POTTS, q_per_replica=q, seed=seed) as sim:
+        for t0, n in ((0, 1), (1, 2)):
+            sim.spin_sweep(beta, 1.0, 0.0, n, t0)
+            oracle_mod.sweep(ref, beta, 1.0, 0.0, seed=seed, n_sweeps=n, sweep_offset=t0, q=q)
+            assert np.array_equal(sim.spin_get_spins(), ref), "lattice differs after sweep %d" % (t0 + n - 1)
+        E, M = sim.spin_observables()
+        Eo, Mo = oracle_mod.potts_observables(ref, q)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+
+
+@pytest.mark.parametrize("batch,L", [(4, 1024), (32, 1024), (60, 1024)])
+def test_bit_packed_bonds_every_plan_equals_oracle(oracle_mod, batch, L):
+    """The +-J variant of the bit-packed kernel has its own instantiations per rows-per-thread."""
+    seed = 500 + batch
+    rng = np.random.default_rng(seed)
+    Jh = (2 * rng.integers(0, 2, size=(1, L, L)) - 1).astype(np.int8)
+    Jv = (2 * rng.integers(0, 2, size=(1, L, L)) - 1).astype(np.int8)
+    beta = np.linspace(0.4, 1.2, batch)
+    ref = oracle_mod.init(batch, L, seed=seed)
+    with sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed, layout=sp.SPIN_LAYOUT_BITPACKED) as sim:
+        sim.spin_set_bonds(Jh[0], Jv[0])
+        sim.spin_sweep(beta, 1.0, 0.05, 3, 7)
+        oracle_mod.sweep_bonds(ref, Jh, Jv, beta, 1.0, 0.05, seed=seed, n_sweeps=3, sweep_offset=7)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        E, M = sim.spin_observables()
+        Eo, Mo = oracle_mod.ising_bonds_observables(ref, Jh, Jv)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
