@@ -18,6 +18,7 @@ __device__ __forceinline__ bool accept_slow(uint32_t r, const uint32_t* tab, int
 // ---- generic kernel: any even L.  One thread per Philox group (4 consecutive same-colour sites, which may
 // span rows when L/2 is not a multiple of 4).  Byte loads; used for L % 32 != 0.
 __global__ void ising_int8_generic_kernel(SweepArgs a) {
+    pdl_wait();   // launched with programmatic stream serialisation: the previous half-sweep must have completed
     const int L = a.L, W = L >> 1;
     const long long half = (long long)L * W;          // sites of one colour
     const long long groups = (half + 3) >> 2;
@@ -354,13 +355,17 @@ __device__ __forceinline__ void tiled_half_sweep(const TiledArgs& a, int colour,
     }
 }
 
-constexpr int kTiledThreads = 512;
+constexpr int kTiledThreads = 1024;
 
+// kOneWord: the region has at most blockDim.x words per colour, so every thread owns ONE word for the whole launch and
+// its coordinates, neighbour offsets and Philox group are computed once; a half-sweep is then one latency chain per
+// thread between two barriers (these shapes are latency-bound: the fewer dependent rounds per half-sweep the better).
+// Otherwise the words are dealt out round-robin every half-sweep (tiled_half_sweep).
+template <bool kOneWord>
 __global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledArgs a) {
     extern __shared__ __align__(16) uint32_t tsm[];
     __shared__ uint32_t stab[kTableStride];
     __shared__ uint32_t sidx[kTiledThreads];
-    pdl_launch_dependents();
     const int L = a.L, W = L >> 1;
     const int SR = a.TR + 2 * a.HR, SWX = (a.TK + 2 * a.HK) >> 2;
     const int perReplica = a.tilesR * a.tilesK;
@@ -394,6 +399,26 @@ __global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledAr
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
     const bool never = stab[kTabNever] != 0u;
+    // the thread's own word (kOneWord)
+    const int task = threadIdx.x;
+    const bool mine = task < SR * SWX;
+    int oU = 0, oD = 0, oNext = 0, oPrev = 0;
+    uint32_t group = 0u, par0 = 0u;
+    if (kOneWord && mine) {
+        const int r = task / SWX, wx = task - r * SWX;
+        int gi = iBase + r;
+        gi = gi >= L ? gi - L : gi;
+        gi = gi >= L ? gi - L : gi;
+        int gk = kBase + 4 * wx;
+        gk = gk >= W ? gk - W : gk;
+        gk = gk >= W ? gk - W : gk;
+        oU = (r == 0 ? 0 : r - 1) * SWX + wx;
+        oD = (r == SR - 1 ? r : r + 1) * SWX + wx;
+        oNext = r * SWX + (wx == SWX - 1 ? wx : wx + 1);
+        oPrev = r * SWX + (wx == 0 ? 0 : wx - 1);
+        group = (uint32_t)gi * (uint32_t)W4 + (uint32_t)(gk >> 2);
+        par0 = (uint32_t)gi & 1u;
+    }
     for (int s = 0; s < a.sweeps; ++s) {
         const unsigned long long t = a.t0 + (unsigned long long)s;
         const uint32_t c2 = (uint32_t)(t & 0xFFFFFFFFull);
@@ -402,7 +427,20 @@ __global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledAr
             const uint32_t c3 = c3lo | ((uint32_t)colour << 24);
             uint32_t* own1 = colour ? reg1 : reg0;
             const uint32_t* oth1 = colour ? reg0 : reg1;
-            if (never) tiled_half_sweep<true>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1);
+            if (kOneWord) {
+                if (mine) {
+                    const uint32_t m = 0x04040404u;
+                    const bool par = ((par0 + (uint32_t)colour) & 1u) != 0u;   // side neighbour of site k: k+1 if par else k-1
+                    const uint32_t um = oth1[oU] & m, cm = oth1[task] & m, dm = oth1[oD] & m;
+                    const uint32_t nb = oth1[par ? oNext : oPrev] & m;
+                    const uint32_t sd = __byte_perm(par ? cm : nb, par ? nb : cm, par ? 0x4321u : 0x6543u);
+                    const uint32_t own = own1[task];
+                    uint32_t rw[4];
+                    philox4x32_10(a.rk, group, c1, c2, c3, rw);
+                    const uint32_t tcls = um + cm + dm + sd + (own & 0x20202020u);
+                    own1[task] = never ? update_word<true, 0>(own, tcls, rw, stab, slot) : update_word<false, 0>(own, tcls, rw, stab, slot);
+                }
+            } else if (never) tiled_half_sweep<true>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1);
             else tiled_half_sweep<false>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1);
             __syncthreads();
         }
@@ -411,8 +449,8 @@ __global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledAr
     const int rows = min(a.TR, L - i0), wcols = min(a.TK, W - k0) >> 2;
     uint32_t* o0 = (uint32_t*)((int8_t*)a.dst + (size_t)b * 2 * half);
     uint32_t* o1 = (uint32_t*)((int8_t*)a.dst + (size_t)b * 2 * half + half);
-    for (int task = threadIdx.x; task < rows * wcols; task += blockDim.x) {
-        const int rr = task / wcols, ww = task - rr * wcols;
+    for (int task2 = threadIdx.x; task2 < rows * wcols; task2 += blockDim.x) {
+        const int rr = task2 / wcols, ww = task2 - rr * wcols;
         const int sidxw = (a.HR + rr) * SWX + (a.HK >> 2) + ww;
         const size_t gw = (size_t)(i0 + rr) * W4 + ((k0 >> 2) + ww);
         o0[gw] = reg0[sidxw];
@@ -632,7 +670,7 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 3) >> 2) * a.batch;
-        ising_int8_generic_kernel<<<(unsigned)((total + 127) / 128), 128, 0, s>>>(a);
+        launch_pdl(ising_int8_generic_kernel, (unsigned)((total + 127) / 128), 128u, s, a);
     }
     return 1;
 }
@@ -687,32 +725,38 @@ struct TileGeom {
     size_t smem;
 };
 
+// At most one tile per SM over the whole batch (a second tile on an SM doubles that SM's time and every launch waits for
+// the slowest tile: 153 tiles ran 1 x 640^2 at 149 flips/ns, 144 tiles at 220), and among those grids the one whose
+// region (tile + halo) has the fewest words per colour: that is the work per half-sweep of every SM.  4 sweeps per launch
+// (halo 8) whenever such a region wraps around the lattice at most once, else 2 (halo 4): measured, 4 beats 2, 3, 5, 6
+// and 8 on every shape AUTO sends here (profiles/r2_pdl_placement.md).
 static bool tile_geometry(int batch, int L, TileGeom& g) {
     if (L % 8 != 0 || L < 16) return false;
     const int W = L >> 1;
-    const long long N = (long long)L * L;
-    int perReplica = (148 + batch - 1) / batch;                 // tiles wanted per replica
+    int perReplica = 148 / batch;                               // tiles allowed per replica
     if (perReplica < 1) perReplica = 1;
-    const double target = (double)N / perReplica;               // sites per tile (both colours)
-    int TK = (int)(sqrt(target / 2.0) / 4.0 + 0.5) * 4;          // same-colour columns: the tile is TR x 2 TK sites
-    if (TK < 16) TK = 16;
-    if (TK > W) TK = W;
-    int tilesK = (W + TK - 1) / TK;
-    TK = ((W + tilesK - 1) / tilesK + 3) / 4 * 4;                // even out, keep a multiple of 4
-    tilesK = (W + TK - 1) / TK;
-    int tilesR = (perReplica + tilesK - 1) / tilesK;
-    if (tilesR < 1) tilesR = 1;
-    int TR = (L + tilesR - 1) / tilesR;
-    if (TR < 8) TR = 8;
-    tilesR = (L + TR - 1) / TR;
-    g.TR = TR; g.TK = TK; g.tilesR = tilesR; g.tilesK = tilesK;
-    g.sweeps = TR >= 32 && TK >= 32 ? 4 : 2;
-    g.HR = 2 * g.sweeps;
-    g.HK = 2 * g.sweeps < 4 ? 4 : (2 * g.sweeps + 3) / 4 * 4;
-    g.smem = (size_t)2 * (TR + 2 * g.HR) * (TK + 2 * g.HK);
-    // the region may wrap around the lattice at most once (two conditional subtractions in the kernel)
-    if (TR + 2 * g.HR > 2 * L || TK + 2 * g.HK > 2 * W) return false;
-    return g.smem <= 200 * 1024;
+    for (int sweeps = 4; sweeps >= 2; sweeps -= 2) {
+        const int HR = 2 * sweeps, HK = 2 * sweeps < 4 ? 4 : (2 * sweeps + 3) / 4 * 4;
+        long long bestWords = -1;
+        for (int tilesK = 1; tilesK <= perReplica && tilesK <= (W + 15) / 16; ++tilesK) {
+            const int TK = ((W + tilesK - 1) / tilesK + 3) / 4 * 4;
+            if ((W + TK - 1) / TK != tilesK) continue;          // rounding merged two columns of tiles
+            for (int tilesR = 1; tilesR * tilesK <= perReplica && tilesR <= (L + 7) / 8; ++tilesR) {
+                const int TR = (L + tilesR - 1) / tilesR;
+                if (TR < 8 || (L + TR - 1) / TR != tilesR) continue;
+                if (TR + 2 * HR > 2 * L || TK + 2 * HK > 2 * W) continue;   // the region may wrap around the lattice at most once
+                const long long words = (long long)(TR + 2 * HR) * ((TK + 2 * HK) >> 2);
+                if ((size_t)words * 8 > 200 * 1024) continue;
+                if (bestWords < 0 || words < bestWords) {
+                    bestWords = words;
+                    g.TR = TR; g.TK = TK; g.tilesR = tilesR; g.tilesK = tilesK; g.sweeps = sweeps; g.HR = HR; g.HK = HK;
+                    g.smem = (size_t)words * 8;
+                }
+            }
+        }
+        if (bestWords >= 0) return true;
+    }
+    return false;
 }
 
 bool ising_int8_tiled_fits(int batch, int L) {
@@ -723,7 +767,8 @@ bool ising_int8_tiled_fits(int batch, int L) {
 int launch_ising_int8_tiled(const SweepArgs& a, void* shadow, unsigned long long t0, long long n_sweeps, cudaStream_t s) {
     TileGeom g;
     if (!tile_geometry(a.batch, a.L, g) || !shadow) return 0;
-    if (cudaFuncSetAttribute(ising_int8_tiled_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
+    if (cudaFuncSetAttribute(ising_int8_tiled_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess ||
+        cudaFuncSetAttribute(ising_int8_tiled_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024) != cudaSuccess) {
         cudaGetLastError();
         return 0;
     }
@@ -732,7 +777,8 @@ int launch_ising_int8_tiled(const SweepArgs& a, void* shadow, unsigned long long
     t.TR = g.TR; t.TK = g.TK; t.HR = g.HR; t.HK = g.HK; t.tilesR = g.tilesR; t.tilesK = g.tilesK; t.rk = a.rk;
     const unsigned grid = (unsigned)((long long)g.tilesR * g.tilesK * a.batch);
     const long long words = (long long)(g.TR + 2 * g.HR) * ((g.TK + 2 * g.HK) >> 2);
-    const unsigned tpb = words >= 1024 ? kTiledThreads : 256;
+    const bool oneWord = words <= kTiledThreads;                // one word per thread for the whole launch
+    const unsigned tpb = oneWord ? (unsigned)((words + 31) / 32 * 32) : (unsigned)kTiledThreads;
     void* cur = a.lattice;
     void* other = shadow;
     int launches = 0;
@@ -749,7 +795,8 @@ int launch_ising_int8_tiled(const SweepArgs& a, void* shadow, unsigned long long
         attr[0].val.programmaticStreamSerializationAllowed = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        cudaLaunchKernelEx(&cfg, ising_int8_tiled_kernel, t);
+        if (oneWord) cudaLaunchKernelEx(&cfg, ising_int8_tiled_kernel<true>, t);
+        else cudaLaunchKernelEx(&cfg, ising_int8_tiled_kernel<false>, t);
         ++launches;
         void* tmp = cur; cur = other; other = tmp;
     }

@@ -13,6 +13,7 @@ __device__ __forceinline__ bool accept_slow(uint32_t r, const uint32_t* tab, int
 
 // ---- generic kernel: any even L, one thread per Philox group (2 consecutive same-colour sites).
 __global__ void potts_int8_generic_kernel(SweepArgs a) {
+    pdl_wait();   // launched with programmatic stream serialisation: the previous half-sweep must have completed
     const int L = a.L, W = L >> 1;
     const long long half = (long long)L * W;
     const long long groups = (half + 1) >> 1;
@@ -316,7 +317,7 @@ int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     } else {
         const long long half = (long long)a.L * (a.L >> 1);
         const long long total = ((half + 1) >> 1) * a.batch;
-        potts_int8_generic_kernel<<<(unsigned)((total + 127) / 128), 128, 0, s>>>(a);
+        launch_pdl(potts_int8_generic_kernel, (unsigned)((total + 127) / 128), 128u, s, a);
     }
     return 1;
 }

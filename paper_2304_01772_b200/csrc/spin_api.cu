@@ -283,6 +283,17 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     return a;
 }
 
+// Shapes AUTO sends to the temporally blocked tile kernel (ising_int8.cu) for plain sweeps: up to 16 replicas and 2^20
+// sites in all, i.e. launches that leave the streaming kernels latency-bound and give one CTA per replica too few CTAs.
+// Measured (profiles/r2_policy_grid.md): 1 x 640^2 231 vs 88 flips/ns streaming, 16 x 128^2 178 vs 74 resident,
+// 16 x 256^2 257 vs 236, 1 x 1024^2 260 vs 224; beyond that it loses (4 x 640^2 302 vs 327, 64 x 128^2 253 vs 291).
+bool prefer_tiled(const spin_sim* sim) {
+    if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || sim->general || sim->d_bond_nat) return false;
+    if (sim->policy != SPIN_POLICY_AUTO) return false;
+    return sim->L >= 64 && sim->batch <= 16 && (long long)sim->batch * sim->L * sim->L <= (1ll << 20) &&
+           ising_int8_tiled_fits(sim->batch, sim->L);
+}
+
 // Shared-memory-resident path (ising_int8.cu): Ising, int8 layout, replica fits one CTA.  AUTO uses it when the
 // batch gives every SM work (or when the lattice is so small that the streaming kernels are launch-bound anyway).
 bool use_resident(const spin_sim* sim, bool measure) {
@@ -294,9 +305,8 @@ bool use_resident(const spin_sim* sim, bool measure) {
     // a replica is a handful of warps (L <= 128: 3.1 vs 0.9 flips/ns at 1 x 64^2, 767 vs 500 at 256 x 128^2); for larger
     // replicas a CTA needs tens of microseconds per sweep, so it only pays when the batch fills the GPU (>= 1 CTA per SM)
     // AND the streaming kernel's blocks would be ragged (L = 160, 224: 766 vs 655 flips/ns at 256 x 224^2); small batches
-    // of large resident-eligible replicas (4 x 416^2: 23 vs 112 flips/ns) go to the persistent / streaming kernels.
-    if (sim->L == 128 && (long long)sim->batch * sim->L * sim->L <= (1ll << 16) && sim->policy == SPIN_POLICY_AUTO && !measure)
-        return false;                                              // 1-4 replicas of 128^2: the tiled kernel spreads them over the SMs
+    // of large resident-eligible replicas (4 x 416^2: 23 vs 112 flips/ns) go to the tiled / streaming kernels.
+    if (!measure && prefer_tiled(sim)) return false;               // few small replicas: the tiled kernel spreads them over the SMs
     if (sim->L <= 128) return true;
     int tpb = 128;
     const int perReplica = (sim->L / 8) * (sim->L / 32);
@@ -342,18 +352,14 @@ bool use_persistent(const spin_sim* sim) {
 
 SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour);
 
-// Temporally blocked tile kernel (ising_int8.cu): uniform Ising model, int8 layout, L % 8 == 0; several sweeps per launch
-// on tiles with halos, one tile per SM.  Measured (profiles/r2_policy_grid.md) its one-thread-per-word shared-memory
-// update costs ~40 instructions per site (17 in the streaming kernel) on top of the halo redundancy, so it only wins
-// where everything else is latency-bound: one to four replicas of 128 <= L <= 256 (1 x 128^2: 7.8 vs 4.7 flips/ns
-// resident; 1 x 224^2: 16.0 vs 10.6 streaming).  AUTO takes it for at most 2^16 sites with L >= 128.
+// Temporally blocked tile kernel (ising_int8.cu): uniform Ising model, int8 layout, L % 8 == 0; four sweeps per launch on
+// tiles with halos, at most one tile per SM, one thread per 4-site word for the whole launch.  AUTO: prefer_tiled().
 bool use_tiled(const spin_sim* sim) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8) return false;
     if (sim->general || sim->d_bond_nat) return false;
     if (!ising_int8_tiled_fits(sim->batch, sim->L)) return false;
     if (sim->policy == SPIN_POLICY_TILED) return true;
-    if (sim->policy != SPIN_POLICY_AUTO) return false;
-    return sim->L >= 128 && (long long)sim->batch * sim->L * sim->L <= (1ll << 16);
+    return prefer_tiled(sim);
 }
 
 bool enqueue_tiled(spin_sim* sim, int64_t t0, int64_t n_sweeps, const uint32_t* tables = nullptr) {

@@ -341,6 +341,27 @@ def test_tiled_kernel_equals_oracle(oracle_mod, batch, L, n):
         assert np.array_equal(sim.spin_get_spins(), ref)
 
 
+@pytest.mark.parametrize("batch,L,variant", [(2, 256, "ising_int8_tiled"), (16, 128, "ising_int8_tiled"),
+                                             (1, 1024, "ising_int8_tiled"), (16, 64, "ising_int8_tiled"),
+                                             (17, 128, "ising_int8_resident"), (4, 32, "ising_int8_resident"),
+                                             (2, 1056, "ising_int8_rows128")])
+def test_auto_policy_small_launches(oracle_mod, batch, L, variant):
+    """What SPIN_POLICY_AUTO picks around the tile kernel's corner (<= 16 replicas, <= 2^20 sites, L >= 64), each pick
+    against the oracle; spin_sweep_measure on the same handle (never tiled) continues the same trajectory."""
+    seed, n = 90 + L, 6
+    beta = np.linspace(0.3, 0.6, batch)
+    ref = oracle_mod.init(batch, L, seed=seed)
+    with _mk_ising(batch, L, seed) as sim:
+        assert sim.spin_kernel_variant() == variant
+        sim.spin_sweep(beta, 1.0, 0.01, n, 0)
+        oracle_mod.sweep(ref, beta, 1.0, 0.01, seed=seed, n_sweeps=n)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        E, M = sim.spin_sweep_measure(beta, 1.0, 0.01, 2, n)
+        Eo, Mo = oracle_mod.sweep(ref, beta, 1.0, 0.01, seed=seed, n_sweeps=2, sweep_offset=n, trace=True)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+
+
 def test_bits_resident_kernel_many_sweeps_in_one_launch(oracle_mod):
     """Bit-packed replica resident in one CTA: 1024^2 = 128 KiB of shared memory, all sweeps of a call in one
     launch; equals the oracle, the streaming bit-packed kernel and continues across calls and a schedule."""
