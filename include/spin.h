@@ -215,9 +215,10 @@ SPIN_API int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_
  *   SPIN_POLICY_PERSISTENT  one cooperative launch for all sweeps of a call, the lattice in L2, a grid-wide barrier between
  *                           half-sweeps: Ising int8, L % 32 == 0, uniform couplings, no class whose threshold is 0.
  *                           Never picked by AUTO (the streaming kernels are faster on every measured shape).
- *   SPIN_POLICY_TILED       temporal blocking: a CTA advances a tile with a halo by 2-4 sweeps per launch in shared memory,
- *                           about one tile per SM; needs a second lattice buffer (allocated by the library on first use):
- *                           Ising int8, L % 8 == 0, L >= 16, uniform couplings.
+ *   SPIN_POLICY_TILED       temporal blocking: a CTA advances a tile with a halo by 4 (small lattices: 2) sweeps per launch in
+ *                           shared memory, at most one tile per SM (AUTO: up to 16 replicas and 2^20 sites); needs a second
+ *                           lattice buffer (allocated by the library on first use): Ising int8, L % 8 == 0, L >= 16,
+ *                           uniform couplings.
  * Returns SPIN_OK or SPIN_ERR_INVALID (NULL handle, unknown policy). */
 enum { SPIN_POLICY_AUTO = 0, SPIN_POLICY_STREAMING = 1, SPIN_POLICY_RESIDENT = 2, SPIN_POLICY_PERSISTENT = 3,
        SPIN_POLICY_TILED = 4 };
