@@ -91,8 +91,14 @@ class ClockSampler:
                     reasons.add(name)
         if not sm:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
-        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
-                "samples": len(sm)}
+        out = {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "reasons": sorted(reasons),
+               "samples": len(sm), "sm_mhz_min": float(min(sm))}
+        try:
+            pw = [float(line.split(",")[2]) for line in self.lines if len(line.split(",")) >= 7]
+            out["power_w_max"] = max(pw)
+        except ValueError:
+            pass
+        return out
 
 
 def _ncu_traffic(kernel_variant, w):
@@ -629,6 +635,9 @@ def main():
                 "algorithmic_bytes_per_launch": bytes_per_site * upd_per_launch,
                 "launches_per_step": int(n_launch),
                 "kernel_avg_launch_us": kern_ms * 1e3, "ops_per_update": ops,
+                # > 1: the batch is swept as that many replica groups on their own streams, whose launches overlap
+                # (csrc/spin_api.cu, streaming_groups): kernel_avg_launch_us is then sweep time / launches, not a duration
+                "concurrent_chains": max(1, int(n_launch) // (2 * w.n_sweeps)),
                 "peak_source": "derived: 64 INT32 lanes/SM/clk x 148 SMs x %.0f MHz (%s sm_max_mhz); DESIGN.md section 6"
                                % (peaks["sm_max_mhz"], peaks["source"]),
                 "hbm": {"achieved_gbs": hbm_achieved, "peak_gbs": peaks["hbm_gbs"], "frac": hbm_achieved / peaks["hbm_gbs"],
@@ -637,10 +646,13 @@ def main():
         }
         sim.spin_destroy()
         if world == 1 and not args.no_per_config:
+            sampler2 = ClockSampler(local_rank)                 # clocks over the whole per_config part of the run
+            sampler2.start()
             line["per_config"] = per_config_block(runner, sp, args, peaks, measured)
             line["per_config"].update(dmc_entries(runner, sp, args, peaks))
             line["per_config"].update(general_entries(runner, sp, args, peaks, measured))
             line["per_config"].update(stencil_cpm_entries(runner, sp, args, peaks, measured))
+            line["per_config_clocks"] = sampler2.stop()
         if not args.no_cpu_baseline and world == 1:
             v, threads, sample, _ = oracle_throughput(w, 12.0)
             line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "sample": sample,

@@ -16,7 +16,7 @@ constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU
 constexpr int kRowsMid = 4;     // under about one wave of 8-row blocks
 constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
 constexpr int kThreads = 128;
-constexpr int kMinBlocks = 8;   // resident blocks per SM (64 registers)
+constexpr int kMinBlocks = kIsingBitsBlocksPerSm;   // resident blocks per SM (spin_internal.cuh)
 
 // One word = 32 sites = 8 Philox calls.  up / dn / ct: other-colour words of rows i-1, i+1, i; sd: the side
 // neighbours (ct shifted by one site, with the bit of the adjacent word).  The class nibbles of the 32 sites are
@@ -284,7 +284,7 @@ int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
     // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots); the
     // smallest launches do best when the next one is released as soon as a thread has its first rows in registers
     const int perReplica8 = (a.L / kRowsLong) * (a.L >> 6);
-    const long long threads8 = (long long)perReplica8 * a.batch;
+    const long long threads8 = (long long)perReplica8 * a.batch * (a.plan_scale > 0 ? a.plan_scale : 1);
     RowsPlan plan = plan_rows(threads8, perReplica8, 148 * kMinBlocks, 0.3, 0.75, false);
     if (plan.rows == kRowsShort && threads8 < 148ll * kMinBlocks * 128 / 10) plan.trigger = kPdlLastRows;
     const int perReplica = (a.L / plan.rows) * (a.L >> 6);

@@ -67,7 +67,7 @@ __global__ void ising_int8_generic_kernel(SweepArgs a) {
 constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU several times over
 constexpr int kRowsMid = 4;     // ... about one wave of 8-row blocks or less: more, shorter blocks
 constexpr int kRowsShort = 2;   // ... and when even those leave SMs idle (latency-bound shapes)
-constexpr int kMinBlocks = 5;   // resident blocks per SM (96 registers)
+constexpr int kMinBlocks = kIsingInt8BlocksPerSm;   // resident blocks per SM (spin_internal.cuh)
 constexpr int kRowsThreads = 128;
 
 template <int kOff>
@@ -655,7 +655,7 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
         // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots)
         const int perReplica8 = (a.L / kRowsLong) * (a.L >> 5);
-        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch, perReplica8, 148 * kMinBlocks, 0.25, 1.2, true);
+        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch * (a.plan_scale > 0 ? a.plan_scale : 1), perReplica8, 148 * kMinBlocks, 0.25, 1.2, true);
         const int perReplica = (a.L / plan.rows) * (a.L >> 5);    // strips x row blocks of one colour
         const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
         const int bpr = (perReplica + tpb - 1) / tpb;

@@ -58,7 +58,7 @@ constexpr int kRowsLong = 8;    // rows per thread when the launch fills the GPU
 constexpr int kRowsMid = 4;     // under about one and a half waves of 8-row blocks
 constexpr int kRowsShort = 2;   // latency-bound shapes: short threads, four times as many
 constexpr int kRowsThreads = 128;
-constexpr int kMinBlocks = 4;   // resident blocks per SM (128 registers)
+constexpr int kMinBlocks = kPottsBlocksPerSm;   // resident blocks per SM (spin_internal.cuh)
 
 template <int kOff>
 __device__ __forceinline__ uint32_t slot_load_u8(uint32_t saddr) {
@@ -302,7 +302,7 @@ int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
         // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots)
         const int perReplica8 = (a.L / kRowsLong) * (a.L >> 5);
-        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch, perReplica8, 148 * kMinBlocks, 0.3, 1.5, false);
+        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch * (a.plan_scale > 0 ? a.plan_scale : 1), perReplica8, 148 * kMinBlocks, 0.3, 1.5, false);
         const int perReplica = (a.L / plan.rows) * (a.L >> 5);    // strips x row blocks of one colour
         const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
         const int bpr = (perReplica + tpb - 1) / tpb;

@@ -133,6 +133,9 @@ struct spin_sim {
     long long* h_EM = nullptr;       // [2][B] pinned, spin_observables
     RoundKeys rk;
     int64_t launches = 0;
+    // second stream for the replica groups of a streaming sweep (streaming_begin / streaming_end), created on first use
+    cudaStream_t aux_stream = nullptr;
+    cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
     int32_t policy = SPIN_POLICY_AUTO;
 };
 
@@ -280,6 +283,7 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     a.bonds = sim->d_bonds;
     a.rk = sim->rk;
     a.pdl_trigger = kPdlAtExit;
+    a.plan_scale = 1;
     return a;
 }
 
@@ -431,6 +435,82 @@ void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour, const uint32_t* ta
     else sim->launches += launch_ising_int8_half_sweep(a, sim->stream);
 }
 
+// ---- streaming sweeps on two replica groups ---------------------------------------------------------------------------
+// A chain of dependent half-sweep launches leaves the GPU idle between them (the drain of one launch, the release and
+// ramp-up of the next).  Replicas are independent, so the batch is split in two halves whose chains run on two streams: the
+// gaps of one are covered by the kernels of the other.  Measured (profiles/r2_pdl_placement.md): 64 x 1024^2 int8 1178 ->
+// 1278 flips/ns, bit-packed 1269 -> 1351; 16 x 2560^2 1089 -> 1226 / 1287 -> 1383; 16 x 1024^2 956 -> 1153; it loses when a
+// half is too small to fill the GPU on its own turn (16 x 640^2 724 -> 695, 4 x 1024^2 598 -> 525), so it is used from 0.3
+// waves of 8-row blocks upwards.  Class-table models only (the general kernels index natural-order coupling arrays).
+int streaming_groups(const spin_sim* sim) {
+    if (sim->batch < 2 || sim->general || sim->d_bond_nat || sim->potts_general) return 1;
+    if (sim->policy != SPIN_POLICY_AUTO && sim->policy != SPIN_POLICY_STREAMING) return 1;
+    const bool bits = sim->layout == SPIN_LAYOUT_BITPACKED;
+    if (sim->L % (bits ? 64 : 32) != 0) return 1;                // the generic kernels are not planned
+    const int perSm = sim->model == SPIN_MODEL_POTTS ? kPottsBlocksPerSm : bits ? kIsingBitsBlocksPerSm : kIsingInt8BlocksPerSm;
+    const double threads8 = (double)(sim->L / 8) * (sim->L >> (bits ? 6 : 5)) * sim->batch;
+    return threads8 >= 0.3 * 128.0 * 148.0 * perSm ? 2 : 1;
+}
+
+// Fork: the second stream waits for everything enqueued so far on the handle's stream.  Returns the number of groups
+// actually available (1 if the stream / events cannot be created).
+int streaming_begin(spin_sim* sim) {
+    int G = streaming_groups(sim);
+    if (G < 2) return 1;
+    if (!sim->aux_stream) {
+        if (cudaStreamCreateWithFlags(&sim->aux_stream, cudaStreamNonBlocking) != cudaSuccess ||
+            cudaEventCreateWithFlags(&sim->ev_fork, cudaEventDisableTiming) != cudaSuccess ||
+            cudaEventCreateWithFlags(&sim->ev_join, cudaEventDisableTiming) != cudaSuccess) {
+            cudaGetLastError();
+            if (sim->aux_stream) cudaStreamDestroy(sim->aux_stream);
+            if (sim->ev_fork) cudaEventDestroy(sim->ev_fork);
+            sim->aux_stream = nullptr; sim->ev_fork = nullptr; sim->ev_join = nullptr;
+            return 1;
+        }
+    }
+    if (cudaEventRecord(sim->ev_fork, sim->stream) != cudaSuccess || cudaStreamWaitEvent(sim->aux_stream, sim->ev_fork, 0) != cudaSuccess) {
+        cudaGetLastError();
+        return 1;
+    }
+    return G;
+}
+
+// Join: the handle's stream waits for the second one (every later operation of the handle sees all replicas done).
+void streaming_end(spin_sim* sim, int G) {
+    if (G < 2) return;
+    cudaEventRecord(sim->ev_join, sim->aux_stream);
+    cudaStreamWaitEvent(sim->stream, sim->ev_join, 0);
+}
+
+// n_sweeps sweeps from t0 for all replicas: the half-sweeps of the groups interleaved in issue order.
+void enqueue_streaming(spin_sim* sim, int G, int64_t t0, int64_t n_sweeps, const uint32_t* tables = nullptr) {
+    if (G < 2) {
+        for (int64_t t = t0; t < t0 + n_sweeps; ++t) {
+            enqueue_half_sweep(sim, t, 0, tables);
+            enqueue_half_sweep(sim, t, 1, tables);
+        }
+        return;
+    }
+    const size_t perReplica = sim->lattice_bytes / (size_t)sim->batch;
+    const size_t bondWords = (size_t)2 * 4 * sim->L * (sim->L >> 6);       // sign planes of one replica (bit-packed +-J)
+    for (int64_t t = t0; t < t0 + n_sweeps; ++t)
+        for (int colour = 0; colour < 2; ++colour)
+            for (int g = 0; g < G; ++g) {
+                const int b0 = (int)((long long)sim->batch * g / G), b1 = (int)((long long)sim->batch * (g + 1) / G);
+                SweepArgs a = sweep_args(sim, t, colour);
+                a.lattice = (char*)sim->lattice + perReplica * (size_t)b0;
+                a.tables = (tables ? tables : sim->d_tables) + (size_t)b0 * kTableStride;
+                a.batch = b1 - b0;
+                a.replica_offset = sim->replica_offset + (uint32_t)b0;
+                if (a.bonds) a.bonds += bondWords * (size_t)b0;
+                a.plan_scale = G;
+                cudaStream_t st = g == 0 ? sim->stream : sim->aux_stream;
+                if (sim->model == SPIN_MODEL_POTTS) sim->launches += launch_potts_int8_half_sweep(a, st);
+                else if (sim->layout == SPIN_LAYOUT_BITPACKED) sim->launches += launch_ising_bits_half_sweep(a, st);
+                else sim->launches += launch_ising_int8_half_sweep(a, st);
+            }
+}
+
 // Enqueue the reductions of the current lattice into E_out[b], M_out[b] (device int64, either may be NULL).
 // The targets are zeroed first (the kernels accumulate).
 int enqueue_observe(spin_sim* sim, long long* E_out, long long* M_out) {
@@ -530,6 +610,12 @@ void spin_destroy(spin_sim* sim) {
     if (!sim) return;
     cudaSetDevice(sim->device);
     if (sim->stream || sim->lattice) cudaStreamSynchronize(sim->stream);
+    if (sim->aux_stream) {
+        cudaStreamSynchronize(sim->aux_stream);
+        cudaStreamDestroy(sim->aux_stream);
+    }
+    if (sim->ev_fork) cudaEventDestroy(sim->ev_fork);
+    if (sim->ev_join) cudaEventDestroy(sim->ev_join);
     if (sim->owns_lattice && sim->lattice) cudaFree(sim->lattice);
     if (sim->d_tables) cudaFree(sim->d_tables);
     if (sim->d_bonds) cudaFree(sim->d_bonds);
@@ -889,6 +975,8 @@ int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps
     sim->any_never = sched_never;
     const bool tiled = !resident && use_tiled(sim);
     const bool persistent = !resident && !tiled && use_persistent(sim);
+    const bool streams = !resident && !tiled && !persistent && !use_bits_resident(sim);
+    const int G = streams ? streaming_begin(sim) : 1;
     for (int64_t k = 0; k < n_steps; ++k) {
         const uint32_t* tab = sim->d_sched + (size_t)k * B * kTableStride;
         const int64_t t0 = sweep_offset + k * sweeps_per_step;
@@ -897,13 +985,9 @@ int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps
         } else if (use_bits_resident(sim) && enqueue_bits_resident(sim, t0, sweeps_per_step, tab)) {
         } else if (tiled && enqueue_tiled(sim, t0, sweeps_per_step, tab)) {
         } else if (persistent && enqueue_persistent(sim, t0, sweeps_per_step, tab)) {
-        } else {
-            for (int64_t t = t0; t < t0 + sweeps_per_step; ++t) {
-                enqueue_half_sweep(sim, t, 0, tab);
-                enqueue_half_sweep(sim, t, 1, tab);
-            }
-        }
+        } else enqueue_streaming(sim, G, t0, sweeps_per_step, tab);
     }
+    streaming_end(sim, G);
     CUDA_TRY(cudaGetLastError());
     return SPIN_OK;
 }
@@ -929,10 +1013,9 @@ int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_
     } else if (use_bits_resident(sim) && enqueue_bits_resident(sim, sweep_offset, n_sweeps)) {
     } else if (use_tiled(sim) && enqueue_tiled(sim, sweep_offset, n_sweeps)) {
     } else if (!(use_persistent(sim) && enqueue_persistent(sim, sweep_offset, n_sweeps))) {
-        for (int64_t t = sweep_offset; t < sweep_offset + n_sweeps; ++t) {
-            enqueue_half_sweep(sim, t, 0);
-            enqueue_half_sweep(sim, t, 1);
-        }
+        const int G = streaming_begin(sim);
+        enqueue_streaming(sim, G, sweep_offset, n_sweeps);
+        streaming_end(sim, G);
     }
     CUDA_TRY(cudaGetLastError());
     return SPIN_OK;

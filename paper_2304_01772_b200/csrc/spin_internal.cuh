@@ -63,6 +63,8 @@ struct SweepArgs {
                               // centre, side of the colour's sites), or nullptr for uniform couplings
     RoundKeys rk;
     int32_t pdl_trigger;      // PdlTrigger: where the row-marching kernels release the next launch (set by the launchers)
+    int32_t plan_scale;       // the launch is one of plan_scale concurrent ones (replica groups on their own streams,
+                              // spin_api.cu): the launch plan is made for the whole batch
 };
 
 // Shared-memory-resident multi-sweep kernel (small lattices: one CTA holds a whole replica and runs all sweeps of a
@@ -158,6 +160,11 @@ inline int pick_block(int units) {
 // the per-thread set-up and the two halo rows; short threads fill the GPU when the launch is small.  The thresholds are
 // the crossovers of a measured (batch, L) grid per kernel (profiles/r2_pdl_placement.md); min8 = fewest 8-row threads
 // per replica for which 8 or 4 rows keep a block reasonably full.
+// Resident blocks per SM of the three row-marching kernels (their __launch_bounds__), i.e. 148 x this = block slots.
+constexpr int kIsingInt8BlocksPerSm = 5;   // 96 registers
+constexpr int kIsingBitsBlocksPerSm = 8;   // 64 registers
+constexpr int kPottsBlocksPerSm = 4;
+
 struct RowsPlan {
     int rows;
     int32_t trigger;

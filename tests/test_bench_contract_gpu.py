@@ -23,7 +23,8 @@ def test_bench_line_has_the_contract_keys():
     assert d["unit"] == "flips/ns" and d["n_gpus"] == 1 and d["steps"] == 2 and d["warmup"] == 3
     assert d["higher_is_better"] is True and d["scaling"] == "weak" and d["vs_baseline"] is None
     assert "workload" in d["config"] and d["config"]["workload"].startswith("C2")
-    assert d["value"] > 0 and d["gpu_launches"] == 2 * (2 * 10 + 1)
+    # per step: 10 sweeps x 2 colours x 2 replica groups (streaming_groups, csrc/spin_api.cu) + the reduction
+    assert d["value"] > 0 and d["gpu_launches"] == 2 * (2 * 2 * 10 + 1)
     r = d["roofline"]
     assert r["bound"] == "alu" and abs(r["frac"] - r["achieved"] / r["peak"]) < 1e-12 and r["traffic"] > 0
     e = d["e2e"]

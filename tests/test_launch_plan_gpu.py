@@ -91,3 +91,38 @@ def test_bit_packed_bonds_every_plan_equals_oracle(oracle_mod, batch, L):
         E, M = sim.spin_observables()
         Eo, Mo = oracle_mod.ising_bonds_observables(ref, Jh, Jv)
         assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+
+
+# ----------------------------------------------------------------- replica groups on two streams (csrc/spin_api.cu)
+@pytest.mark.parametrize("model,batch,L,layout", [("ising", 31, 1024, "bits"), ("ising", 13, 1024, "int8"),
+                                                  ("potts", 27, 512, "int8")])
+def test_two_replica_groups_sweep_schedule_and_later_calls(oracle_mod, model, batch, L, layout):
+    """From 0.3 waves of 8-row blocks upwards a streaming sweep runs as two replica groups on two streams (odd batches
+    split unevenly); later operations of the handle (observables, a schedule, a measured sweep, get_spins) must see both
+    groups finished, and spin_sweep_schedule runs every step on both."""
+    seed = 600 + batch
+    slots = {"bits": 8, "int8": 5}[layout] if model == "ising" else 4
+    assert _w8(batch, L, layout, slots) >= 0.3, "the case no longer runs as two groups"
+    q = None if model == "ising" else np.array([3 + (b % 6) for b in range(batch)], dtype=np.int32)
+    h = 0.02 if model == "ising" else 0.0
+    beta = np.linspace(0.4, 1.1, batch)
+    ref = oracle_mod.init(batch, L, seed=seed, q=q)
+    lay = sp.SPIN_LAYOUT_BITPACKED if layout == "bits" else sp.SPIN_LAYOUT_INT8
+    mdl = sp.SPIN_MODEL_ISING if model == "ising" else sp.SPIN_MODEL_POTTS
+    obs = oracle_mod.ising_observables if model == "ising" else (lambda s: oracle_mod.potts_observables(s, q))
+    with sp.spin_create_ex(batch, L, mdl, q_per_replica=q, seed=seed, layout=lay) as sim:
+        l0 = sim.spin_kernel_launches()
+        sim.spin_sweep(beta, 1.0, h, 2, 0)
+        assert sim.spin_kernel_launches() - l0 == 2 * 2 * 2          # sweeps x colours x groups
+        oracle_mod.sweep(ref, beta, 1.0, h, seed=seed, n_sweeps=2, q=q)
+        E, M = sim.spin_observables()                                 # on the handle's stream, right after the join
+        Eo, Mo = obs(ref)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+        steps = np.stack([beta, beta[::-1], 0.5 * beta])
+        sim.spin_sweep_schedule(steps, 1.0, h, 2, sweep_offset=2)
+        oracle_mod.sweep_schedule(ref, steps, 1.0, h, seed, 2, sweep_offset=2, q=q)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        Et, Mt = sim.spin_sweep_measure(beta, 1.0, h, 2, 8)
+        Eo, Mo = oracle_mod.sweep(ref, beta, 1.0, h, seed=seed, n_sweeps=2, sweep_offset=8, q=q, trace=True)
+        assert np.array_equal(Et, Eo) and np.array_equal(Mt, Mo)
+        assert np.array_equal(sim.spin_get_spins(), ref)
