@@ -226,7 +226,7 @@ class Runner:
             prepare(sim)
         E_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
         M_dev = torch.zeros(w.batch, dtype=torch.int64, device="cuda")
-        state = {"offset": 0, "per_call": None}
+        state = {"offset": 0, "per_call": None, "host_ms": []}
 
         def step(events=None):
             off = state["offset"]
@@ -234,7 +234,9 @@ class Runner:
                 events[0].record(stream)
             if mode == "sweep":
                 l0 = sim.spin_kernel_launches()
+                th = time.perf_counter()
                 sim.spin_sweep(w.beta, w.J, w.h, w.n_sweeps, off)
+                state["host_ms"].append((time.perf_counter() - th) * 1e3)     # host time to enqueue the call's launches
                 state["per_call"] = sim.spin_kernel_launches() - l0
                 if events:
                     events[1].record(stream)
@@ -271,6 +273,7 @@ class Runner:
         launches0 = sim.spin_kernel_launches()
         barrier()
         torch.cuda.synchronize()
+        state["host_ms"] = []
         for k in range(steps):
             with torch.cuda.stream(stream):
                 self.flush.fill_(k)  # L2 flush, outside the timed interval of the step
@@ -287,6 +290,7 @@ class Runner:
             kernel += " (thermalisation) + ising_int8_resident (measured sweeps, reductions fused)"
         res = {"sim": sim, "step_ms": step_ms, "sweep_ms": sweep_ms, "launches": int(launches),
                "launches_per_sweep_call": state["per_call"], "kernel": kernel, "state": state,
+               "host_enqueue_ms": list(state["host_ms"][:steps]),
                "step_fn": step}
         if e2e_steps:
             host_lat = torch.empty((w.batch, w.L, w.L), dtype=torch.int8).pin_memory()
@@ -340,6 +344,10 @@ def summarise(w, res, peaks, measured_words_per_ns):
                                            if measured_words_per_ns else None)}}
     if "e2e" in res:
         d["e2e"] = res["e2e"]
+    if res.get("host_enqueue_ms"):
+        # host time of the spin_sweep call (it only enqueues): when this approaches ms_per_step the shape is bound by the
+        # host's launch rate, not by the GPU
+        d["host_enqueue_ms"] = float(np.mean(res["host_enqueue_ms"]))
     return d
 
 

@@ -655,7 +655,10 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
         // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots)
         const int perReplica8 = (a.L / kRowsLong) * (a.L >> 5);
-        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch * (a.plan_scale > 0 ? a.plan_scale : 1), perReplica8, 148 * kMinBlocks, 0.25, 1.2, true);
+        // (as one of two replica groups every launch has half the blocks: 2-row threads stay ahead up to 0.6 waves)
+        const bool grouped = a.plan_scale > 1;
+        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch * (grouped ? a.plan_scale : 1), perReplica8, 148 * kMinBlocks,
+                                        grouped ? 0.6 : 0.25, 1.2, true);
         const int perReplica = (a.L / plan.rows) * (a.L >> 5);    // strips x row blocks of one colour
         const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
         const int bpr = (perReplica + tpb - 1) / tpb;

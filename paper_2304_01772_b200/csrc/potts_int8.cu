@@ -302,7 +302,9 @@ int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
         // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots)
         const int perReplica8 = (a.L / kRowsLong) * (a.L >> 5);
-        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch * (a.plan_scale > 0 ? a.plan_scale : 1), perReplica8, 148 * kMinBlocks, 0.3, 1.5, false);
+        const bool grouped = a.plan_scale > 1;                 // one of two replica groups: half the blocks per launch
+        const RowsPlan plan = plan_rows((long long)perReplica8 * a.batch * (grouped ? a.plan_scale : 1), perReplica8, 148 * kMinBlocks,
+                                        grouped ? 0.55 : 0.3, grouped ? 1.2 : 1.5, false);
         const int perReplica = (a.L / plan.rows) * (a.L >> 5);    // strips x row blocks of one colour
         const int tpb = pick_block(perReplica);               // the last block of a replica may be ragged
         const int bpr = (perReplica + tpb - 1) / tpb;

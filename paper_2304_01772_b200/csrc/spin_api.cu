@@ -440,8 +440,8 @@ void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour, const uint32_t* ta
 // ramp-up of the next).  Replicas are independent, so the batch is split in two halves whose chains run on two streams: the
 // gaps of one are covered by the kernels of the other.  Measured (profiles/r2_pdl_placement.md): 64 x 1024^2 int8 1178 ->
 // 1278 flips/ns, bit-packed 1269 -> 1351; 16 x 2560^2 1089 -> 1226 / 1287 -> 1383; 16 x 1024^2 956 -> 1153; it loses when a
-// half is too small to fill the GPU on its own turn (16 x 640^2 724 -> 695, 4 x 1024^2 598 -> 525), so it is used from 0.3
-// waves of 8-row blocks upwards.  Class-table models only (the general kernels index natural-order coupling arrays).
+// half is too small to fill the GPU on its own turn (16 x 640^2 724 -> 695, 4 x 1024^2 598 -> 525), so it is used from 0.15
+// (bit-packed), 0.2 (Potts), 0.3 (int8) waves of 8-row blocks upwards.  Class-table models only (the general kernels index natural-order coupling arrays).
 int streaming_groups(const spin_sim* sim) {
     if (sim->batch < 2 || sim->general || sim->d_bond_nat || sim->potts_general) return 1;
     if (sim->policy != SPIN_POLICY_AUTO && sim->policy != SPIN_POLICY_STREAMING) return 1;
@@ -449,7 +449,8 @@ int streaming_groups(const spin_sim* sim) {
     if (sim->L % (bits ? 64 : 32) != 0) return 1;                // the generic kernels are not planned
     const int perSm = sim->model == SPIN_MODEL_POTTS ? kPottsBlocksPerSm : bits ? kIsingBitsBlocksPerSm : kIsingInt8BlocksPerSm;
     const double threads8 = (double)(sim->L / 8) * (sim->L >> (bits ? 6 : 5)) * sim->batch;
-    return threads8 >= 0.3 * 128.0 * 148.0 * perSm ? 2 : 1;
+    const double from = sim->model == SPIN_MODEL_POTTS ? 0.2 : bits ? 0.15 : 0.3;   // measured crossovers, in waves of 8-row blocks
+    return threads8 >= from * 128.0 * 148.0 * perSm ? 2 : 1;
 }
 
 // Fork: the second stream waits for everything enqueued so far on the handle's stream.  Returns the number of groups

@@ -3,9 +3,9 @@ thread and the point where a half-sweep releases the next launch (at block exit,
 last rows) are chosen from the size of the launch.  The result may not depend on any of it: one shape per branch of each
 kernel's planner, streaming policy, lattice and observables against the oracle after every compared sweep.
 
-w8 = threads of the 8-row grid / (128 x 148 x resident blocks per SM) — int8 Ising: 5 blocks, < 0.25 -> 2 rows,
-< 1.2 -> 4 rows, else 8 rows released at the first instruction; bit-packed: 8 blocks, < 0.3 -> 2 rows (< 0.1: released
-at the last rows), < 0.75 -> 4, else 8; Potts: 4 blocks, < 0.3 -> 2, < 1.5 -> 4, else 8."""
+w8 = threads of the 8-row grid / (128 x 148 x resident blocks per SM: int8 Ising 5, bit-packed 8, Potts 4).  From
+0.3 / 0.15 / 0.2 waves upwards (and batch >= 2) the batch runs as two replica groups on two streams with their own
+thresholds; `_plan` below restates the rules of csrc/ (ising_int8.cu, ising_bits.cu, potts_int8.cu, spin_api.cu)."""
 import numpy as np
 import pytest
 
@@ -19,35 +19,48 @@ def _w8(batch, L, layout, slots_per_sm):
     return per * batch / (128.0 * 148 * slots_per_sm)
 
 
+def _plan(kind, batch, L):
+    """(rows per thread, replica groups) the library picks for a streaming half-sweep of this shape."""
+    layout = "bits" if kind == "bits" else "int8"
+    w8 = _w8(batch, L, layout, {"int8": 5, "bits": 8, "potts": 4}[kind])
+    groups = 2 if batch >= 2 and w8 >= {"int8": 0.3, "bits": 0.15, "potts": 0.2}[kind] else 1
+    lo, hi = {"int8": ((0.25, 1.2), (0.6, 1.2)), "bits": ((0.3, 0.75), (0.3, 0.75)), "potts": ((0.3, 1.5), (0.55, 1.2))}[kind][groups - 1]
+    per8 = (L // 8) * (L >> (6 if layout == "bits" else 5))
+    return (2 if per8 < 64 or w8 < lo else 4 if w8 < hi else 8), groups
+
+
 ISING_PLANS = [
-    # batch, L, layout, expected rows, J, h
-    (2, 1024, "int8", 2, 1.0, 0.0),        # w8 0.09
-    (8, 1024, "int8", 4, 1.0, 0.01),       # w8 0.35
-    (100, 256, "int8", 4, -1.0, 0.2),      # w8 0.27, many replicas per wave
-    (30, 1024, "int8", 8, 1.0, 0.0),       # w8 1.30, released at the first instruction
-    (3, 64, "int8", 2, 1.0, 0.0),          # fewer than 64 eight-row threads per replica
-    (4, 1024, "bits", 2, 1.0, 0.01),       # w8 0.05, released at the last rows
-    (12, 1024, "bits", 2, 1.0, 0.0),       # w8 0.16, released at exit
-    (32, 1024, "bits", 4, -1.0, 0.2),      # w8 0.43
-    (60, 1024, "bits", 8, 1.0, 0.0),       # w8 0.81
+    # batch, L, layout, expected (rows, groups), J, h
+    (2, 1024, "int8", (2, 1), 1.0, 0.0),        # w8 0.09
+    (100, 256, "int8", (4, 1), -1.0, 0.2),      # w8 0.27, many replicas per wave
+    (1, 4096, "int8", (4, 1), 1.0, 0.01),       # w8 0.69, one replica: no groups
+    (8, 1024, "int8", (2, 2), 1.0, 0.01),       # w8 0.35
+    (16, 1024, "int8", (4, 2), 1.0, 0.0),       # w8 0.69
+    (30, 1024, "int8", (8, 2), 1.0, 0.0),       # w8 1.30, released at the first instruction
+    (3, 64, "int8", (2, 1), 1.0, 0.0),          # fewer than 64 eight-row threads per replica
+    (4, 1024, "bits", (2, 1), 1.0, 0.01),       # w8 0.05, released at the last rows
+    (12, 1024, "bits", (2, 2), 1.0, 0.0),       # w8 0.16, released at exit
+    (32, 1024, "bits", (4, 2), -1.0, 0.2),      # w8 0.43
+    (60, 1024, "bits", (8, 2), 1.0, 0.0),       # w8 0.81
+    (1, 8192, "bits", (8, 1), 1.0, 0.0),        # w8 0.86, one replica
 ]
 
 
 @pytest.mark.parametrize("batch,L,layout,rows,J,h", ISING_PLANS)
 def test_ising_every_plan_equals_oracle(oracle_mod, batch, L, layout, rows, J, h):
-    w8 = _w8(batch, L, layout, 8 if layout == "bits" else 5)
-    lo, hi = (0.3, 0.75) if layout == "bits" else (0.25, 1.2)
-    per8 = (L // 8) * (L >> (6 if layout == "bits" else 5))
-    assert rows == (2 if per8 < 64 or w8 < lo else 4 if w8 < hi else 8), "the case no longer hits the branch it names"
+    assert rows == _plan(layout, batch, L), "the case no longer hits the branch it names"
     seed = 300 + batch
     beta = np.linspace(0.3, 0.6, batch)
-    beta[-1] = 20.0                                           # one replica with never-accepted classes
+    if batch > 1:
+        beta[-1] = 20.0                                       # one replica with never-accepted classes
     lay = sp.SPIN_LAYOUT_BITPACKED if layout == "bits" else sp.SPIN_LAYOUT_INT8
     ref = oracle_mod.init(batch, L, seed=seed)
     with sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed, layout=lay) as sim:
         sim.spin_set_policy(sp.SPIN_POLICY_STREAMING)
         for t0, n in ((0, 1), (1, 3)):
+            l0 = sim.spin_kernel_launches()
             sim.spin_sweep(beta, J, h, n, t0)
+            assert sim.spin_kernel_launches() - l0 == 2 * n * rows[1]        # colours x sweeps x replica groups
             oracle_mod.sweep(ref, beta, J, h, seed=seed, n_sweeps=n, sweep_offset=t0)
             assert np.array_equal(sim.spin_get_spins(), ref), "lattice differs after sweep %d" % (t0 + n - 1)
         E, M = sim.spin_observables()
@@ -55,18 +68,21 @@ def test_ising_every_plan_equals_oracle(oracle_mod, batch, L, layout, rows, J, h
         assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
 
 
-@pytest.mark.parametrize("batch,L,rows", [(2, 512, 2), (32, 512, 4), (4, 1024, 2), (120, 512, 8)])
+@pytest.mark.parametrize("batch,L,rows", [(2, 512, (2, 1)), (1, 4096, (4, 1)), (32, 512, (2, 2)), (64, 512, (4, 2)),
+                                          (120, 512, (8, 2))])
 def test_potts_every_plan_equals_oracle(oracle_mod, batch, L, rows):
-    w8 = _w8(batch, L, "int8", 4)
-    assert rows == (2 if w8 < 0.3 else 4 if w8 < 1.5 else 8), "the case no longer hits the branch it names"
+    assert rows == _plan("potts", batch, L), "the case no longer hits the branch it names"
     seed = 400 + batch
     q = np.array([3, 8, 5, 127][: min(batch, 4)] + [3 + (b % 6) for b in range(max(0, batch - 4))], dtype=np.int32)
     beta = np.linspace(0.5, 1.6, batch)
-    beta[0] = 25.0                                            # never-accepted classes
+    if batch > 1:
+        beta[0] = 25.0                                        # never-accepted classes
     ref = oracle_mod.init(batch, L, seed=seed, q=q)
     with sp.spin_create_ex(batch, L, sp.SPIN_MODEL_POTTS, q_per_replica=q, seed=seed) as sim:
         for t0, n in ((0, 1), (1, 2)):
+            l0 = sim.spin_kernel_launches()
             sim.spin_sweep(beta, 1.0, 0.0, n, t0)
+            assert sim.spin_kernel_launches() - l0 == 2 * n * rows[1]        # colours x sweeps x replica groups
             oracle_mod.sweep(ref, beta, 1.0, 0.0, seed=seed, n_sweeps=n, sweep_offset=t0, q=q)
             assert np.array_equal(sim.spin_get_spins(), ref), "lattice differs after sweep %d" % (t0 + n - 1)
         E, M = sim.spin_observables()
@@ -101,8 +117,7 @@ def test_two_replica_groups_sweep_schedule_and_later_calls(oracle_mod, model, ba
     split unevenly); later operations of the handle (observables, a schedule, a measured sweep, get_spins) must see both
     groups finished, and spin_sweep_schedule runs every step on both."""
     seed = 600 + batch
-    slots = {"bits": 8, "int8": 5}[layout] if model == "ising" else 4
-    assert _w8(batch, L, layout, slots) >= 0.3, "the case no longer runs as two groups"
+    assert _plan("potts" if model == "potts" else layout, batch, L)[1] == 2, "the case no longer runs as two groups"
     q = None if model == "ising" else np.array([3 + (b % 6) for b in range(batch)], dtype=np.int32)
     h = 0.02 if model == "ising" else 0.0
     beta = np.linspace(0.4, 1.1, batch)
