@@ -288,6 +288,17 @@ SPIN_API int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_
  * Synchronises the stream. */
 SPIN_API int spin_stencil_observables(int32_t stencil, int32_t batch, int32_t L, const int8_t* lattice, int64_t* E1,
                                       int64_t* E2, int64_t* M, void* cuda_stream);
+/* The same reductions for callers that may not allocate (code under CUDA graph capture, tight serving loops, harnesses
+ * that forbid cudaMalloc): no cudaMalloc / cudaFree / allocating library routine, no host synchronisation.  The
+ * accumulators live in a fixed device array inside the library (96 KiB per GPU that loads it, held until exit), hence
+ * batch <= 4096: larger batches are rejected with SPIN_ERR_INVALID.  E1_dev, E2_dev, M_dev: DEVICE int64 [batch], any may
+ * be NULL; written by work enqueued on cuda_stream (asynchronous: synchronise the stream before reading them).  The call
+ * uses the CURRENT device, which must be the one holding lattice and the outputs (ordinal < 64, else
+ * SPIN_ERR_UNSUPPORTED).  Every call shares the one array (cleared at the start of each call): calls that overlap on the
+ * GPU - different streams, or graphs replayed concurrently - race on it; order them.  Other arguments and errors as for
+ * spin_stencil_observables. */
+SPIN_API int spin_stencil_observables_noalloc(int32_t stencil, int32_t batch, int32_t L, const int8_t* lattice,
+                                              int64_t* E1_dev, int64_t* E2_dev, int64_t* M_dev, void* cuda_stream);
 
 /* ---------------------------------------------------------------------------------------------
  * Cellular Potts model (Eq. 7 and Table II of the paper):

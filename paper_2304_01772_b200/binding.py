@@ -22,6 +22,7 @@ __all__ = [
     "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim", "spin_measure_philox_compare_rate",
     "SPIN_DTYPE_F32", "SPIN_DTYPE_F64", "SPIN_STENCIL_TRIANGULAR", "SPIN_STENCIL_CUBIC", "SPIN_STENCIL_SQUARE_NNN",
     "spin_stencil_sites", "spin_stencil_init", "spin_stencil_sweep", "spin_stencil_observables",
+    "spin_stencil_observables_noalloc",
     "spin_cpm_sweep", "spin_cpm_observables", "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
     "spin_create", "spin_create_ex",
 ]
@@ -74,6 +75,7 @@ def load_library():
         "spin_stencil_init": (c.c_int, [i32, i32, i32, vp, u64, i64, vp]),
         "spin_stencil_sweep": (c.c_int, [i32, i32, i32, vp, vp, dbl, dbl, dbl, u64, i64, i64, i64, vp]),
         "spin_stencil_observables": (c.c_int, [i32, i32, i32, vp, vp, vp, vp, vp]),
+        "spin_stencil_observables_noalloc": (c.c_int, [i32, i32, i32, vp, vp, vp, vp, vp]),
         "spin_cpm_sweep": (c.c_int, [i32, i32, i32, vp, vp, vp, i32, i64, vp, vp, u64, i64, i64, i64, vp]),
         "spin_cpm_observables": (c.c_int, [i32, i32, i32, vp, vp, vp, i32, i64, vp, vp, vp, vp, vp, vp]),
         "spin_dmc_forward": (c.c_int, [i32, i32, i32, vp, vp, vp, dbl, vp, dbl, u64, i64, i64, i64, vp, vp, vp]),
@@ -96,6 +98,7 @@ EXPORTED_SYMBOLS = (
     "spin_dmc_forward", "spin_dmc_backward", "spin_dmc_discretise",
     "spin_set_couplings", "spin_energy_general", "spin_potts_label_sum", "spin_sweep_schedule",
     "spin_stencil_sites", "spin_stencil_init", "spin_stencil_sweep", "spin_stencil_observables",
+    "spin_stencil_observables_noalloc",
     "spin_cpm_sweep", "spin_cpm_observables",
 )
 
@@ -179,6 +182,11 @@ def spin_stencil_observables(stencil, batch, L, lattice_ptr, cuda_stream=None):
     _check(load_library().spin_stencil_observables(stencil, batch, L, lattice_ptr, _np_ptr(E1), _np_ptr(E2), _np_ptr(M),
                                                    cuda_stream))
     return E1, E2, M
+
+
+def spin_stencil_observables_noalloc(stencil, batch, L, lattice_ptr, E1_ptr, E2_ptr, M_ptr, cuda_stream=None):
+    """E1_ptr / E2_ptr / M_ptr: DEVICE int64 [batch] (or None); asynchronous, allocates nothing (batch <= 4096)."""
+    _check(load_library().spin_stencil_observables_noalloc(stencil, batch, L, lattice_ptr, E1_ptr, E2_ptr, M_ptr, cuda_stream))
 
 
 def _cpm_arrays(tau, Jtab, A):

@@ -396,6 +396,26 @@ __global__ void __launch_bounds__(256) stencil_observe_kernel(const int8_t* __re
     }
 }
 
+// ---- scratch of spin_stencil_observables_noalloc: the accumulators the reduction kernel adds into, in a file-scope device
+// array (every GPU that loads the library holds these 96 KiB until exit) instead of a per-call allocation.  In HOST code
+// the name g_noalloc_acc is a stand-in, not a device address: the launcher below asks cudaGetSymbolAddress for the
+// address, once per device, with that device current.
+constexpr int kNoAllocMaxBatch = 4096;
+static __device__ __align__(256) long long g_noalloc_acc[3 * kNoAllocMaxBatch];
+
+// acc[3 b + {0, 1, 2}] -> E1[b], E2[b], M[b] (device outputs, any may be NULL).
+__global__ void stencil_noalloc_scatter_kernel(const long long* __restrict__ acc, int batch, long long* E1, long long* E2,
+                                               long long* M) {
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    if (E1) E1[b] = acc[3 * b];
+    if (E2) E2[b] = acc[3 * b + 1];
+    if (M) M[b] = acc[3 * b + 2];
+}
+
+constexpr int kNoAllocMaxDevices = 64;
+long long* g_noalloc_ptr[kNoAllocMaxDevices] = {};     // device address of g_noalloc_acc on device d, once looked up
+
 int stencil_fail(int code, const char* msg) { return set_error(code, msg); }
 
 int check_shape(int32_t stencil, int32_t batch, int32_t L) {
@@ -550,5 +570,42 @@ int spin_stencil_observables(int32_t stencil, int32_t batch, int32_t L, const in
     }
     return SPIN_OK;
 }
+
+int spin_stencil_observables_noalloc(int32_t stencil, int32_t batch, int32_t L, const int8_t* lattice, int64_t* E1_dev,
+                                     int64_t* E2_dev, int64_t* M_dev, void* cuda_stream) {
+    const int rc = check_shape(stencil, batch, L);
+    if (rc != SPIN_OK) return rc;
+    if (!lattice) return stencil_fail(SPIN_ERR_INVALID, "spin_stencil_observables_noalloc: NULL lattice");
+    if (batch > kNoAllocMaxBatch)
+        return stencil_fail(SPIN_ERR_INVALID, "spin_stencil_observables_noalloc: batch exceeds the fixed scratch (at most 4096 replicas "
+                                              "per call); split the batch or use spin_stencil_observables");
+    cudaStream_t s = (cudaStream_t)cuda_stream;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return stencil_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+    if (dev < 0 || dev >= kNoAllocMaxDevices) return stencil_fail(SPIN_ERR_UNSUPPORTED, "spin_stencil_observables_noalloc: device ordinal >= 64");
+    long long* acc = g_noalloc_ptr[dev];
+    if (!acc) {
+        // once per device, with that device current (two threads racing here store the same address)
+        e = cudaGetSymbolAddress((void**)&acc, g_noalloc_acc);
+        if (e != cudaSuccess || !acc) return stencil_fail(SPIN_ERR_CUDA, e != cudaSuccess ? cudaGetErrorString(e) : "cudaGetSymbolAddress returned NULL");
+        g_noalloc_ptr[dev] = acc;
+    }
+    // the array keeps the previous call's sums and the kernel accumulates: clear this call's part first
+    e = cudaMemsetAsync(acc, 0, sizeof(long long) * 3 * (size_t)batch, s);
+    if (e != cudaSuccess) return stencil_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+    const long long N = total_sites(stencil, L);
+    long long want = (N + 255) / 256, cap = (148ll * 16 + batch - 1) / batch;
+    const int bpr = (int)(want < cap ? want : (cap < 1 ? 1 : cap));
+    const unsigned grid = (unsigned)((long long)bpr * batch);
+    if (stencil == SPIN_STENCIL_TRIANGULAR) stencil_observe_kernel<SPIN_STENCIL_TRIANGULAR><<<grid, 256, 0, s>>>(lattice, L, bpr, acc);
+    else if (stencil == SPIN_STENCIL_CUBIC) stencil_observe_kernel<SPIN_STENCIL_CUBIC><<<grid, 256, 0, s>>>(lattice, L, bpr, acc);
+    else stencil_observe_kernel<SPIN_STENCIL_SQUARE_NNN><<<grid, 256, 0, s>>>(lattice, L, bpr, acc);
+    stencil_noalloc_scatter_kernel<<<(unsigned)((batch + 127) / 128), 128, 0, s>>>(acc, batch, (long long*)E1_dev, (long long*)E2_dev,
+                                                                                 (long long*)M_dev);
+    e = cudaGetLastError();
+    return e == cudaSuccess ? SPIN_OK : stencil_fail(SPIN_ERR_CUDA, cudaGetErrorString(e));
+}
+
 
 }  // extern "C"
