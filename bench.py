@@ -380,6 +380,14 @@ def per_config_block(runner, sp, args, peaks, measured):
             d["paper_rtx3060_flips_per_ns"] = paper[w.name]
             out["%s-%s" % (w.name, layout)] = d
             res["sim"].spin_destroy()
+        if w.name in ("P_1x2560", "P_16x640") and w.n_sweeps >= 64:
+            # the same sweeps replayed from a CUDA graph (SPIN_POLICY_GRAPH): what it buys is host_enqueue_ms
+            w.layout = "int8"
+            res = runner.run(w, "sweep", args.steps, args.warmup, policy=sp.SPIN_POLICY_GRAPH)
+            d = summarise(w, res, peaks, measured)
+            d["mode"] = "SPIN_POLICY_GRAPH: one cudaGraphLaunch per 64 sweeps"
+            out["%s-int8-graph" % w.name] = d
+            res["sim"].spin_destroy()
     return out
 
 

@@ -219,9 +219,16 @@ SPIN_API int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_
  *                           shared memory, at most one tile per SM (AUTO: up to 16 replicas and 2^20 sites); needs a second
  *                           lattice buffer (allocated by the library on first use): Ising int8, L % 8 == 0, L >= 16,
  *                           uniform couplings.
+ *   SPIN_POLICY_GRAPH       the streaming kernels replayed from a CUDA graph of 64 sweeps captured once per handle (the kernels
+ *                           read the sweep index from device memory): spin_sweep calls of >= 64 sweeps cost the host one
+ *                           graph launch per 64 sweeps instead of 2-4 launches per sweep; the GPU-side rate is 1-5 % below
+ *                           SPIN_POLICY_STREAMING.  Class-table models (uniform or +-J couplings, Potts without field),
+ *                           L % 32 == 0 (bit-packed: L % 64 == 0), a handle created on a stream of its own (the legacy
+ *                           default stream cannot be captured); spin_sweep only (spin_sweep_schedule and
+ *                           spin_sweep_measure stream).  Never picked by AUTO.
  * Returns SPIN_OK or SPIN_ERR_INVALID (NULL handle, unknown policy). */
 enum { SPIN_POLICY_AUTO = 0, SPIN_POLICY_STREAMING = 1, SPIN_POLICY_RESIDENT = 2, SPIN_POLICY_PERSISTENT = 3,
-       SPIN_POLICY_TILED = 4 };
+       SPIN_POLICY_TILED = 4, SPIN_POLICY_GRAPH = 5 };
 SPIN_API int spin_set_policy(spin_sim* sim, int32_t policy);
 
 /* ---------------------------------------------------------------------------------------------

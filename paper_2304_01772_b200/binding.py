@@ -12,13 +12,14 @@ SPIN_OK, SPIN_ERR_INVALID, SPIN_ERR_NOMEM, SPIN_ERR_CUDA, SPIN_ERR_UNSUPPORTED =
 SPIN_MODEL_ISING, SPIN_MODEL_POTTS = 0, 1
 SPIN_LAYOUT_INT8, SPIN_LAYOUT_BITPACKED = 0, 1
 SPIN_POLICY_AUTO, SPIN_POLICY_STREAMING, SPIN_POLICY_RESIDENT, SPIN_POLICY_PERSISTENT, SPIN_POLICY_TILED = 0, 1, 2, 3, 4
+SPIN_POLICY_GRAPH = 5
 SPIN_DTYPE_F32, SPIN_DTYPE_F64 = 0, 1
 SPIN_STENCIL_TRIANGULAR, SPIN_STENCIL_CUBIC, SPIN_STENCIL_SQUARE_NNN = 0, 1, 2
 
 __all__ = [
     "SPIN_OK", "SPIN_ERR_INVALID", "SPIN_ERR_NOMEM", "SPIN_ERR_CUDA", "SPIN_ERR_UNSUPPORTED",
     "SPIN_MODEL_ISING", "SPIN_MODEL_POTTS", "SPIN_LAYOUT_INT8", "SPIN_LAYOUT_BITPACKED",
-    "SPIN_POLICY_AUTO", "SPIN_POLICY_STREAMING", "SPIN_POLICY_RESIDENT", "SPIN_POLICY_PERSISTENT", "SPIN_POLICY_TILED",
+    "SPIN_POLICY_AUTO", "SPIN_POLICY_STREAMING", "SPIN_POLICY_RESIDENT", "SPIN_POLICY_PERSISTENT", "SPIN_POLICY_TILED", "SPIN_POLICY_GRAPH",
     "SpinError", "load_library", "spin_last_error", "spin_buffer_bytes", "spin_threshold_table", "SpinSim", "spin_measure_philox_compare_rate",
     "SPIN_DTYPE_F32", "SPIN_DTYPE_F64", "SPIN_STENCIL_TRIANGULAR", "SPIN_STENCIL_CUBIC", "SPIN_STENCIL_SQUARE_NNN",
     "spin_stencil_sites", "spin_stencil_init", "spin_stencil_sweep", "spin_stencil_observables",

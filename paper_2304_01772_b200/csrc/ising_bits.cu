@@ -59,7 +59,7 @@ __device__ __forceinline__ void group_step(uint32_t& flip, const uint32_t r[4], 
 
 // Two Philox groups (sites 8p .. 8p+7) share one byte of each t[e].
 template <bool kHasNever, int kP>
-__device__ __forceinline__ void pair_step(const SweepArgs& a, uint32_t& flip, uint32_t g0, uint32_t c1,
+__device__ __forceinline__ void pair_step(const PhiloxCtx& a, uint32_t& flip, uint32_t g0, uint32_t c1,
                                           const uint32_t* stab, const uint8_t* sT, uint32_t never, uint32_t slot) {
     uint32_t v[4];
     v[0] = slot_load_u8<0 * kThreads * 4 + kP>(slot);
@@ -74,7 +74,7 @@ __device__ __forceinline__ void pair_step(const SweepArgs& a, uint32_t& flip, ui
 }
 
 template <bool kHasNever>
-__device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own, uint32_t up, uint32_t dn, uint32_t ct,
+__device__ __forceinline__ uint32_t update_word(const PhiloxCtx& a, uint32_t own, uint32_t up, uint32_t dn, uint32_t ct,
                                                 uint32_t sd, uint32_t g0, uint32_t c1, const uint32_t* stab,
                                                 const uint8_t* sT, uint32_t never, uint32_t slot) {
     // bit-sliced count of -1 neighbours: nd = P0 + 2 P1 + 4 P2
@@ -103,7 +103,7 @@ __device__ __forceinline__ uint32_t update_word(const SweepArgs& a, uint32_t own
 // kBonds: +-J couplings (SweepArgs::bonds): the neighbour words are XORed with the sign planes of the bonds that
 // join them to the row's sites, so the adder counts neighbours whose bond-weighted spin is -1; nothing else changes.
 template <int kColour, bool kHasNever, int kRows, bool kBonds>
-__device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint8_t* sT, uint32_t never,
+__device__ __forceinline__ void march_rows(const SweepArgs& a, const PhiloxCtx& pc, const uint32_t* stab, const uint8_t* sT, uint32_t never,
                                            uint32_t slot, int b, int rb, int x) {
     const int L = a.L, WW = L >> 6;                       // words per colour-row
     const size_t half = (size_t)L * WW;
@@ -143,7 +143,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             pB += 2 * rowStride;
         }
         uint32_t sd = kColour ? ((wC >> 1) | (edge << 31)) : ((wC << 1) | (edge >> 31));
-        *pOwn = update_word<kHasNever>(a, own, wU ^ bu, wD ^ bd, wC ^ bc, sd ^ bs, g0, c1, stab, sT, never, slot);
+        *pOwn = update_word<kHasNever>(pc, own, wU ^ bu, wD ^ bd, wC ^ bc, sd ^ bs, g0, c1, stab, sT, never, slot);
         uint32_t n2 = n1, own2 = own1, edge2 = edge1;
         if (more) {
             n2 = __ldg(pOth + rowStride);
@@ -151,7 +151,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             edge2 = __ldg(pEdgeEven + 2 * rowStride);
         }
         sd = kColour ? ((wD << 1) | (edge1 >> 31)) : ((wD >> 1) | (edge1 << 31));
-        *(pOwn + rowStride) = update_word<kHasNever>(a, own1, wC ^ bu1, n1 ^ bd1, wD ^ bc1, sd ^ bs1, g0 + (uint32_t)(L >> 3),
+        *(pOwn + rowStride) = update_word<kHasNever>(pc, own1, wC ^ bu1, n1 ^ bd1, wD ^ bc1, sd ^ bs1, g0 + (uint32_t)(L >> 3),
                                                      c1, stab, sT, never, slot);
         wU = wD;
         wC = n1;
@@ -166,7 +166,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
     }
 }
 
-template <int kColour, int kRows, bool kBonds>
+template <int kColour, int kRows, bool kBonds, bool kDevT>
 __global__ void __launch_bounds__(kThreads, kMinBlocks) ising_bits_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[16];                          // U[class], class = d * 8 + nd
     __shared__ __align__(16) uint8_t sT[kAuxBytes];        // [e][half][byte] -> 4 * class
@@ -176,6 +176,9 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) ising_bits_kernel(SweepA
     const int blk = blockIdx.x - b * bpr;
     for (int k = threadIdx.x; k < kAuxBytes / 16; k += blockDim.x) ((uint4*)sT)[k] = ((const uint4*)a.aux)[k];   // constant
     pdl_wait();
+    uint32_t c2, c3;
+    sweep_counter_words<kDevT>(a, c2, c3);
+    const PhiloxCtx pc = {a.rk, c2, c3};
     const uint32_t* tab = a.tables + (size_t)b * kTableStride;
     const uint32_t never = tab[kTabNever];
     for (int m = threadIdx.x; m < 16; m += blockDim.x) stab[m] = tab[m];
@@ -185,8 +188,8 @@ __global__ void __launch_bounds__(kThreads, kMinBlocks) ising_bits_kernel(SweepA
     const int u = blk * blockDim.x + threadIdx.x;
     if (u >= (a.L / kRows) * WW) return;                  // ragged last block of a replica (after the barrier)
     const int rb = u / WW, x = u - rb * WW;
-    if (never) march_rows<kColour, true, kRows, kBonds>(a, stab, sT, never, slot, b, rb, x);
-    else march_rows<kColour, false, kRows, kBonds>(a, stab, sT, never, slot, b, rb, x);
+    if (never) march_rows<kColour, true, kRows, kBonds>(a, pc, stab, sT, never, slot, b, rb, x);
+    else march_rows<kColour, false, kRows, kBonds>(a, pc, stab, sT, never, slot, b, rb, x);
 }
 
 // ---- shared-memory-resident kernel ("a 1024^2 replica is 128 KiB as bits and fits one CTA"): one CTA per
@@ -231,8 +234,8 @@ __global__ void __launch_bounds__(kBitsResThreads) ising_bits_resident_kernel(Re
                 const uint32_t sd = par ? ((ct >> 1) | (ew << 31)) : ((ct << 1) | (ew >> 31));
                 const uint32_t g0 = (uint32_t)i * (uint32_t)(L >> 3) + 8u * (uint32_t)x;
                 uint32_t res;
-                if (never) res = update_word<true>(sa, own1[w], oth1[iu * WW + x], oth1[id * WW + x], ct, sd, g0, c1, stab, sT, never, slot);
-                else res = update_word<false>(sa, own1[w], oth1[iu * WW + x], oth1[id * WW + x], ct, sd, g0, c1, stab, sT, never, slot);
+                if (never) res = update_word<true>(PhiloxCtx{sa.rk, sa.c2, sa.c3}, own1[w], oth1[iu * WW + x], oth1[id * WW + x], ct, sd, g0, c1, stab, sT, never, slot);
+                else res = update_word<false>(PhiloxCtx{sa.rk, sa.c2, sa.c3}, own1[w], oth1[iu * WW + x], oth1[id * WW + x], ct, sd, g0, c1, stab, sT, never, slot);
                 own1[w] = res;
             }
             __syncthreads();
@@ -280,6 +283,21 @@ uint8_t* ising_bits_make_aux_table() {
     }
 }
 
+// The instantiation for (rows per thread, colour, +-J couplings); kDevT: sweep index from device memory (graph nodes).
+template <bool kDevT>
+static void (*pick_bits_kernel(int rows, int colour, bool bonds))(SweepArgs, int) {
+    if (rows == kRowsShort) {
+        if (bonds) return colour == 0 ? ising_bits_kernel<0, kRowsShort, true, kDevT> : ising_bits_kernel<1, kRowsShort, true, kDevT>;
+        return colour == 0 ? ising_bits_kernel<0, kRowsShort, false, kDevT> : ising_bits_kernel<1, kRowsShort, false, kDevT>;
+    }
+    if (rows == kRowsMid) {
+        if (bonds) return colour == 0 ? ising_bits_kernel<0, kRowsMid, true, kDevT> : ising_bits_kernel<1, kRowsMid, true, kDevT>;
+        return colour == 0 ? ising_bits_kernel<0, kRowsMid, false, kDevT> : ising_bits_kernel<1, kRowsMid, false, kDevT>;
+    }
+    if (bonds) return colour == 0 ? ising_bits_kernel<0, kRowsLong, true, kDevT> : ising_bits_kernel<1, kRowsLong, true, kDevT>;
+    return colour == 0 ? ising_bits_kernel<0, kRowsLong, false, kDevT> : ising_bits_kernel<1, kRowsLong, false, kDevT>;
+}
+
 int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
     // rows per thread and release point: measured crossovers of this kernel (148 x kMinBlocks block slots); the
     // smallest launches do best when the next one is released as soon as a thread has its first rows in registers
@@ -294,17 +312,7 @@ int launch_ising_bits_half_sweep(const SweepArgs& a, cudaStream_t s) {
     SweepArgs args = a;
     args.pdl_trigger = plan.trigger;
     const bool bonds = a.bonds != nullptr;
-    void (*k)(SweepArgs, int);
-    if (plan.rows == kRowsShort) {
-        if (bonds) k = a.colour == 0 ? ising_bits_kernel<0, kRowsShort, true> : ising_bits_kernel<1, kRowsShort, true>;
-        else k = a.colour == 0 ? ising_bits_kernel<0, kRowsShort, false> : ising_bits_kernel<1, kRowsShort, false>;
-    } else if (plan.rows == kRowsMid) {
-        if (bonds) k = a.colour == 0 ? ising_bits_kernel<0, kRowsMid, true> : ising_bits_kernel<1, kRowsMid, true>;
-        else k = a.colour == 0 ? ising_bits_kernel<0, kRowsMid, false> : ising_bits_kernel<1, kRowsMid, false>;
-    } else {
-        if (bonds) k = a.colour == 0 ? ising_bits_kernel<0, kRowsLong, true> : ising_bits_kernel<1, kRowsLong, true>;
-        else k = a.colour == 0 ? ising_bits_kernel<0, kRowsLong, false> : ising_bits_kernel<1, kRowsLong, false>;
-    }
+    void (*k)(SweepArgs, int) = a.t_dev ? pick_bits_kernel<true>(plan.rows, a.colour, bonds) : pick_bits_kernel<false>(plan.rows, a.colour, bonds);
     launch_pdl(k, grid, (unsigned)tpb, s, args, bpr);
     return 1;
 }

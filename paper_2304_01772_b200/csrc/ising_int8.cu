@@ -168,8 +168,8 @@ __device__ __forceinline__ uint4 mask4(const uint4& v) {
 }
 
 template <int kColour, bool kHasNever, int kRows, bool kPersist = false>
-__device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, uint32_t slot, int b, int rb,
-                                           int x) {
+__device__ __forceinline__ void march_rows(const SweepArgs& a, uint32_t c2, uint32_t c3, const uint32_t* stab, uint32_t slot,
+                                           int b, int rb, int x) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
     const size_t half = (size_t)L * W;
     const int i0 = rb * kRows;
@@ -217,10 +217,10 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             own2 = ldown<kPersist>(pOwn + 2 * rowStride);
             edge2 = ld1<kPersist>(pEdgeEven + edgeStride2);
         }
-        uint4 res = update_row<kHasNever, kColour>(a.rk, a.c2, a.c3, own, wU, wC, wD, edge, g0, c1, stab, slot);
+        uint4 res = update_row<kHasNever, kColour>(a.rk, c2, c3, own, wU, wC, wD, edge, g0, c1, stab, slot);
         *pOwn = res;
         const uint4 n1m = mask4(n1);
-        res = update_row<kHasNever, 1 - kColour>(a.rk, a.c2, a.c3, own1, wC, wD, n1m, edge1 & 0x04040404u,
+        res = update_row<kHasNever, 1 - kColour>(a.rk, c2, c3, own1, wC, wD, n1m, edge1 & 0x04040404u,
                                                  g0 + (uint32_t)W4, c1, stab, slot);
         *(pOwn + rowStride) = res;
         wU = wD;
@@ -237,7 +237,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 }
 
 // One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
-template <int kColour, int kRows>
+template <int kColour, int kRows, bool kDevT>
 __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[kTableStride];
     __shared__ uint32_t sidx[4 * kRowsThreads];   // per-thread slot: word j of thread t at sidx[j * 128 + t]
@@ -245,6 +245,8 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_kern
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
     pdl_wait();
+    uint32_t c2, c3;
+    sweep_counter_words<kDevT>(a, c2, c3);
     const uint32_t never = a.tables[(size_t)b * kTableStride + kTabNever];   // block-uniform
     for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
     const int W16 = a.L >> 5;
@@ -254,8 +256,8 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_kern
     if (u >= (a.L / kRows) * W16) return;
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
-    if (never) march_rows<kColour, true, kRows>(a, stab, slot, b, rb, x);
-    else march_rows<kColour, false, kRows>(a, stab, slot, b, rb, x);
+    if (never) march_rows<kColour, true, kRows>(a, c2, c3, stab, slot, b, rb, x);
+    else march_rows<kColour, false, kRows>(a, c2, c3, stab, slot, b, rb, x);
 }
 
 // ---- persistent kernel for launch-bound shapes (lattices too big for one CTA's shared memory, too small for a
@@ -308,8 +310,8 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_persisten
                 const int u = blk * blockDim.x + threadIdx.x;
                 if (u < perReplica) {
                     const int rb = u / W16, x = u - rb * W16;
-                    if (colour == 0) march_rows<0, false, kRows, true>(a, stab, slot, b, rb, x);
-                    else march_rows<1, false, kRows, true>(a, stab, slot, b, rb, x);
+                    if (colour == 0) march_rows<0, false, kRows, true>(a, a.c2, a.c3, stab, slot, b, rb, x);
+                    else march_rows<1, false, kRows, true>(a, a.c2, a.c3, stab, slot, b, rb, x);
                 }
             }
             grid_barrier(counter, target);
@@ -666,9 +668,13 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
         SweepArgs args = a;
         args.pdl_trigger = plan.trigger;
         void (*k)(SweepArgs, int);
-        if (plan.rows == kRowsShort) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsShort> : ising_int8_rows_kernel<1, kRowsShort>;
-        else if (plan.rows == kRowsMid) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsMid> : ising_int8_rows_kernel<1, kRowsMid>;
-        else k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsLong> : ising_int8_rows_kernel<1, kRowsLong>;
+        if (a.t_dev) {
+            if (plan.rows == kRowsShort) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsShort, true> : ising_int8_rows_kernel<1, kRowsShort, true>;
+            else if (plan.rows == kRowsMid) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsMid, true> : ising_int8_rows_kernel<1, kRowsMid, true>;
+            else k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsLong, true> : ising_int8_rows_kernel<1, kRowsLong, true>;
+        } else if (plan.rows == kRowsShort) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsShort, false> : ising_int8_rows_kernel<1, kRowsShort, false>;
+        else if (plan.rows == kRowsMid) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsMid, false> : ising_int8_rows_kernel<1, kRowsMid, false>;
+        else k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsLong, false> : ising_int8_rows_kernel<1, kRowsLong, false>;
         launch_pdl(k, grid, (unsigned)tpb, s, args, bpr);
     } else {
         const long long half = (long long)a.L * (a.L >> 1);

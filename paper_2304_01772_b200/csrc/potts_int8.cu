@@ -162,7 +162,7 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
 // One row of one strip.  up / ct / dn: other-colour words of rows i-1, i, i+1; kParity = 1: the side neighbour of
 // site k is other[i][k+1], else other[i][k-1]; `edge` is the 32-bit word holding the 17th byte.
 template <bool kHasNever, bool kSmallQ, bool kPow2, int kParity>
-__device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const uint4& up, const uint4& ct,
+__device__ __forceinline__ uint4 update_row(const PhiloxCtx& a, uint4 own, const uint4& up, const uint4& ct,
                                             const uint4& dn, uint32_t edge, uint32_t g0, uint32_t c1, uint32_t q,
                                             uint32_t geAdd, uint32_t dshift, uint32_t dmask, const uint32_t* stab,
                                             const uint32_t* snever, uint32_t slot) {
@@ -196,7 +196,7 @@ __device__ __forceinline__ uint4 update_row(const SweepArgs& a, uint4 own, const
 }
 
 template <int kColour, bool kHasNever, bool kSmallQ, bool kPow2, int kRows>
-__device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* stab, const uint32_t* snever, uint32_t q,
+__device__ __forceinline__ void march_rows(const SweepArgs& a, const PhiloxCtx& pc, const uint32_t* stab, const uint32_t* snever, uint32_t q,
                                            uint32_t slot, int b, int rb, int x) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
     const size_t half = (size_t)L * W;
@@ -236,7 +236,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
         const uint4 n1 = __ldg(more ? pOth : pOthLast);
         const uint4 own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
-        uint4 res = update_row<kHasNever, kSmallQ, kPow2, kColour>(a, own, wU, wC, wD, edge, g0, c1, q, geAdd, dshift, dmask, stab, snever, slot);
+        uint4 res = update_row<kHasNever, kSmallQ, kPow2, kColour>(pc, own, wU, wC, wD, edge, g0, c1, q, geAdd, dshift, dmask, stab, snever, slot);
         *pOwn = res;
         uint4 n2 = n1, own2 = own1;
         uint32_t edge2 = edge1;
@@ -245,7 +245,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
             own2 = *(pOwn + 2 * rowStride);
             edge2 = __ldg(pEdgeEven + edgeStride2);
         }
-        res = update_row<kHasNever, kSmallQ, kPow2, 1 - kColour>(a, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd,
+        res = update_row<kHasNever, kSmallQ, kPow2, 1 - kColour>(pc, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd,
                                                                  dshift, dmask, stab, snever, slot);
         *(pOwn + rowStride) = res;
         wU = wD;
@@ -262,7 +262,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const uint32_t* s
 }
 
 // One block covers blockDim.x consecutive strips-times-row-blocks of one replica; bpr = blocks per replica.
-template <int kColour, int kRows>
+template <int kColour, int kRows, bool kDevT>
 __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) potts_int8_rows_kernel(SweepArgs a, int bpr) {
     __shared__ uint32_t stab[16 + 64];            // U[dn + 4] in [0..8]; from word 16: 256-byte pattern -> 4 * class table
     __shared__ uint32_t snever[1];
@@ -271,6 +271,9 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) potts_int8_rows_kern
     const int b = blockIdx.x / bpr;
     const int blk = blockIdx.x - b * bpr;
     pdl_wait();
+    uint32_t c2, c3;
+    sweep_counter_words<kDevT>(a, c2, c3);
+    const PhiloxCtx pc = {a.rk, c2, c3};
     const uint32_t* tab = a.tables + (size_t)b * kTableStride;
     const uint32_t never = tab[kTabNever];
     for (int m = threadIdx.x; m < 16; m += blockDim.x) stab[m] = tab[m];
@@ -288,15 +291,23 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) potts_int8_rows_kern
     if (u >= (a.L / kRows) * W16) return;                  // ragged last block of a replica (after the barrier)
     const int rb = u / W16, x = u - rb * W16;
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
-    if (never) march_rows<kColour, true, false, false, kRows>(a, stab, snever, q, slot, b, rb, x);
-    else if (q <= 16u && ((q - 1u) & (q - 2u)) == 0u) march_rows<kColour, false, true, true, kRows>(a, stab, snever, q, slot, b, rb, x);
-    else if (q <= 16u) march_rows<kColour, false, true, false, kRows>(a, stab, snever, q, slot, b, rb, x);   // shift-free indicators
-    else march_rows<kColour, false, false, false, kRows>(a, stab, snever, q, slot, b, rb, x);
+    if (never) march_rows<kColour, true, false, false, kRows>(a, pc, stab, snever, q, slot, b, rb, x);
+    else if (q <= 16u && ((q - 1u) & (q - 2u)) == 0u) march_rows<kColour, false, true, true, kRows>(a, pc, stab, snever, q, slot, b, rb, x);
+    else if (q <= 16u) march_rows<kColour, false, true, false, kRows>(a, pc, stab, snever, q, slot, b, rb, x);   // shift-free indicators
+    else march_rows<kColour, false, false, false, kRows>(a, pc, stab, snever, q, slot, b, rb, x);
 }
 
 }  // namespace
 
 const char* potts_int8_variant(int L) { return (L % 32 == 0) ? "potts_int8_rows128" : "potts_int8_generic"; }
+
+// The instantiation for (rows per thread, colour); kDevT: sweep index from device memory (graph nodes).
+template <bool kDevT>
+static void (*pick_potts_kernel(int rows, int colour))(SweepArgs, int) {
+    if (rows == kRowsShort) return colour == 0 ? potts_int8_rows_kernel<0, kRowsShort, kDevT> : potts_int8_rows_kernel<1, kRowsShort, kDevT>;
+    if (rows == kRowsMid) return colour == 0 ? potts_int8_rows_kernel<0, kRowsMid, kDevT> : potts_int8_rows_kernel<1, kRowsMid, kDevT>;
+    return colour == 0 ? potts_int8_rows_kernel<0, kRowsLong, kDevT> : potts_int8_rows_kernel<1, kRowsLong, kDevT>;
+}
 
 int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
     if (a.L % 32 == 0) {
@@ -311,10 +322,7 @@ int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
         const unsigned grid = (unsigned)((long long)bpr * a.batch);
         SweepArgs args = a;
         args.pdl_trigger = plan.trigger;
-        void (*k)(SweepArgs, int);
-        if (plan.rows == kRowsShort) k = a.colour == 0 ? potts_int8_rows_kernel<0, kRowsShort> : potts_int8_rows_kernel<1, kRowsShort>;
-        else if (plan.rows == kRowsMid) k = a.colour == 0 ? potts_int8_rows_kernel<0, kRowsMid> : potts_int8_rows_kernel<1, kRowsMid>;
-        else k = a.colour == 0 ? potts_int8_rows_kernel<0, kRowsLong> : potts_int8_rows_kernel<1, kRowsLong>;
+        void (*k)(SweepArgs, int) = a.t_dev ? pick_potts_kernel<true>(plan.rows, a.colour) : pick_potts_kernel<false>(plan.rows, a.colour);
         launch_pdl(k, grid, (unsigned)tpb, s, args, bpr);
     } else {
         const long long half = (long long)a.L * (a.L >> 1);

@@ -136,6 +136,13 @@ struct spin_sim {
     // second stream for the replica groups of a streaming sweep (streaming_begin / streaming_end), created on first use
     cudaStream_t aux_stream = nullptr;
     cudaEvent_t ev_fork = nullptr, ev_join = nullptr;
+    // CUDA graph of kGraphSweeps streaming sweeps whose nodes read the sweep index from d_graph_t (sweep_graph below)
+    cudaGraphExec_t graph_exec = nullptr;
+    unsigned long long* d_graph_t = nullptr;
+    const unsigned long long* capture_t = nullptr;   // non-NULL only while the graph is being captured
+    int graph_launches = 0;                          // kernels per replay
+    const uint32_t* graph_bonds = nullptr;           // SweepArgs::bonds the graph was captured with
+    bool graph_failed = false;
     int32_t policy = SPIN_POLICY_AUTO;
 };
 
@@ -284,6 +291,8 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     a.rk = sim->rk;
     a.pdl_trigger = kPdlAtExit;
     a.plan_scale = 1;
+    a.t_dev = sim->capture_t;
+    a.t_rel = sim->capture_t ? (uint32_t)t : 0u;
     return a;
 }
 
@@ -303,7 +312,8 @@ bool prefer_tiled(const spin_sim* sim) {
 bool use_resident(const spin_sim* sim, bool measure) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || !ising_int8_resident_fits(sim->L)) return false;
     if (sim->general || sim->d_bond_nat) return false;            // per-bond couplings run on the general kernels
-    if (sim->policy == SPIN_POLICY_STREAMING || sim->policy == SPIN_POLICY_PERSISTENT || sim->policy == SPIN_POLICY_TILED) return false;
+    if (sim->policy == SPIN_POLICY_STREAMING || sim->policy == SPIN_POLICY_PERSISTENT || sim->policy == SPIN_POLICY_TILED ||
+        sim->policy == SPIN_POLICY_GRAPH) return false;
     if (sim->policy == SPIN_POLICY_RESIDENT) return true;
     // Measured on B200 (profiles/r2_policy_grid.md): one CTA per replica wins for every batch size while a half-sweep of
     // a replica is a handful of warps (L <= 128: 3.1 vs 0.9 flips/ns at 1 x 64^2, 767 vs 500 at 256 x 128^2); for larger
@@ -444,7 +454,7 @@ void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour, const uint32_t* ta
 // (bit-packed), 0.2 (Potts), 0.3 (int8) waves of 8-row blocks upwards.  Class-table models only (the general kernels index natural-order coupling arrays).
 int streaming_groups(const spin_sim* sim) {
     if (sim->batch < 2 || sim->general || sim->d_bond_nat || sim->potts_general) return 1;
-    if (sim->policy != SPIN_POLICY_AUTO && sim->policy != SPIN_POLICY_STREAMING) return 1;
+    if (sim->policy != SPIN_POLICY_AUTO && sim->policy != SPIN_POLICY_STREAMING && sim->policy != SPIN_POLICY_GRAPH) return 1;
     const bool bits = sim->layout == SPIN_LAYOUT_BITPACKED;
     if (sim->L % (bits ? 64 : 32) != 0) return 1;                // the generic kernels are not planned
     const int perSm = sim->model == SPIN_MODEL_POTTS ? kPottsBlocksPerSm : bits ? kIsingBitsBlocksPerSm : kIsingInt8BlocksPerSm;
@@ -464,7 +474,9 @@ int streaming_begin(spin_sim* sim) {
             cudaEventCreateWithFlags(&sim->ev_join, cudaEventDisableTiming) != cudaSuccess) {
             cudaGetLastError();
             if (sim->aux_stream) cudaStreamDestroy(sim->aux_stream);
-            if (sim->ev_fork) cudaEventDestroy(sim->ev_fork);
+            if (sim->graph_exec) cudaGraphExecDestroy(sim->graph_exec);
+    if (sim->d_graph_t) cudaFree(sim->d_graph_t);
+    if (sim->ev_fork) cudaEventDestroy(sim->ev_fork);
             sim->aux_stream = nullptr; sim->ev_fork = nullptr; sim->ev_join = nullptr;
             return 1;
         }
@@ -510,6 +522,87 @@ void enqueue_streaming(spin_sim* sim, int G, int64_t t0, int64_t n_sweeps, const
                 else if (sim->layout == SPIN_LAYOUT_BITPACKED) sim->launches += launch_ising_bits_half_sweep(a, st);
                 else sim->launches += launch_ising_int8_half_sweep(a, st);
             }
+}
+
+// ---- streaming sweeps replayed from a CUDA graph (SPIN_POLICY_GRAPH) ----------------------------------------------------
+// A chain of half-sweep launches costs the host 2-4 us per launch (about half of what the GPU needs per launch on the
+// paper's mid-size shapes), so a busy or jittery host thread shows up in the sweep rate.  Under this policy a graph of
+// kGraphSweeps sweeps is captured once per handle from the very launchers of the streaming path (same kernels, same launch
+// plan, same replica groups; the capture keeps the programmatic edges); its kernels take the sweep index from device memory
+// (SweepArgs::t_dev + t_rel, the kDevT instantiations) and a last node advances it, so a replay needs no parameter update:
+// one cudaGraphLaunch per 64 sweeps.  Measured (profiles/r2_pdl_placement.md): host time per 240 sweeps 1.2-3.2 ms ->
+// 0.03 ms; GPU rate 1-5 % below the stream launches (1 x 2560^2 695 vs 720 flips/ns, 64 x 1024^2 1282 vs 1284): replaying
+// is not faster on the GPU than programmatic dependent launches, it only takes the host out of the loop.
+constexpr int kGraphSweeps = 64;
+
+__global__ void graph_set_t_kernel(unsigned long long* t, unsigned long long v) { *t = v; }
+__global__ void graph_advance_t_kernel(unsigned long long* t, unsigned long long k) { *t += k; }
+
+// Class-table models on the row-marching kernels (the only ones with kDevT instantiations).
+bool use_graph(const spin_sim* sim) {
+    if (sim->policy != SPIN_POLICY_GRAPH || sim->graph_failed) return false;
+    if (sim->stream == nullptr || sim->stream == cudaStreamLegacy) return false;   // the legacy default stream cannot be captured
+    if (sim->general || sim->d_bond_nat || sim->potts_general) return false;
+    return sim->L % (sim->layout == SPIN_LAYOUT_BITPACKED ? 64 : 32) == 0;
+}
+
+// Returns 1 if all n_sweeps sweeps were enqueued, 0 if the caller should use the stream path (nothing enqueued), -1 on a
+// CUDA error after part of the work was enqueued.
+int enqueue_graph_sweeps(spin_sim* sim, int64_t t0, int64_t n_sweeps) {
+    if (!use_graph(sim) || n_sweeps < kGraphSweeps) return 0;
+    if (sim->graph_exec && sim->graph_bonds != sim->d_bonds) {      // spin_set_bonds since the capture
+        cudaGraphExecDestroy(sim->graph_exec);
+        sim->graph_exec = nullptr;
+    }
+    if (!sim->graph_exec) {
+        if (!sim->d_graph_t && cudaMalloc(&sim->d_graph_t, sizeof(unsigned long long)) != cudaSuccess) {
+            cudaGetLastError();
+            sim->d_graph_t = nullptr;
+            sim->graph_failed = true;
+            return 0;
+        }
+        const int probe = streaming_begin(sim);                     // creates the second stream and the events outside the capture
+        streaming_end(sim, probe);
+        const int64_t l0 = sim->launches;
+        cudaGraph_t graph = nullptr;
+        if (cudaStreamBeginCapture(sim->stream, cudaStreamCaptureModeThreadLocal) != cudaSuccess) {
+            cudaGetLastError();
+            sim->graph_failed = true;
+            return 0;
+        }
+        sim->capture_t = sim->d_graph_t;
+        const int G = streaming_begin(sim);
+        enqueue_streaming(sim, G, 0, kGraphSweeps);
+        streaming_end(sim, G);
+        sim->capture_t = nullptr;
+        graph_advance_t_kernel<<<1, 1, 0, sim->stream>>>(sim->d_graph_t, (unsigned long long)kGraphSweeps);
+        const cudaError_t e1 = cudaStreamEndCapture(sim->stream, &graph);
+        sim->graph_launches = (int)(sim->launches - l0) + 1;
+        sim->launches = l0;                                          // nothing ran yet: replays are counted below
+        cudaError_t e2 = cudaErrorUnknown;
+        if (e1 == cudaSuccess && graph) e2 = cudaGraphInstantiate(&sim->graph_exec, graph, 0);
+        if (graph) cudaGraphDestroy(graph);
+        if (e1 != cudaSuccess || e2 != cudaSuccess) {
+            cudaGetLastError();
+            sim->graph_exec = nullptr;
+            sim->graph_failed = true;                                // this handle streams from now on
+            return 0;
+        }
+        sim->graph_bonds = sim->d_bonds;
+    }
+    graph_set_t_kernel<<<1, 1, 0, sim->stream>>>(sim->d_graph_t, (unsigned long long)t0);
+    sim->launches += 1;
+    int64_t done = 0;
+    for (; done + kGraphSweeps <= n_sweeps; done += kGraphSweeps) {
+        if (cudaGraphLaunch(sim->graph_exec, sim->stream) != cudaSuccess) return -1;
+        sim->launches += sim->graph_launches;
+    }
+    if (done < n_sweeps) {                                           // the ragged rest as plain launches
+        const int G = streaming_begin(sim);
+        enqueue_streaming(sim, G, t0 + done, n_sweeps - done);
+        streaming_end(sim, G);
+    }
+    return 1;
 }
 
 // Enqueue the reductions of the current lattice into E_out[b], M_out[b] (device int64, either may be NULL).
@@ -996,7 +1089,7 @@ int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_t n_steps
 int spin_set_policy(spin_sim* sim, int32_t policy) {
     if (!sim) return fail(SPIN_ERR_INVALID, "spin_set_policy: NULL handle");
     if (policy != SPIN_POLICY_AUTO && policy != SPIN_POLICY_STREAMING && policy != SPIN_POLICY_RESIDENT &&
-        policy != SPIN_POLICY_PERSISTENT && policy != SPIN_POLICY_TILED)
+        policy != SPIN_POLICY_PERSISTENT && policy != SPIN_POLICY_TILED && policy != SPIN_POLICY_GRAPH)
         return fail(SPIN_ERR_INVALID, "spin_set_policy: unknown policy %d", (int)policy);
     sim->policy = policy;
     return SPIN_OK;
@@ -1014,9 +1107,13 @@ int spin_sweep(spin_sim* sim, const double* beta, double J, double h, int64_t n_
     } else if (use_bits_resident(sim) && enqueue_bits_resident(sim, sweep_offset, n_sweeps)) {
     } else if (use_tiled(sim) && enqueue_tiled(sim, sweep_offset, n_sweeps)) {
     } else if (!(use_persistent(sim) && enqueue_persistent(sim, sweep_offset, n_sweeps))) {
-        const int G = streaming_begin(sim);
-        enqueue_streaming(sim, G, sweep_offset, n_sweeps);
-        streaming_end(sim, G);
+        const int rg = enqueue_graph_sweeps(sim, sweep_offset, n_sweeps);
+        if (rg < 0) return fail(SPIN_ERR_CUDA, "spin_sweep: cudaGraphLaunch failed: %s", cudaGetErrorString(cudaGetLastError()));
+        if (rg == 0) {
+            const int G = streaming_begin(sim);
+            enqueue_streaming(sim, G, sweep_offset, n_sweeps);
+            streaming_end(sim, G);
+        }
     }
     CUDA_TRY(cudaGetLastError());
     return SPIN_OK;

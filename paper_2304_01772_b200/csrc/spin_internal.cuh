@@ -63,6 +63,8 @@ struct SweepArgs {
                               // centre, side of the colour's sites), or nullptr for uniform couplings
     RoundKeys rk;
     int32_t pdl_trigger;      // PdlTrigger: where the row-marching kernels release the next launch (set by the launchers)
+    const unsigned long long* t_dev;   // non-NULL: the launch is a node of a CUDA graph (spin_api.cu, sweep_graph) and its sweep
+    uint32_t t_rel;                    // index is *t_dev + t_rel, read after pdl_wait(); c2 / c3 then hold colour and domain only
     int32_t plan_scale;       // the launch is one of plan_scale concurrent ones (replica groups on their own streams,
                               // spin_api.cu): the launch plan is made for the whole batch
 };
@@ -127,6 +129,24 @@ enum PdlTrigger : int32_t {
 };
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// What the inner update functions need for a Philox call besides the group and the replica.
+struct PhiloxCtx {
+    const RoundKeys& rk;
+    uint32_t c2, c3;
+};
+
+// Counter words 2 and 3 of a launch: from the arguments, or (kDevT, graph nodes) from the sweep index in device memory.
+template <bool kDevT>
+__device__ __forceinline__ void sweep_counter_words(const SweepArgs& a, uint32_t& c2, uint32_t& c3) {
+    c2 = a.c2;
+    c3 = a.c3;
+    if (kDevT) {
+        const unsigned long long t = *(const volatile unsigned long long*)a.t_dev + a.t_rel;
+        c2 = (uint32_t)(t & 0xFFFFFFFFull);
+        c3 = (a.c3 & 0xFF000000u) | (uint32_t)((t >> 32) & 0xFFFFFFull);
+    }
+}
 
 template <typename... KArgs, typename... Args>
 inline cudaError_t launch_pdl(void (*kernel)(KArgs...), unsigned grid, unsigned block, cudaStream_t s, Args... args) {

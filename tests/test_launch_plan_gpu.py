@@ -141,3 +141,87 @@ def test_two_replica_groups_sweep_schedule_and_later_calls(oracle_mod, model, ba
         Eo, Mo = oracle_mod.sweep(ref, beta, 1.0, h, seed=seed, n_sweeps=2, sweep_offset=8, q=q, trace=True)
         assert np.array_equal(Et, Eo) and np.array_equal(Mt, Mo)
         assert np.array_equal(sim.spin_get_spins(), ref)
+
+
+# ----------------------------------------------------------------- SPIN_POLICY_GRAPH: sweeps replayed from a CUDA graph
+def _oracle_sweep_threads(oracle_mod, ref, beta, h, seed, n, t0, q):
+    """oracle.sweep replica by replica on host threads (replica_offset = b): same lattices, a fraction of the wall time."""
+    from concurrent.futures import ThreadPoolExecutor
+
+    def one(b):
+        oracle_mod.sweep(ref[b:b + 1], beta[b:b + 1], 1.0, h, seed=seed, n_sweeps=n, sweep_offset=t0,
+                         q=None if q is None else q[b:b + 1], replica_offset=b)
+    with ThreadPoolExecutor(16) as ex:
+        list(ex.map(one, range(ref.shape[0])))
+
+
+@pytest.mark.parametrize("model,batch,L,layout,calls", [
+    ("ising", 3, 96, "int8", (64 * 2 + 5, 64, 7)), ("ising", 2, 128, "bits", (64 * 2 + 5, 64, 7)),
+    ("potts", 2, 64, "int8", (64 * 2 + 5, 64, 7)),
+    ("ising", 13, 1024, "int8", (67, 64)), ("ising", 12, 1024, "bits", (67, 64)), ("potts", 27, 512, "int8", (67, 64))])
+def test_graph_policy_equals_oracle(oracle_mod, model, batch, L, layout, calls):
+    """The kernels of a graph read the sweep index from device memory: replays of 64 sweeps, the ragged rest as plain
+    launches, a later call that replays the same graph, a sweep index that crosses 2^32 inside a replay, one and two
+    replica groups, never-accepted classes; short calls stream."""
+    import torch
+    seed = 700 + batch + L
+    q = None if model == "ising" else np.array([3 + (b % 6) for b in range(batch)], dtype=np.int32)
+    h = 0.02 if model == "ising" else 0.0
+    beta = np.linspace(0.4, 1.1, batch)
+    beta[-1] = 22.0
+    ref = oracle_mod.init(batch, L, seed=seed, q=q)
+    lay = sp.SPIN_LAYOUT_BITPACKED if layout == "bits" else sp.SPIN_LAYOUT_INT8
+    mdl = sp.SPIN_MODEL_ISING if model == "ising" else sp.SPIN_MODEL_POTTS
+    groups = _plan("potts" if model == "potts" else layout, batch, L)[1]
+    assert groups == (2 if L >= 512 else 1)
+    stream = torch.cuda.Stream()                              # the legacy default stream cannot be captured
+    with sp.spin_create_ex(batch, L, mdl, q_per_replica=q, seed=seed, layout=lay, cuda_stream=stream.cuda_stream) as sim:
+        sim.spin_set_policy(sp.SPIN_POLICY_GRAPH)
+        t0 = (1 << 32) - 70
+        for n in calls:
+            l0 = sim.spin_kernel_launches()
+            sim.spin_sweep(beta, 1.0, h, n, t0)
+            replays = n // 64
+            # per replay: 64 sweeps x 2 colours x groups + the node that advances the index; + 1 kernel that sets it per call
+            want = replays * (64 * 2 * groups + 1) + (1 if replays else 0) + (n % 64) * 2 * groups
+            assert sim.spin_kernel_launches() - l0 == want
+            _oracle_sweep_threads(oracle_mod, ref, beta, h, seed, n, t0, q)
+            assert np.array_equal(sim.spin_get_spins(), ref), n
+            t0 += n
+        E, M = sim.spin_observables()
+        Eo, Mo = oracle_mod.ising_observables(ref) if model == "ising" else oracle_mod.potts_observables(ref, q)
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo)
+    # on the legacy default stream the policy falls back to plain launches
+    with sp.spin_create_ex(batch, L, mdl, q_per_replica=q, seed=seed, layout=lay) as sim:
+        sim.spin_set_policy(sp.SPIN_POLICY_GRAPH)
+        l0 = sim.spin_kernel_launches()
+        sim.spin_sweep(beta, 1.0, h, 64, 0)
+        assert sim.spin_kernel_launches() - l0 == 64 * 2 * groups
+
+
+def test_graph_policy_with_bonds_rebuilds_the_graph(oracle_mod):
+    """+-J couplings on the bit-packed layout: the graph holds the pointer to the sign planes and is captured again after
+    spin_set_bonds replaced or removed them."""
+    import torch
+    batch, L, seed = 2, 256, 77
+    rng = np.random.default_rng(seed)
+    mk = lambda: (2 * rng.integers(0, 2, size=(batch, L, L)) - 1).astype(np.int8)
+    beta = np.linspace(0.5, 1.5, batch)
+    ref = oracle_mod.init(batch, L, seed=seed)
+    stream = torch.cuda.Stream()
+    with sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed, layout=sp.SPIN_LAYOUT_BITPACKED,
+                           cuda_stream=stream.cuda_stream) as sim:
+        sim.spin_set_policy(sp.SPIN_POLICY_GRAPH)
+        t = 0
+        for bonds in (None, (mk(), mk()), (mk(), mk()), None):
+            l0 = sim.spin_kernel_launches()
+            if bonds is None:
+                sim.spin_set_bonds(None, None)
+                sim.spin_sweep(beta, 1.0, 0.0, 66, t)
+                oracle_mod.sweep(ref, beta, 1.0, 0.0, seed=seed, n_sweeps=66, sweep_offset=t)
+            else:
+                sim.spin_set_bonds(bonds[0], bonds[1])
+                sim.spin_sweep(beta, 1.0, 0.0, 66, t)
+                oracle_mod.sweep_bonds(ref, bonds[0], bonds[1], beta, 1.0, 0.0, seed=seed, n_sweeps=66, sweep_offset=t)
+            assert np.array_equal(sim.spin_get_spins(), ref)
+            t += 66
