@@ -124,7 +124,7 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t t, const 
 template <bool kHasNever, int kParity>
 __device__ __forceinline__ uint4 update_row(const RoundKeys& rk, uint32_t c2, uint32_t c3, uint4 own, const uint4& um,
                                             const uint4& cm, const uint4& dm, uint32_t edge, uint32_t g0, uint32_t c1,
-                                            const uint32_t* stab, uint32_t slot) {
+                                            const uint32_t* stab, uint32_t slot, uint4* tout = nullptr) {
     uint32_t s0, s1, s2, s3;
     if (kParity) {
         s0 = __byte_perm(cm.x, cm.y, 0x4321);
@@ -142,6 +142,7 @@ __device__ __forceinline__ uint4 update_row(const RoundKeys& rk, uint32_t c2, ui
     const uint32_t t1 = (um.y + cm.y + dm.y) + s1 + (own.y & kOwn);
     const uint32_t t2 = (um.z + cm.z + dm.z) + s2 + (own.z & kOwn);
     const uint32_t t3 = (um.w + cm.w + dm.w) + s3 + (own.w & kOwn);
+    if (tout) *tout = make_uint4(t0, t1, t2, t3);   // bytes 4 * nd + 32 * d (fused measurement)
     uint32_t r0[4], r1[4], r2[4], r3[4];
     philox4x32_10(rk, g0 + 0, c1, c2, c3, r0);
     philox4x32_10(rk, g0 + 1, c1, c2, c3, r1);
@@ -167,9 +168,32 @@ __device__ __forceinline__ uint4 mask4(const uint4& v) {
     return make_uint4(v.x & m, v.y & m, v.z & m, v.w & m);
 }
 
-template <int kColour, bool kHasNever, int kRows, bool kPersist = false>
+// Sums for the fused E / M reduction (kMeasure, colour-1 launches), kept as packed byte counters so that a row costs a few
+// full-rate logic / add instructions (IDP4A shares the pipe of the Philox multiplies, which is the kernel's bottleneck):
+//   cS  += 4 per -1 spin of the updated strip `res`            (bit 2 of a +-1 byte)
+//   cC  += the masked centre word (4 per -1 colour-0 spin: every colour-0 site is the centre word of exactly one strip)
+//   cB[j] += 4 nd of the sites of word j whose NEW spin is -1   (t & res & 0x1C: t = 4 nd + 32 d, res = 0xFF / 0x01)
+// A byte grows by at most 16 per row (cB) or 16 per row over the four words (cS, cC): no overflow for <= 8 rows.
+// With nS, nC, nB the byte sums: number of -1 colour-1 spins = nS / 4, of -1 colour-0 spins = nC / 4,
+// sum over colour-1 sites of 4 nd = 4 nC (every colour-0 site is a neighbour of four colour-1 sites), so
+//   sum s = N/2 - nS/2,   sum s * 4 nd = 4 nC - 2 nB,   E_int = -(4 sum s - (sum s * 4 nd) / 2),   M = N - (nS + nC) / 2.
+struct MeasureCounters {
+    uint32_t cS, cC;
+    uint4 cB;
+};
+__device__ __forceinline__ void measure_row(const uint4& res, const uint4& t, const uint4& cm, MeasureCounters& mc) {
+    const uint32_t m = 0x04040404u, k = 0x1C1C1C1Cu;
+    mc.cS += ((res.x & m) + (res.y & m)) + ((res.z & m) + (res.w & m));
+    mc.cC += (cm.x + cm.y) + (cm.z + cm.w);
+    mc.cB.x += t.x & res.x & k;
+    mc.cB.y += t.y & res.y & k;
+    mc.cB.z += t.z & res.z & k;
+    mc.cB.w += t.w & res.w & k;
+}
+
+template <int kColour, bool kHasNever, int kRows, bool kPersist = false, bool kMeasure = false>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, uint32_t c2, uint32_t c3, const uint32_t* stab, uint32_t slot,
-                                           int b, int rb, int x) {
+                                           int b, int rb, int x, MeasureCounters* mc = nullptr) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
     const size_t half = (size_t)L * W;
     const int i0 = rb * kRows;
@@ -198,7 +222,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, uint32_t c2, uint
     uint32_t edge = ld1<kPersist>(pEdgeEven) & 0x04040404u;
     uint32_t g0 = (uint32_t)i0 * (uint32_t)W4 + 4u * (uint32_t)x;
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
-    if (!kPersist) __syncthreads();   // the block's threshold table (filled by the caller) is first read below: the loads
+    if (!kPersist && !kMeasure) __syncthreads();   // the block's threshold table (filled by the caller) is first read below: the loads
                                       // above are already in flight while the block waits for it
     // Two rows per iteration (the side-neighbour parity alternates); the four iterations of an 8-row thread are
     // unrolled so that the register window rotates by renaming instead of moves (measured: +2.5 % over the rolled loop).
@@ -217,12 +241,15 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, uint32_t c2, uint
             own2 = ldown<kPersist>(pOwn + 2 * rowStride);
             edge2 = ld1<kPersist>(pEdgeEven + edgeStride2);
         }
-        uint4 res = update_row<kHasNever, kColour>(a.rk, c2, c3, own, wU, wC, wD, edge, g0, c1, stab, slot);
+        uint4 tw;
+        uint4 res = update_row<kHasNever, kColour>(a.rk, c2, c3, own, wU, wC, wD, edge, g0, c1, stab, slot, kMeasure ? &tw : nullptr);
         *pOwn = res;
+        if (kMeasure) measure_row(res, tw, wC, *mc);
         const uint4 n1m = mask4(n1);
         res = update_row<kHasNever, 1 - kColour>(a.rk, c2, c3, own1, wC, wD, n1m, edge1 & 0x04040404u,
-                                                 g0 + (uint32_t)W4, c1, stab, slot);
+                                                 g0 + (uint32_t)W4, c1, stab, slot, kMeasure ? &tw : nullptr);
         *(pOwn + rowStride) = res;
+        if (kMeasure) measure_row(res, tw, wD, *mc);
         wU = wD;
         wC = n1m;
         wD = mask4(n2);
@@ -258,6 +285,114 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_kern
     const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
     if (never) march_rows<kColour, true, kRows>(a, c2, c3, stab, slot, b, rb, x);
     else march_rows<kColour, false, kRows>(a, c2, c3, stab, slot, b, rb, x);
+}
+
+// Colour-1 half-sweep with the E / M reduction fused in (spin_sweep_measure on the streaming path): the same marching
+// code; every thread also sums measure_row() over its rows, the block adds its three sums to a.measure_acc[b][0..2]
+// (nS, nC, nB), and launch_ising_measure_finalize turns them into E and M once the launch is complete.
+template <int kRows>
+__global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_measure_kernel(SweepArgs a, int bpr) {
+    __shared__ uint32_t stab[kTableStride];
+    __shared__ uint32_t sidx[4 * kRowsThreads];
+    __shared__ int ssum[3 * (kRowsThreads / 32)];
+    if (a.pdl_trigger == kPdlAtStart) pdl_launch_dependents();
+    const int b = blockIdx.x / bpr;
+    const int blk = blockIdx.x - b * bpr;
+    pdl_wait();
+    const uint32_t never = a.tables[(size_t)b * kTableStride + kTabNever];   // block-uniform
+    for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
+    const int W16 = a.L >> 5;
+    const int u = blk * blockDim.x + threadIdx.x;
+    MeasureCounters mc = {0u, 0u, make_uint4(0u, 0u, 0u, 0u)};
+    __syncthreads();                       // the table; here and not inside march_rows: the spare threads of a ragged last
+                                           // block stay for the block sum, and a barrier may not sit in divergent code
+    if (u < (a.L / kRows) * W16) {
+        const int rb = u / W16, x = u - rb * W16;
+        const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
+        if (never) march_rows<1, true, kRows, false, true>(a, a.c2, a.c3, stab, slot, b, rb, x, &mc);
+        else march_rows<1, false, kRows, false, true>(a, a.c2, a.c3, stab, slot, b, rb, x, &mc);
+    }
+    // byte sums nS, nC, nB of the thread (unsigned bytes, one IDP4A per counter word)
+    int msum[3];
+    msum[0] = __dp4a(mc.cS, 0x01010101u, 0u);
+    msum[1] = __dp4a(mc.cC, 0x01010101u, 0u);
+    msum[2] = __dp4a(mc.cB.x, 0x01010101u, __dp4a(mc.cB.y, 0x01010101u, __dp4a(mc.cB.z, 0x01010101u, __dp4a(mc.cB.w, 0x01010101u, 0u))));
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        msum[0] += __shfl_xor_sync(0xFFFFFFFFu, msum[0], o);
+        msum[1] += __shfl_xor_sync(0xFFFFFFFFu, msum[1], o);
+        msum[2] += __shfl_xor_sync(0xFFFFFFFFu, msum[2], o);
+    }
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) { ssum[3 * w] = msum[0]; ssum[3 * w + 1] = msum[1]; ssum[3 * w + 2] = msum[2]; }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        long long t = 0;
+        for (int k = 0; k < (int)((blockDim.x + 31) >> 5); ++k) t += ssum[3 * k + threadIdx.x];
+        atomicAdd((unsigned long long*)a.measure_acc + 3 * (size_t)b + threadIdx.x, (unsigned long long)t);
+    }
+}
+
+// r[0..2] = the byte sums (nS, nC, nB) of one replica (measure_row) -> E_int, M; moments as accumulate_moments_kernel
+// (observe.cu); the sums are cleared.
+__device__ __forceinline__ void measure_finalize_replica(long long* r, long long sites, long long* E_out, long long* M_out,
+                                                         long long* m) {
+    const long long nS = r[0], nC = r[1], nB = r[2];
+    r[0] = 0; r[1] = 0; r[2] = 0;
+    const long long sum1 = sites / 2 - nS / 2;                  // sum of the colour-1 spins
+    const long long e = -(4 * sum1 - (4 * nC - 2 * nB) / 2);
+    const long long mag = sites - (nS + nC) / 2;
+    if (E_out) *E_out = e;
+    if (M_out) *M_out = mag;
+    if (m) {
+        const unsigned long long ae = e < 0 ? (unsigned long long)(-e) : (unsigned long long)e;
+        const unsigned long long lo = ae * ae, hi = __umul64hi(ae, ae);
+        const unsigned long long old_lo = (unsigned long long)m[2];
+        const unsigned long long new_lo = old_lo + lo;
+        m[0] += 1;
+        m[1] += e;
+        m[2] = (long long)new_lo;
+        m[3] = (long long)((unsigned long long)m[3] + hi + (new_lo < old_lo ? 1ull : 0ull));
+        m[4] += mag;
+        m[5] += mag < 0 ? -mag : mag;
+        m[6] += mag * mag;
+        m[7] += e * mag;
+    }
+}
+
+// After the last sweep of a measured call (the sweeps before it are finalised by the next sweep's colour-0 launch).
+__global__ void ising_measure_finalize_kernel(long long* acc, int batch, long long sites, long long* E_out, long long* M_out,
+                                              long long* moments) {
+    pdl_wait();
+    const int b = blockIdx.x * blockDim.x + threadIdx.x;
+    if (b >= batch) return;
+    measure_finalize_replica(acc + 3 * (size_t)b, sites, E_out ? E_out + b : nullptr, M_out ? M_out + b : nullptr,
+                             moments ? moments + 8 * (size_t)b : nullptr);
+}
+
+// Colour-0 half-sweep of a measured run: ising_int8_rows_kernel<0, kRows> plus the finalisation of the previous sweep's sums
+// by the first thread of every replica's first block (its colour-1 launch is complete once pdl_wait returns, and the next
+// colour-1 launch, which adds to the same sums, starts after this one).
+template <int kRows>
+__global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_rows_fin_kernel(SweepArgs a, int bpr) {
+    __shared__ uint32_t stab[kTableStride];
+    __shared__ uint32_t sidx[4 * kRowsThreads];
+    if (a.pdl_trigger == kPdlAtStart) pdl_launch_dependents();
+    const int b = blockIdx.x / bpr;
+    const int blk = blockIdx.x - b * bpr;
+    pdl_wait();
+    if (blk == 0 && threadIdx.x == 0 && a.fin_pending)
+        measure_finalize_replica(a.measure_acc + 3 * (size_t)b, (long long)a.L * a.L, a.fin_E ? a.fin_E + b : nullptr,
+                                 a.fin_M ? a.fin_M + b : nullptr, a.fin_mom ? a.fin_mom + 8 * (size_t)b : nullptr);
+    const uint32_t never = a.tables[(size_t)b * kTableStride + kTabNever];   // block-uniform
+    for (int k = threadIdx.x; k < kTableStride; k += blockDim.x) stab[k] = a.tables[(size_t)b * kTableStride + k];
+    const int W16 = a.L >> 5;
+    const int u = blk * blockDim.x + threadIdx.x;
+    if (u >= (a.L / kRows) * W16) return;
+    const int rb = u / W16, x = u - rb * W16;
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
+    if (never) march_rows<0, true, kRows>(a, a.c2, a.c3, stab, slot, b, rb, x);
+    else march_rows<0, false, kRows>(a, a.c2, a.c3, stab, slot, b, rb, x);
 }
 
 // ---- persistent kernel for launch-bound shapes (lattices too big for one CTA's shared memory, too small for a
@@ -668,7 +803,13 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
         SweepArgs args = a;
         args.pdl_trigger = plan.trigger;
         void (*k)(SweepArgs, int);
-        if (a.t_dev) {
+        if (a.measure_acc && a.colour == 1) {
+            k = plan.rows == kRowsShort ? ising_int8_rows_measure_kernel<kRowsShort>
+                : plan.rows == kRowsMid ? ising_int8_rows_measure_kernel<kRowsMid> : ising_int8_rows_measure_kernel<kRowsLong>;
+        } else if (a.measure_acc) {
+            k = plan.rows == kRowsShort ? ising_int8_rows_fin_kernel<kRowsShort>
+                : plan.rows == kRowsMid ? ising_int8_rows_fin_kernel<kRowsMid> : ising_int8_rows_fin_kernel<kRowsLong>;
+        } else if (a.t_dev) {
             if (plan.rows == kRowsShort) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsShort, true> : ising_int8_rows_kernel<1, kRowsShort, true>;
             else if (plan.rows == kRowsMid) k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsMid, true> : ising_int8_rows_kernel<1, kRowsMid, true>;
             else k = a.colour == 0 ? ising_int8_rows_kernel<0, kRowsLong, true> : ising_int8_rows_kernel<1, kRowsLong, true>;
@@ -687,6 +828,12 @@ int launch_ising_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
 }  // namespace spin
 
 namespace spin {
+
+int launch_ising_measure_finalize(long long* acc, int batch, long long sites, long long* E_out, long long* M_out,
+                                  long long* moments, cudaStream_t s) {
+    launch_pdl(ising_measure_finalize_kernel, (unsigned)((batch + 127) / 128), 128u, s, acc, batch, sites, E_out, M_out, moments);
+    return 1;
+}
 
 static size_t resident_smem_bytes(int L) {
     return (size_t)L * L + sizeof(uint32_t) * (kTableStride + 4 * kResThreads) + sizeof(int) * 32;

@@ -123,6 +123,7 @@ struct spin_sim {
     int8_t* d_stage = nullptr;       // natural-layout staging for spin_get_spins / spin_set_spins / spin_set_bonds (grow-only)
     size_t stage_bytes = 0;
     long long* d_mom = nullptr;      // [B][8] moments of spin_sweep_measure
+    long long* d_macc = nullptr;     // [B][3] sums of the fused E / M reduction (streaming spin_sweep_measure), lazily allocated
     long long* d_trace = nullptr;    // trace buffer of spin_sweep_measure (grow-only)
     size_t trace_bytes = 0;
     // scratch (host, pinned): two table buffers used alternately, each guarded by the event recorded after its upload,
@@ -291,6 +292,8 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     a.rk = sim->rk;
     a.pdl_trigger = kPdlAtExit;
     a.plan_scale = 1;
+    a.measure_acc = nullptr;
+    a.fin_E = nullptr; a.fin_M = nullptr; a.fin_mom = nullptr; a.fin_pending = 0;
     a.t_dev = sim->capture_t;
     a.t_rel = sim->capture_t ? (uint32_t)t : 0u;
     return a;
@@ -327,7 +330,9 @@ bool use_resident(const spin_sim* sim, bool measure) {
     while (perReplica % tpb) tpb >>= 1;
     if (sim->L > 256) return false;                                // one CTA per SM only: 256 x 416^2 runs 692 resident vs 1020 streaming
     if (tpb < 64 && sim->batch >= 148) return true;
-    return measure && sim->batch >= 296;                           // fused per-sweep reductions, >= 2 CTAs per SM
+    // (measured runs of larger replicas stream as well: the E / M reduction is fused into the colour-1 launch,
+    // 1024 x 256^2 with moments 1171 flips/ns against 1047 for this kernel)
+    return false;
 }
 
 // Bit-packed resident kernel (ising_bits.cu): uniform couplings, replica fits one CTA.  Measured:
@@ -522,6 +527,61 @@ void enqueue_streaming(spin_sim* sim, int G, int64_t t0, int64_t n_sweeps, const
                 else if (sim->layout == SPIN_LAYOUT_BITPACKED) sim->launches += launch_ising_bits_half_sweep(a, st);
                 else sim->launches += launch_ising_int8_half_sweep(a, st);
             }
+}
+
+// ---- streaming sweeps with the E / M reduction fused into the colour-1 launch (spin_sweep_measure) ----------------------
+// Uniform Ising model, int8 layout, L % 32 == 0: the colour-1 kernel variant adds three sums per replica into d_macc and a
+// thread per replica of the NEXT sweep's colour-0 launch (a finalisation kernel after the last sweep) turns them into E
+// and M, writes the trace sample and / or accumulates the moments, and clears the sums.  Two launches per sweep, as for
+// spin_sweep, instead of two launches, a memset, a reduction over the whole lattice and the moment kernel; the same replica
+// groups as spin_sweep.  (A finalisation kernel per sweep in the chain cost 10 us per sweep: it keeps the next colour-0
+// launch from being staged behind the colour-1 launch.)
+bool fused_measure_eligible(const spin_sim* sim) {
+    return sim->model == SPIN_MODEL_ISING && sim->layout == SPIN_LAYOUT_INT8 && sim->L % 32 == 0 && !sim->general && !sim->d_bond_nat;
+}
+
+// E_trace / M_trace: device [n_sweeps][B] or nullptr; d_mom: device [B][8] or nullptr.
+int enqueue_streaming_measure(spin_sim* sim, int64_t t0, int64_t n_sweeps, long long* E_trace, long long* M_trace, long long* d_mom) {
+    const size_t B = (size_t)sim->batch;
+    if (!sim->d_macc) {
+        const cudaError_t e = cudaMalloc(&sim->d_macc, sizeof(long long) * 3 * B);
+        if (e != cudaSuccess) { sim->d_macc = nullptr; return fail(SPIN_ERR_NOMEM, "cudaMalloc for the measurement sums: %s", cudaGetErrorString(e)); }
+    }
+    CUDA_TRY(cudaMemsetAsync(sim->d_macc, 0, sizeof(long long) * 3 * B, sim->stream));
+    const int G = streaming_begin(sim);
+    const size_t perReplica = sim->lattice_bytes / B;
+    const long long sites = (long long)sim->L * sim->L;
+    for (int64_t local = 0; local <= n_sweeps; ++local) {
+        // sweep `local` (none after the last); its colour-0 launch first finalises sweep local - 1
+        for (int colour = 0; colour < (local < n_sweeps ? 2 : 0); ++colour)
+            for (int g = 0; g < G; ++g) {
+                const int b0 = (int)((long long)sim->batch * g / G), b1 = (int)((long long)sim->batch * (g + 1) / G);
+                SweepArgs a = sweep_args(sim, t0 + local, colour);
+                a.lattice = (char*)sim->lattice + perReplica * (size_t)b0;
+                a.tables = sim->d_tables + (size_t)b0 * kTableStride;
+                a.batch = b1 - b0;
+                a.replica_offset = sim->replica_offset + (uint32_t)b0;
+                a.plan_scale = G;
+                a.measure_acc = sim->d_macc + 3 * (size_t)b0;
+                if (colour == 0 && local > 0) {
+                    a.fin_pending = 1;
+                    a.fin_E = E_trace ? E_trace + (size_t)(local - 1) * B + b0 : nullptr;
+                    a.fin_M = M_trace ? M_trace + (size_t)(local - 1) * B + b0 : nullptr;
+                    a.fin_mom = d_mom ? d_mom + 8 * (size_t)b0 : nullptr;
+                }
+                sim->launches += launch_ising_int8_half_sweep(a, g == 0 ? sim->stream : sim->aux_stream);
+            }
+        if (local == n_sweeps)
+            for (int g = 0; g < G; ++g) {
+                const int b0 = (int)((long long)sim->batch * g / G), b1 = (int)((long long)sim->batch * (g + 1) / G);
+                sim->launches += launch_ising_measure_finalize(sim->d_macc + 3 * (size_t)b0, b1 - b0, sites,
+                                                               E_trace ? E_trace + (size_t)(local - 1) * B + b0 : nullptr,
+                                                               M_trace ? M_trace + (size_t)(local - 1) * B + b0 : nullptr,
+                                                               d_mom ? d_mom + 8 * (size_t)b0 : nullptr, g == 0 ? sim->stream : sim->aux_stream);
+            }
+    }
+    streaming_end(sim, G);
+    return SPIN_OK;
 }
 
 // ---- streaming sweeps replayed from a CUDA graph (SPIN_POLICY_GRAPH) ----------------------------------------------------
@@ -730,6 +790,7 @@ void spin_destroy(spin_sim* sim) {
     if (sim->d_aux) cudaFree(sim->d_aux);
     if (sim->d_stage) cudaFree(sim->d_stage);
     if (sim->d_mom) cudaFree(sim->d_mom);
+    if (sim->d_macc) cudaFree(sim->d_macc);
     if (sim->d_trace) cudaFree(sim->d_trace);
     for (int k = 0; k < 2; ++k) {
         if (sim->h_tables[k]) cudaFreeHost(sim->h_tables[k]);
@@ -1209,6 +1270,10 @@ int spin_sweep_measure(spin_sim* sim, const double* beta, double J, double h, in
     if (resident) {
         enqueue_resident(sim, sweep_offset, n_sweeps, true, want_trace ? d_trace : nullptr,
                          want_trace ? d_trace + trace_elems : nullptr, d_mom);
+    } else if (fused_measure_eligible(sim)) {
+        const int rf = enqueue_streaming_measure(sim, sweep_offset, n_sweeps, want_trace ? d_trace : nullptr,
+                                                 want_trace ? d_trace + trace_elems : nullptr, d_mom);
+        if (rf != SPIN_OK) { cudaStreamSynchronize(sim->stream); return rf; }
     } else {
         for (int64_t local = 0; local < n_sweeps; ++local) {
             const int64_t t = sweep_offset + local;

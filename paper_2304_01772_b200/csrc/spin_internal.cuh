@@ -63,6 +63,15 @@ struct SweepArgs {
                               // centre, side of the colour's sites), or nullptr for uniform couplings
     RoundKeys rk;
     int32_t pdl_trigger;      // PdlTrigger: where the row-marching kernels release the next launch (set by the launchers)
+    long long* measure_acc;   // non-NULL (int8 Ising rows kernel, colour 1): [batch][3] sums the launch adds into for the fused
+                              // E / M reduction (ising_int8.cu, kMeasure); indexed by the launch's own replica index
+    // colour-0 launches of a measured run (fin_pending != 0): before its own work, one thread per replica turns the sums the
+    // previous sweep's colour-1 launch left in measure_acc into E / M (fin_E / fin_M: that sweep's trace sample, device
+    // [batch] or NULL; fin_mom: device [batch][8] or NULL) and clears them - no separate launch in the chain
+    long long* fin_E;
+    long long* fin_M;
+    long long* fin_mom;
+    int32_t fin_pending;
     const unsigned long long* t_dev;   // non-NULL: the launch is a node of a CUDA graph (spin_api.cu, sweep_graph) and its sweep
     uint32_t t_rel;                    // index is *t_dev + t_rel, read after pdl_wait(); c2 / c3 then hold colour and domain only
     int32_t plan_scale;       // the launch is one of plan_scale concurrent ones (replica groups on their own streams,
@@ -243,6 +252,10 @@ int launch_potts_int8_observe(const void* lattice, int batch, int L, const int32
 // M_out[b] = max_k hist[b][k], then hist is cleared for the next use.
 int launch_potts_finalize(unsigned int* hist, const int32_t* q, int batch, long long* M_out, cudaStream_t s);
 // moments[b][8] += sample (E[b], M[b])
+// Fused E / M of the int8 Ising streaming path: turns the sums the colour-1 launch left in acc[batch][3] into E, M (written
+// to E_out / M_out if non-NULL), accumulates the moments (if non-NULL) and clears acc.  sites = L * L.
+int launch_ising_measure_finalize(long long* acc, int batch, long long sites, long long* E_out, long long* M_out,
+                                  long long* moments, cudaStream_t s);
 int launch_accumulate_moments(long long* moments, const long long* E, const long long* M, int batch, cudaStream_t s);
 
 // Natural <-> internal layout.  natural: [B][L][L] int8 on the device.

@@ -225,3 +225,35 @@ def test_graph_policy_with_bonds_rebuilds_the_graph(oracle_mod):
                 oracle_mod.sweep_bonds(ref, bonds[0], bonds[1], beta, 1.0, 0.0, seed=seed, n_sweeps=66, sweep_offset=t)
             assert np.array_equal(sim.spin_get_spins(), ref)
             t += 66
+
+
+# ----------------------------------------------------------------- spin_sweep_measure on the streaming path (fused E / M)
+@pytest.mark.parametrize("batch,L", [(13, 1024), (40, 256), (3, 96)])
+def test_fused_measure_two_groups_traces_and_moments(oracle_mod, batch, L):
+    """The colour-1 launch adds the E / M sums, the next sweep's colour-0 launch (or the finalisation kernel after the last
+    sweep) turns them into the sample: traces and moments against the oracle, two replica groups, a replica with
+    never-accepted classes, a second call that continues, launch counts (no reduction launches any more)."""
+    seed, n = 800 + batch, 5
+    groups = _plan("int8", batch, L)[1]
+    beta = np.linspace(0.3, 0.6, batch)
+    beta[-1] = 20.0
+    ref = oracle_mod.init(batch, L, seed=seed)
+    mom_o = np.zeros((batch, 8), dtype=np.int64)
+    Eo, Mo = oracle_mod.sweep(ref, beta, 1.0, 0.03, seed=seed, n_sweeps=n, sweep_offset=4, trace=True, moments=mom_o)
+    with sp.spin_create_ex(batch, L, sp.SPIN_MODEL_ISING, seed=seed) as sim:
+        sim.spin_set_policy(sp.SPIN_POLICY_STREAMING)
+        mom = np.zeros((batch, 8), dtype=np.int64)
+        l0 = sim.spin_kernel_launches()
+        E1, M1 = sim.spin_sweep_measure(beta, 1.0, 0.03, 2, 4, moments=mom)
+        assert sim.spin_kernel_launches() - l0 == (2 * 2 + 1) * groups      # sweeps x colours + one finalisation, per group
+        E2, M2 = sim.spin_sweep_measure(beta, 1.0, 0.03, n - 2, 6, moments=mom)
+        assert np.array_equal(np.vstack([E1, E2]), Eo) and np.array_equal(np.vstack([M1, M2]), Mo)
+        assert np.array_equal(mom, mom_o)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        # moments only (no trace), then a plain sweep and the stand-alone reduction agree with the oracle
+        sim.spin_sweep_measure(beta, 1.0, 0.03, 2, 4 + n, trace=False, moments=mom)
+        oracle_mod.sweep(ref, beta, 1.0, 0.03, seed=seed, n_sweeps=2, sweep_offset=4 + n, moments=mom_o)
+        assert np.array_equal(mom, mom_o)
+        E, M = sim.spin_observables()
+        Eo2, Mo2 = oracle_mod.ising_observables(ref)
+        assert np.array_equal(E, Eo2) and np.array_equal(M, Mo2)
