@@ -467,10 +467,10 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) ising_int8_persisten
 template <bool kHasNever>
 __device__ __forceinline__ void tiled_half_sweep(const TiledArgs& a, int colour, uint32_t c2, uint32_t c3, uint32_t* own1,
                                                  const uint32_t* oth1, int SR, int SWX, int iBase, int kBase,
-                                                 const uint32_t* stab, uint32_t slot, uint32_t c1) {
+                                                 const uint32_t* stab, uint32_t slot, uint32_t c1, int rLo, int rHi) {
     const int L = a.L, W = L >> 1, W4 = W >> 2;
     const uint32_t m = 0x04040404u;
-    for (int task = threadIdx.x; task < SR * SWX; task += blockDim.x) {
+    for (int task = rLo * SWX + threadIdx.x; task < rHi * SWX; task += blockDim.x) {   // rows [rLo, rHi): see the kernel
         const int r = task / SWX, wx = task - r * SWX;
         int gi = iBase + r;                                    // iBase in [0, L): at most two wraps for regions <= 2 L
         gi = gi >= L ? gi - L : gi;
@@ -539,7 +539,7 @@ __global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledAr
     // the thread's own word (kOneWord)
     const int task = threadIdx.x;
     const bool mine = task < SR * SWX;
-    int oU = 0, oD = 0, oNext = 0, oPrev = 0;
+    int oU = 0, oD = 0, oNext = 0, oPrev = 0, dr = 0;          // dr: distance of the thread's row from the tile's interior rows
     uint32_t group = 0u, par0 = 0u;
     if (kOneWord && mine) {
         const int r = task / SWX, wx = task - r * SWX;
@@ -551,6 +551,7 @@ __global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledAr
         gk = gk >= W ? gk - W : gk;
         oU = (r == 0 ? 0 : r - 1) * SWX + wx;
         oD = (r == SR - 1 ? r : r + 1) * SWX + wx;
+        dr = r < a.HR ? a.HR - r : (r >= a.HR + a.TR ? r - (a.HR + a.TR - 1) : 0);
         oNext = r * SWX + (wx == SWX - 1 ? wx : wx + 1);
         oPrev = r * SWX + (wx == 0 ? 0 : wx - 1);
         group = (uint32_t)gi * (uint32_t)W4 + (uint32_t)(gk >> 2);
@@ -564,8 +565,11 @@ __global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledAr
             const uint32_t c3 = c3lo | ((uint32_t)colour << 24);
             uint32_t* own1 = colour ? reg1 : reg0;
             const uint32_t* oth1 = colour ? reg0 : reg1;
+            // a site can still reach the interior by the end of the launch only if it is within `reach` sites of it: rows
+            // farther out are not updated any more (their values are stale by then anyway)
+            const int reach = 2 * (a.sweeps - s) - 1 - colour;
             if (kOneWord) {
-                if (mine) {
+                if (mine && dr <= reach) {
                     const uint32_t m = 0x04040404u;
                     const bool par = ((par0 + (uint32_t)colour) & 1u) != 0u;   // side neighbour of site k: k+1 if par else k-1
                     const uint32_t um = oth1[oU] & m, cm = oth1[task] & m, dm = oth1[oD] & m;
@@ -577,8 +581,8 @@ __global__ void __launch_bounds__(kTiledThreads) ising_int8_tiled_kernel(TiledAr
                     const uint32_t tcls = um + cm + dm + sd + (own & 0x20202020u);
                     own1[task] = never ? update_word<true, 0>(own, tcls, rw, stab, slot) : update_word<false, 0>(own, tcls, rw, stab, slot);
                 }
-            } else if (never) tiled_half_sweep<true>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1);
-            else tiled_half_sweep<false>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1);
+            } else if (never) tiled_half_sweep<true>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1, max(0, a.HR - reach), min(SR, a.HR + a.TR + reach));
+            else tiled_half_sweep<false>(a, colour, c2, c3, own1, oth1, SR, SWX, iBase, kBase, stab, slot, c1, max(0, a.HR - reach), min(SR, a.HR + a.TR + reach));
             __syncthreads();
         }
     }
@@ -892,7 +896,9 @@ static bool tile_geometry(int batch, int L, TileGeom& g) {
     int perReplica = 148 / batch;                               // tiles allowed per replica
     if (perReplica < 1) perReplica = 1;
     for (int sweeps = 4; sweeps >= 2; sweeps -= 2) {
-        const int HR = 2 * sweeps, HK = 2 * sweeps < 4 ? 4 : (2 * sweeps + 3) / 4 * 4;
+        // staleness moves one SITE per half-sweep: 2 * sweeps rows, and 2 * sweeps actual columns = `sweeps` same-colour
+        // columns (k indexes every other column), rounded up to a whole 4-site word
+        const int HR = 2 * sweeps, HK = (sweeps + 3) / 4 * 4;
         long long bestWords = -1;
         for (int tilesK = 1; tilesK <= perReplica && tilesK <= (W + 15) / 16; ++tilesK) {
             const int TK = ((W + tilesK - 1) / tilesK + 3) / 4 * 4;

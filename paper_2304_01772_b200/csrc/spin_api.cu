@@ -299,14 +299,15 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     return a;
 }
 
-// Shapes AUTO sends to the temporally blocked tile kernel (ising_int8.cu) for plain sweeps: up to 16 replicas and 2^20
+// Shapes AUTO sends to the temporally blocked tile kernel (ising_int8.cu) for plain sweeps: up to 16 replicas and 2^21
 // sites in all, i.e. launches that leave the streaming kernels latency-bound and give one CTA per replica too few CTAs.
-// Measured (profiles/r2_policy_grid.md): 1 x 640^2 231 vs 88 flips/ns streaming, 16 x 128^2 178 vs 74 resident,
-// 16 x 256^2 257 vs 236, 1 x 1024^2 260 vs 224; beyond that it loses (4 x 640^2 302 vs 327, 64 x 128^2 253 vs 291).
+// Measured (profiles/r2_policy_grid.md): 1 x 640^2 271 vs 87 flips/ns streaming, 16 x 128^2 201 vs 73 resident,
+// 16 x 256^2 265 vs 235, 1 x 1024^2 265 vs 219, 4 x 640^2 351 vs 325; beyond that it loses (16 x 416^2 412 vs 407 is a
+// tie, 4 x 1024^2 470 vs 576, 64 x 128^2 269 vs 291 resident).
 bool prefer_tiled(const spin_sim* sim) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_INT8 || sim->general || sim->d_bond_nat) return false;
     if (sim->policy != SPIN_POLICY_AUTO) return false;
-    return sim->L >= 64 && sim->batch <= 16 && (long long)sim->batch * sim->L * sim->L <= (1ll << 20) &&
+    return sim->L >= 64 && sim->batch <= 16 && (long long)sim->batch * sim->L * sim->L <= (1ll << 21) &&
            ising_int8_tiled_fits(sim->batch, sim->L);
 }
 
@@ -318,31 +319,22 @@ bool use_resident(const spin_sim* sim, bool measure) {
     if (sim->policy == SPIN_POLICY_STREAMING || sim->policy == SPIN_POLICY_PERSISTENT || sim->policy == SPIN_POLICY_TILED ||
         sim->policy == SPIN_POLICY_GRAPH) return false;
     if (sim->policy == SPIN_POLICY_RESIDENT) return true;
-    // Measured on B200 (profiles/r2_policy_grid.md): one CTA per replica wins for every batch size while a half-sweep of
-    // a replica is a handful of warps (L <= 128: 3.1 vs 0.9 flips/ns at 1 x 64^2, 767 vs 500 at 256 x 128^2); for larger
-    // replicas a CTA needs tens of microseconds per sweep, so it only pays when the batch fills the GPU (>= 1 CTA per SM)
-    // AND the streaming kernel's blocks would be ragged (L = 160, 224: 766 vs 655 flips/ns at 256 x 224^2); small batches
-    // of large resident-eligible replicas (4 x 416^2: 23 vs 112 flips/ns) go to the tiled / streaming kernels.
+    // Measured on B200 (profiles/r2_policy_grid.md): one CTA per replica wins while a half-sweep of a replica is a handful
+    // of warps and there are many replicas (L <= 128: 503 vs 229 flips/ns at 256 x 64^2, 767 vs 579 at 256 x 128^2).
     if (!measure && prefer_tiled(sim)) return false;               // few small replicas: the tiled kernel spreads them over the SMs
-    if (sim->L <= 128) return true;
-    int tpb = 128;
-    const int perReplica = (sim->L / 8) * (sim->L / 32);
-    while (perReplica % tpb) tpb >>= 1;
-    if (sim->L > 256) return false;                                // one CTA per SM only: 256 x 416^2 runs 692 resident vs 1020 streaming
-    if (tpb < 64 && sim->batch >= 148) return true;
-    // (measured runs of larger replicas stream as well: the E / M reduction is fused into the colour-1 launch,
-    // 1024 x 256^2 with moments 1171 flips/ns against 1047 for this kernel)
-    return false;
+    // larger replicas stream: with the batch swept as two replica groups even the ragged L = 160 / 224 shapes are faster
+    // there (256 x 224^2: 930 vs 763 flips/ns), and measured runs have the reduction fused into the colour-1 launch
+    // (1024 x 256^2 with moments: 1171 vs 1047)
+    return sim->L <= 128;
 }
 
-// Bit-packed resident kernel (ising_bits.cu): uniform couplings, replica fits one CTA.  Measured:
-// 64 x 1024^2 406 vs 1123 flips/ns streaming (84 SMs idle), 148 x 1024^2 939 vs 1339, 296 x 512^2 1181 vs 1293,
-// 1024 x 256^2 1220 vs 1096: AUTO takes it only for many small replicas; SPIN_POLICY_RESIDENT forces it.
+// Bit-packed resident kernel (ising_bits.cu): uniform couplings, replica fits one CTA.  On request only
+// (SPIN_POLICY_RESIDENT): one CTA per replica idles SMs or loses to the two-group streaming path on every measured shape
+// (64 x 1024^2 406 vs 1266 flips/ns, 148 x 1024^2 939 vs 1339, 1024 x 256^2 1220 vs 1330).
 bool use_bits_resident(const spin_sim* sim) {
     if (sim->model != SPIN_MODEL_ISING || sim->layout != SPIN_LAYOUT_BITPACKED || sim->d_bonds) return false;
     if (!ising_bits_resident_fits(sim->L)) return false;
-    if (sim->policy == SPIN_POLICY_RESIDENT) return true;
-    return sim->policy == SPIN_POLICY_AUTO && sim->L <= 256 && sim->batch >= 592;
+    return sim->policy == SPIN_POLICY_RESIDENT;
 }
 
 bool enqueue_bits_resident(spin_sim* sim, int64_t t0, int64_t n_sweeps, const uint32_t* tables = nullptr) {

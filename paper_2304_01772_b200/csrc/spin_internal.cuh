@@ -105,7 +105,7 @@ struct TiledArgs {
     int32_t batch, L;
     uint32_t replica_offset;
     unsigned long long t0;    // first sweep index of this launch
-    int32_t sweeps;           // sweeps in this launch (2 * sweeps <= HR and <= HK)
+    int32_t sweeps;           // sweeps in this launch (2 * sweeps <= HR rows, sweeps <= HK same-colour columns)
     int32_t TR, TK, HR, HK;   // TK, HK multiples of 4 (k = same-colour column index)
     int32_t tilesR, tilesK;
     RoundKeys rk;

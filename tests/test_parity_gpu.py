@@ -344,9 +344,10 @@ def test_tiled_kernel_equals_oracle(oracle_mod, batch, L, n):
 @pytest.mark.parametrize("batch,L,variant", [(2, 256, "ising_int8_tiled"), (16, 128, "ising_int8_tiled"),
                                              (1, 1024, "ising_int8_tiled"), (16, 64, "ising_int8_tiled"),
                                              (17, 128, "ising_int8_resident"), (4, 32, "ising_int8_resident"),
-                                             (2, 1056, "ising_int8_rows128")])
+                                             (4, 640, "ising_int8_tiled"), (2, 1056, "ising_int8_rows128"),
+                                             (150, 224, "ising_int8_rows128")])
 def test_auto_policy_small_launches(oracle_mod, batch, L, variant):
-    """What SPIN_POLICY_AUTO picks around the tile kernel's corner (<= 16 replicas, <= 2^20 sites, L >= 64), each pick
+    """What SPIN_POLICY_AUTO picks around the tile kernel's corner (<= 16 replicas, <= 2^21 sites, L >= 64), each pick
     against the oracle; spin_sweep_measure on the same handle (never tiled) continues the same trajectory."""
     seed, n = 90 + L, 6
     beta = np.linspace(0.3, 0.6, batch)
