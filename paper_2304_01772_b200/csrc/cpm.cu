@@ -68,13 +68,17 @@ __device__ __forceinline__ int cpm_site(const int8_t* lat, int L, int i, int j, 
                                         const int32_t* areas, const P& p, const uint32_t* T, int dmax, bool beta_zero) {
     const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1, jl = j == 0 ? L - 1 : j - 1, jr = j == L - 1 ? 0 : j + 1;
     const int old = lat[(size_t)i * L + j];
+    // the proposed value first: most sites sit inside a cell or the medium, where it equals the old one and nothing else
+    // is needed.  Direction k of the Moore order (-1,-1) (-1,0) (-1,1) (0,-1) (0,1) (1,-1) (1,0) (1,1): cell k + (k >= 4)
+    // of the 3 x 3 block around the site.
+    const uint32_t dir = r_prop >> 29;
+    const int cell = (int)dir + (dir >= 4u ? 1 : 0);
+    const int cr = cell / 3, cc = cell - 3 * cr;
+    const int pi = cr == 0 ? iu : (cr == 1 ? i : id), pj = cc == 0 ? jl : (cc == 1 ? j : jr);
+    const int nw = lat[(size_t)pi * L + pj];
+    if (nw == old) return -1;
     const int nb[8] = {lat[(size_t)iu * L + jl], lat[(size_t)iu * L + j], lat[(size_t)iu * L + jr], lat[(size_t)i * L + jl],
                        lat[(size_t)i * L + jr], lat[(size_t)id * L + jl], lat[(size_t)id * L + j], lat[(size_t)id * L + jr]};
-    const uint32_t dir = r_prop >> 29;
-    int nw = nb[0];
-#pragma unroll
-    for (int k = 1; k < 8; ++k) nw = dir == (uint32_t)k ? nb[k] : nw;
-    if (nw == old) return -1;
     const int tn = p.tau[nw], to = p.tau[old];
     long long dH = 0;
 #pragma unroll
@@ -123,7 +127,7 @@ __global__ void __launch_bounds__(128) cpm_pass_kernel(CpmArgs a, CpmParams p) {
 // replica keeps the lattice and the area counters in shared memory and runs every sweep of the call in one launch.  The
 // areas are counted once; during a colour pass accepted copies add to a separate delta array, which is folded into the
 // areas after the pass - so every proposal of a pass still sees the counts of the start of that pass (reading C3).
-__global__ void __launch_bounds__(256) cpm_resident_kernel(CpmArgs a, CpmParams pp, unsigned long long t0, long long n_sweeps) {
+__global__ void __launch_bounds__(512) cpm_resident_kernel(CpmArgs a, CpmParams pp, unsigned long long t0, long long n_sweeps) {
     extern __shared__ __align__(16) int8_t slat[];
     __shared__ int32_t sarea[128], sdelta[128];
     __shared__ int8_t stau[128];
@@ -147,6 +151,7 @@ __global__ void __launch_bounds__(256) cpm_resident_kernel(CpmArgs a, CpmParams 
     }
     __syncthreads();
     const int per = W * W, groups = (per + 1) >> 1;
+    const int wshift = (W & (W - 1)) == 0 ? __ffs(W) - 1 : -1;
     const uint32_t* T = a.T + (size_t)b * (a.dmax + 1);
     const bool bz = a.beta_zero[b] != 0;
     for (long long s = 0; s < n_sweeps; ++s) {
@@ -161,7 +166,8 @@ __global__ void __launch_bounds__(256) cpm_resident_kernel(CpmArgs a, CpmParams 
                 for (int e = 0; e < 2; ++e) {
                     const int n = 2 * g + e;
                     if (n >= per) break;
-                    const int i = 2 * (n / W) + (colour >> 1), j = 2 * (n % W) + (colour & 1);
+                    const int row = wshift >= 0 ? n >> wshift : n / W, col = n - row * W;   // no division for L = 2^k
+                    const int i = 2 * row + (colour >> 1), j = 2 * col + (colour & 1);
                     const int nw = cpm_site(slat, L, i, j, r[2 * e], r[2 * e + 1], sarea, p, T, a.dmax, bz);
                     if (nw >= 0) {
                         const int old = slat[i * L + j];
@@ -300,8 +306,11 @@ int spin_cpm_sweep(int32_t batch, int32_t L, int32_t q, int8_t* lattice, const i
         const bool resident = N <= 65536 && (N & 3) == 0 && (L <= 128 || batch >= 148);
         if (resident) {
             a.colour = 0; a.c2 = 0; a.c3 = 0;
+            // one Philox group (two sites) per thread and colour pass where the lattice has that many (the passes are latency
+            // chains: 60 -> measured below with 512 threads for L = 64)
+            const unsigned res_threads = (L / 2) * (L / 2) / 2 >= 512 ? 512u : 256u;
             if (N > 32768) e = cudaFuncSetAttribute(cpm_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
-            if (e == cudaSuccess) cpm_resident_kernel<<<(unsigned)batch, 256, (size_t)N, s>>>(a, p, (unsigned long long)sweep_offset, (long long)n_sweeps);
+            if (e == cudaSuccess) cpm_resident_kernel<<<(unsigned)batch, res_threads, (size_t)N, s>>>(a, p, (unsigned long long)sweep_offset, (long long)n_sweeps);
         }
         for (int64_t t = sweep_offset; !resident && t < sweep_offset + n_sweeps && e == cudaSuccess; ++t)
             for (int c = 0; c < 4; ++c) {
