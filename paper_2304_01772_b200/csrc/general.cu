@@ -37,9 +37,10 @@ __device__ __forceinline__ GroupPos group_pos(const SweepArgs& a, int sites_per_
 
 // Natural coordinates of same-colour site n of colour c.
 __device__ __forceinline__ void site_coords(int L, int colour, long long n, int& i, int& j) {
-    const int W = L >> 1;
-    i = (int)(n / W);
-    const int k = (int)(n % W);
+    const uint32_t W = (uint32_t)L >> 1, un = (uint32_t)n;      // n < L * L / 2 <= 2^31: 32-bit arithmetic, no division for L = 2^k
+    const uint32_t row = (W & (W - 1u)) == 0u ? un >> (__ffs((int)W) - 1) : un / W;
+    const int k = (int)(un - row * W);
+    i = (int)row;
     j = 2 * k + ((i + colour) & 1);
 }
 
