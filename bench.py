@@ -483,7 +483,7 @@ def general_entries(runner, sp, args, peaks, measured):
     w = Workload("F2-potts-field", "potts", B, L, 9, np.full(B, 1.0), 1.0, 0.1, n, q=q)
     res = runner.run(w, "sweep", args.steps, args.warmup)
     d = summarise(w, res, peaks, measured)
-    d["kernel"] = "potts_int8_general_kernel"
+    d["kernel"] = "potts_int8_rows_field_kernel"
     out[w.name] = d
     res["sim"].spin_destroy()
     B, L, n_steps, per = 4, 1024, 50, 4

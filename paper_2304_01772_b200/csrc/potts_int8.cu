@@ -122,15 +122,27 @@ __device__ __forceinline__ void site_step(uint32_t& acc_mask, uint32_t o, uint32
     }
 }
 
+// One site with a field on the state label (kField): the threshold depends on the class AND on new - old.  ftab: the
+// replica's [9][255] entries (always << 32) | T (accept iff always or r < T: a threshold of 0 never accepts, so there is no
+// never-mask on this path); df = new - old + 127 of the site.
+template <int kE>
+__device__ __forceinline__ void site_step_field(uint32_t& acc_mask, uint32_t o, uint32_t df, uint32_t r, const uint32_t* stab,
+                                                const unsigned long long* ftab) {
+    const uint32_t c4 = ((const uint8_t*)(stab + 16))[o];             // 4 * (dn + 4)
+    const unsigned long long ent = __ldg(ftab + (c4 >> 2) * 255u + df);
+    if ((uint32_t)(ent >> 32) != 0u || r < (uint32_t)ent) acc_mask |= 0xFFu << (8 * kE);
+}
+
 // One 4-site word: r0 feeds sites 0, 1 (proposal words r0[0], r0[2]; acceptance words r0[1], r0[3]), r1 sites 2, 3.
 // kPow2: q - 1 is a power of two 2^k <= 8 (q = 2, 3, 5, 9): floor(r (q-1) / 2^32) is the top k bits of r, so the four
 // proposal offsets of a word come from the top bytes of the four words with three PRMT, a shift and a mask
 // (dshift = 8 - k, dmask = (2^k - 1) per byte) instead of four IMAD.HI (half-rate) and three merges.
-template <bool kHasNever, bool kSmallQ, bool kPow2, int kJ>
+template <bool kHasNever, bool kSmallQ, bool kPow2, int kJ, bool kField = false>
 __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint32_t dn, uint32_t ct, uint32_t sd,
                                                 const uint32_t r0[4], const uint32_t r1[4], uint32_t q, uint32_t geAdd,
                                                 uint32_t dshift, uint32_t dmask,
-                                                const uint32_t* stab, const uint32_t* snever, uint32_t slot) {
+                                                const uint32_t* stab, const uint32_t* snever, uint32_t slot,
+                                                const unsigned long long* ftab = nullptr) {
     // proposal (O6): new = old + 1 + floor(r_prop (q-1) / 2^32), minus q if >= q
     const uint32_t qm1 = q - 1u;
     uint32_t d;
@@ -152,6 +164,14 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
     const uint32_t o2 = slot_load_u8<kJ * kRowsThreads * 4 + 2>(slot);
     const uint32_t o3 = slot_load_u8<kJ * kRowsThreads * 4 + 3>(slot);
     uint32_t am = 0u;                                                 // 0xFF in the bytes whose proposal is accepted
+    if (kField) {
+        const uint32_t df = (nw + 0x7F7F7F7Fu) - own;                 // new - old + 127 per byte (states <= 126: no carries)
+        site_step_field<0>(am, o0, df & 0xFFu, r0[1], stab, ftab);
+        site_step_field<1>(am, o1, (df >> 8) & 0xFFu, r0[3], stab, ftab);
+        site_step_field<2>(am, o2, (df >> 16) & 0xFFu, r1[1], stab, ftab);
+        site_step_field<3>(am, o3, df >> 24, r1[3], stab, ftab);
+        return (own & ~am) | (nw & am);
+    }
     site_step<kHasNever, 0>(am, o0, r0[1], stab, snever);
     site_step<kHasNever, 1>(am, o1, r0[3], stab, snever);
     site_step<kHasNever, 2>(am, o2, r1[1], stab, snever);
@@ -161,11 +181,11 @@ __device__ __forceinline__ uint32_t update_word(uint32_t own, uint32_t up, uint3
 
 // One row of one strip.  up / ct / dn: other-colour words of rows i-1, i, i+1; kParity = 1: the side neighbour of
 // site k is other[i][k+1], else other[i][k-1]; `edge` is the 32-bit word holding the 17th byte.
-template <bool kHasNever, bool kSmallQ, bool kPow2, int kParity>
+template <bool kHasNever, bool kSmallQ, bool kPow2, int kParity, bool kField = false>
 __device__ __forceinline__ uint4 update_row(const PhiloxCtx& a, uint4 own, const uint4& up, const uint4& ct,
                                             const uint4& dn, uint32_t edge, uint32_t g0, uint32_t c1, uint32_t q,
                                             uint32_t geAdd, uint32_t dshift, uint32_t dmask, const uint32_t* stab,
-                                            const uint32_t* snever, uint32_t slot) {
+                                            const uint32_t* snever, uint32_t slot, const unsigned long long* ftab = nullptr) {
     uint32_t s0, s1, s2, s3;
     if (kParity) {
         s0 = __byte_perm(ct.x, ct.y, 0x4321);
@@ -182,22 +202,22 @@ __device__ __forceinline__ uint4 update_row(const PhiloxCtx& a, uint4 own, const
     uint32_t r0[4], r1[4];
     philox4x32_10(a.rk, g0 + 0, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 1, c1, a.c2, a.c3, r1);
-    res.x = update_word<kHasNever, kSmallQ, kPow2, 0>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot);
+    res.x = update_word<kHasNever, kSmallQ, kPow2, 0, kField>(own.x, up.x, dn.x, ct.x, s0, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot, ftab);
     philox4x32_10(a.rk, g0 + 2, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 3, c1, a.c2, a.c3, r1);
-    res.y = update_word<kHasNever, kSmallQ, kPow2, 1>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot);
+    res.y = update_word<kHasNever, kSmallQ, kPow2, 1, kField>(own.y, up.y, dn.y, ct.y, s1, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot, ftab);
     philox4x32_10(a.rk, g0 + 4, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 5, c1, a.c2, a.c3, r1);
-    res.z = update_word<kHasNever, kSmallQ, kPow2, 2>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot);
+    res.z = update_word<kHasNever, kSmallQ, kPow2, 2, kField>(own.z, up.z, dn.z, ct.z, s2, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot, ftab);
     philox4x32_10(a.rk, g0 + 6, c1, a.c2, a.c3, r0);
     philox4x32_10(a.rk, g0 + 7, c1, a.c2, a.c3, r1);
-    res.w = update_word<kHasNever, kSmallQ, kPow2, 3>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot);
+    res.w = update_word<kHasNever, kSmallQ, kPow2, 3, kField>(own.w, up.w, dn.w, ct.w, s3, r0, r1, q, geAdd, dshift, dmask, stab, snever, slot, ftab);
     return res;
 }
 
-template <int kColour, bool kHasNever, bool kSmallQ, bool kPow2, int kRows>
+template <int kColour, bool kHasNever, bool kSmallQ, bool kPow2, int kRows, bool kField = false>
 __device__ __forceinline__ void march_rows(const SweepArgs& a, const PhiloxCtx& pc, const uint32_t* stab, const uint32_t* snever, uint32_t q,
-                                           uint32_t slot, int b, int rb, int x) {
+                                           uint32_t slot, int b, int rb, int x, const unsigned long long* ftab = nullptr) {
     const int L = a.L, W = L >> 1, W16 = W >> 4, W4 = W >> 2;
     const size_t half = (size_t)L * W;
     const int i0 = rb * kRows;
@@ -236,7 +256,7 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const PhiloxCtx& 
         const uint4 n1 = __ldg(more ? pOth : pOthLast);
         const uint4 own1 = *(pOwn + rowStride);
         const uint32_t edge1 = __ldg(pEdgeOdd);
-        uint4 res = update_row<kHasNever, kSmallQ, kPow2, kColour>(pc, own, wU, wC, wD, edge, g0, c1, q, geAdd, dshift, dmask, stab, snever, slot);
+        uint4 res = update_row<kHasNever, kSmallQ, kPow2, kColour, kField>(pc, own, wU, wC, wD, edge, g0, c1, q, geAdd, dshift, dmask, stab, snever, slot, ftab);
         *pOwn = res;
         uint4 n2 = n1, own2 = own1;
         uint32_t edge2 = edge1;
@@ -245,8 +265,8 @@ __device__ __forceinline__ void march_rows(const SweepArgs& a, const PhiloxCtx& 
             own2 = *(pOwn + 2 * rowStride);
             edge2 = __ldg(pEdgeEven + edgeStride2);
         }
-        res = update_row<kHasNever, kSmallQ, kPow2, 1 - kColour>(pc, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd,
-                                                                 dshift, dmask, stab, snever, slot);
+        res = update_row<kHasNever, kSmallQ, kPow2, 1 - kColour, kField>(pc, own1, wC, wD, n1, edge1, g0 + (uint32_t)(W >> 1), c1, q, geAdd,
+                                                                         dshift, dmask, stab, snever, slot, ftab);
         *(pOwn + rowStride) = res;
         wU = wD;
         wC = n1;
@@ -297,6 +317,34 @@ __global__ void __launch_bounds__(kRowsThreads, kMinBlocks) potts_int8_rows_kern
     else march_rows<kColour, false, false, false, kRows>(a, pc, stab, snever, q, slot, b, rb, x);
 }
 
+// Half-sweep with a field on the state label (Eq. 5 of the paper with its field term): the same marching
+// code; the acceptance entry of a site comes from the replica's [9][255] table in global memory (L1-resident: a replica
+// touches at most 9 x (2 q - 1) entries), indexed by the class and by new - old.
+template <int kColour, int kRows>
+__global__ void __launch_bounds__(kRowsThreads, kMinBlocks) potts_int8_rows_field_kernel(SweepArgs a, int bpr) {
+    __shared__ uint32_t stab[16 + 64];            // from word 16: 256-byte pattern -> 4 * class table (words 0..15 unused)
+    __shared__ uint32_t snever[1];
+    __shared__ uint32_t sidx[4 * kRowsThreads];
+    if (a.pdl_trigger == kPdlAtStart) pdl_launch_dependents();
+    const int b = blockIdx.x / bpr;
+    const int blk = blockIdx.x - b * bpr;
+    pdl_wait();
+    const PhiloxCtx pc = {a.rk, a.c2, a.c3};
+    const uint32_t q = a.tables[(size_t)b * kTableStride + kTabQ];
+    if (threadIdx.x == 0) snever[0] = 0u;
+    for (int m = threadIdx.x; m < 256; m += blockDim.x) {
+        const int cls = nibble_count(m >> 4, false) - nibble_count(m & 15, false) + 4;
+        ((uint8_t*)(stab + 16))[m] = (uint8_t)(4 * cls);
+    }
+    __syncthreads();
+    const int W16 = a.L >> 5;
+    const int u = blk * blockDim.x + threadIdx.x;
+    if (u >= (a.L / kRows) * W16) return;
+    const int rb = u / W16, x = u - rb * W16;
+    const uint32_t slot = (uint32_t)__cvta_generic_to_shared(&sidx[threadIdx.x]);
+    march_rows<kColour, false, false, false, kRows, true>(a, pc, stab, snever, q, slot, b, rb, x, a.potts_tab2 + (size_t)b * 9 * 255);
+}
+
 }  // namespace
 
 const char* potts_int8_variant(int L) { return (L % 32 == 0) ? "potts_int8_rows128" : "potts_int8_generic"; }
@@ -323,6 +371,11 @@ int launch_potts_int8_half_sweep(const SweepArgs& a, cudaStream_t s) {
         SweepArgs args = a;
         args.pdl_trigger = plan.trigger;
         void (*k)(SweepArgs, int) = a.t_dev ? pick_potts_kernel<true>(plan.rows, a.colour) : pick_potts_kernel<false>(plan.rows, a.colour);
+        if (a.potts_tab2) {
+            if (plan.rows == kRowsShort) k = a.colour == 0 ? potts_int8_rows_field_kernel<0, kRowsShort> : potts_int8_rows_field_kernel<1, kRowsShort>;
+            else if (plan.rows == kRowsMid) k = a.colour == 0 ? potts_int8_rows_field_kernel<0, kRowsMid> : potts_int8_rows_field_kernel<1, kRowsMid>;
+            else k = a.colour == 0 ? potts_int8_rows_field_kernel<0, kRowsLong> : potts_int8_rows_field_kernel<1, kRowsLong>;
+        }
         launch_pdl(k, grid, (unsigned)tpb, s, args, bpr);
     } else {
         const long long half = (long long)a.L * (a.L >> 1);

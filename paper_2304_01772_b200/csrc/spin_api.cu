@@ -292,6 +292,7 @@ SweepArgs sweep_args(const spin_sim* sim, int64_t t, int colour) {
     a.rk = sim->rk;
     a.pdl_trigger = kPdlAtExit;
     a.plan_scale = 1;
+    a.potts_tab2 = nullptr;
     a.measure_acc = nullptr;
     a.fin_E = nullptr; a.fin_M = nullptr; a.fin_mom = nullptr; a.fin_pending = 0;
     a.t_dev = sim->capture_t;
@@ -432,10 +433,13 @@ void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour, const uint32_t* ta
     if (tables) a.tables = tables;                          // a step of spin_sweep_schedule
     const size_t nat = (size_t)sim->batch * sim->L * sim->L;
     if (sim->model == SPIN_MODEL_POTTS) {
-        if (sim->potts_general)
+        if (sim->potts_general && (sim->d_bond_nat || sim->L % 32 != 0))
             sim->launches += launch_potts_int8_general_half_sweep(a, sim->d_tab2, sim->d_bond_nat,
                                                                   sim->d_bond_nat ? sim->d_bond_nat + nat : nullptr, sim->stream);
-        else sim->launches += launch_potts_int8_half_sweep(a, sim->stream);
+        else {
+            if (sim->potts_general) a.potts_tab2 = sim->d_tab2;   // a field, uniform couplings: the row-marching kernel's field variant
+            sim->launches += launch_potts_int8_half_sweep(a, sim->stream);
+        }
     } else if (sim->layout == SPIN_LAYOUT_BITPACKED) sim->launches += launch_ising_bits_half_sweep(a, sim->stream);
     else if (sim->general) sim->launches += launch_ising_int8_general_half_sweep(a, sim->d_thr, sim->d_alw, sim->stream);
     else if (sim->d_bond_nat) sim->launches += launch_ising_int8_bonds_half_sweep(a, sim->d_bond_nat, sim->d_bond_nat + nat, sim->stream);
@@ -450,7 +454,7 @@ void enqueue_half_sweep(spin_sim* sim, int64_t t, int colour, const uint32_t* ta
 // half is too small to fill the GPU on its own turn (16 x 640^2 724 -> 695, 4 x 1024^2 598 -> 525), so it is used from 0.15
 // (bit-packed), 0.2 (Potts), 0.3 (int8) waves of 8-row blocks upwards.  Class-table models only (the general kernels index natural-order coupling arrays).
 int streaming_groups(const spin_sim* sim) {
-    if (sim->batch < 2 || sim->general || sim->d_bond_nat || sim->potts_general) return 1;
+    if (sim->batch < 2 || sim->general || sim->d_bond_nat) return 1;   // (Potts with a field and uniform couplings: groups as usual)
     if (sim->policy != SPIN_POLICY_AUTO && sim->policy != SPIN_POLICY_STREAMING && sim->policy != SPIN_POLICY_GRAPH) return 1;
     const bool bits = sim->layout == SPIN_LAYOUT_BITPACKED;
     if (sim->L % (bits ? 64 : 32) != 0) return 1;                // the generic kernels are not planned
@@ -514,6 +518,7 @@ void enqueue_streaming(spin_sim* sim, int G, int64_t t0, int64_t n_sweeps, const
                 a.replica_offset = sim->replica_offset + (uint32_t)b0;
                 if (a.bonds) a.bonds += bondWords * (size_t)b0;
                 a.plan_scale = G;
+                if (sim->potts_general) a.potts_tab2 = sim->d_tab2 + (size_t)9 * 255 * b0;
                 cudaStream_t st = g == 0 ? sim->stream : sim->aux_stream;
                 if (sim->model == SPIN_MODEL_POTTS) sim->launches += launch_potts_int8_half_sweep(a, st);
                 else if (sim->layout == SPIN_LAYOUT_BITPACKED) sim->launches += launch_ising_bits_half_sweep(a, st);

@@ -72,6 +72,8 @@ struct SweepArgs {
     long long* fin_M;
     long long* fin_mom;
     int32_t fin_pending;
+    const unsigned long long* potts_tab2;   // non-NULL (Potts rows kernel): field on the state label - entries
+                                            // (always << 32) | T indexed [replica][dn + 4][new - old + 127] (spin_api.cu)
     const unsigned long long* t_dev;   // non-NULL: the launch is a node of a CUDA graph (spin_api.cu, sweep_graph) and its sweep
     uint32_t t_rel;                    // index is *t_dev + t_rel, read after pdl_wait(); c2 / c3 then hold colour and domain only
     int32_t plan_scale;       // the launch is one of plan_scale concurrent ones (replica groups on their own streams,

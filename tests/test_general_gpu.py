@@ -182,3 +182,30 @@ def test_schedule_with_int8_bond_signs_and_for_potts():
         with pytest.raises(sp.SpinError) as e:                       # a Potts field needs the general kernel: per-call only
             sim.spin_sweep_schedule(steps, 1.0, 0.1, 3)
         assert e.value.code == sp.SPIN_ERR_UNSUPPORTED
+
+
+@pytest.mark.parametrize("L,B,h", [(32, 3, 0.25), (96, 5, -0.2), (256, 64, 0.1)])
+def test_potts_field_on_the_row_marching_kernel(L, B, h):
+    """A field on the state label with uniform couplings and L % 32 == 0 runs the row-marching Potts kernel's field variant
+    (threshold by class and by new - old): ragged blocks, two replica groups (64 x 256^2), q from 2 to 127, thresholds of 0
+    (beta = 30) and always-accept entries, chunked calls; E, M and the label sum against the oracle."""
+    seed = 300 + L
+    q = np.array([2, 3, 8, 127, 5, 16, 9][:min(B, 7)] + [3 + (b % 6) for b in range(max(0, B - 7))], dtype=np.int32)
+    beta = np.linspace(0.4, 1.6, B)
+    beta[-1] = 30.0
+    ref = oracle.init(B, L, seed=seed, q=q)
+    with sp.spin_create_ex(B, L, sp.SPIN_MODEL_POTTS, q_per_replica=q, seed=seed) as sim:
+        l0 = sim.spin_kernel_launches()
+        sim.spin_sweep(beta, 1.0, h, 3, 0)
+        assert sim.spin_kernel_launches() - l0 == 3 * 2 * (2 if B >= 60 else 1)
+        oracle.sweep_potts_general(ref, q, beta, 1.0, h, seed, 3, None, None, sweep_offset=0)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        sim.spin_sweep(beta, -0.5, -h, 2, (1 << 32) - 1)
+        oracle.sweep_potts_general(ref, q, beta, -0.5, -h, seed, 2, None, None, sweep_offset=(1 << 32) - 1)
+        assert np.array_equal(sim.spin_get_spins(), ref)
+        Eo, So, Mo = oracle.potts_general_observables(ref, q, None, None)
+        E, M = sim.spin_observables()
+        assert np.array_equal(E, Eo) and np.array_equal(M, Mo) and np.array_equal(sim.spin_potts_label_sum(), So)
+        sim.spin_sweep(beta, 1.0, 0.0, 2, 9)                            # back to the plain model on the same handle
+        oracle.sweep(ref, beta, 1.0, 0.0, seed=seed, n_sweeps=2, sweep_offset=9, q=q)
+        assert np.array_equal(sim.spin_get_spins(), ref)
