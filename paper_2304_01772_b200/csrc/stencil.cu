@@ -33,6 +33,24 @@ struct StencilArgs {
 __device__ __forceinline__ int wrap_inc(int a, int L) { return a == L - 1 ? 0 : a + 1; }
 __device__ __forceinline__ int wrap_dec(int a, int L) { return a == 0 ? L - 1 : a - 1; }
 
+// Index arithmetic of the byte-SIMD kernels without 64-bit divisions (each costs ~100 instructions, against ~40 for the
+// update of a site): the thread index splits into (replica, rest) in 32 bits whenever the launch has fewer than 2^32
+// threads, and divisions by a power of two are shifts.
+__device__ __forceinline__ void split_replica(long long gid, long long total, uint32_t per, int& b, uint32_t& rem) {
+    if (total <= 0xFFFFFFFFll) {
+        const uint32_t g = (uint32_t)gid;
+        b = (int)(g / per);
+        rem = g - (uint32_t)b * per;
+    } else {
+        b = (int)(gid / per);
+        rem = (uint32_t)(gid - (long long)b * per);
+    }
+}
+__device__ __forceinline__ void divmod_u32(uint32_t x, uint32_t d, uint32_t& quo, uint32_t& r) {
+    if ((d & (d - 1u)) == 0u) { quo = x >> (__ffs((int)d) - 1); r = x & (d - 1u); }
+    else { quo = x / d; r = x - quo * d; }
+}
+
 // Number of sites of one colour, and coordinates of same-colour site n (row-major order among that colour).
 __device__ __host__ __forceinline__ long long colour_sites(int stencil, int L) {
     if (stencil == SPIN_STENCIL_TRIANGULAR) return (long long)L * (L / 3);
@@ -119,7 +137,9 @@ __global__ void __launch_bounds__(128) cubic_pass_vec_kernel(StencilArgs a) {
     const long long total = lines * V * a.batch;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     // a block never straddles replicas when (L^2 * V) % 128 == 0; otherwise the table is re-read per thread below
-    const int b0 = (int)(((long long)blockIdx.x * blockDim.x) / (lines * V));
+    int b0;
+    uint32_t rem0;
+    split_replica((long long)blockIdx.x * blockDim.x, total, (uint32_t)(lines * V), b0, rem0);
     if (threadIdx.x < 16) {
         const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
         const int d = threadIdx.x >> 3, nd = threadIdx.x & 7;
@@ -132,11 +152,12 @@ __global__ void __launch_bounds__(128) cubic_pass_vec_kernel(StencilArgs a) {
     }
     __syncthreads();
     if (gid >= total) return;
-    const int b = (int)(gid / (lines * V));
-    const long long rem = gid - (long long)b * lines * V;
-    const int v = (int)(rem % V);
-    const long long ij = rem / V;
-    const int i = (int)(ij / L), j = (int)(ij % L);
+    int b;
+    uint32_t rem, uv, uij, ui, uj;
+    split_replica(gid, total, (uint32_t)(lines * V), b, rem);     // L^3 / 16 < 2^32 for every legal L
+    divmod_u32(rem, (uint32_t)V, uij, uv);
+    divmod_u32(uij, (uint32_t)L, ui, uj);
+    const int v = (int)uv, i = (int)ui, j = (int)uj;
     const int iu = wrap_dec(i, L), id = wrap_inc(i, L), jl = wrap_dec(j, L), jr = wrap_inc(j, L);
     int8_t* lat = a.lattice + (size_t)b * lines * L;
     const int k0 = v << 4;
@@ -213,8 +234,10 @@ __global__ void __launch_bounds__(128) nnn_pass_vec_kernel(StencilArgs a) {
     const long long per = (long long)H * V;                    // words of the colour's rows per replica
     const long long total = per * a.batch;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int b0 = (int)(((long long)blockIdx.x * blockDim.x) / per);
-    const bool uniform = (per % blockDim.x) == 0;              // then a block never straddles replicas
+    int b0;
+    uint32_t rem0;
+    split_replica((long long)blockIdx.x * blockDim.x, total, (uint32_t)per, b0, rem0);
+    const bool uniform = ((uint32_t)per % blockDim.x) == 0u;     // then a block never straddles replicas
     if (uniform) {
         const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
         if (threadIdx.x < 50) stab[threadIdx.x] = tab[threadIdx.x];
@@ -222,9 +245,11 @@ __global__ void __launch_bounds__(128) nnn_pass_vec_kernel(StencilArgs a) {
         __syncthreads();
     }
     if (gid >= total) return;
-    const int b = (int)(gid / per);
-    const long long rem = gid - (long long)b * per;
-    const int v = (int)(rem % V), ar = (int)(rem / V);
+    int b;
+    uint32_t rem, uv, uar;
+    split_replica(gid, total, (uint32_t)per, b, rem);
+    divmod_u32(rem, (uint32_t)V, uar, uv);
+    const int v = (int)uv, ar = (int)uar;
     const int i = 2 * ar + (a.colour >> 1);
     const uint32_t pj = (uint32_t)(a.colour & 1);
     const int iu = wrap_dec(i, L), id = wrap_inc(i, L), j0 = v << 4;
@@ -277,8 +302,10 @@ __global__ void __launch_bounds__(128) triangular_pass_vec_kernel(StencilArgs a)
     const long long per = (long long)L * V;
     const long long total = per * a.batch;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    const int b0 = (int)(((long long)blockIdx.x * blockDim.x) / per);
-    const bool uniform = (per % blockDim.x) == 0;              // then a block never straddles replicas
+    int b0;
+    uint32_t rem0;
+    split_replica((long long)blockIdx.x * blockDim.x, total, (uint32_t)per, b0, rem0);
+    const bool uniform = ((uint32_t)per % blockDim.x) == 0u;     // then a block never straddles replicas
     if (uniform) {
         if (threadIdx.x < 16) {
             const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
@@ -289,9 +316,11 @@ __global__ void __launch_bounds__(128) triangular_pass_vec_kernel(StencilArgs a)
         __syncthreads();
     }
     if (gid >= total) return;
-    const int b = (int)(gid / per);
-    const long long rem = gid - (long long)b * per;
-    const int v = (int)(rem % V), i = (int)(rem / V);
+    int b;
+    uint32_t rem, uv, ui;
+    split_replica(gid, total, (uint32_t)per, b, rem);
+    divmod_u32(rem, (uint32_t)V, ui, uv);
+    const int v = (int)uv, i = (int)ui;
     const int iu = wrap_dec(i, L), id = wrap_inc(i, L), j0 = 12 * v;
     const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 12 == L ? 0 : j0 + 12;
     int8_t* lat = a.lattice + (size_t)b * L * L;
