@@ -216,7 +216,7 @@ SPIN_API int spin_sweep_schedule(spin_sim* sim, const double* beta_steps, int64_
  *                           half-sweeps: Ising int8, L % 32 == 0, uniform couplings, no class whose threshold is 0.
  *                           Never picked by AUTO (the streaming kernels are faster on every measured shape).
  *   SPIN_POLICY_TILED       temporal blocking: a CTA advances a tile with a halo by 4 (small lattices: 2) sweeps per launch in
- *                           shared memory, at most one tile per SM (AUTO: up to 16 replicas and 2^20 sites); needs a second
+ *                           shared memory, at most one tile per SM (AUTO: up to 16 replicas and 2^21 sites); needs a second
  *                           lattice buffer (allocated by the library on first use): Ising int8, L % 8 == 0, L >= 16,
  *                           uniform couplings.
  *   SPIN_POLICY_GRAPH       the streaming kernels replayed from a CUDA graph of 64 sweeps captured once per handle (the kernels
