@@ -372,6 +372,116 @@ __global__ void __launch_bounds__(128) triangular_pass_vec_kernel(StencilArgs a)
     wc[2] = cw[2] ^ flip[2];
 }
 
+// ---- triangular lattice, L % 12 == 0, row-marching variant of the kernel above: a thread owns a 12-site chunk of kRows
+// consecutive rows and keeps the masked words (and the two edge bytes) of the rows above / of / below the current one in
+// registers, so a row costs one row of loads instead of three and the index arithmetic is paid once per thread.  The
+// updated sites never neighbour each other, so the masked words of a row stay valid as "row above" after the row was
+// updated (only bytes of the current colour changed, and those are never read as neighbours in this pass); rows written by
+// the neighbouring thread are read word-wise with their other-colour bytes unchanged, as in the kernel above.
+template <int kRows>
+__global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a) {
+    pdl_wait();
+    __shared__ uint32_t stab[16];
+    __shared__ uint32_t salways;
+    const int L = a.L, V = L / 12, RB = L / kRows;             // chunks per row, row blocks per replica
+    const long long per = (long long)RB * V;
+    const long long total = per * a.batch;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    int b0;
+    uint32_t rem0;
+    split_replica((long long)blockIdx.x * blockDim.x, total, (uint32_t)per, b0, rem0);
+    const bool uniform = ((uint32_t)per % blockDim.x) == 0u;     // then a block never straddles replicas
+    if (uniform) {
+        if (threadIdx.x < 16) {
+            const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
+            const int d = threadIdx.x >> 3, nd = threadIdx.x & 7;
+            stab[threadIdx.x] = nd <= 6 ? tab[d * 7 + nd] : 0u;
+            if (threadIdx.x == 0) salways = (tab[62] & 0x7Fu) | (((tab[62] >> 7) & 0x7Fu) << 8);
+        }
+        __syncthreads();
+    }
+    if (gid >= total) return;
+    int b;
+    uint32_t rem, uv, urb;
+    split_replica(gid, total, (uint32_t)per, b, rem);
+    divmod_u32(rem, (uint32_t)V, urb, uv);
+    const int v = (int)uv, i0 = (int)urb * kRows;
+    const int j0 = 12 * v, jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 12 == L ? 0 : j0 + 12;
+    int8_t* lat = a.lattice + (size_t)b * L * L;
+    const uint32_t m = 0x04040404u;
+    const uint32_t* gtab = a.tables + (size_t)b * kStencilRec;
+    uint32_t always = salways;
+    if (!uniform) always = (gtab[62] & 0x7Fu) | (((gtab[62] >> 7) & 0x7Fu) << 8);
+    // rows i - 1, i, i + 1: masked words, edge bytes (masked), and the raw words of row i
+    uint32_t um[3], cm[3], dm[3], cw[3], nw[3];
+    uint32_t uL, cL, cR, dL, dR;
+    {
+        const int iu = wrap_dec(i0, L), id = wrap_inc(i0, L);
+        const uint32_t* ru = (const uint32_t*)(lat + (size_t)iu * L + j0);
+        const uint32_t* rc = (const uint32_t*)(lat + (size_t)i0 * L + j0);
+        const uint32_t* rd = (const uint32_t*)(lat + (size_t)id * L + j0);
+#pragma unroll
+        for (int w = 0; w < 3; ++w) { um[w] = ru[w] & m; cw[w] = rc[w]; cm[w] = cw[w] & m; nw[w] = rd[w]; dm[w] = nw[w] & m; }
+        uL = (uint32_t)(uint8_t)lat[(size_t)iu * L + jl] & 4u;
+        cL = (uint32_t)(uint8_t)lat[(size_t)i0 * L + jl] & 4u;
+        cR = (uint32_t)(uint8_t)lat[(size_t)i0 * L + jr] & 4u;
+        dL = (uint32_t)(uint8_t)lat[(size_t)id * L + jl] & 4u;
+        dR = (uint32_t)(uint8_t)lat[(size_t)id * L + jr] & 4u;
+    }
+    int p = ((a.colour - i0) % 3 + 3) % 3;                     // byte offset of the first updated site of row i
+    uint32_t group = (uint32_t)((long long)i0 * V + v);
+    const uint32_t c1 = (uint32_t)b + a.replica_offset;
+#pragma unroll
+    for (int rr = 0; rr < kRows; ++rr) {
+        const int i = i0 + rr;
+        // the row after next (the only load of this step), issued before the arithmetic of the current row
+        uint32_t xw[3] = {0u, 0u, 0u}, xL = 0u, xR = 0u;
+        if (rr + 1 < kRows) {
+            int i2 = i + 2;
+            i2 = i2 >= L ? i2 - L : i2;
+            const uint32_t* rx = (const uint32_t*)(lat + (size_t)i2 * L + j0);
+            xw[0] = rx[0]; xw[1] = rx[1]; xw[2] = rx[2];
+            xL = (uint32_t)(uint8_t)lat[(size_t)i2 * L + jl] & 4u;
+            xR = (uint32_t)(uint8_t)lat[(size_t)i2 * L + jr] & 4u;
+        }
+        uint32_t r[4];
+        philox4x32_10(a.rk, group, c1, a.c2, a.c3, r);
+        uint32_t t[3];
+#pragma unroll
+        for (int w = 0; w < 3; ++w) {
+            const uint32_t cprev = w == 0 ? cL : (cm[w - 1] >> 24), cnext = w == 2 ? cR : (cm[w + 1] & 0xFFu);
+            const uint32_t uprev = w == 0 ? uL : (um[w - 1] >> 24), dnext = w == 2 ? dR : (dm[w + 1] & 0xFFu);
+            const uint32_t left = (cm[w] << 8) | cprev, right = (cm[w] >> 8) | (cnext << 24);
+            const uint32_t upleft = (um[w] << 8) | uprev, downright = (dm[w] >> 8) | (dnext << 24);
+            t[w] = um[w] + dm[w] + left + right + upleft + downright + (cw[w] & 0x20202020u);   // bytes: 4 nd + 32 d
+        }
+        uint32_t flip[3] = {0u, 0u, 0u};
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+            const int pos = p + 3 * e;                         // byte of the updated site within the 12
+            const uint32_t word = pos < 4 ? t[0] : (pos < 8 ? t[1] : t[2]);
+            const uint32_t idx = ((word >> (8 * (pos & 3))) & 0xFFu) >> 2;      // d * 8 + nd
+            uint32_t T;
+            if (uniform) T = stab[idx];
+            else T = gtab[(idx >> 3) * 7u + (idx & 7u)];
+            if (((always >> idx) & 1u) || r[e] < T) {
+                const uint32_t bit = 0xFEu << (8 * (pos & 3));
+                if (pos < 4) flip[0] |= bit; else if (pos < 8) flip[1] |= bit; else flip[2] |= bit;
+            }
+        }
+        uint32_t* wc = (uint32_t*)(lat + (size_t)i * L + j0);
+        wc[0] = cw[0] ^ flip[0];
+        wc[1] = cw[1] ^ flip[1];
+        wc[2] = cw[2] ^ flip[2];
+        // next row: (above, current, below) <- (current as it was, below, the row just loaded)
+#pragma unroll
+        for (int w = 0; w < 3; ++w) { um[w] = cm[w]; cw[w] = nw[w]; cm[w] = dm[w]; nw[w] = xw[w]; dm[w] = xw[w] & m; }
+        uL = cL; cL = dL; cR = dR; dL = xL; dR = xR;
+        p = p == 0 ? 2 : p - 1;                                // (colour - (i + 1)) mod 3
+        group += (uint32_t)V;
+    }
+}
+
 __global__ void stencil_init_kernel(int8_t* lattice, long long N, int batch, uint32_t replica_offset, RoundKeys rk) {
     const long long groups = (N + 3) >> 2;
     const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -552,7 +662,9 @@ int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_t* lattic
             a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)c << 24) | (kDomainStencil << 28);
             if (stencil == SPIN_STENCIL_TRIANGULAR && L % 12 == 0) {
                 const long long chunks = (long long)L * (L / 12) * batch;
-                launch_pdl(triangular_pass_vec_kernel, (unsigned)((chunks + 127) / 128), 128u, s, a);
+                // 12 or 4 rows per thread (L % 12 == 0): the longer march when it still gives every SM several blocks
+                if (chunks / 12 >= 148ll * 8 * 128) launch_pdl(triangular_march_vec_kernel<12>, (unsigned)((chunks / 12 + 127) / 128), 128u, s, a);
+                else launch_pdl(triangular_march_vec_kernel<4>, (unsigned)((chunks / 4 + 127) / 128), 128u, s, a);
             } else if (stencil == SPIN_STENCIL_TRIANGULAR) launch_pdl(stencil_pass_kernel<SPIN_STENCIL_TRIANGULAR>, grid, 128u, s, a);
             else if (stencil == SPIN_STENCIL_CUBIC && L % 16 == 0) {
                 const long long words = (long long)L * L * (L >> 4) * batch;

@@ -52,3 +52,27 @@ def test_invalid_shapes_and_arguments():
         with pytest.raises(sp.SpinError):
             sp.spin_stencil_sweep(sp.SPIN_STENCIL_CUBIC, 1, a["L"], d.data_ptr(), a["beta"], a["J1"], 0.0, 0.0, 1, a["n_sweeps"])
     assert torch.all(d == 1).item()
+
+
+@pytest.mark.parametrize("L,B", [(24, 5), (96, 2400)])
+def test_triangular_row_marching_kernel(L, B):
+    """The triangular byte-SIMD kernel marches 4 rows per thread, 12 when the launch is large (2400 x 96^2): every replica
+    against the oracle after each of 2 sweeps and after a 3-sweep call, ragged blocks that straddle replicas (5 x 24^2)."""
+    st = sp.SPIN_STENCIL_TRIANGULAR
+    seed = 40 + L
+    beta = np.linspace(0.05, 0.6, B)
+    beta[-1] = 20.0
+    n = sp.spin_stencil_sites(st, L)
+    d = torch.empty(B * n, dtype=torch.int8, device="cuda")
+    cs = torch.cuda.current_stream().cuda_stream
+    sp.spin_stencil_init(st, B, L, d.data_ptr(), seed, cuda_stream=cs)
+    ref = oracle.stencil_init(st, B, L, seed=seed)
+    t = 0
+    for k in (1, 1, 3):
+        sp.spin_stencil_sweep(st, B, L, d.data_ptr(), beta, 1.0, 0.0, 0.07, seed, k, sweep_offset=t, cuda_stream=cs)
+        oracle.stencil_sweep(st, ref, beta, 1.0, 0.0, 0.07, seed, k, sweep_offset=t)
+        assert np.array_equal(d.cpu().numpy().reshape(ref.shape), ref), t
+        t += k
+    E1, E2, M = sp.spin_stencil_observables(st, B, L, d.data_ptr(), cuda_stream=cs)
+    o1, o2, om = oracle.stencil_observables(st, ref)
+    assert np.array_equal(E1, o1) and np.array_equal(M, om)
