@@ -290,94 +290,16 @@ __global__ void __launch_bounds__(128) nnn_pass_vec_kernel(StencilArgs a) {
     *(uint4*)(lat + (size_t)i * L + j0) = make_uint4(out[0], out[1], out[2], out[3]);
 }
 
-// ---- triangular lattice, L % 12 == 0: byte-SIMD kernel.  One thread owns 12 consecutive sites of a row (three words):
-// the sites of the current colour are every third one, at byte p + 3 m (p = (colour - i) mod 3, m = 0..3) = exactly one
-// Philox group.  Neighbour sums per byte as in the kernels above: (i-1, j) + (i+1, j) + (i, j-1) + (i, j+1) + (i+1, j+1) +
-// (i-1, j-1), every spin masked to "4 per -1 spin"; 4 nd + 32 d indexes the [d][8] threshold table.
-__global__ void __launch_bounds__(128) triangular_pass_vec_kernel(StencilArgs a) {
-    pdl_wait();   // launched with programmatic stream serialisation: the previous pass must have completed
-    __shared__ uint32_t stab[16];
-    __shared__ uint32_t salways;
-    const int L = a.L, V = L / 12;                             // 12-site chunks per row
-    const long long per = (long long)L * V;
-    const long long total = per * a.batch;
-    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    int b0;
-    uint32_t rem0;
-    split_replica((long long)blockIdx.x * blockDim.x, total, (uint32_t)per, b0, rem0);
-    const bool uniform = ((uint32_t)per % blockDim.x) == 0u;     // then a block never straddles replicas
-    if (uniform) {
-        if (threadIdx.x < 16) {
-            const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
-            const int d = threadIdx.x >> 3, nd = threadIdx.x & 7;
-            stab[threadIdx.x] = nd <= 6 ? tab[d * 7 + nd] : 0u;
-            if (threadIdx.x == 0) salways = (tab[62] & 0x7Fu) | (((tab[62] >> 7) & 0x7Fu) << 8);
-        }
-        __syncthreads();
-    }
-    if (gid >= total) return;
-    int b;
-    uint32_t rem, uv, ui;
-    split_replica(gid, total, (uint32_t)per, b, rem);
-    divmod_u32(rem, (uint32_t)V, ui, uv);
-    const int v = (int)uv, i = (int)ui;
-    const int iu = wrap_dec(i, L), id = wrap_inc(i, L), j0 = 12 * v;
-    const int jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 12 == L ? 0 : j0 + 12;
-    int8_t* lat = a.lattice + (size_t)b * L * L;
-    const uint32_t m = 0x04040404u;
-    const uint32_t* rc = (const uint32_t*)(lat + (size_t)i * L + j0);
-    const uint32_t* ru = (const uint32_t*)(lat + (size_t)iu * L + j0);
-    const uint32_t* rd = (const uint32_t*)(lat + (size_t)id * L + j0);
-    const uint32_t cw[3] = {rc[0], rc[1], rc[2]};
-    const uint32_t cm[3] = {cw[0] & m, cw[1] & m, cw[2] & m}, um[3] = {ru[0] & m, ru[1] & m, ru[2] & m},
-                   dm[3] = {rd[0] & m, rd[1] & m, rd[2] & m};
-    const uint32_t cL = (uint32_t)(uint8_t)lat[(size_t)i * L + jl] & 4u, cR = (uint32_t)(uint8_t)lat[(size_t)i * L + jr] & 4u;
-    const uint32_t uL = (uint32_t)(uint8_t)lat[(size_t)iu * L + jl] & 4u, dR = (uint32_t)(uint8_t)lat[(size_t)id * L + jr] & 4u;
-    const int p = ((a.colour - i) % 3 + 3) % 3;                // byte offset of the first updated site
-    uint32_t r[4];
-    philox4x32_10(a.rk, (uint32_t)((long long)i * V + v), (uint32_t)b + a.replica_offset, a.c2, a.c3, r);
-    uint32_t t[3];
-#pragma unroll
-    for (int w = 0; w < 3; ++w) {
-        const uint32_t cprev = w == 0 ? cL : (cm[w - 1] >> 24), cnext = w == 2 ? cR : (cm[w + 1] & 0xFFu);
-        const uint32_t uprev = w == 0 ? uL : (um[w - 1] >> 24), dnext = w == 2 ? dR : (dm[w + 1] & 0xFFu);
-        const uint32_t left = (cm[w] << 8) | cprev, right = (cm[w] >> 8) | (cnext << 24);
-        const uint32_t upleft = (um[w] << 8) | uprev, downright = (dm[w] >> 8) | (dnext << 24);
-        t[w] = um[w] + dm[w] + left + right + upleft + downright + (cw[w] & 0x20202020u);   // bytes: 4 nd + 32 d
-    }
-    const uint32_t* tab = uniform ? stab : nullptr;
-    uint32_t flip[3] = {0u, 0u, 0u};
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-        const int pos = p + 3 * e;                             // byte of the updated site within the 12
-        const uint32_t word = pos < 4 ? t[0] : (pos < 8 ? t[1] : t[2]);
-        const uint32_t idx = ((word >> (8 * (pos & 3))) & 0xFFu) >> 2;      // d * 8 + nd
-        uint32_t T;
-        bool al;
-        if (tab) { T = tab[idx]; al = (salways >> idx) & 1u; }
-        else {
-            const uint32_t* g = a.tables + (size_t)b * kStencilRec;
-            const uint32_t k7 = (idx >> 3) * 7u + (idx & 7u);
-            T = g[k7];
-            al = (g[62] >> k7) & 1u;
-        }
-        if (al || r[e] < T) {
-            const uint32_t bit = 0xFEu << (8 * (pos & 3));
-            if (pos < 4) flip[0] |= bit; else if (pos < 8) flip[1] |= bit; else flip[2] |= bit;
-        }
-    }
-    uint32_t* wc = (uint32_t*)(lat + (size_t)i * L + j0);
-    wc[0] = cw[0] ^ flip[0];
-    wc[1] = cw[1] ^ flip[1];
-    wc[2] = cw[2] ^ flip[2];
-}
-
-// ---- triangular lattice, L % 12 == 0, row-marching variant of the kernel above: a thread owns a 12-site chunk of kRows
-// consecutive rows and keeps the masked words (and the two edge bytes) of the rows above / of / below the current one in
-// registers, so a row costs one row of loads instead of three and the index arithmetic is paid once per thread.  The
-// updated sites never neighbour each other, so the masked words of a row stay valid as "row above" after the row was
-// updated (only bytes of the current colour changed, and those are never read as neighbours in this pass); rows written by
-// the neighbouring thread are read word-wise with their other-colour bytes unchanged, as in the kernel above.
+// ---- triangular lattice, L % 12 == 0: byte-SIMD row-marching kernel.  A thread owns a chunk of 12 consecutive sites (three
+// words) of kRows consecutive rows; the four sites of the pass's colour in a chunk, at bytes p + 3 m with
+// p = (colour - i) mod 3, are one Philox group (group index i * (L / 12) + v).  Neighbours (i+-1, j), (i, j+-1),
+// (i+1, j+1), (i-1, j-1): with every spin masked to "4 per -1 spin", up + down + left + right + upleft + downright +
+// 32 d per byte is the byte offset of the class threshold in a shared-memory table laid out [d][8].  The masked words (and
+// the two edge bytes) of the rows above / of / below the current one stay in registers, so a row costs one row of loads
+// and the index arithmetic is paid once per thread.  The updated sites never neighbour each other, so the masked words of
+// a row stay valid as "row above" after the row was updated (only bytes of the current colour changed, and those are
+// never read as neighbours in this pass); rows of the neighbouring threads are read word-wise, their other-colour bytes
+// are rewritten with the values they already have.
 template <int kRows>
 __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a) {
     pdl_wait();
