@@ -539,7 +539,7 @@ def stencil_cpm_entries(runner, sp, args, peaks, measured):
         ms = _time_calls(runner, args, lambda k: sp.spin_stencil_sweep(stencil, B, L, lat.data_ptr(), beta, 1.0, 0.2, 0.0, 21, n,
                                                                        sweep_offset=k * n, cuda_stream=stream.cuda_stream))
         ncol = {sp.SPIN_STENCIL_TRIANGULAR: 3, sp.SPIN_STENCIL_CUBIC: 2, sp.SPIN_STENCIL_SQUARE_NNN: 4}[stencil]
-        kern = {sp.SPIN_STENCIL_TRIANGULAR: "triangular_march_vec_kernel", sp.SPIN_STENCIL_CUBIC: "cubic_pass_vec_kernel",
+        kern = {sp.SPIN_STENCIL_TRIANGULAR: "triangular_march_vec_kernel", sp.SPIN_STENCIL_CUBIC: "cubic_march_vec_kernel",
                 sp.SPIN_STENCIL_SQUARE_NNN: "nnn_pass_vec_kernel"}[stencil]
         out[key] = _alu_entry(key, "%s: Ising, batch %d, L = %d (%d sites per replica), %d sweeps" % (key, B, L, sites, n),
                               float(B) * sites * n, ms, 11.0, 1.0, kern, ncol * n, peaks, measured)
