@@ -540,7 +540,7 @@ def stencil_cpm_entries(runner, sp, args, peaks, measured):
                                                                        sweep_offset=k * n, cuda_stream=stream.cuda_stream))
         ncol = {sp.SPIN_STENCIL_TRIANGULAR: 3, sp.SPIN_STENCIL_CUBIC: 2, sp.SPIN_STENCIL_SQUARE_NNN: 4}[stencil]
         kern = {sp.SPIN_STENCIL_TRIANGULAR: "triangular_march_vec_kernel", sp.SPIN_STENCIL_CUBIC: "cubic_march_vec_kernel",
-                sp.SPIN_STENCIL_SQUARE_NNN: "nnn_pass_vec_kernel"}[stencil]
+                sp.SPIN_STENCIL_SQUARE_NNN: "nnn_march_vec_kernel"}[stencil]
         out[key] = _alu_entry(key, "%s: Ising, batch %d, L = %d (%d sites per replica), %d sweeps" % (key, B, L, sites, n),
                               float(B) * sites * n, ms, 11.0, 1.0, kern, ncol * n, peaks, measured)
     B, L = 256, 64
