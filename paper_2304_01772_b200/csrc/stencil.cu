@@ -132,7 +132,7 @@ __global__ void __launch_bounds__(128) stencil_pass_kernel(StencilArgs a) {
 // of the current one) instead of five: one word per thread was bound by its L2 traffic (80 bytes per 8 updates; 380 vs 449
 // flips/ns on 8 x 128^3).  The updated sites never neighbour each other, so a plane's word stays valid as the "i - 1"
 // neighbour after it was updated.
-template <int kRows>
+template <int kRows, bool kUniform>
 __global__ void __launch_bounds__(128) cubic_march_vec_kernel(StencilArgs a) {
     pdl_wait();
     __shared__ uint32_t stab[16];
@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(128) cubic_march_vec_kernel(StencilArgs a) {
     int b0;
     uint32_t rem0;
     split_replica((long long)blockIdx.x * blockDim.x, total, (uint32_t)per, b0, rem0);
-    const bool uniform = ((uint32_t)per % blockDim.x) == 0u;     // then a block never straddles replicas
+    constexpr bool uniform = kUniform;                           // per % blockDim.x == 0 (the launcher): a block never straddles replicas
     if (uniform) {
         if (threadIdx.x < 16) {
             const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
@@ -219,7 +219,9 @@ __global__ void __launch_bounds__(128) cubic_march_vec_kernel(StencilArgs a) {
                 uint32_t T;
                 if (uniform) T = stab[idx];
                 else T = gtab[(idx >> 3) * 7u + (idx & 7u)];
-                if (((always >> idx) & 1u) || r[2 * w + e] < T) flip |= 0xFEu << (8u * pos);
+                // branch-free (a short-circuit `||` compiles to a divergent branch per site): accept -> all ones
+                const uint32_t acc = ((always >> idx) & 1u) | (uint32_t)(r[2 * w + e] < T);
+                flip |= (0u - acc) & (0xFEu << (8u * pos));
             }
             out[w] = cw[w] ^ flip;
         }
@@ -249,7 +251,7 @@ __device__ __forceinline__ void shifted_words(const uint32_t x[4], uint32_t edge
 // an updated row is the row above the next one and is not touched in this pass, so its masked and shifted words are
 // reused: two rows of loads per step instead of three (one word per thread: 326 flips/ns on 16 x 1024^2, marching 4 rows:
 // 355, 8 rows: 282).
-template <int kRows>
+template <int kRows, bool kUniform>
 __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
     pdl_wait();
     __shared__ uint32_t stab[50];
@@ -261,7 +263,7 @@ __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
     int b0;
     uint32_t rem0;
     split_replica((long long)blockIdx.x * blockDim.x, total, (uint32_t)per, b0, rem0);
-    const bool uniform = ((uint32_t)per % blockDim.x) == 0u;     // then a block never straddles replicas
+    constexpr bool uniform = kUniform;                           // per % blockDim.x == 0 (the launcher): a block never straddles replicas
     if (uniform) {
         const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
         if (threadIdx.x < 50) stab[threadIdx.x] = tab[threadIdx.x];
@@ -315,7 +317,8 @@ __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
             for (int e = 0; e < 2; ++e) {
                 const uint32_t pos = 2u * (uint32_t)e + pj;
                 const uint32_t idx = ((t >> (8u * pos)) & 0xFFu) >> 2;
-                if (((always >> idx) & 1ull) || r[2 * w + e] < tab[idx]) flip |= 0xFEu << (8u * pos);
+                const uint32_t acc = (uint32_t)((always >> idx) & 1ull) | (uint32_t)(r[2 * w + e] < tab[idx]);   // branch-free
+                flip |= (0u - acc) & (0xFEu << (8u * pos));
             }
             out[w] = cw[w] ^ flip;
         }
@@ -336,7 +339,7 @@ __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
 // a row stay valid as "row above" after the row was updated (only bytes of the current colour changed, and those are
 // never read as neighbours in this pass); rows of the neighbouring threads are read word-wise, their other-colour bytes
 // are rewritten with the values they already have.
-template <int kRows>
+template <int kRows, bool kUniform>
 __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a) {
     pdl_wait();
     __shared__ uint32_t stab[16];
@@ -348,7 +351,7 @@ __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a
     int b0;
     uint32_t rem0;
     split_replica((long long)blockIdx.x * blockDim.x, total, (uint32_t)per, b0, rem0);
-    const bool uniform = ((uint32_t)per % blockDim.x) == 0u;     // then a block never straddles replicas
+    constexpr bool uniform = kUniform;                           // per % blockDim.x == 0 (the launcher): a block never straddles replicas
     if (uniform) {
         if (threadIdx.x < 16) {
             const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
@@ -422,10 +425,11 @@ __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a
             uint32_t T;
             if (uniform) T = stab[idx];
             else T = gtab[(idx >> 3) * 7u + (idx & 7u)];
-            if (((always >> idx) & 1u) || r[e] < T) {
-                const uint32_t bit = 0xFEu << (8 * (pos & 3));
-                if (pos < 4) flip[0] |= bit; else if (pos < 8) flip[1] |= bit; else flip[2] |= bit;
-            }
+            const uint32_t acc = ((always >> idx) & 1u) | (uint32_t)(r[e] < T);                  // branch-free
+            const uint32_t bit = (0u - acc) & (0xFEu << (8 * (pos & 3)));
+            flip[0] |= pos < 4 ? bit : 0u;
+            flip[1] |= (pos >= 4 && pos < 8) ? bit : 0u;
+            flip[2] |= pos >= 8 ? bit : 0u;
         }
         uint32_t* wc = (uint32_t*)(lat + (size_t)i * L + j0);
         wc[0] = cw[0] ^ flip[0];
@@ -621,16 +625,28 @@ int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_t* lattic
             if (stencil == SPIN_STENCIL_TRIANGULAR && L % 12 == 0) {
                 const long long chunks = (long long)L * (L / 12) * batch;
                 // 12 or 4 rows per thread (L % 12 == 0): the longer march when it still gives every SM several blocks
-                if (chunks / 12 >= 148ll * 8 * 128) launch_pdl(triangular_march_vec_kernel<12>, (unsigned)((chunks / 12 + 127) / 128), 128u, s, a);
-                else launch_pdl(triangular_march_vec_kernel<4>, (unsigned)((chunks / 4 + 127) / 128), 128u, s, a);
+                // (kUniform: the threads of one replica fill whole blocks, so a block's table comes from shared memory)
+                if (chunks / 12 >= 148ll * 8 * 128) {
+                    const bool uni = ((long long)(L / 12) * (L / 12)) % 128 == 0;
+                    launch_pdl(uni ? triangular_march_vec_kernel<12, true> : triangular_march_vec_kernel<12, false>,
+                               (unsigned)((chunks / 12 + 127) / 128), 128u, s, a);
+                } else {
+                    const bool uni = ((long long)(L / 4) * (L / 12)) % 128 == 0;
+                    launch_pdl(uni ? triangular_march_vec_kernel<4, true> : triangular_march_vec_kernel<4, false>,
+                               (unsigned)((chunks / 4 + 127) / 128), 128u, s, a);
+                }
             } else if (stencil == SPIN_STENCIL_TRIANGULAR) launch_pdl(stencil_pass_kernel<SPIN_STENCIL_TRIANGULAR>, grid, 128u, s, a);
             else if (stencil == SPIN_STENCIL_CUBIC && L % 16 == 0) {
                 const long long words = (long long)L * L * (L >> 4) * batch;
-                launch_pdl(cubic_march_vec_kernel<4>, (unsigned)((words / 4 + 127) / 128), 128u, s, a);   // 4 planes per thread (8: 407 flips/ns)
+                const bool uni = ((long long)(L / 4) * L * (L >> 4)) % 128 == 0;
+                launch_pdl(uni ? cubic_march_vec_kernel<4, true> : cubic_march_vec_kernel<4, false>,
+                           (unsigned)((words / 4 + 127) / 128), 128u, s, a);   // 4 planes per thread (8: 407 flips/ns)
             } else if (stencil == SPIN_STENCIL_CUBIC) launch_pdl(stencil_pass_kernel<SPIN_STENCIL_CUBIC>, grid, 128u, s, a);
             else if (L % 16 == 0) {
                 const long long words = (long long)(L >> 1) * (L >> 4) * batch;
-                launch_pdl(nnn_march_vec_kernel<4>, (unsigned)((words / 4 + 127) / 128), 128u, s, a);
+                const bool uni = ((long long)(L / 8) * (L >> 4)) % 128 == 0;
+                launch_pdl(uni ? nnn_march_vec_kernel<4, true> : nnn_march_vec_kernel<4, false>,
+                           (unsigned)((words / 4 + 127) / 128), 128u, s, a);
             } else launch_pdl(stencil_pass_kernel<SPIN_STENCIL_SQUARE_NNN>, grid, 128u, s, a);
         }
     if (e == cudaSuccess) e = cudaGetLastError();
