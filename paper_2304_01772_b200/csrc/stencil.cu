@@ -339,8 +339,9 @@ __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
 // a row stay valid as "row above" after the row was updated (only bytes of the current colour changed, and those are
 // never read as neighbours in this pass); rows of the neighbouring threads are read word-wise, their other-colour bytes
 // are rewritten with the values they already have.
-template <int kRows, bool kUniform>
+template <int kRows, bool kUniform, int kColour>
 __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a) {
+    static_assert(kRows % 3 == 0, "the byte positions of the updated sites are compile-time only if a thread starts at a row that is a multiple of 3");
     pdl_wait();
     __shared__ uint32_t stab[16];
     __shared__ uint32_t salways;
@@ -389,7 +390,8 @@ __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a
         dL = (uint32_t)(uint8_t)lat[(size_t)id * L + jl] & 4u;
         dR = (uint32_t)(uint8_t)lat[(size_t)id * L + jr] & 4u;
     }
-    int p = ((a.colour - i0) % 3 + 3) % 3;                     // byte offset of the first updated site of row i
+    // byte offset of the first updated site of row i0 + rr: (colour - i) mod 3 = (kColour - rr) mod 3, as i0 % 3 == 0 - a
+    // compile-time constant in the unrolled loop, so the word selects, shifts and flip masks below are immediates
     uint32_t group = (uint32_t)((long long)i0 * V + v);
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
 #pragma unroll
@@ -419,7 +421,7 @@ __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a
         uint32_t flip[3] = {0u, 0u, 0u};
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
-            const int pos = p + 3 * e;                         // byte of the updated site within the 12
+            const int pos = ((kColour - rr) % 3 + 3) % 3 + 3 * e;   // byte of the updated site within the 12
             const uint32_t word = pos < 4 ? t[0] : (pos < 8 ? t[1] : t[2]);
             const uint32_t idx = ((word >> (8 * (pos & 3))) & 0xFFu) >> 2;      // d * 8 + nd
             uint32_t T;
@@ -439,7 +441,6 @@ __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a
 #pragma unroll
         for (int w = 0; w < 3; ++w) { um[w] = cm[w]; cw[w] = nw[w]; cm[w] = dm[w]; nw[w] = xw[w]; dm[w] = xw[w] & m; }
         uL = cL; cL = dL; cR = dR; dL = xL; dR = xR;
-        p = p == 0 ? 2 : p - 1;                                // (colour - (i + 1)) mod 3
         group += (uint32_t)V;
     }
 }
@@ -624,16 +625,24 @@ int spin_stencil_sweep(int32_t stencil, int32_t batch, int32_t L, int8_t* lattic
             a.c3 = (uint32_t)(((uint64_t)t >> 32) & 0xFFFFFFull) | ((uint32_t)c << 24) | (kDomainStencil << 28);
             if (stencil == SPIN_STENCIL_TRIANGULAR && L % 12 == 0) {
                 const long long chunks = (long long)L * (L / 12) * batch;
-                // 12 or 4 rows per thread (L % 12 == 0): the longer march when it still gives every SM several blocks
-                // (kUniform: the threads of one replica fill whole blocks, so a block's table comes from shared memory)
+                // 12 or 6 rows per thread (L % 12 == 0): the longer march when it still gives every SM several blocks.
+                // (kUniform: the threads of one replica fill whole blocks, so a block's table comes from shared memory;
+                // the colour is a template parameter: see the kernel)
+                typedef void (*Kern)(StencilArgs);
+                static const Kern k12[2][3] = {{triangular_march_vec_kernel<12, false, 0>, triangular_march_vec_kernel<12, false, 1>,
+                                                triangular_march_vec_kernel<12, false, 2>},
+                                               {triangular_march_vec_kernel<12, true, 0>, triangular_march_vec_kernel<12, true, 1>,
+                                                triangular_march_vec_kernel<12, true, 2>}};
+                static const Kern k6[2][3] = {{triangular_march_vec_kernel<6, false, 0>, triangular_march_vec_kernel<6, false, 1>,
+                                               triangular_march_vec_kernel<6, false, 2>},
+                                              {triangular_march_vec_kernel<6, true, 0>, triangular_march_vec_kernel<6, true, 1>,
+                                               triangular_march_vec_kernel<6, true, 2>}};
                 if (chunks / 12 >= 148ll * 8 * 128) {
                     const bool uni = ((long long)(L / 12) * (L / 12)) % 128 == 0;
-                    launch_pdl(uni ? triangular_march_vec_kernel<12, true> : triangular_march_vec_kernel<12, false>,
-                               (unsigned)((chunks / 12 + 127) / 128), 128u, s, a);
+                    launch_pdl(k12[uni][c], (unsigned)((chunks / 12 + 127) / 128), 128u, s, a);
                 } else {
-                    const bool uni = ((long long)(L / 4) * (L / 12)) % 128 == 0;
-                    launch_pdl(uni ? triangular_march_vec_kernel<4, true> : triangular_march_vec_kernel<4, false>,
-                               (unsigned)((chunks / 4 + 127) / 128), 128u, s, a);
+                    const bool uni = ((long long)(L / 6) * (L / 12)) % 128 == 0;
+                    launch_pdl(k6[uni][c], (unsigned)((chunks / 6 + 127) / 128), 128u, s, a);
                 }
             } else if (stencil == SPIN_STENCIL_TRIANGULAR) launch_pdl(stencil_pass_kernel<SPIN_STENCIL_TRIANGULAR>, grid, 128u, s, a);
             else if (stencil == SPIN_STENCIL_CUBIC && L % 16 == 0) {
