@@ -135,7 +135,7 @@ __global__ void __launch_bounds__(128) stencil_pass_kernel(StencilArgs a) {
 template <int kRows, bool kUniform>
 __global__ void __launch_bounds__(128) cubic_march_vec_kernel(StencilArgs a) {
     pdl_wait();
-    __shared__ uint32_t stab[16];
+    __shared__ unsigned long long stab[16];   // entry (always << 32) | T: accepted iff (64-bit) r < entry, one compare
     __shared__ uint32_t salways;
     const int L = a.L, V = L >> 4, RB = L / kRows;
     const long long per = (long long)RB * L * V;               // threads per replica: (plane block, j, v)
@@ -149,8 +149,9 @@ __global__ void __launch_bounds__(128) cubic_march_vec_kernel(StencilArgs a) {
         if (threadIdx.x < 16) {
             const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
             const int d = threadIdx.x >> 3, nd = threadIdx.x & 7;
-            stab[threadIdx.x] = nd <= 6 ? tab[d * 7 + nd] : 0u;
-            if (threadIdx.x == 0) salways = (tab[62] & 0x7Fu) | (((tab[62] >> 7) & 0x7Fu) << 8);
+            const uint32_t alw = (tab[62] & 0x7Fu) | (((tab[62] >> 7) & 0x7Fu) << 8);
+            stab[threadIdx.x] = nd <= 6 ? ((unsigned long long)((alw >> threadIdx.x) & 1u) << 32) | tab[d * 7 + nd] : 0ull;
+            if (threadIdx.x == 0) salways = alw;
         }
         __syncthreads();
     }
@@ -216,11 +217,10 @@ __global__ void __launch_bounds__(128) cubic_march_vec_kernel(StencilArgs a) {
             for (int e = 0; e < 2; ++e) {
                 const uint32_t pos = 2u * (uint32_t)e + par;                                    // byte of the updated site
                 const uint32_t idx = ((t >> (8u * pos)) & 0xFFu) >> 2;                          // d * 8 + nd
-                uint32_t T;
-                if (uniform) T = stab[idx];
-                else T = gtab[(idx >> 3) * 7u + (idx & 7u)];
                 // branch-free (a short-circuit `||` compiles to a divergent branch per site): accept -> all ones
-                const uint32_t acc = ((always >> idx) & 1u) | (uint32_t)(r[2 * w + e] < T);
+                uint32_t acc;
+                if (uniform) acc = (uint32_t)((unsigned long long)r[2 * w + e] < stab[idx]);
+                else acc = ((always >> idx) & 1u) | (uint32_t)(r[2 * w + e] < gtab[(idx >> 3) * 7u + (idx & 7u)]);
                 flip |= (0u - acc) & (0xFEu << (8u * pos));
             }
             out[w] = cw[w] ^ flip;
@@ -254,8 +254,7 @@ __device__ __forceinline__ void shifted_words(const uint32_t x[4], uint32_t edge
 template <int kRows, bool kUniform>
 __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
     pdl_wait();
-    __shared__ uint32_t stab[50];
-    __shared__ uint32_t salw[2];
+    __shared__ unsigned long long stab[50];   // entry (always << 32) | T: accepted iff (64-bit) r < entry, one compare
     const int L = a.L, V = L >> 4, H = L >> 1, RB = H / kRows;
     const long long per = (long long)RB * V;
     const long long total = per * a.batch;
@@ -266,8 +265,8 @@ __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
     constexpr bool uniform = kUniform;                           // per % blockDim.x == 0 (the launcher): a block never straddles replicas
     if (uniform) {
         const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
-        if (threadIdx.x < 50) stab[threadIdx.x] = tab[threadIdx.x];
-        if (threadIdx.x < 2) salw[threadIdx.x] = tab[62 + threadIdx.x];
+        if (threadIdx.x < 50)
+            stab[threadIdx.x] = ((unsigned long long)((tab[62 + (threadIdx.x >> 5)] >> (threadIdx.x & 31)) & 1u) << 32) | tab[threadIdx.x];
         __syncthreads();
     }
     if (gid >= total) return;
@@ -280,9 +279,9 @@ __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
     const int j0 = v << 4, jl = j0 == 0 ? L - 1 : j0 - 1, jr = j0 + 16 == L ? 0 : j0 + 16;
     int8_t* lat = a.lattice + (size_t)b * L * L;
     const uint32_t m = 0x04040404u;
-    const uint32_t* tab = uniform ? stab : a.tables + (size_t)b * kStencilRec;
-    const unsigned long long always = uniform ? ((unsigned long long)salw[0] | ((unsigned long long)salw[1] << 32))
-                                              : ((unsigned long long)tab[62] | ((unsigned long long)tab[63] << 32));
+    const uint32_t* tab = a.tables + (size_t)b * kStencilRec;   // read by the ragged launches only (!uniform)
+    unsigned long long always = 0ull;
+    if (!uniform) always = (unsigned long long)tab[62] | ((unsigned long long)tab[63] << 32);
     const uint32_t c1 = (uint32_t)b + a.replica_offset;
     // the row above the first updated row: masked word and its shifted forms
     uint32_t um[4], ul[4], ur[4];
@@ -317,7 +316,9 @@ __global__ void __launch_bounds__(128) nnn_march_vec_kernel(StencilArgs a) {
             for (int e = 0; e < 2; ++e) {
                 const uint32_t pos = 2u * (uint32_t)e + pj;
                 const uint32_t idx = ((t >> (8u * pos)) & 0xFFu) >> 2;
-                const uint32_t acc = (uint32_t)((always >> idx) & 1ull) | (uint32_t)(r[2 * w + e] < tab[idx]);   // branch-free
+                uint32_t acc;                                                                    // branch-free
+                if (uniform) acc = (uint32_t)((unsigned long long)r[2 * w + e] < stab[idx]);
+                else acc = (uint32_t)((always >> idx) & 1ull) | (uint32_t)(r[2 * w + e] < tab[idx]);
                 flip |= (0u - acc) & (0xFEu << (8u * pos));
             }
             out[w] = cw[w] ^ flip;
@@ -343,7 +344,7 @@ template <int kRows, bool kUniform, int kColour>
 __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a) {
     static_assert(kRows % 3 == 0, "the byte positions of the updated sites are compile-time only if a thread starts at a row that is a multiple of 3");
     pdl_wait();
-    __shared__ uint32_t stab[16];
+    __shared__ unsigned long long stab[16];   // entry (always << 32) | T: accepted iff (64-bit) r < entry, one compare
     __shared__ uint32_t salways;
     const int L = a.L, V = L / 12, RB = L / kRows;             // chunks per row, row blocks per replica
     const long long per = (long long)RB * V;
@@ -357,8 +358,9 @@ __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a
         if (threadIdx.x < 16) {
             const uint32_t* tab = a.tables + (size_t)b0 * kStencilRec;
             const int d = threadIdx.x >> 3, nd = threadIdx.x & 7;
-            stab[threadIdx.x] = nd <= 6 ? tab[d * 7 + nd] : 0u;
-            if (threadIdx.x == 0) salways = (tab[62] & 0x7Fu) | (((tab[62] >> 7) & 0x7Fu) << 8);
+            const uint32_t alw = (tab[62] & 0x7Fu) | (((tab[62] >> 7) & 0x7Fu) << 8);
+            stab[threadIdx.x] = nd <= 6 ? ((unsigned long long)((alw >> threadIdx.x) & 1u) << 32) | tab[d * 7 + nd] : 0ull;
+            if (threadIdx.x == 0) salways = alw;
         }
         __syncthreads();
     }
@@ -424,10 +426,9 @@ __global__ void __launch_bounds__(128) triangular_march_vec_kernel(StencilArgs a
             const int pos = ((kColour - rr) % 3 + 3) % 3 + 3 * e;   // byte of the updated site within the 12
             const uint32_t word = pos < 4 ? t[0] : (pos < 8 ? t[1] : t[2]);
             const uint32_t idx = ((word >> (8 * (pos & 3))) & 0xFFu) >> 2;      // d * 8 + nd
-            uint32_t T;
-            if (uniform) T = stab[idx];
-            else T = gtab[(idx >> 3) * 7u + (idx & 7u)];
-            const uint32_t acc = ((always >> idx) & 1u) | (uint32_t)(r[e] < T);                  // branch-free
+            uint32_t acc;                                                                        // branch-free
+            if (uniform) acc = (uint32_t)((unsigned long long)r[e] < stab[idx]);
+            else acc = ((always >> idx) & 1u) | (uint32_t)(r[e] < gtab[(idx >> 3) * 7u + (idx & 7u)]);
             const uint32_t bit = (0u - acc) & (0xFEu << (8 * (pos & 3)));
             flip[0] |= pos < 4 ? bit : 0u;
             flip[1] |= (pos >= 4 && pos < 8) ? bit : 0u;
