@@ -56,7 +56,7 @@ def test_invalid_shapes_and_arguments():
 
 @pytest.mark.parametrize("L,B", [(24, 5), (96, 2400)])
 def test_triangular_row_marching_kernel(L, B):
-    """The triangular byte-SIMD kernel marches 4 rows per thread, 12 when the launch is large (2400 x 96^2): every replica
+    """The triangular byte-SIMD kernel marches 6 rows per thread, 12 when the launch is large (2400 x 96^2): every replica
     against the oracle after each of 2 sweeps and after a 3-sweep call, ragged blocks that straddle replicas (5 x 24^2)."""
     st = sp.SPIN_STENCIL_TRIANGULAR
     seed = 40 + L
