@@ -80,15 +80,20 @@ __device__ __forceinline__ int cpm_site(const int8_t* lat, int L, int i, int j, 
     const int nb[8] = {lat[(size_t)iu * L + jl], lat[(size_t)iu * L + j], lat[(size_t)iu * L + jr], lat[(size_t)i * L + jl],
                        lat[(size_t)i * L + jr], lat[(size_t)id * L + jl], lat[(size_t)id * L + j], lat[(size_t)id * L + jr]};
     const int tn = p.tau[nw], to = p.tau[old];
-    long long dH = 0;
+    // Branch-free: both J entries are read for every neighbour and selected (conditional adds compile to a divergent branch
+    // each).  |J| <= 2^20 and 16 terms: the adhesion part is exact in 32 bits.
+    const int32_t* Jn = p.J + tn * p.ntypes;
+    const int32_t* Jo = p.J + to * p.ntypes;
+    int dJ = 0;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         const int ty = p.tau[nb[k]];
-        if (nw != nb[k]) dH += p.J[tn * p.ntypes + ty];
-        if (old != nb[k]) dH -= p.J[to * p.ntypes + ty];
+        const int jn = Jn[ty], jo = Jo[ty];
+        dJ += (nw != nb[k] ? jn : 0) - (old != nb[k] ? jo : 0);
     }
-    if (nw != 0) dH += p.lambda * (2ll * ((long long)areas[nw] - p.A[nw]) + 1);
-    if (old != 0) dH += p.lambda * (-2ll * ((long long)areas[old] - p.A[old]) + 1);
+    const long long an = p.lambda * (2ll * ((long long)areas[nw] - p.A[nw]) + 1);
+    const long long ao = p.lambda * (-2ll * ((long long)areas[old] - p.A[old]) + 1);
+    const long long dH = (long long)dJ + (nw != 0 ? an : 0ll) + (old != 0 ? ao : 0ll);
     bool acc = dH <= 0 || beta_zero;
     if (!acc && dH <= (long long)dmax) acc = r_acc < T[dH];
     return acc ? nw : -1;
