@@ -63,9 +63,12 @@ struct CpmTables {
     int ntypes;
 };
 
-template <typename P>   // CpmParams (kernel parameters) or CpmTables (shared-memory copies): same member names
+// kPair: D[a * qs + b] = (a != b) ? J[tau a][tau b] : 0 for all pairs of identifiers (shared memory, resident kernel): the
+// adhesion change is then two reads and two adds per neighbour.
+template <typename P, bool kPair = false>   // CpmParams (kernel parameters) or CpmTables (shared-memory copies): same member names
 __device__ __forceinline__ int cpm_site(const int8_t* lat, int L, int i, int j, uint32_t r_prop, uint32_t r_acc,
-                                        const int32_t* areas, const P& p, const uint32_t* T, int dmax, bool beta_zero) {
+                                        const int32_t* areas, const P& p, const uint32_t* T, int dmax, bool beta_zero,
+                                        const int32_t* D = nullptr, int qs = 0) {
     const int iu = i == 0 ? L - 1 : i - 1, id = i == L - 1 ? 0 : i + 1, jl = j == 0 ? L - 1 : j - 1, jr = j == L - 1 ? 0 : j + 1;
     const int old = lat[(size_t)i * L + j];
     // the proposed value first: most sites sit inside a cell or the medium, where it equals the old one and nothing else
@@ -79,17 +82,24 @@ __device__ __forceinline__ int cpm_site(const int8_t* lat, int L, int i, int j, 
     if (nw == old) return -1;
     const int nb[8] = {lat[(size_t)iu * L + jl], lat[(size_t)iu * L + j], lat[(size_t)iu * L + jr], lat[(size_t)i * L + jl],
                        lat[(size_t)i * L + jr], lat[(size_t)id * L + jl], lat[(size_t)id * L + j], lat[(size_t)id * L + jr]};
+    int dJ = 0;
+    if (kPair) {
+        const int32_t* Dn = D + nw * qs;
+        const int32_t* Do = D + old * qs;
+#pragma unroll
+        for (int k = 0; k < 8; ++k) dJ += Dn[nb[k]] - Do[nb[k]];
+    } else {
     const int tn = p.tau[nw], to = p.tau[old];
     // Branch-free: both J entries are read for every neighbour and selected (conditional adds compile to a divergent branch
     // each).  |J| <= 2^20 and 16 terms: the adhesion part is exact in 32 bits.
     const int32_t* Jn = p.J + tn * p.ntypes;
     const int32_t* Jo = p.J + to * p.ntypes;
-    int dJ = 0;
 #pragma unroll
     for (int k = 0; k < 8; ++k) {
         const int ty = p.tau[nb[k]];
         const int jn = Jn[ty], jo = Jo[ty];
         dJ += (nw != nb[k] ? jn : 0) - (old != nb[k] ? jo : 0);
+    }
     }
     const long long an = p.lambda * (2ll * ((long long)areas[nw] - p.A[nw]) + 1);
     const long long ao = p.lambda * (-2ll * ((long long)areas[old] - p.A[old]) + 1);
@@ -132,6 +142,7 @@ __global__ void __launch_bounds__(128) cpm_pass_kernel(CpmArgs a, CpmParams p) {
 // replica keeps the lattice and the area counters in shared memory and runs every sweep of the call in one launch.  The
 // areas are counted once; during a colour pass accepted copies add to a separate delta array, which is folded into the
 // areas after the pass - so every proposal of a pass still sees the counts of the start of that pass (reading C3).
+template <bool kPair>
 __global__ void __launch_bounds__(512) cpm_resident_kernel(CpmArgs a, CpmParams pp, unsigned long long t0, long long n_sweeps) {
     extern __shared__ __align__(16) int8_t slat[];
     __shared__ int32_t sarea[128], sdelta[128];
@@ -144,6 +155,13 @@ __global__ void __launch_bounds__(512) cpm_resident_kernel(CpmArgs a, CpmParams 
     for (int k = threadIdx.x; k < 128; k += blockDim.x) { sarea[k] = 0; sdelta[k] = 0; }
     for (int k = threadIdx.x; k < (N >> 2); k += blockDim.x) ((uint32_t*)slat)[k] = ((const uint32_t*)glat)[k];
     __syncthreads();
+    int32_t* D = (int32_t*)(slat + ((N + 15) & ~15));          // kPair: [q][q] behind the lattice
+    const int qs = pp.q;
+    if (kPair)
+        for (int k = threadIdx.x; k < qs * qs; k += blockDim.x) {
+            const int ia = k / qs, ib = k - ia * qs;
+            D[k] = ia != ib ? sJ[stau[ia] * p.ntypes + stau[ib]] : 0;
+        }
     {   // initial count: the medium (0) usually dominates, so it is counted in a register and reduced per warp
         int zeros = 0;
         for (int x = threadIdx.x; x < N; x += blockDim.x) {
@@ -173,7 +191,7 @@ __global__ void __launch_bounds__(512) cpm_resident_kernel(CpmArgs a, CpmParams 
                     if (n >= per) break;
                     const int row = wshift >= 0 ? n >> wshift : n / W, col = n - row * W;   // no division for L = 2^k
                     const int i = 2 * row + (colour >> 1), j = 2 * col + (colour & 1);
-                    const int nw = cpm_site(slat, L, i, j, r[2 * e], r[2 * e + 1], sarea, p, T, a.dmax, bz);
+                    const int nw = cpm_site<CpmTables, kPair>(slat, L, i, j, r[2 * e], r[2 * e + 1], sarea, p, T, a.dmax, bz, D, qs);
                     if (nw >= 0) {
                         const int old = slat[i * L + j];
                         slat[i * L + j] = (int8_t)nw;         // only this thread touches a site of the current colour
@@ -314,8 +332,15 @@ int spin_cpm_sweep(int32_t batch, int32_t L, int32_t q, int8_t* lattice, const i
             // one Philox group (two sites) per thread and colour pass where the lattice has that many (the passes are latency
             // chains: 60 -> measured below with 512 threads for L = 64)
             const unsigned res_threads = (L / 2) * (L / 2) / 2 >= 512 ? 512u : 256u;
-            if (N > 32768) e = cudaFuncSetAttribute(cpm_resident_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 65536);
-            if (e == cudaSuccess) cpm_resident_kernel<<<(unsigned)batch, res_threads, (size_t)N, s>>>(a, p, (unsigned long long)sweep_offset, (long long)n_sweeps);
+            // the pair table of the adhesion energies ([q][q] int32 behind the lattice) while it stays small (q <= 64: 16 KiB)
+            const bool pair = q <= 64;
+            const size_t smem = pair ? (size_t)((N + 15) & ~15ll) + sizeof(int32_t) * q * q : (size_t)N;
+            if (smem > 49152) e = cudaFuncSetAttribute(pair ? cpm_resident_kernel<true> : cpm_resident_kernel<false>,
+                                                       cudaFuncAttributeMaxDynamicSharedMemorySize, 65536 + 16384);
+            if (e == cudaSuccess) {
+                if (pair) cpm_resident_kernel<true><<<(unsigned)batch, res_threads, smem, s>>>(a, p, (unsigned long long)sweep_offset, (long long)n_sweeps);
+                else cpm_resident_kernel<false><<<(unsigned)batch, res_threads, smem, s>>>(a, p, (unsigned long long)sweep_offset, (long long)n_sweeps);
+            }
         }
         for (int64_t t = sweep_offset; !resident && t < sweep_offset + n_sweeps && e == cudaSuccess; ++t)
             for (int c = 0; c < 4; ++c) {
