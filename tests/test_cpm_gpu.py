@@ -56,6 +56,23 @@ def test_random_lattices_equal_oracle(L, q, lam):
     _check_obs(d, ref, B, L, tau, A, lam, st)
 
 
+@pytest.mark.parametrize("L,cells,size,B", [(192, 8, 6, 3), (260, 11, 8, 2)])
+def test_large_lattices_take_the_three_launch_path(L, cells, size, B):
+    """Lattices beyond one CTA's shared memory, or few large replicas (L > 128 with fewer than 148 replicas), run
+    cpm_area_kernel + cpm_pass_kernel per colour pass instead of the resident kernel: same oracle, same bar."""
+    seed, lam = 21, 2
+    spins, tau, A = workloads.cpm_initial(B, L, cells, size, seed=4)
+    beta = np.linspace(0.05, 0.5, B)
+    ref = spins.copy()
+    d = torch.from_numpy(spins.copy()).cuda()
+    st = torch.cuda.current_stream().cuda_stream
+    for t0, n in ((0, 1), (1, 1), (2, 3)):
+        sp.spin_cpm_sweep(B, L, d.data_ptr(), tau, JT, lam, A, beta, seed, n, sweep_offset=t0, replica_offset=1, cuda_stream=st)
+        oracle.cpm_sweep(ref, tau, JT, lam, A, beta, seed, n, sweep_offset=t0, replica_offset=1)
+        assert np.array_equal(d.cpu().numpy(), ref), t0
+    _check_obs(d, ref, B, L, tau, A, lam, st)
+
+
 def test_argument_checks():
     spins, tau, A = workloads.cpm_initial(1, 16, 3, 4, seed=1)
     d = torch.from_numpy(spins.copy()).cuda()
